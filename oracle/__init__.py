@@ -1,0 +1,149 @@
+"""ctypes front of the CPU oracle (oracle/dash_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It imports nothing from
+paper_2507_19141_b200 and shares no code with the CUDA path.
+
+All arrays are host numpy arrays.  Function names mirror the C ABI of the product
+(include/dash_hash4d.h) with the prefix `oracle_`; semantics: DESIGN.md §2-§3.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+FLAG_DENSE_COARSE = 1
+
+
+class OracleConfig(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("L", C.c_uint32), ("F", C.c_uint32), ("T", C.c_uint32),
+                ("res_s_min", C.c_uint32), ("res_s_max", C.c_uint32),
+                ("res_t_min", C.c_uint32), ("res_t_max", C.c_uint32),
+                ("primes", C.c_uint32 * 4), ("table_dtype", C.c_uint32), ("flags", C.c_uint32)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.dash_oracle_threads.restype = C.c_int
+    return _lib
+
+
+def make_config(L, F, T, res_s_min, res_s_max, res_t_min, res_t_max, table_dtype="fp32",
+                primes=(0, 0, 0, 0), dense_coarse=True) -> OracleConfig:
+    c = OracleConfig()
+    c.struct_size = C.sizeof(OracleConfig)
+    c.L, c.F, c.T = L, F, T
+    c.res_s_min, c.res_s_max, c.res_t_min, c.res_t_max = res_s_min, res_s_max, res_t_min, res_t_max
+    c.primes = (C.c_uint32 * 4)(*primes)
+    c.table_dtype = {"fp32": 0, "fp16": 1}[table_dtype]
+    c.flags = FLAG_DENSE_COARSE if dense_coarse else 0
+    return c
+
+
+def config_from_params(enc, **kw) -> OracleConfig:
+    """enc: dash_inputs.EncoderParams (plain numbers only)."""
+    return make_config(enc.L, enc.F, enc.T, enc.res_s_min, enc.res_s_max, enc.res_t_min,
+                       enc.res_t_max, enc.table_dtype, **kw)
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise RuntimeError(f"{what} failed with oracle status {rc}")
+
+
+def _query_args(xyz, t, index, t_stride):
+    assert xyz.dtype == np.float32 and xyz.ndim == 2 and xyz.shape[1] in (3, 4) and xyz.flags.c_contiguous
+    assert t.dtype == np.float32 and t.flags.c_contiguous
+    if index is not None:
+        assert index.dtype == np.int32 and index.flags.c_contiguous
+    return C.c_uint32(xyz.shape[1]), C.c_uint32(t_stride)
+
+
+def threads() -> int:
+    return int(lib().dash_oracle_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().dash_oracle_set_threads(C.c_int(n))
+
+
+def oracle_resolutions(cfg: OracleConfig):
+    L = cfg.L
+    rs, rt, dn = np.zeros(L, np.uint32), np.zeros(L, np.uint32), np.zeros(L, np.uint8)
+    _check(lib().dash_oracle_resolutions(C.byref(cfg), _p(rs), _p(rt), _p(dn)), "resolutions")
+    return rs, rt, dn.astype(bool)
+
+
+def oracle_indices(cfg, N, xyz, t, index=None, t_stride=1, want_weights=True):
+    xs, ts = _query_args(xyz, t, index, t_stride)
+    idx = np.zeros((N, cfg.L, 16), np.uint32)
+    w = np.zeros((N, cfg.L, 16), np.float64) if want_weights else None
+    _check(lib().dash_oracle_indices(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(t), ts, _p(index),
+                                     _p(idx), _p(w)), "indices")
+    return idx, w
+
+
+def oracle_fwd(cfg, N, xyz, t, table, index=None, t_stride=1, want_abs=False):
+    xs, ts = _query_args(xyz, t, index, t_stride)
+    want = np.float16 if cfg.table_dtype == 1 else np.float32
+    assert table.dtype == want and table.flags.c_contiguous and table.size == cfg.L * cfg.T * cfg.F
+    out = np.zeros((N, cfg.L * cfg.F), np.float32)
+    mag = np.zeros((N, cfg.L * cfg.F), np.float64) if want_abs else None
+    _check(lib().dash_oracle_fwd(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(t), ts, _p(index),
+                                 _p(table), _p(out), _p(mag)), "fwd")
+    return (out, mag) if want_abs else out
+
+
+def oracle_bwd(cfg, N, xyz, t, dout, index=None, t_stride=1, dtable=None, want_abs=False,
+               want_hits=False):
+    """Returns dtable [L][T][F] fp32 (accumulated into `dtable` if given), and optionally
+    sum|W*dY| per entry (double) and contributions per slot (uint32)."""
+    xs, ts = _query_args(xyz, t, index, t_stride)
+    assert dout.dtype == np.float32 and dout.flags.c_contiguous and dout.size == N * cfg.L * cfg.F
+    if dtable is None:
+        dtable = np.zeros((cfg.L, cfg.T, cfg.F), np.float32)
+    assert dtable.dtype == np.float32 and dtable.flags.c_contiguous
+    mag = np.zeros((cfg.L, cfg.T, cfg.F), np.float64) if want_abs else None
+    hits = np.zeros((cfg.L, cfg.T), np.uint32) if want_hits else None
+    _check(lib().dash_oracle_bwd(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(t), ts, _p(index),
+                                 _p(dout), _p(dtable), _p(mag), _p(hits)), "bwd")
+    res = [dtable]
+    if want_abs:
+        res.append(mag)
+    if want_hits:
+        res.append(hits)
+    return res[0] if len(res) == 1 else tuple(res)
+
+
+# ---- debug exports used only by the pin tests ----
+
+def oracle_vertex_slot(cfg, level: int, g) -> int:
+    garr = (C.c_uint32 * 4)(*[int(v) for v in g])
+    out = C.c_uint32(0)
+    _check(lib().dash_oracle_vertex_slot(C.byref(cfg), C.c_uint32(level), garr, C.byref(out)), "vertex_slot")
+    return int(out.value)
+
+
+def oracle_locate(x: float, n: int):
+    cell, frac = C.c_uint32(0), C.c_float(0)
+    lib().dash_oracle_locate(C.c_float(x), C.c_uint32(n), C.byref(cell), C.byref(frac))
+    return int(cell.value), float(frac.value)
+
+
+def oracle_half_to_double(h: int) -> float:
+    f = lib().dash_oracle_half_to_double
+    f.restype = C.c_double
+    return float(f(C.c_uint16(h)))

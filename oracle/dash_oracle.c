@@ -1,0 +1,341 @@
+/*
+ * dash_oracle.c — CPU ORACLE for the DASH multiresolution 4D hash encoder G_4D.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may load it.  It shares no code, header,
+ * table or constant generator with the CUDA path (paper_2507_19141_b200/csrc, include/).
+ *
+ * What it computes: the plain definition of, written out in the paper's order
+ *   Eq. 7  resolution schedule N_l            -> dash_oracle_resolutions
+ *   PAPER.md:129           cell location  floor(x * N_l)      -> locate()
+ *   Eq. 8  spatial-temporal hash of a vertex  -> vertex_slot()
+ *   PAPER.md:133 / Eq. 9   quadrilinear interpolation, levels concatenated to f_h in R^{LF}
+ *                                                              -> dash_oracle_fwd
+ *   PAPER.md:133 ("learnable feature vectors"): the transpose of that linear map, i.e. the
+ *   table gradient dtable[l][h] += W * dY                      -> dash_oracle_bwd
+ * Where the paper is silent or garbled the reading taken is the numbered one in DESIGN.md §3
+ * (Q1..Q21); each is marked "Q<n>" below.
+ *
+ * Precision: cell location is ONE binary32 multiply (Q4) so that indices are a bit-exact
+ * contract; interpolation weights, feature sums and gradient sums are formed in double and
+ * rounded to fp32 once (Q11, Q14).  No blocking, no SIMD, no reordering.  OpenMP only splits
+ * independent work: queries in fwd/indices, levels (disjoint tables) in bwd.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): printed resolution lists, hand-derived hash
+ * values, dense-index bijection by brute force, weights sum to 1, exact table value at grid
+ * vertices, multi-affine reproduction, scipy RegularGridInterpolator on dense levels,
+ * linearity, adjoint identity, finite differences, pure-Python brute force on tiny inputs.
+ * Parity with the paper's OWN (unavailable) CUDA code on hashed levels: "parity unpinned"
+ * (its primes / scale convention are not in the paper) — see DESIGN.md §3.
+ *
+ * Build: gcc -O2 -std=c11 -fopenmp -ffp-contract=off -shared -fPIC (oracle/build.py).
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct dash_oracle_config {
+    uint32_t struct_size;
+    uint32_t L, F, T;
+    uint32_t res_s_min, res_s_max;
+    uint32_t res_t_min, res_t_max;
+    uint32_t primes[4];
+    uint32_t table_dtype; /* 0 fp32, 1 fp16 */
+    uint32_t flags;       /* bit0: dense indexing on coarse levels (Q10) */
+} dash_oracle_config;
+
+enum { ORACLE_OK = 0, ORACLE_INVALID = 1, ORACLE_NOMEM = 5 };
+#define ORACLE_MAX_L 32
+
+/* Q7: default multipliers (pi_1 = 1 keeps x-neighbours adjacent; the other three are large primes) */
+static const uint32_t k_default_primes[4] = {1u, 2654435761u, 805459861u, 3674653429u};
+
+static int config_ok(const dash_oracle_config *c) {
+    if (!c || c->struct_size != sizeof(dash_oracle_config)) return 0;
+    if (c->L < 1 || c->L > ORACLE_MAX_L) return 0;
+    if (!(c->F == 1 || c->F == 2 || c->F == 4 || c->F == 8)) return 0;
+    if (c->T < 1) return 0;
+    if (c->res_s_min < 1 || c->res_s_min > c->res_s_max) return 0;
+    if (c->res_t_min < 1 || c->res_t_min > c->res_t_max) return 0;
+    if (c->table_dtype > 1) return 0;
+    return 1;
+}
+
+static void get_primes(const dash_oracle_config *c, uint32_t pi[4]) {
+    int all_zero = !(c->primes[0] | c->primes[1] | c->primes[2] | c->primes[3]);
+    for (int d = 0; d < 4; ++d) pi[d] = all_zero ? k_default_primes[d] : c->primes[d];
+}
+
+/* Eq. 7 read as N_l = floor(N_min * b^l), b = exp((ln N_max - ln N_min)/(L-1))
+ * (Q1: the exponent l is lost in the extracted text; "geometric progression").
+ * Q2: evaluated in IEEE double as N_min * pow(N_max/N_min, l/(L-1)), floor(r + 1e-6) so that
+ * levels that are mathematically integers (64, 128, 300, 4096 ...) do not fall one short. */
+static uint32_t level_resolution(uint32_t n_min, uint32_t n_max, uint32_t l, uint32_t L) {
+    if (L == 1) return n_min;
+    double r = (double)n_min * pow((double)n_max / (double)n_min, (double)l / (double)(L - 1));
+    return (uint32_t)floor(r + 1e-6);
+}
+
+/* Q10: a level is dense iff its vertex count (Ns+1)^3 (Nt+1) fits in T. */
+static int level_is_dense(const dash_oracle_config *c, uint32_t ns, uint32_t nt) {
+    if (!(c->flags & 1u)) return 0;
+    long double v = (long double)(ns + 1.0L) * (ns + 1.0L) * (ns + 1.0L) * (nt + 1.0L);
+    return v <= (long double)c->T;
+}
+
+int dash_oracle_resolutions(const dash_oracle_config *c, uint32_t *res_s, uint32_t *res_t,
+                            uint8_t *is_dense) {
+    if (!config_ok(c) || !res_s || !res_t) return ORACLE_INVALID;
+    for (uint32_t l = 0; l < c->L; ++l) {
+        res_s[l] = level_resolution(c->res_s_min, c->res_s_max, l, c->L); /* Q3: spatial range */
+        res_t[l] = level_resolution(c->res_t_min, c->res_t_max, l, c->L); /* Q3: temporal range */
+        if (is_dense) is_dense[l] = (uint8_t)level_is_dense(c, res_s[l], res_t[l]);
+    }
+    return ORACLE_OK;
+}
+
+/* Q12: inputs live in [0,1); clamp to [0, 1-2^-24], NaN -> 0. */
+static float clamp_unit(float v) {
+    if (isnan(v)) return 0.0f;
+    if (v < 0.0f) return 0.0f;
+    if (v > 0x1.fffffep-1f) return 0x1.fffffep-1f;
+    return v;
+}
+
+/* floor(x_l) = floor(x * N_l).  Q4: one binary32 multiply, no offset.
+ * (volatile + -ffp-contract=off keep the compiler from widening or fusing it.) */
+static void locate(float x, uint32_t n, uint32_t *cell, float *frac) {
+    volatile float pos = x * (float)n;
+    float fl = floorf(pos);
+    *cell = (uint32_t)fl;
+    *frac = pos - fl; /* exact in fp32 */
+}
+
+/* Eq. 8: h = (XOR_i g_i * pi_i) mod T, products in uint32 wraparound (Q8),
+ * uniform T (Q9); or the dense injective index on coarse levels (Q10), x fastest. */
+static uint32_t vertex_slot(const uint32_t g[4], const uint32_t pi[4], uint32_t T, int dense,
+                            uint32_t ns) {
+    if (dense) {
+        uint32_t S = ns + 1u;
+        return g[0] + S * (g[1] + S * (g[2] + S * g[3]));
+    }
+    uint32_t h = 0;
+    for (int d = 0; d < 4; ++d) h ^= g[d] * pi[d];
+    return h % T;
+}
+
+/* Q13: IEEE half -> double, exact, by the format's definition. */
+static double half_to_double(uint16_t h) {
+    int sign = (h >> 15) & 1, e = (h >> 10) & 0x1f, m = h & 0x3ff;
+    double v;
+    if (e == 0) v = ldexp((double)m, -24);
+    else if (e == 31) v = m ? NAN : INFINITY;
+    else v = ldexp((double)(m + 1024), e - 25);
+    return sign ? -v : v;
+}
+
+typedef struct {
+    uint32_t res_s[ORACLE_MAX_L], res_t[ORACLE_MAX_L];
+    uint8_t dense[ORACLE_MAX_L];
+    uint32_t pi[4];
+} level_plan;
+
+static int make_plan(const dash_oracle_config *c, level_plan *p) {
+    int rc = dash_oracle_resolutions(c, p->res_s, p->res_t, p->dense);
+    if (rc) return rc;
+    get_primes(c, p->pi);
+    return ORACLE_OK;
+}
+
+/* Steps 1-5 of DESIGN.md §2 for one (query, level): the 16 slots and 16 weights.
+ * Corner k: bit d of k set => +1 along dimension d, d = 0:x 1:y 2:z 3:t (Q5, Q6). */
+static void corners(const dash_oracle_config *c, const level_plan *p, uint32_t l,
+                    const float q[4], uint32_t slot[16], double W[16]) {
+    uint32_t cell[4];
+    float frac[4];
+    for (int d = 0; d < 4; ++d) {
+        uint32_t n = (d < 3) ? p->res_s[l] : p->res_t[l];
+        locate(clamp_unit(q[d]), n, &cell[d], &frac[d]);
+    }
+    for (int k = 0; k < 16; ++k) {
+        uint32_t g[4];
+        double w = 1.0;
+        for (int d = 0; d < 4; ++d) {
+            int up = (k >> d) & 1;
+            g[d] = cell[d] + (uint32_t)up; /* Q5: upper corner is floor+1 always */
+            w *= up ? (double)frac[d] : 1.0 - (double)frac[d];
+        }
+        slot[k] = vertex_slot(g, p->pi, c->T, p->dense[l], p->res_s[l]);
+        W[k] = w;
+    }
+}
+
+static void fetch_query(uint64_t n, const float *xyz, uint32_t xyz_stride, const float *t,
+                        uint32_t t_stride, const int32_t *index, float q[4]) {
+    uint64_t row = index ? (uint64_t)index[n] : n;
+    q[0] = xyz[row * xyz_stride + 0];
+    q[1] = xyz[row * xyz_stride + 1];
+    q[2] = xyz[row * xyz_stride + 2];
+    q[3] = t[n * (uint64_t)t_stride]; /* Q21: t_stride 0 = one timestamp for all */
+}
+
+static int args_ok(const float *xyz, uint32_t xyz_stride, const float *t, uint32_t t_stride) {
+    if (!xyz || !t) return 0;
+    if (!(xyz_stride == 3 || xyz_stride == 4)) return 0;
+    if (!(t_stride == 0 || t_stride == 1 || t_stride == 4)) return 0;
+    return 1;
+}
+
+/* idx_out [N][L][16] u32; w_out [N][L][16] double (nullable). */
+int dash_oracle_indices(const dash_oracle_config *c, uint64_t N, const float *xyz,
+                        uint32_t xyz_stride, const float *t, uint32_t t_stride,
+                        const int32_t *index, uint32_t *idx_out, double *w_out) {
+    level_plan p;
+    if (!config_ok(c) || make_plan(c, &p)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!args_ok(xyz, xyz_stride, t, t_stride) || !idx_out) return ORACLE_INVALID;
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < (int64_t)N; ++n) {
+        float q[4];
+        fetch_query((uint64_t)n, xyz, xyz_stride, t, t_stride, index, q);
+        for (uint32_t l = 0; l < c->L; ++l) {
+            uint32_t slot[16];
+            double W[16];
+            corners(c, &p, l, q, slot, W);
+            size_t base = ((size_t)n * c->L + l) * 16;
+            for (int k = 0; k < 16; ++k) {
+                idx_out[base + k] = slot[k];
+                if (w_out) w_out[base + k] = W[k];
+            }
+        }
+    }
+    return ORACLE_OK;
+}
+
+static double table_value(const dash_oracle_config *c, const void *table, uint32_t l,
+                          uint32_t slot, uint32_t f) {
+    size_t e = ((size_t)l * c->T + slot) * c->F + f; /* D1: [L][T][F] */
+    if (c->table_dtype == 1) return half_to_double(((const uint16_t *)table)[e]);
+    return (double)((const float *)table)[e];
+}
+
+/* Eq. 9: out[n][l*F+f] = sum_k W_k * table[l][slot_k][f]  (Q11: level-major).
+ * out_abs (nullable, [N][L*F] double) receives sum_k |W_k * v_k| — the conditioning term A of
+ * the elementwise tolerance (DESIGN.md §3 Q17). */
+int dash_oracle_fwd(const dash_oracle_config *c, uint64_t N, const float *xyz, uint32_t xyz_stride,
+                    const float *t, uint32_t t_stride, const int32_t *index, const void *table,
+                    float *out, double *out_abs) {
+    level_plan p;
+    if (!config_ok(c) || make_plan(c, &p)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!args_ok(xyz, xyz_stride, t, t_stride) || !table || !out) return ORACLE_INVALID;
+    const uint32_t L = c->L, F = c->F;
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < (int64_t)N; ++n) {
+        float q[4];
+        fetch_query((uint64_t)n, xyz, xyz_stride, t, t_stride, index, q);
+        for (uint32_t l = 0; l < L; ++l) {
+            uint32_t slot[16];
+            double W[16];
+            corners(c, &p, l, q, slot, W);
+            for (uint32_t f = 0; f < F; ++f) {
+                double acc = 0.0, mag = 0.0;
+                for (int k = 0; k < 16; ++k) {
+                    double term = W[k] * table_value(c, table, l, slot[k], f);
+                    acc += term;
+                    mag += fabs(term);
+                }
+                size_t o = (size_t)n * L * F + (size_t)l * F + f;
+                out[o] = (float)acc; /* rounded to fp32 once */
+                if (out_abs) out_abs[o] = mag;
+            }
+        }
+    }
+    return ORACLE_OK;
+}
+
+/* Transpose of Eq. 9: dtable[l][slot_k][f] += W_k * dout[n][l*F+f]   (Q15: accumulate).
+ * Per level: a double accumulator over the whole level, queries in order n = 0..N-1, rounded to
+ * fp32 once and added to the caller's dtable.  grad_abs (nullable, [L][T][F] double) receives
+ * sum |W * dY| per entry; hits (nullable, [L][T] u32) the number of contributions per slot. */
+int dash_oracle_bwd(const dash_oracle_config *c, uint64_t N, const float *xyz, uint32_t xyz_stride,
+                    const float *t, uint32_t t_stride, const int32_t *index, const float *dout,
+                    float *dtable, double *grad_abs, uint32_t *hits) {
+    level_plan p;
+    if (!config_ok(c) || make_plan(c, &p)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!args_ok(xyz, xyz_stride, t, t_stride) || !dout || !dtable) return ORACLE_INVALID;
+    const uint32_t L = c->L, F = c->F;
+    const size_t TF = (size_t)c->T * F;
+    int failed = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t l = 0; l < (int32_t)L; ++l) {
+        double *acc = (double *)calloc(TF, sizeof(double));
+        double *mag = grad_abs ? grad_abs + (size_t)l * TF : NULL;
+        uint32_t *cnt = hits ? hits + (size_t)l * c->T : NULL;
+        if (!acc) {
+            failed = 1;
+            continue;
+        }
+        if (mag) memset(mag, 0, TF * sizeof(double));
+        if (cnt) memset(cnt, 0, (size_t)c->T * sizeof(uint32_t));
+        for (uint64_t n = 0; n < N; ++n) {
+            float q[4];
+            uint32_t slot[16];
+            double W[16];
+            fetch_query(n, xyz, xyz_stride, t, t_stride, index, q);
+            corners(c, &p, (uint32_t)l, q, slot, W);
+            for (int k = 0; k < 16; ++k) {
+                for (uint32_t f = 0; f < F; ++f) {
+                    double term = W[k] * (double)dout[(size_t)n * L * F + (size_t)l * F + f];
+                    acc[(size_t)slot[k] * F + f] += term;
+                    if (mag) mag[(size_t)slot[k] * F + f] += fabs(term);
+                }
+                if (cnt) cnt[slot[k]] += 1u;
+            }
+        }
+        float *dst = dtable + (size_t)l * TF;
+        for (size_t e = 0; e < TF; ++e) dst[e] = (float)((double)dst[e] + acc[e]);
+        free(acc);
+    }
+    return failed ? ORACLE_NOMEM : ORACLE_OK;
+}
+
+int dash_oracle_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void dash_oracle_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* ---- debug exports used only by the pin tests ---- */
+
+/* Slot of grid vertex g = (gx,gy,gz,gt) at level l (Eq. 8 or the dense index). */
+int dash_oracle_vertex_slot(const dash_oracle_config *c, uint32_t l, const uint32_t g[4],
+                            uint32_t *slot) {
+    level_plan p;
+    if (!config_ok(c) || make_plan(c, &p) || l >= c->L || !g || !slot) return ORACLE_INVALID;
+    *slot = vertex_slot(g, p.pi, c->T, p.dense[l], p.res_s[l]);
+    return ORACLE_OK;
+}
+
+/* Cell and fractional offset of coordinate x at resolution n (after the Q12 clamp). */
+void dash_oracle_locate(float x, uint32_t n, uint32_t *cell, float *frac) {
+    locate(clamp_unit(x), n, cell, frac);
+}
+
+double dash_oracle_half_to_double(uint16_t h) { return half_to_double(h); }
