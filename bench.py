@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py — DASH 4D hash encoder, fwd + bwd, on B200 (metric: BASELINE.json "4D hash encode fwd+bwd
+Mqueries/s at 1 B200; achieved GB/s vs HBM peak").
+
+One STEP = one pass of the whole hot path over one batch of synthetic queries:
+    zero the table gradient  ->  dash_hash4d_fwd  ->  dash_hash4d_bwd
+all through the C ABI (include/dash_hash4d.h), on one stream.  Default workload: BASELINE.json configs[3]
+("C4": N=1M, L=16, F=4, T=2^21, fp16 table) — the config the north_star's roofline bar is quoted on.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C1..C5] [--impl reference]
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/) instead — the only
+place besides the cpu_baseline leg where this file executes oracle code.
+N > 1: replicas (the path needs no exchange step) — every rank runs the same workload on its
+own GPU, value = N * queries / max-over-ranks time, scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from dash_inputs import CONFIGS, make_workload  # noqa: E402
+
+METRIC = "4d_hash_encode_fwd_bwd_mqueries_per_s"
+UNIT = "Mqueries/s"
+REFERENCE_SAMPLE_QUERIES = 100_000     # per step of --impl reference
+CPU_BASELINE_QUERIES = 500_000         # bounded sample of the cpu_baseline leg (~10 s of CPU work)
+
+
+# ------------------------------------------------------------------------------------------ helpers
+
+def algorithmic_bytes(enc, has_index: bool):
+    """SURVEY.md §8d / DESIGN.md §6: bytes the method itself must move, per query and fixed."""
+    s_table = 2 if enc.table_dtype == "fp16" else 4
+    inp = 20 if has_index else 16
+    fwd = inp + 16 * enc.L * enc.F * s_table + 4 * enc.L * enc.F
+    bwd = inp + 4 * enc.L * enc.F + 16 * enc.L * enc.F * 4
+    zero = 4 * enc.L * enc.T * enc.F
+    return fwd, bwd, zero
+
+
+def measured_hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:  # noqa: BLE001
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:  # noqa: BLE001
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:  # noqa: BLE001
+            self.proc.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_oracle(wl, n_queries: int, repeats: int = 1):
+    """Oracle fwd+bwd on the first n_queries queries of the workload, as it stands.  -> (seconds, threads)."""
+    import oracle
+    enc = wl.spec.enc
+    cfg = oracle.config_from_params(enc)
+    n = min(n_queries, wl.N)
+    t = np.ascontiguousarray(wl.t[:n])
+    dout = np.ascontiguousarray(wl.dout[:n])
+    if wl.index is not None:
+        xyz, index = wl.xyz, np.ascontiguousarray(wl.index[:n])
+    else:
+        xyz, index = np.ascontiguousarray(wl.xyz[:n]), None
+    best = float("inf")
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        oracle.oracle_fwd(cfg, n, xyz, t, wl.table, index=index)
+        oracle.oracle_bwd(cfg, n, xyz, t, dout, index=index)
+        best = min(best, time.perf_counter() - t0)
+    return best, n, oracle.threads()
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl = make_workload(args.config)
+    times = []
+    n = threads = 0
+    for i in range(args.warmup + args.steps):
+        sec, n, threads = time_oracle(wl, REFERENCE_SAMPLE_QUERIES)
+        if i >= args.warmup:
+            times.append(sec)
+    sec = sum(times) / len(times)
+    value = n / sec / 1e6
+    enc = wl.spec.enc
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.config}: first {n} of {wl.N} queries per step, L={enc.L} F={enc.F} "
+                               f"T=2^{enc.T.bit_length() - 1} table {enc.table_dtype}",
+                   "queries_per_step": n},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                         "sample": f"first {n} queries of {args.config}, fwd+bwd, mean of {args.steps} steps"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ CUDA arm
+
+def run_cuda(args):
+    import torch
+    import paper_2507_19141_b200 as dh
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    wl = make_workload(args.config)
+    enc, N = wl.spec.enc, wl.N
+    flags = dh.FLAG_DENSE_COARSE | (dh.FLAG_ZERO_GRAD if args.zero_grad_fused else 0)
+    cfg = dh.config_from_params(enc, flags=flags)
+    to_dev = lambda a: None if a is None else torch.from_numpy(a).cuda()
+    xyz, t, index = to_dev(wl.xyz), to_dev(wl.t), to_dev(wl.index)
+    table, dout = to_dev(wl.table), to_dev(wl.dout)
+    out = torch.empty((N, enc.L * enc.F), dtype=torch.float32, device="cuda")
+    dtable = torch.empty((enc.L, enc.T, enc.F), dtype=torch.float32, device="cuda")
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(marks=None):
+        if marks is not None:
+            marks[0].record()
+        if not args.zero_grad_fused:
+            dh.dash_hash4d_zero(cfg, dtable)
+        if marks is not None:
+            marks[1].record()
+        dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index)
+        if marks is not None:
+            marks[2].record()
+        dh.dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=index)
+        if marks is not None:
+            marks[3].record()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    marks = [[ev() for _ in range(4)] for _ in range(args.steps)]
+    start, stop = ev(), ev()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler is not None:
+        time.sleep(0.25)                       # let the sampler come up before the timed region
+    dh.dash_hash4d_launch_count(reset=True)
+    barrier()
+    start.record()
+    for i in range(args.steps):
+        step(marks[i])
+    stop.record()
+    barrier()
+    launches = dh.dash_hash4d_launch_count()
+    clocks = sampler.stop() if sampler is not None else None
+    ms_total = start.elapsed_time(stop)
+    if dist is not None:
+        tt = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+    seg = np.array([[m[0].elapsed_time(m[1]), m[1].elapsed_time(m[2]), m[2].elapsed_time(m[3])]
+                    for m in marks])
+    ms_zero, ms_fwd, ms_bwd = (float(v) for v in seg.mean(0))
+
+    # ---- roofline of the dominant kernel (the bwd scatter), live CUDA-event durations
+    b_fwd, b_bwd, b_zero = algorithmic_bytes(enc, index is not None)
+    peak, peak_src = measured_hbm_peak()
+    dominant = "bwd" if ms_bwd >= ms_fwd else "fwd"
+    dom_bytes = (b_bwd if dominant == "bwd" else b_fwd) * N
+    if dominant == "bwd" and args.zero_grad_fused:
+        dom_bytes += b_zero
+    dom_ms = ms_bwd if dominant == "bwd" else ms_fwd
+    achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
+    step_bytes = (b_fwd + b_bwd) * N + b_zero
+    roofline = {
+        "bound": "hbm", "kernel": f"hash4d_{dominant}_kernel", "achieved": achieved, "peak": peak,
+        "unit": "GB/s", "frac": achieved / peak, "traffic": args.traffic_bytes,
+        "peak_source": peak_src,
+        "algorithmic_bytes_per_launch": dom_bytes,
+        "step": {"algorithmic_bytes": step_bytes, "achieved": step_bytes / (ms_step * 1e-3) / 1e9,
+                 "frac": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
+                 "ms": {"zero": ms_zero, "fwd": ms_fwd, "bwd": ms_bwd}},
+    }
+
+    # ---- e2e: HOST (pinned) buffers through the binding's *_host calls, copies inside the timed region
+    pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory()
+    xyz_h, t_h, index_h, dout_h = pin(wl.xyz), pin(wl.t), pin(wl.index), pin(wl.dout)
+    out_h = torch.empty((N, enc.L * enc.F), dtype=torch.float32).pin_memory()
+    dtable_h = torch.empty((enc.L, enc.T, enc.F), dtype=torch.float32).pin_memory()
+    staging = {"xyz": xyz, "t": t, "dout": dout, "out": out, "dtable": dtable}
+    if index is not None:
+        staging["index"] = index
+
+    def e2e_step():
+        dh.dash_hash4d_fwd_host(cfg, xyz_h, t_h, table, out_h, index_h=index_h, staging=staging)
+        dh.dash_hash4d_bwd_host(cfg, xyz_h, t_h, dout_h, dtable_h, index_h=index_h, staging=staging,
+                                reuse_queries=True)
+
+    e2e_steps = max(3, min(args.steps, 10))
+    e2e_step(); e2e_step()
+    barrier()
+    e0, e1 = ev(), ev()
+    e0.record()
+    for _ in range(e2e_steps):
+        e2e_step()
+    e1.record()
+    barrier()
+    e2e_ms = e0.elapsed_time(e1) / e2e_steps
+    if dist is not None:
+        tt = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_ms = float(tt.item())
+    nbytes = lambda x: 0 if x is None else x.numel() * x.element_size()
+    h2d = nbytes(xyz_h) + nbytes(t_h) + nbytes(index_h) + nbytes(dout_h)
+    d2h = nbytes(out_h) + nbytes(dtable_h)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- cpu_baseline: the oracle as it stands, bounded sample, on this box's host cores
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        sec, n_s, threads = time_oracle(wl, CPU_BASELINE_QUERIES)
+        cpu = {"value": n_s / sec / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"first {n_s} of {N} queries of {args.config}, fwd+bwd once ({sec:.2f} s)"}
+
+    value = N * world / (ms_step * 1e-3) / 1e6
+    ws_mb = (nbytes(table) + nbytes(dtable) + nbytes(out) + nbytes(dout) + nbytes(xyz) + nbytes(t)) / 1e6
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{args.config}: N={N} queries, L={enc.L} F={enc.F} T=2^{enc.T.bit_length() - 1} "
+                               f"table {enc.table_dtype}, spatial {enc.res_s_min}->{enc.res_s_max}, "
+                               f"temporal {enc.res_t_min}->{enc.res_t_max}; step = zero(dtable)+fwd+bwd",
+                   "queries_per_step_per_gpu": N, "parallelism": f"replicas x{world}",
+                   "l2": f"working set {ws_mb:.0f} MB > L2 (126 MB): no flush between iterations",
+                   "zero_grad_fused": bool(args.zero_grad_fused)},
+        "roofline": roofline,
+        "e2e": {"value": N * world / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", default="C4", choices=sorted(CONFIGS))
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--zero-grad-fused", type=int, default=0,
+                    help="1: bwd zeroes each level group itself (DASH_HASH4D_FLAG_ZERO_GRAD)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic-bytes", type=float, default=None,
+                    help="ncu dram bytes per launch of the dominant kernel (from profiles/), else null")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,154 @@
+/*
+ * dash_hash4d.h — C ABI of the B200-native multiresolution 4D hash encoder G_4D of DASH
+ * (arxiv 2507.19141, §4.2 "4D Hash Encoding", lines 123-138).
+ *
+ * The encoder maps a query x = (P, t) = (x, y, z, t) in [0,1)^4 to f_h = G_4D(x) in R^{L*F}
+ * (Eq. 9): for each of L levels with per-axis resolutions N_l in geometric progression
+ * (Eq. 7) it locates the enclosing 4D cell floor(x*N_l), maps each of
+ * the cell's 16 vertices to a table slot with the spatial-temporal hash h_l = (XOR_i x_i*pi_i) mod T
+ * (Eq. 8), and quadrilinearly interpolates the F-dimensional "learnable feature
+ * vectors" stored there.  The backward call is the transpose of that linear map: it
+ * scatter-adds upstream gradients into a table-shaped gradient buffer.  Every reading of a point the
+ * paper leaves open (Q1..Q21) is listed in DESIGN.md §3.
+ *
+ * General conventions
+ *   - All data pointers are DEVICE pointers unless marked "host".  Every buffer is caller-owned; the
+ *     library allocates nothing persistent, keeps no state between calls and never frees.
+ *   - Calls enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream) and
+ *     return without synchronising, except under DASH_HASH4D_FLAG_VALIDATE_INPUTS.
+ *   - `table`, `out`, `dout`, `dtable`, `workspace` must be 16-byte aligned; `xyz`, `t`, `index`,
+ *     `idx_out`, `w_out` 4-byte aligned.
+ *   - Return codes: see dash_hash4d_status.  No exceptions, no abort.  N == 0 is DASH_HASH4D_OK and
+ *     a no-op.  dash_hash4d_last_error() gives a thread-local message for the last non-OK return.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns
+ *     DASH_HASH4D_CUDA_ERROR.
+ */
+#ifndef DASH_HASH4D_H_
+#define DASH_HASH4D_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(_WIN32)
+#define DASH_API __declspec(dllexport)
+#else
+#define DASH_API __attribute__((visibility("default")))
+#endif
+
+enum dash_hash4d_status {
+    DASH_HASH4D_OK = 0,
+    DASH_HASH4D_INVALID_ARG = 1,         /* null pointer, bad L/F/T/resolutions/stride/alignment/struct_size,
+                                            or (VALIDATE_INPUTS) a NaN / out-of-[0,1) coordinate          */
+    DASH_HASH4D_UNSUPPORTED = 2,         /* e.g. F not in {1,2,4,8}, N too large for one launch          */
+    DASH_HASH4D_WORKSPACE_TOO_SMALL = 3, /* workspace_bytes < dash_hash4d_workspace_bytes(...)            */
+    DASH_HASH4D_CUDA_ERROR = 4           /* launch / runtime error; text via dash_hash4d_last_error()    */
+};
+
+enum dash_hash4d_dtype { DASH_HASH4D_FP32 = 0, DASH_HASH4D_FP16 = 1 };
+
+enum dash_hash4d_flags {
+    DASH_HASH4D_FLAG_DENSE_COARSE = 1u,     /* levels with (Ns+1)^3 (Nt+1) <= T use the injective dense index
+                                               x + S(y + S(z + S t)), S = Ns+1, instead of Eq. 8 (reading Q10).
+                                               Clear => Eq. 8 literally on every level.                      */
+    DASH_HASH4D_FLAG_DETERMINISTIC_BWD = 2u,/* bwd accumulates in 64-bit fixed point (order-independent):
+                                               bitwise identical results run to run; needs workspace.       */
+    DASH_HASH4D_FLAG_VALIDATE_INPUTS = 4u,  /* debug: scan coordinates for NaN / values outside [0,1) before
+                                               the op; synchronises the stream; needs workspace.            */
+    DASH_HASH4D_FLAG_ZERO_GRAD = 8u         /* bwd OVERWRITES: the library zeroes each level group of dtable
+                                               immediately before scattering into it (keeps it L2-resident)
+                                               instead of accumulating into the caller's contents.          */
+};
+
+enum dash_hash4d_op { DASH_HASH4D_OP_FWD = 0, DASH_HASH4D_OP_BWD = 1, DASH_HASH4D_OP_INDICES = 2 };
+
+/* Encoder hyper-parameters.  POD, passed by pointer (host memory). */
+typedef struct dash_hash4d_config {
+    uint32_t struct_size;          /* = sizeof(dash_hash4d_config): ABI versioning                          */
+    uint32_t L;                    /* number of levels, 1..32                                               */
+    uint32_t F;                    /* features per table entry: 1, 2, 4 or 8                                */
+    uint32_t T;                    /* entries per level (T_l of Eq. 8; uniform over levels), >= 1.
+                                      Power of two uses `& (T-1)`, anything else an unsigned remainder.     */
+    uint32_t res_s_min, res_s_max; /* N_min, N_max of Eq. 7 for the three spatial axes                      */
+    uint32_t res_t_min, res_t_max; /* N_min, N_max of Eq. 7 for the temporal axis; all resolutions <= 2^22 */
+    uint32_t primes[4];            /* pi_x, pi_y, pi_z, pi_t of Eq. 8; all zero => defaults
+                                      (1, 2654435761, 805459861, 3674653429), reading Q7                    */
+    uint32_t table_dtype;          /* dash_hash4d_dtype of `table`; out/dout/dtable are always fp32         */
+    uint32_t flags;                /* OR of dash_hash4d_flags                                               */
+} dash_hash4d_config;
+
+/* Eq. 7: the per-level resolutions N_l = floor(N_min * b^l), b = (N_max/N_min)^(1/(L-1)),
+ * for the spatial and the temporal range, and which levels use the dense index (reading Q10).
+ * res_s, res_t: host arrays of L uint32 (written).  is_dense: host array of L bytes, nullable.
+ * Returns INVALID_ARG on a bad config or null output pointer.  Needs no GPU. */
+DASH_API int dash_hash4d_resolutions(const dash_hash4d_config* cfg, uint32_t* res_s, uint32_t* res_t,
+                                     uint8_t* is_dense);
+
+/* Bytes of device workspace `op` needs for N queries under cfg->flags (0 for the default paths).
+ * Returns 0 on a bad config as well.  Needs no GPU. */
+DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op);
+
+/* Forward, Eq. 9:  out[n][l*F + f] = sum_{k<16} W_k * table[l][slot_k][f].
+ *   N          number of queries.
+ *   xyz        query n reads the three floats at xyz + row*xyz_stride, row = index ? index[n] : n;
+ *              xyz_stride (in floats) is 3 or 4.
+ *   t          query n reads t[n * t_stride]; t_stride is 0 (one timestamp for the whole call), 1 or 4.
+ *              A packed [N][4] array is the view xyz = base, xyz_stride = 4, t = base + 3, t_stride = 4.
+ *   index      nullable int32 [N] row list (the dynamic subset of PAPER.md:111); rows must be valid.
+ *   table      [L][T][F] row-major, element type cfg->table_dtype (read only).
+ *   out        [N][L*F] fp32, level-major columns (written, every element).
+ *   workspace  only read when dash_hash4d_workspace_bytes(cfg, N, OP_FWD) > 0.
+ * Coordinates are clamped to [0, 1-2^-24], NaN -> 0 (reading Q12).  fp16 tables are converted to fp32
+ * exactly; weights, products and sums are fp32 (reading Q13). */
+DASH_API int dash_hash4d_fwd(const dash_hash4d_config* cfg, uint64_t N,
+                             const float* xyz, uint32_t xyz_stride,
+                             const float* t, uint32_t t_stride,
+                             const int32_t* index,
+                             const void* table,
+                             float* out,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Backward (table gradient), the transpose of Eq. 9:
+ *     dtable[l][slot_k][f] += W_k * dout[n][l*F + f]      for every query n, level l, corner k.
+ *   dout       [N][L*F] fp32 upstream gradient (read only).
+ *   dtable     [L][T][F] fp32, ACCUMULATED into (+=) — the caller zeroes it (dash_hash4d_zero) unless
+ *              DASH_HASH4D_FLAG_ZERO_GRAD is set, in which case it is overwritten.
+ * Default path: fp32 vector reductions at L2 (`red.global.add.v2/.v4.f32`): summation order, hence the
+ * last bits, vary run to run; subnormal partial sums flush to zero.  DETERMINISTIC_BWD: 64-bit
+ * fixed-point accumulation in `workspace`, bitwise reproducible.  Other arguments as in fwd. */
+DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N,
+                             const float* xyz, uint32_t xyz_stride,
+                             const float* t, uint32_t t_stride,
+                             const int32_t* index,
+                             const float* dout,
+                             float* dtable,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Debug: the 16 table slots and interpolation weights of every (query, level)
+ * (Eq. 8).  Corner k: bit d of k set => vertex floor(x_d*N_l)+1 along axis d,
+ * d = 0:x 1:y 2:z 3:t (readings Q5, Q6).
+ *   idx_out    [N][L][16] uint32 (written).     w_out  [N][L][16] fp32, nullable. */
+DASH_API int dash_hash4d_indices(const dash_hash4d_config* cfg, uint64_t N,
+                                 const float* xyz, uint32_t xyz_stride,
+                                 const float* t, uint32_t t_stride,
+                                 const int32_t* index,
+                                 uint32_t* idx_out, float* w_out, void* cuda_stream);
+
+/* dtable <- 0 for the whole [L][T][F] fp32 gradient buffer (the accumulation's initial state), with the
+ * library's own fill kernel on `cuda_stream`. */
+DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream);
+
+/* Thread-local, never NULL; empty string when the last call on this thread succeeded. */
+DASH_API const char* dash_hash4d_last_error(void);
+
+/* Number of kernels the library launched on this thread since the last call with reset != 0
+ * (used by bench.py for "gpu_launches"). */
+DASH_API uint64_t dash_hash4d_launch_count(int reset);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DASH_HASH4D_H_ */

@@ -1,0 +1,262 @@
+"""ctypes binding of libdash_hash4d.so — same names as include/dash_hash4d.h.
+
+Marshalling only: torch tensors give device pointers and the current CUDA stream; nothing of the
+method is computed here.  PyTorch is used for device memory and streams, nothing else.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import torch
+
+from . import build as _build
+
+FLAG_DENSE_COARSE = 1
+FLAG_DETERMINISTIC_BWD = 2
+FLAG_VALIDATE_INPUTS = 4
+FLAG_ZERO_GRAD = 8
+OP_FWD, OP_BWD, OP_INDICES = 0, 1, 2
+
+_STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUDA_ERROR"}
+
+EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4d_fwd",
+           "dash_hash4d_bwd", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
+           "dash_hash4d_launch_count"]
+
+
+class Hash4DError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"dash_hash4d status {status} ({_STATUS.get(status, '?')}): {message}")
+        self.status = status
+
+
+class Hash4DConfig(C.Structure):
+    """Mirror of `struct dash_hash4d_config` (include/dash_hash4d.h)."""
+    _fields_ = [("struct_size", C.c_uint32), ("L", C.c_uint32), ("F", C.c_uint32), ("T", C.c_uint32),
+                ("res_s_min", C.c_uint32), ("res_s_max", C.c_uint32),
+                ("res_t_min", C.c_uint32), ("res_t_max", C.c_uint32),
+                ("primes", C.c_uint32 * 4), ("table_dtype", C.c_uint32), ("flags", C.c_uint32)]
+
+
+_lib: Optional[C.CDLL] = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def _load() -> C.CDLL:
+    """Load the in-tree library; build it if the sources are newer and nvcc is present.  Fails loudly:
+    there is no fallback implementation."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.is_stale():
+        try:
+            _build.build()
+        except Exception as exc:  # noqa: BLE001
+            if not os.path.exists(path):
+                raise ImportError(f"libdash_hash4d.so is not built and nvcc failed: {exc}") from exc
+    lib = C.CDLL(path)
+    vp, u32, u64, sz = C.c_void_p, C.c_uint32, C.c_uint64, C.c_size_t
+    cfgp = C.POINTER(Hash4DConfig)
+    lib.dash_hash4d_resolutions.argtypes = [cfgp, vp, vp, vp]
+    lib.dash_hash4d_resolutions.restype = C.c_int
+    lib.dash_hash4d_workspace_bytes.argtypes = [cfgp, u64, C.c_int]
+    lib.dash_hash4d_workspace_bytes.restype = sz
+    lib.dash_hash4d_fwd.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp, sz, vp]
+    lib.dash_hash4d_fwd.restype = C.c_int
+    lib.dash_hash4d_bwd.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp, sz, vp]
+    lib.dash_hash4d_bwd.restype = C.c_int
+    lib.dash_hash4d_indices.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp]
+    lib.dash_hash4d_indices.restype = C.c_int
+    lib.dash_hash4d_zero.argtypes = [cfgp, vp, vp]
+    lib.dash_hash4d_zero.restype = C.c_int
+    lib.dash_hash4d_last_error.argtypes = []
+    lib.dash_hash4d_last_error.restype = C.c_char_p
+    lib.dash_hash4d_launch_count.argtypes = [C.c_int]
+    lib.dash_hash4d_launch_count.restype = u64
+    _lib = lib
+    return lib
+
+
+def exported_symbols() -> list[str]:
+    """Names include/dash_hash4d.h declares that resolve in the loaded library."""
+    lib = _load()
+    return [n for n in EXPORTS if hasattr(lib, n)]
+
+
+def make_config(L, F, T, res_s_min, res_s_max, res_t_min, res_t_max, table_dtype="fp32",
+                primes=(0, 0, 0, 0), flags=FLAG_DENSE_COARSE) -> Hash4DConfig:
+    c = Hash4DConfig()
+    c.struct_size = C.sizeof(Hash4DConfig)
+    c.L, c.F, c.T = L, F, T
+    c.res_s_min, c.res_s_max, c.res_t_min, c.res_t_max = res_s_min, res_s_max, res_t_min, res_t_max
+    c.primes = (C.c_uint32 * 4)(*primes)
+    c.table_dtype = {"fp32": 0, "fp16": 1}[table_dtype]
+    c.flags = flags
+    return c
+
+
+def config_from_params(enc, **kw) -> Hash4DConfig:
+    """enc: dash_inputs.EncoderParams (plain numbers)."""
+    return make_config(enc.L, enc.F, enc.T, enc.res_s_min, enc.res_s_max, enc.res_t_min,
+                       enc.res_t_max, enc.table_dtype, **kw)
+
+
+def with_flags(cfg: Hash4DConfig, flags: int) -> Hash4DConfig:
+    c = Hash4DConfig.from_buffer_copy(bytes(cfg))
+    c.flags = flags
+    return c
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise Hash4DError(rc, dash_hash4d_last_error())
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t: Optional[torch.Tensor], dtype, what: str):
+    if t is None:
+        return
+    if not t.is_cuda:
+        raise ValueError(f"{what} must be a CUDA tensor (no CPU fallback exists)")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise ValueError(f"{what} must be contiguous {dtype}")
+
+
+def _strides(xyz: torch.Tensor, t: torch.Tensor, t_stride: Optional[int]):
+    if xyz.dim() != 2 or xyz.shape[1] not in (3, 4):
+        raise ValueError("xyz must be [rows][3] or [rows][4]")
+    if t_stride is None:
+        t_stride = 0 if t.numel() == 1 else 1
+    return int(xyz.shape[1]), int(t_stride)
+
+
+def dash_hash4d_last_error() -> str:
+    return _load().dash_hash4d_last_error().decode()
+
+
+def dash_hash4d_launch_count(reset: bool = False) -> int:
+    return int(_load().dash_hash4d_launch_count(1 if reset else 0))
+
+
+def dash_hash4d_resolutions(cfg: Hash4DConfig):
+    """-> (res_s, res_t, is_dense) as Python lists (host only; needs no GPU)."""
+    L = max(int(cfg.L), 1)
+    rs, rt, dn = (C.c_uint32 * L)(), (C.c_uint32 * L)(), (C.c_uint8 * L)()
+    _check(_load().dash_hash4d_resolutions(C.byref(cfg), rs, rt, dn))
+    return list(rs), list(rt), [bool(v) for v in dn]
+
+
+def dash_hash4d_workspace_bytes(cfg: Hash4DConfig, N: int, op: int) -> int:
+    return int(_load().dash_hash4d_workspace_bytes(C.byref(cfg), N, op))
+
+
+def _workspace(cfg, N, op, workspace):
+    need = dash_hash4d_workspace_bytes(cfg, N, op)
+    if need and workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+    return workspace, (0 if workspace is None else workspace.numel() * workspace.element_size())
+
+
+def dash_hash4d_fwd(cfg, xyz, t, table, out=None, index=None, t_stride=None, N=None, workspace=None):
+    """out[n][l*F+f] = sum_k W_k table[l][slot_k][f]; returns `out` ([N][L*F] fp32, CUDA)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(t, torch.float32, "t"); _dev(index, torch.int32, "index")
+    _dev(table, torch.float16 if cfg.table_dtype == 1 else torch.float32, "table")
+    xs, ts = _strides(xyz, t, t_stride)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    if out is None:
+        out = torch.empty((N, cfg.L * cfg.F), dtype=torch.float32, device=xyz.device)
+    _dev(out, torch.float32, "out")
+    workspace, wbytes = _workspace(cfg, N, OP_FWD, workspace)
+    _check(_load().dash_hash4d_fwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
+                                   _ptr(table), _ptr(out), _ptr(workspace), wbytes, _stream()))
+    return out
+
+
+def dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=None, t_stride=None, N=None, workspace=None):
+    """dtable[l][slot_k][f] += W_k dout[n][l*F+f]; returns `dtable` ([L][T][F] fp32, CUDA)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(t, torch.float32, "t"); _dev(index, torch.int32, "index")
+    _dev(dout, torch.float32, "dout"); _dev(dtable, torch.float32, "dtable")
+    xs, ts = _strides(xyz, t, t_stride)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    workspace, wbytes = _workspace(cfg, N, OP_BWD, workspace)
+    _check(_load().dash_hash4d_bwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
+                                   _ptr(dout), _ptr(dtable), _ptr(workspace), wbytes, _stream()))
+    return dtable
+
+
+def dash_hash4d_indices(cfg, xyz, t, index=None, t_stride=None, N=None, want_weights=True):
+    """-> (idx [N][L][16] int32-viewed uint32, w [N][L][16] fp32 or None)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(t, torch.float32, "t"); _dev(index, torch.int32, "index")
+    xs, ts = _strides(xyz, t, t_stride)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    idx = torch.empty((N, cfg.L, 16), dtype=torch.int32, device=xyz.device)   # bits are uint32
+    w = torch.empty((N, cfg.L, 16), dtype=torch.float32, device=xyz.device) if want_weights else None
+    _check(_load().dash_hash4d_indices(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
+                                       _ptr(idx), _ptr(w), _stream()))
+    return idx, w
+
+
+def dash_hash4d_zero(cfg, dtable):
+    _dev(dtable, torch.float32, "dtable")
+    _check(_load().dash_hash4d_zero(C.byref(cfg), _ptr(dtable), _stream()))
+    return dtable
+
+
+# ---- host-buffer entry points (bench.py "e2e"): copies in, C-ABI calls, copies out -----------------
+
+def dash_hash4d_fwd_host(cfg, xyz_h, t_h, table_d, out_h, index_h=None, t_stride=None, staging=None):
+    """Forward with HOST (pinned) query and output buffers; the table stays resident on the device
+    (it is the model's parameter).  Copies are async on the current stream; caller synchronises."""
+    st = staging if staging is not None else {}
+    xyz_d = _stage(st, "xyz", xyz_h); t_d = _stage(st, "t", t_h)
+    index_d = _stage(st, "index", index_h) if index_h is not None else None
+    out_d = st.get("out")
+    if out_d is None or out_d.shape != out_h.shape:
+        out_d = st["out"] = torch.empty(out_h.shape, dtype=torch.float32, device="cuda")
+    dash_hash4d_fwd(cfg, xyz_d, t_d, table_d, out=out_d, index=index_d, t_stride=t_stride)
+    out_h.copy_(out_d, non_blocking=True)
+    return out_h
+
+
+def dash_hash4d_bwd_host(cfg, xyz_h, t_h, dout_h, dtable_h, index_h=None, t_stride=None, staging=None,
+                         reuse_queries=False):
+    """Backward with HOST (pinned) buffers: dout in, dtable out (zeroed on the device first)."""
+    st = staging if staging is not None else {}
+    if reuse_queries and "xyz" in st:
+        xyz_d, t_d, index_d = st["xyz"], st["t"], st.get("index")
+    else:
+        xyz_d = _stage(st, "xyz", xyz_h); t_d = _stage(st, "t", t_h)
+        index_d = _stage(st, "index", index_h) if index_h is not None else None
+    dout_d = _stage(st, "dout", dout_h)
+    dt_d = st.get("dtable")
+    if dt_d is None or dt_d.shape != dtable_h.shape:
+        dt_d = st["dtable"] = torch.empty(dtable_h.shape, dtype=torch.float32, device="cuda")
+    if not (cfg.flags & FLAG_ZERO_GRAD):
+        dash_hash4d_zero(cfg, dt_d)
+    dash_hash4d_bwd(cfg, xyz_d, t_d, dout_d, dt_d, index=index_d, t_stride=t_stride)
+    dtable_h.copy_(dt_d, non_blocking=True)
+    return dtable_h
+
+
+def _stage(st: dict, key: str, host: torch.Tensor) -> torch.Tensor:
+    dev = st.get(key)
+    if dev is None or dev.shape != host.shape or dev.dtype != host.dtype:
+        dev = st[key] = torch.empty(host.shape, dtype=host.dtype, device="cuda")
+    dev.copy_(host, non_blocking=True)
+    return dev

@@ -1,0 +1,388 @@
+// hash4d_api.cu — C ABI (include/dash_hash4d.h) and host-side scheduler of the 4D hash encoder.
+//
+// Host work per call: validate, evaluate Eq. 7 once, decide dense vs hashed per
+// level (reading Q10), pick the level-group size G from the L2 capacity, launch.  No allocation,
+// no synchronisation (except VALIDATE_INPUTS), no state kept between calls.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#include "../../include/dash_hash4d.h"
+#include "hash4d_kernels.h"
+#include "hash4d_plan.h"
+
+namespace {
+
+using dash::Plan;
+using dash::WorkspaceHeader;
+
+thread_local char g_error[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_error, sizeof(g_error), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int ok() {
+    g_error[0] = '\0';
+    return DASH_HASH4D_OK;
+}
+
+const uint32_t kDefaultPrimes[4] = {1u, 2654435761u, 805459861u, 3674653429u};  // reading Q7
+constexpr uint32_t kMaxResolution = 1u << 22;
+constexpr size_t kHeaderBytes = sizeof(WorkspaceHeader);
+
+int check_config(const dash_hash4d_config* c) {
+    if (!c) return fail(DASH_HASH4D_INVALID_ARG, "config is NULL");
+    if (c->struct_size != sizeof(dash_hash4d_config))
+        return fail(DASH_HASH4D_INVALID_ARG, "struct_size %u != %zu", c->struct_size,
+                    sizeof(dash_hash4d_config));
+    if (c->L < 1 || c->L > dash::kMaxLevels)
+        return fail(DASH_HASH4D_INVALID_ARG, "L = %u outside 1..%d", c->L, dash::kMaxLevels);
+    if (c->F == 0 || c->F > 8) return fail(DASH_HASH4D_INVALID_ARG, "F = %u outside 1..8", c->F);
+    if (!(c->F == 1 || c->F == 2 || c->F == 4 || c->F == 8))
+        return fail(DASH_HASH4D_UNSUPPORTED, "F = %u not in {1,2,4,8}", c->F);
+    if (c->T < 1) return fail(DASH_HASH4D_INVALID_ARG, "T = 0");
+    if (c->res_s_min < 1 || c->res_s_min > c->res_s_max || c->res_s_max > kMaxResolution)
+        return fail(DASH_HASH4D_INVALID_ARG, "spatial resolution range [%u, %u] invalid",
+                    c->res_s_min, c->res_s_max);
+    if (c->res_t_min < 1 || c->res_t_min > c->res_t_max || c->res_t_max > kMaxResolution)
+        return fail(DASH_HASH4D_INVALID_ARG, "temporal resolution range [%u, %u] invalid",
+                    c->res_t_min, c->res_t_max);
+    if (c->table_dtype != DASH_HASH4D_FP32 && c->table_dtype != DASH_HASH4D_FP16)
+        return fail(DASH_HASH4D_INVALID_ARG, "table_dtype = %u", c->table_dtype);
+    if (c->flags & ~15u) return fail(DASH_HASH4D_INVALID_ARG, "unknown flag bits 0x%x", c->flags);
+    return DASH_HASH4D_OK;
+}
+
+// Eq. 7 with the exponent restored (reading Q1): N_l = floor(N_min * (N_max/N_min)^(l/(L-1))).
+// Reading Q2: IEEE double, +1e-6 before the floor so mathematically-integer levels are not lost.
+uint32_t geometric_level(uint32_t lo, uint32_t hi, uint32_t l, uint32_t L) {
+    if (L == 1) return lo;
+    const double ratio = static_cast<double>(hi) / static_cast<double>(lo);
+    const double expo = static_cast<double>(l) / static_cast<double>(L - 1);
+    return static_cast<uint32_t>(std::floor(static_cast<double>(lo) * std::pow(ratio, expo) + 1e-6));
+}
+
+bool fits_dense(uint32_t ns, uint32_t nt, uint32_t T) {  // (Ns+1)^3 (Nt+1) <= T, in 128-bit-safe steps
+    const unsigned long long S = static_cast<unsigned long long>(ns) + 1ull;
+    unsigned long long v = S * S;               // <= 2^46
+    if (v > T) return false;
+    v *= S;                                      // v <= T * S < 2^55
+    if (v > T) return false;
+    v *= static_cast<unsigned long long>(nt) + 1ull;
+    return v <= T;
+}
+
+struct Schedule {
+    uint32_t res_s[dash::kMaxLevels], res_t[dash::kMaxLevels];
+    uint8_t dense[dash::kMaxLevels];
+};
+
+void make_schedule(const dash_hash4d_config* c, Schedule* s) {
+    for (uint32_t l = 0; l < c->L; ++l) {
+        s->res_s[l] = geometric_level(c->res_s_min, c->res_s_max, l, c->L);
+        s->res_t[l] = geometric_level(c->res_t_min, c->res_t_max, l, c->L);
+        s->dense[l] = (c->flags & DASH_HASH4D_FLAG_DENSE_COARSE) &&
+                      fits_dense(s->res_s[l], s->res_t[l], c->T);
+    }
+}
+
+size_t l2_bytes() {
+    static size_t cached = 0;
+    if (!cached) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&v, cudaDevAttrL2CacheSize, dev) == cudaSuccess && v > 0)
+            cached = static_cast<size_t>(v);
+        else
+            cached = 64u << 20;
+    }
+    return cached;
+}
+
+uint32_t env_u32(const char* name) {
+    const char* v = std::getenv(name);
+    return v ? static_cast<uint32_t>(std::strtoul(v, nullptr, 10)) : 0u;
+}
+
+// Level-group size G (power of two <= 16): as many levels as keep the group's randomly accessed
+// bytes (tables in fwd, fp32 gradient slices in bwd) within a fraction of L2, but at least enough
+// that one lane-quad writes a full 32-byte sector of `out` (G*F*4 >= 32), and without wasting more
+// than a quarter of the lanes when L is not a multiple of G.  DASH_HASH4D_{FWD,BWD}_GROUP override.
+uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, const char* env_name) {
+    uint32_t forced = env_u32(env_name);
+    if (forced) {
+        uint32_t g = 1;
+        while (g * 2 <= forced && g * 2 <= dash::kMaxGroup) g *= 2;
+        return g;
+    }
+    const size_t budget = l2_bytes() * 6 / 10;
+    uint32_t g_min = 1;
+    while (g_min * c->F * 4 < 32 && g_min < dash::kMaxGroup) g_min *= 2;
+    uint32_t best = 0;
+    for (uint32_t g = dash::kMaxGroup; g >= 1; g /= 2) {
+        const uint32_t groups = (c->L + g - 1) / g;
+        const bool efficient = 4 * c->L >= 3 * groups * g;
+        const bool resident = g * bytes_per_level <= budget;
+        if (efficient && (resident || g <= g_min)) {
+            best = g;
+            break;
+        }
+    }
+    return best ? best : 1;
+}
+
+int fill_plan(const dash_hash4d_config* c, uint64_t N, uint32_t xyz_stride, uint32_t t_stride,
+              uint32_t group, Plan* P) {
+    Schedule s;
+    make_schedule(c, &s);
+    std::memset(P, 0, sizeof(*P));
+    P->N = N;
+    P->L = c->L;
+    P->F = c->F;
+    P->T = c->T;
+    P->t_pow2 = (c->T & (c->T - 1)) == 0;
+    P->t_mask = c->T - 1;
+    P->xyz_stride = xyz_stride;
+    P->t_stride = t_stride;
+    P->group = group;
+    uint32_t lg = 0;
+    while ((1u << lg) < group) ++lg;
+    P->group_log2 = lg;
+    P->level_begin = 0;
+    P->num_groups = (c->L + group - 1) / group;
+    P->q_per_block = dash::kItemsPerBlock >> lg;
+    const bool defaults = !(c->primes[0] | c->primes[1] | c->primes[2] | c->primes[3]);
+    for (uint32_t l = 0; l < c->L; ++l) {
+        dash::LevelParams& lp = P->lv[l];
+        lp.ns_f = static_cast<float>(s.res_s[l]);
+        lp.nt_f = static_cast<float>(s.res_t[l]);
+        lp.dense = s.dense[l];
+        if (s.dense[l]) {
+            const uint32_t S = s.res_s[l] + 1;
+            lp.m[0] = 1;
+            lp.m[1] = S;
+            lp.m[2] = S * S;
+            lp.m[3] = S * S * S;
+        } else {
+            for (int d = 0; d < 4; ++d) lp.m[d] = defaults ? kDefaultPrimes[d] : c->primes[d];
+        }
+    }
+    if (N) {
+        const uint64_t tiles = (N + P->q_per_block - 1) / P->q_per_block;
+        if (tiles > 0x7fffffffull)
+            return fail(DASH_HASH4D_UNSUPPORTED, "N = %llu too large for one launch",
+                        static_cast<unsigned long long>(N));
+    }
+    return DASH_HASH4D_OK;
+}
+
+int check_queries(const float* xyz, uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                  const int32_t* index) {
+    if (!xyz || !t) return fail(DASH_HASH4D_INVALID_ARG, "xyz or t is NULL");
+    if (!(xyz_stride == 3 || xyz_stride == 4))
+        return fail(DASH_HASH4D_INVALID_ARG, "xyz_stride = %u (want 3 or 4)", xyz_stride);
+    if (!(t_stride == 0 || t_stride == 1 || t_stride == 4))
+        return fail(DASH_HASH4D_INVALID_ARG, "t_stride = %u (want 0, 1 or 4)", t_stride);
+    if ((reinterpret_cast<uintptr_t>(xyz) | reinterpret_cast<uintptr_t>(t) |
+         reinterpret_cast<uintptr_t>(index)) & 3u)
+        return fail(DASH_HASH4D_INVALID_ARG, "xyz / t / index not 4-byte aligned");
+    return DASH_HASH4D_OK;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int cuda_fail(cudaError_t e, const char* what) {
+    return fail(DASH_HASH4D_CUDA_ERROR, "%s: %s", what, cudaGetErrorString(e));
+}
+
+size_t table_elems(const dash_hash4d_config* c) {
+    return static_cast<size_t>(c->L) * c->T * c->F;
+}
+
+int run_validation(const dash_hash4d_config* c, const Plan& P, const float* xyz, const float* t,
+                   const int32_t* index, void* workspace, size_t workspace_bytes, cudaStream_t s) {
+    if (!(c->flags & DASH_HASH4D_FLAG_VALIDATE_INPUTS)) return DASH_HASH4D_OK;
+    if (!workspace || workspace_bytes < kHeaderBytes)
+        return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "VALIDATE_INPUTS needs %zu workspace bytes",
+                    kHeaderBytes);
+    WorkspaceHeader* hdr = static_cast<WorkspaceHeader*>(workspace);
+    cudaError_t e = dash::launch_zero(hdr, kHeaderBytes, s);
+    if (e == cudaSuccess) e = dash::launch_validate(P, xyz, t, index, hdr, s);
+    if (e != cudaSuccess) return cuda_fail(e, "validate launch");
+    uint32_t bad = 0;
+    e = cudaMemcpyAsync(&bad, &hdr->bad_inputs, sizeof(bad), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(e, "validate readback");
+    if (bad)
+        return fail(DASH_HASH4D_INVALID_ARG, "%u coordinates are NaN or outside [0,1)", bad);
+    return DASH_HASH4D_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+DASH_API const char* dash_hash4d_last_error(void) { return g_error; }
+
+DASH_API uint64_t dash_hash4d_launch_count(int reset) { return dash::launch_counter(reset != 0); }
+
+DASH_API int dash_hash4d_resolutions(const dash_hash4d_config* cfg, uint32_t* res_s,
+                                     uint32_t* res_t, uint8_t* is_dense) {
+    if (int rc = check_config(cfg)) return rc;
+    if (!res_s || !res_t) return fail(DASH_HASH4D_INVALID_ARG, "res_s or res_t is NULL");
+    Schedule s;
+    make_schedule(cfg, &s);
+    for (uint32_t l = 0; l < cfg->L; ++l) {
+        res_s[l] = s.res_s[l];
+        res_t[l] = s.res_t[l];
+        if (is_dense) is_dense[l] = s.dense[l];
+    }
+    return ok();
+}
+
+DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op) {
+    (void)N;
+    if (check_config(cfg)) return 0;
+    size_t bytes = 0;
+    if ((cfg->flags & DASH_HASH4D_FLAG_VALIDATE_INPUTS) && op != DASH_HASH4D_OP_INDICES)
+        bytes = kHeaderBytes;
+    if (op == DASH_HASH4D_OP_BWD && (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD))
+        bytes = kHeaderBytes + table_elems(cfg) * sizeof(long long);
+    g_error[0] = '\0';
+    return bytes;
+}
+
+DASH_API int dash_hash4d_fwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                             uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                             const int32_t* index, const void* table, float* out, void* workspace,
+                             size_t workspace_bytes, void* cuda_stream) {
+    if (int rc = check_config(cfg)) return rc;
+    if (N == 0) return ok();
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
+    if (!table || !out) return fail(DASH_HASH4D_INVALID_ARG, "table or out is NULL");
+    if (!aligned16(table) || !aligned16(out))
+        return fail(DASH_HASH4D_INVALID_ARG, "table / out not 16-byte aligned");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const bool half = cfg->table_dtype == DASH_HASH4D_FP16;
+    const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * (half ? 2 : 4);
+    Plan P;
+    if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
+                           pick_group(cfg, level_bytes, "DASH_HASH4D_FWD_GROUP"), &P))
+        return rc;
+    if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
+    cudaError_t e = dash::launch_fwd(P, xyz, t, index, table, half, out, s);
+    if (e != cudaSuccess) return cuda_fail(e, "fwd launch");
+    return ok();
+}
+
+DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                             uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                             const int32_t* index, const float* dout, float* dtable,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (int rc = check_config(cfg)) return rc;
+    if (!dtable && (N || (cfg->flags & DASH_HASH4D_FLAG_ZERO_GRAD)))
+        return fail(DASH_HASH4D_INVALID_ARG, "dtable is NULL");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const bool zero_first = (cfg->flags & DASH_HASH4D_FLAG_ZERO_GRAD) != 0;
+    const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * sizeof(float);
+    if (N == 0) {
+        if (zero_first) {
+            if (!aligned16(dtable))
+                return fail(DASH_HASH4D_INVALID_ARG, "dtable not 16-byte aligned");
+            cudaError_t e = dash::launch_zero(dtable, level_bytes * cfg->L, s);
+            if (e != cudaSuccess) return cuda_fail(e, "zero launch");
+        }
+        return ok();
+    }
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
+    if (!dout) return fail(DASH_HASH4D_INVALID_ARG, "dout is NULL");
+    if (!aligned16(dout) || !aligned16(dtable))
+        return fail(DASH_HASH4D_INVALID_ARG, "dout / dtable not 16-byte aligned");
+    const bool fixed = (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD) != 0;
+    const size_t need = dash_hash4d_workspace_bytes(cfg, N, DASH_HASH4D_OP_BWD);
+    if (need && (!workspace || workspace_bytes < need))
+        return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "bwd needs %zu workspace bytes, got %zu", need,
+                    workspace_bytes);
+    if (need && !aligned16(workspace))
+        return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
+    Plan P;
+    const size_t scatter_bytes = fixed ? 2 * level_bytes : level_bytes;
+    if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
+                           pick_group(cfg, scatter_bytes, "DASH_HASH4D_BWD_GROUP"), &P))
+        return rc;
+    if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
+
+    cudaError_t e = cudaSuccess;
+    if (fixed) {
+        WorkspaceHeader* hdr = static_cast<WorkspaceHeader*>(workspace);
+        long long* acc = reinterpret_cast<long long*>(static_cast<char*>(workspace) + kHeaderBytes);
+        const size_t elems = table_elems(cfg);
+        e = dash::launch_zero(workspace, kHeaderBytes + elems * sizeof(long long), s);
+        if (e == cudaSuccess)
+            e = dash::launch_absmax(dout, static_cast<size_t>(N) * cfg->L * cfg->F, hdr, N, s);
+        if (e == cudaSuccess) e = dash::launch_bwd_fixed(P, xyz, t, index, dout, acc, hdr, s);
+        if (e == cudaSuccess) e = dash::launch_fixed_finalize(acc, dtable, elems, hdr, zero_first, s);
+        if (e != cudaSuccess) return cuda_fail(e, "deterministic bwd launch");
+        return ok();
+    }
+    if (!zero_first) {
+        e = dash::launch_bwd(P, xyz, t, index, dout, dtable, s);
+        if (e != cudaSuccess) return cuda_fail(e, "bwd launch");
+        return ok();
+    }
+    // ZERO_GRAD: zero one level group, scatter into it while the zeros are still in L2, next group.
+    const uint32_t groups = P.num_groups;
+    for (uint32_t g = 0; g < groups; ++g) {
+        const uint32_t l0 = g * P.group;
+        const uint32_t l1 = (l0 + P.group < cfg->L) ? l0 + P.group : cfg->L;
+        char* base = reinterpret_cast<char*>(dtable) + static_cast<size_t>(l0) * level_bytes;
+        const size_t bytes = static_cast<size_t>(l1 - l0) * level_bytes;
+        e = dash::launch_zero(base, bytes, s);  // handles slices that are only 4-byte aligned
+        if (e != cudaSuccess) return cuda_fail(e, "zero launch");
+        Plan Pg = P;
+        Pg.level_begin = l0;
+        Pg.num_groups = 1;
+        e = dash::launch_bwd(Pg, xyz, t, index, dout, dtable, s);
+        if (e != cudaSuccess) return cuda_fail(e, "bwd launch");
+    }
+    return ok();
+}
+
+DASH_API int dash_hash4d_indices(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                                 uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                                 const int32_t* index, uint32_t* idx_out, float* w_out,
+                                 void* cuda_stream) {
+    if (int rc = check_config(cfg)) return rc;
+    if (N == 0) return ok();
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
+    if (!idx_out) return fail(DASH_HASH4D_INVALID_ARG, "idx_out is NULL");
+    if (N * cfg->L > 0x7fffffffull * dash::kBlockThreads)
+        return fail(DASH_HASH4D_UNSUPPORTED, "N*L too large for one launch");
+    Plan P;
+    if (int rc = fill_plan(cfg, N, xyz_stride, t_stride, 1, &P)) return rc;
+    cudaError_t e = dash::launch_indices(P, xyz, t, index, idx_out, w_out,
+                                         static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "indices launch");
+    return ok();
+}
+
+DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream) {
+    if (int rc = check_config(cfg)) return rc;
+    if (!dtable) return fail(DASH_HASH4D_INVALID_ARG, "dtable is NULL");
+    if (!aligned16(dtable)) return fail(DASH_HASH4D_INVALID_ARG, "dtable not 16-byte aligned");
+    cudaError_t e = dash::launch_zero(dtable, table_elems(cfg) * sizeof(float),
+                                      static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "zero launch");
+    return ok();
+}
+
+}  // extern "C"

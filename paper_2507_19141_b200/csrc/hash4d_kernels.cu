@@ -1,0 +1,549 @@
+// hash4d_kernels.cu — hand-written sm_100a kernels of the DASH 4D hash encoder.
+//
+// Work decomposition: one LANE PAIR per (query n, level l) item.  The two lanes of
+// a pair take the two x-corners of the 4D cell (pi_x = 1 keeps them in adjacent table slots, so a
+// pair's two 8/16-byte accesses fall in one 32-byte sector 50-75 % of the time and almost always
+// in one 128-byte line: half the L1 wavefronts of a lane-per-item mapping), each lane walks the 8
+// (y,z,t) corners, and one shuffle folds the two halves.  A warp holds 16 items = (16/G) queries x
+// G consecutive levels, so the warp's store of `out` (and load of `dout`) covers G*F*4 contiguous
+// bytes per query.  Blocks are ordered level-group-major (blockIdx.y = group) so that the tables
+// (fwd) / gradient slices (bwd) of one group stay L2-resident while all queries stream past.
+//
+// This is a gather/scatter path: no tensor cores (no dense contraction), no TMA (8-byte random
+// accesses cannot be expressed as tiles).
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+
+#include "hash4d_kernels.h"
+
+namespace dash {
+
+namespace {
+
+thread_local uint64_t g_launches = 0;
+
+// ------------------------------------------------------------------------------------------------
+// Cell location and vertex -> slot (Eq. 8 / dense index)
+// ------------------------------------------------------------------------------------------------
+
+// Reading Q12: clamp to [0, 1-2^-24]; fmaxf(NaN, 0) = 0.
+__device__ __forceinline__ float clamp_unit(float v) { return fminf(fmaxf(v, 0.0f), 0x1.fffffep-1f); }
+
+// floor(x * N_l) with ONE binary32 multiply (reading Q4): __fmul_rn is never contracted into an FMA.
+__device__ __forceinline__ void locate(float x, float res, uint32_t& cell, float& frac) {
+    const float pos = __fmul_rn(clamp_unit(x), res);
+    const float fl = floorf(pos);
+    cell = static_cast<uint32_t>(fl);
+    frac = pos - fl;  // exact
+}
+
+struct Query {
+    uint32_t c[4];  // cell (floor) per axis x,y,z,t
+    float w[4];     // fractional offset per axis
+};
+
+__device__ __forceinline__ Query load_query(const Plan& P, const LevelParams& lp, uint64_t n,
+                                            const float* __restrict__ xyz,
+                                            const float* __restrict__ t,
+                                            const int32_t* __restrict__ index) {
+    const uint64_t row = index ? static_cast<uint64_t>(__ldg(index + n)) : n;
+    const float* p = xyz + row * P.xyz_stride;
+    Query q;
+    locate(__ldg(p + 0), lp.ns_f, q.c[0], q.w[0]);
+    locate(__ldg(p + 1), lp.ns_f, q.c[1], q.w[1]);
+    locate(__ldg(p + 2), lp.ns_f, q.c[2], q.w[2]);
+    locate(__ldg(t + n * P.t_stride), lp.nt_f, q.c[3], q.w[3]);
+    return q;
+}
+
+// The 8 (y,z,t) corners that share x-corner `xc` (0: floor, 1: floor+1).  Corner j: bit0 = y, bit1 =
+// z, bit2 = t, i.e. full corner number k = xc | (j << 1) (reading Q6).  Hashed level: slot = (XOR of
+// g_d*pi_d) mod T (Eq. 8, uint32 wraparound, Q8/Q9); dense level: slot = sum of g_d*stride_d (Q10).
+__device__ __forceinline__ void half_cell(const Plan& P, const LevelParams& lp, const Query& q,
+                                          uint32_t xc, uint32_t slot[8], float W[8]) {
+    const uint32_t ax = (q.c[0] + xc) * lp.m[0];
+    const uint32_t ay0 = q.c[1] * lp.m[1], ay1 = ay0 + lp.m[1];
+    const uint32_t az0 = q.c[2] * lp.m[2], az1 = az0 + lp.m[2];
+    const uint32_t at0 = q.c[3] * lp.m[3], at1 = at0 + lp.m[3];
+    if (lp.dense) {
+        const uint32_t p0 = ax + ay0, p1 = ax + ay1;
+        const uint32_t q0 = az0 + at0, q1 = az1 + at0, q2 = az0 + at1, q3 = az1 + at1;
+        slot[0] = p0 + q0; slot[1] = p1 + q0; slot[2] = p0 + q1; slot[3] = p1 + q1;
+        slot[4] = p0 + q2; slot[5] = p1 + q2; slot[6] = p0 + q3; slot[7] = p1 + q3;
+    } else {
+        const uint32_t p0 = ax ^ ay0, p1 = ax ^ ay1;
+        const uint32_t q0 = az0 ^ at0, q1 = az1 ^ at0, q2 = az0 ^ at1, q3 = az1 ^ at1;
+        slot[0] = p0 ^ q0; slot[1] = p1 ^ q0; slot[2] = p0 ^ q1; slot[3] = p1 ^ q1;
+        slot[4] = p0 ^ q2; slot[5] = p1 ^ q2; slot[6] = p0 ^ q3; slot[7] = p1 ^ q3;
+        if (P.t_pow2) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) slot[j] &= P.t_mask;
+        } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) slot[j] %= P.T;
+        }
+    }
+    // quadrilinear weights: W = prod_d (corner bit ? w_d : 1 - w_d), fp32
+    const float wx = xc ? q.w[0] : 1.0f - q.w[0];
+    const float py0 = wx * (1.0f - q.w[1]), py1 = wx * q.w[1];
+    const float z0 = 1.0f - q.w[2], z1 = q.w[2], t0 = 1.0f - q.w[3], t1 = q.w[3];
+    const float r0 = z0 * t0, r1 = z1 * t0, r2 = z0 * t1, r3 = z1 * t1;
+    W[0] = py0 * r0; W[1] = py1 * r0; W[2] = py0 * r1; W[3] = py1 * r1;
+    W[4] = py0 * r2; W[5] = py1 * r2; W[6] = py0 * r3; W[7] = py1 * r3;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Table slot access
+// ------------------------------------------------------------------------------------------------
+
+template <int F, bool HALF>
+__device__ __forceinline__ void load_slot(const void* __restrict__ level_base, uint32_t slot,
+                                          float v[F]) {
+    if constexpr (!HALF) {
+        const float* p = static_cast<const float*>(level_base) + static_cast<size_t>(slot) * F;
+        if constexpr (F == 1) {
+            v[0] = __ldg(p);
+        } else if constexpr (F == 2) {
+            const float2 a = __ldg(reinterpret_cast<const float2*>(p));
+            v[0] = a.x; v[1] = a.y;
+        } else if constexpr (F == 4) {
+            const float4 a = __ldg(reinterpret_cast<const float4*>(p));
+            v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
+        } else {
+            const float4 a = __ldg(reinterpret_cast<const float4*>(p));
+            const float4 b = __ldg(reinterpret_cast<const float4*>(p) + 1);
+            v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
+            v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+        }
+    } else {  // IEEE half table, converted exactly to fp32 (reading Q13)
+        const __half* p = static_cast<const __half*>(level_base) + static_cast<size_t>(slot) * F;
+        if constexpr (F == 1) {
+            const unsigned short raw = __ldg(reinterpret_cast<const unsigned short*>(p));
+            v[0] = __half2float(__ushort_as_half(raw));
+        } else if constexpr (F == 2) {
+            const uint32_t raw = __ldg(reinterpret_cast<const uint32_t*>(p));
+            const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&raw));
+            v[0] = a.x; v[1] = a.y;
+        } else if constexpr (F == 4) {
+            const uint2 raw = __ldg(reinterpret_cast<const uint2*>(p));
+            const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&raw.x));
+            const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&raw.y));
+            v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+        } else {
+            const uint4 raw = __ldg(reinterpret_cast<const uint4*>(p));
+            const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&raw.x));
+            const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&raw.y));
+            const float2 c = __half22float2(*reinterpret_cast<const __half2*>(&raw.z));
+            const float2 d = __half22float2(*reinterpret_cast<const __half2*>(&raw.w));
+            v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+            v[4] = c.x; v[5] = c.y; v[6] = d.x; v[7] = d.y;
+        }
+    }
+}
+
+// fp32 vector reduction at L2, no return value (REDG.E.ADD.F32x2 / .F32x4 on sm_100a).
+template <int F>
+__device__ __forceinline__ void red_add(float* p, const float v[F]) {
+    if constexpr (F == 1) {
+        asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(v[0]) : "memory");
+    } else if constexpr (F == 2) {
+        asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(v[0]), "f"(v[1])
+                     : "memory");
+    } else if constexpr (F == 4) {
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v[0]),
+                     "f"(v[1]), "f"(v[2]), "f"(v[3])
+                     : "memory");
+    } else {
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v[0]),
+                     "f"(v[1]), "f"(v[2]), "f"(v[3])
+                     : "memory");
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p + 4), "f"(v[4]),
+                     "f"(v[5]), "f"(v[6]), "f"(v[7])
+                     : "memory");
+    }
+}
+
+// Item coordinates of this lane pair.  Inactive pairs (tail tile, L not a multiple of G) are clamped
+// onto a valid item so that every lane reaches the shuffles; they skip their stores / reductions.
+struct Item {
+    uint64_t n;
+    uint32_t l;
+    uint32_t xc;
+    bool active;
+};
+
+__device__ __forceinline__ Item this_item(const Plan& P) {
+    const uint32_t pair = threadIdx.x >> 1;
+    Item it;
+    it.xc = threadIdx.x & 1u;
+    it.n = static_cast<uint64_t>(blockIdx.x) * P.q_per_block + (pair >> P.group_log2);
+    it.l = P.level_begin + blockIdx.y * P.group + (pair & (P.group - 1u));
+    it.active = (it.n < P.N) && (it.l < P.L);
+    if (it.n >= P.N) it.n = P.N - 1;
+    if (it.l >= P.L) it.l = P.L - 1;
+    return it;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Forward: gather + quadrilinear interpolation (Eq. 9)
+// ------------------------------------------------------------------------------------------------
+template <int F, bool HALF>
+__global__ void __launch_bounds__(kBlockThreads)
+hash4d_fwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
+                  const float* __restrict__ t, const int32_t* __restrict__ index,
+                  const void* __restrict__ table, float* __restrict__ out) {
+    const Item it = this_item(P);
+    const LevelParams lp = P.lv[it.l];
+    const Query q = load_query(P, lp, it.n, xyz, t, index);
+    uint32_t slot[8];
+    float W[8];
+    half_cell(P, lp, q, it.xc, slot, W);
+
+    constexpr size_t kElem = HALF ? 2 : 4;
+    const char* level_base =
+        static_cast<const char*>(table) + static_cast<size_t>(it.l) * P.T * (F * kElem);
+    float v[8][F];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);  // 8 loads in flight
+    float acc[F];
+#pragma unroll
+    for (int f = 0; f < F; ++f) acc[f] = 0.0f;
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+#pragma unroll
+        for (int f = 0; f < F; ++f) acc[f] = fmaf(W[j], v[j][f], acc[f]);
+#pragma unroll
+    for (int f = 0; f < F; ++f) acc[f] += __shfl_xor_sync(0xffffffffu, acc[f], 1);  // fold x-corners
+
+    if (!it.active) return;
+    float* o = out + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F;
+    if constexpr (F == 1) {
+        if (it.xc == 0) __stcs(o, acc[0]);
+    } else if constexpr (F == 2) {
+        __stcs(o + it.xc, it.xc ? acc[1] : acc[0]);
+    } else if constexpr (F == 4) {
+        const float2 s = it.xc ? make_float2(acc[2], acc[3]) : make_float2(acc[0], acc[1]);
+        __stcs(reinterpret_cast<float2*>(o) + it.xc, s);
+    } else {
+        const float4 s = it.xc ? make_float4(acc[4], acc[5], acc[6], acc[7])
+                               : make_float4(acc[0], acc[1], acc[2], acc[3]);
+        __stcs(reinterpret_cast<float4*>(o) + it.xc, s);
+    }
+}
+
+// Each lane of a pair loads half of the item's F upstream gradients; one shuffle gives both all F.
+template <int F>
+__device__ __forceinline__ void load_dout(const float* __restrict__ d, uint32_t xc, float g[F]) {
+    if constexpr (F == 1) {
+        g[0] = __ldcs(d);
+    } else if constexpr (F == 2) {
+        const float mine = __ldcs(d + xc);
+        const float other = __shfl_xor_sync(0xffffffffu, mine, 1);
+        g[0] = xc ? other : mine;
+        g[1] = xc ? mine : other;
+    } else if constexpr (F == 4) {
+        const float2 mine = __ldcs(reinterpret_cast<const float2*>(d) + xc);
+        float2 other;
+        other.x = __shfl_xor_sync(0xffffffffu, mine.x, 1);
+        other.y = __shfl_xor_sync(0xffffffffu, mine.y, 1);
+        const float2 lo = xc ? other : mine, hi = xc ? mine : other;
+        g[0] = lo.x; g[1] = lo.y; g[2] = hi.x; g[3] = hi.y;
+    } else {
+        const float4 mine = __ldcs(reinterpret_cast<const float4*>(d) + xc);
+        float4 other;
+        other.x = __shfl_xor_sync(0xffffffffu, mine.x, 1);
+        other.y = __shfl_xor_sync(0xffffffffu, mine.y, 1);
+        other.z = __shfl_xor_sync(0xffffffffu, mine.z, 1);
+        other.w = __shfl_xor_sync(0xffffffffu, mine.w, 1);
+        const float4 lo = xc ? other : mine, hi = xc ? mine : other;
+        g[0] = lo.x; g[1] = lo.y; g[2] = lo.z; g[3] = lo.w;
+        g[4] = hi.x; g[5] = hi.y; g[6] = hi.z; g[7] = hi.w;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Backward: scatter-add of W_k * dY into the table gradient (transpose of Eq. 9)
+// ------------------------------------------------------------------------------------------------
+template <int F>
+__global__ void __launch_bounds__(kBlockThreads)
+hash4d_bwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
+                  const float* __restrict__ t, const int32_t* __restrict__ index,
+                  const float* __restrict__ dout, float* __restrict__ dtable) {
+    const Item it = this_item(P);
+    const LevelParams lp = P.lv[it.l];
+    float g[F];
+    load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F,
+                 it.xc, g);
+    const Query q = load_query(P, lp, it.n, xyz, t, index);
+    uint32_t slot[8];
+    float W[8];
+    half_cell(P, lp, q, it.xc, slot, W);  // recomputed, never cached from fwd (128 B per item)
+    if (!it.active) return;
+    float* level_base = dtable + static_cast<size_t>(it.l) * P.T * F;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        float c[F];
+#pragma unroll
+        for (int f = 0; f < F; ++f) c[f] = W[j] * g[f];
+        red_add<F>(level_base + static_cast<size_t>(slot[j]) * F, c);
+    }
+}
+
+// Deterministic variant: 64-bit fixed-point accumulation.  Integer addition is associative, so the
+// sums do not depend on the order in which the L2 applies the reductions.
+template <int F>
+__global__ void __launch_bounds__(kBlockThreads)
+hash4d_bwd_fixed_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
+                        const float* __restrict__ t, const int32_t* __restrict__ index,
+                        const float* __restrict__ dout, long long* __restrict__ acc,
+                        const WorkspaceHeader* __restrict__ hdr) {
+    const Item it = this_item(P);
+    const LevelParams lp = P.lv[it.l];
+    float g[F];
+    load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F,
+                 it.xc, g);
+    const Query q = load_query(P, lp, it.n, xyz, t, index);
+    uint32_t slot[8];
+    float W[8];
+    half_cell(P, lp, q, it.xc, slot, W);
+    if (!it.active) return;
+    const float scale = hdr->scale;  // power of two: the products below are exact rescalings
+    unsigned long long* level_base =
+        reinterpret_cast<unsigned long long*>(acc) + static_cast<size_t>(it.l) * P.T * F;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+#pragma unroll
+        for (int f = 0; f < F; ++f) {
+            const long long fx = __float2ll_rn(__fmul_rn(__fmul_rn(W[j], g[f]), scale));
+            atomicAdd(level_base + static_cast<size_t>(slot[j]) * F + f,
+                      static_cast<unsigned long long>(fx));
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Debug: all 16 slots + weights per (query, level)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlockThreads)
+hash4d_indices_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
+                      const float* __restrict__ t, const int32_t* __restrict__ index,
+                      uint32_t* __restrict__ idx_out, float* __restrict__ w_out) {
+    const uint64_t i = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x;
+    if (i >= P.N * P.L) return;
+    const uint64_t n = i / P.L;
+    const uint32_t l = static_cast<uint32_t>(i - n * P.L);
+    const LevelParams lp = P.lv[l];
+    const Query q = load_query(P, lp, n, xyz, t, index);
+#pragma unroll
+    for (uint32_t xc = 0; xc < 2; ++xc) {
+        uint32_t slot[8];
+        float W[8];
+        half_cell(P, lp, q, xc, slot, W);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            idx_out[i * 16 + (xc | (j << 1))] = slot[j];
+            if (w_out) w_out[i * 16 + (xc | (j << 1))] = W[j];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Small helpers: fill, |dout| max, fixed-point finalize, input validation
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlockThreads)
+zero_kernel(unsigned char* __restrict__ base, size_t head, size_t n16, size_t tail) {
+    // [base, base+head) bytes up to 16-byte alignment, then n16 aligned 16-byte stores, then tail bytes
+    uint4* body = reinterpret_cast<uint4*>(base + head);
+    const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
+    for (size_t i = static_cast<size_t>(blockIdx.x) * kBlockThreads + threadIdx.x; i < n16;
+         i += stride)
+        body[i] = make_uint4(0u, 0u, 0u, 0u);
+    if (blockIdx.x == 0) {
+        if (threadIdx.x < head) base[threadIdx.x] = 0;
+        if (threadIdx.x < tail) base[head + n16 * 16 + threadIdx.x] = 0;
+    }
+}
+
+__global__ void __launch_bounds__(kBlockThreads)
+absmax_kernel(const float* __restrict__ v, size_t count, WorkspaceHeader* __restrict__ hdr) {
+    const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
+    uint32_t m = 0;
+    for (size_t i = static_cast<size_t>(blockIdx.x) * kBlockThreads + threadIdx.x; i < count;
+         i += stride)
+        m = max(m, __float_as_uint(fabsf(__ldg(v + i))));  // non-negative floats order as uints
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(&hdr->absmax_bits, m);
+}
+
+// scale = 2^s with N * max|dY| * 2^s <= 2^61: no slot can overflow int64 (weights of one query sum to 1).
+__global__ void fixed_scale_kernel(WorkspaceHeader* hdr, uint64_t N) {
+    const float amax = __uint_as_float(hdr->absmax_bits);
+    int e = 0;
+    if (amax > 0.0f && amax < __int_as_float(0x7f800000)) frexpf(amax, &e);  // amax < 2^e
+    int k = 0;
+    while ((1ull << k) < N && k < 62) ++k;  // N <= 2^k
+    int s = 61 - e - k;
+    s = max(-100, min(100, s));
+    hdr->scale = ldexpf(1.0f, s);
+    hdr->inv_scale = ldexp(1.0, -s);
+}
+
+__global__ void __launch_bounds__(kBlockThreads)
+fixed_finalize_kernel(const long long* __restrict__ acc, float* __restrict__ dtable, size_t count,
+                      const WorkspaceHeader* __restrict__ hdr, int overwrite) {
+    const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
+    const double inv = hdr->inv_scale;
+    for (size_t i = static_cast<size_t>(blockIdx.x) * kBlockThreads + threadIdx.x; i < count;
+         i += stride) {
+        const double sum = __ll2double_rn(acc[i]) * inv;
+        dtable[i] = static_cast<float>(overwrite ? sum : static_cast<double>(dtable[i]) + sum);
+    }
+}
+
+__global__ void __launch_bounds__(kBlockThreads)
+validate_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
+                const float* __restrict__ t, const int32_t* __restrict__ index,
+                WorkspaceHeader* __restrict__ hdr) {
+    const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
+    uint32_t bad = 0;
+    for (uint64_t n = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x; n < P.N;
+         n += stride) {
+        const uint64_t row = index ? static_cast<uint64_t>(index[n]) : n;
+        const float* p = xyz + row * P.xyz_stride;
+        const float c[4] = {p[0], p[1], p[2], t[n * P.t_stride]};
+#pragma unroll
+        for (int d = 0; d < 4; ++d) bad += !(c[d] >= 0.0f && c[d] < 1.0f);  // NaN fails both
+    }
+    if (bad) atomicAdd(&hdr->bad_inputs, bad);
+}
+
+int sm_count() {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            sms <= 0)
+            sms = 148;
+    }
+    return sms;
+}
+
+inline cudaError_t after_launch() {
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+inline dim3 item_grid(const Plan& P) {
+    const uint64_t tiles = (P.N + P.q_per_block - 1) / P.q_per_block;
+    return dim3(static_cast<unsigned>(tiles), P.num_groups, 1);
+}
+
+}  // namespace
+
+uint64_t launch_counter(bool reset) {
+    const uint64_t v = g_launches;
+    if (reset) g_launches = 0;
+    return v;
+}
+
+cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                       const void* table, bool table_half, float* out, cudaStream_t s) {
+    const dim3 grid = item_grid(P), block(kBlockThreads);
+#define DASH_FWD(FV, HV) \
+    hash4d_fwd_kernel<FV, HV><<<grid, block, 0, s>>>(P, xyz, t, index, table, out)
+    switch (P.F * 2 + (table_half ? 1 : 0)) {
+        case 2: DASH_FWD(1, false); break;
+        case 3: DASH_FWD(1, true); break;
+        case 4: DASH_FWD(2, false); break;
+        case 5: DASH_FWD(2, true); break;
+        case 8: DASH_FWD(4, false); break;
+        case 9: DASH_FWD(4, true); break;
+        case 16: DASH_FWD(8, false); break;
+        case 17: DASH_FWD(8, true); break;
+        default: return cudaErrorInvalidValue;
+    }
+#undef DASH_FWD
+    return after_launch();
+}
+
+cudaError_t launch_bwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                       const float* dout, float* dtable, cudaStream_t s) {
+    const dim3 grid = item_grid(P), block(kBlockThreads);
+    switch (P.F) {
+        case 1: hash4d_bwd_kernel<1><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); break;
+        case 2: hash4d_bwd_kernel<2><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); break;
+        case 4: hash4d_bwd_kernel<4><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); break;
+        case 8: hash4d_bwd_kernel<8><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return after_launch();
+}
+
+cudaError_t launch_bwd_fixed(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                             const float* dout, long long* acc, const WorkspaceHeader* hdr,
+                             cudaStream_t s) {
+    const dim3 grid = item_grid(P), block(kBlockThreads);
+    switch (P.F) {
+        case 1: hash4d_bwd_fixed_kernel<1><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); break;
+        case 2: hash4d_bwd_fixed_kernel<2><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); break;
+        case 4: hash4d_bwd_fixed_kernel<4><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); break;
+        case 8: hash4d_bwd_fixed_kernel<8><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return after_launch();
+}
+
+cudaError_t launch_indices(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                           uint32_t* idx_out, float* w_out, cudaStream_t s) {
+    const uint64_t items = P.N * P.L;
+    const uint64_t blocks = (items + kBlockThreads - 1) / kBlockThreads;
+    hash4d_indices_kernel<<<static_cast<unsigned>(blocks), kBlockThreads, 0, s>>>(P, xyz, t, index,
+                                                                                 idx_out, w_out);
+    return after_launch();
+}
+
+cudaError_t launch_zero(void* ptr, size_t bytes, cudaStream_t s) {
+    if (bytes == 0) return cudaSuccess;
+    size_t head = (16 - (reinterpret_cast<uintptr_t>(ptr) & 15u)) & 15u;
+    if (head > bytes) head = bytes;
+    const size_t n16 = (bytes - head) / 16, tail = (bytes - head) % 16;
+    const size_t want = (n16 + kBlockThreads - 1) / kBlockThreads;
+    const size_t cap = static_cast<size_t>(sm_count()) * 16;
+    const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
+    zero_kernel<<<blocks, kBlockThreads, 0, s>>>(static_cast<unsigned char*>(ptr), head, n16, tail);
+    return after_launch();
+}
+
+cudaError_t launch_absmax(const float* v, size_t count, WorkspaceHeader* hdr, uint64_t N,
+                          cudaStream_t s) {
+    const size_t want = (count + kBlockThreads - 1) / kBlockThreads;
+    const size_t cap = static_cast<size_t>(sm_count()) * 8;
+    const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
+    absmax_kernel<<<blocks, kBlockThreads, 0, s>>>(v, count, hdr);
+    cudaError_t e = after_launch();
+    if (e != cudaSuccess) return e;
+    fixed_scale_kernel<<<1, 1, 0, s>>>(hdr, N);
+    return after_launch();
+}
+
+cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t count,
+                                  const WorkspaceHeader* hdr, bool overwrite, cudaStream_t s) {
+    const size_t want = (count + kBlockThreads - 1) / kBlockThreads;
+    const size_t cap = static_cast<size_t>(sm_count()) * 16;
+    const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
+    fixed_finalize_kernel<<<blocks, kBlockThreads, 0, s>>>(acc, dtable, count, hdr, overwrite ? 1 : 0);
+    return after_launch();
+}
+
+cudaError_t launch_validate(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                            WorkspaceHeader* hdr, cudaStream_t s) {
+    const size_t want = (P.N + kBlockThreads - 1) / kBlockThreads;
+    const size_t cap = static_cast<size_t>(sm_count()) * 8;
+    const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
+    validate_kernel<<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, hdr);
+    return after_launch();
+}
+
+}  // namespace dash

@@ -1,0 +1,41 @@
+// hash4d_kernels.h — host-callable launchers of the sm_100a kernels (hash4d_kernels.cu).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+
+#include "hash4d_plan.h"
+
+namespace dash {
+
+// Header of the caller's workspace when a flag needs one (DETERMINISTIC_BWD / VALIDATE_INPUTS).
+struct WorkspaceHeader {
+    uint32_t absmax_bits;   // max |dout| as binary32 bits (deterministic bwd)
+    float scale;            // fixed-point scale 2^s
+    double inv_scale;       // 2^-s
+    uint32_t bad_inputs;    // VALIDATE_INPUTS: coordinates that are NaN or outside [0,1)
+    uint32_t pad[27];
+};
+static_assert(sizeof(WorkspaceHeader) == 128, "workspace header is 128 bytes");
+
+cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                       const void* table, bool table_half, float* out, cudaStream_t s);
+cudaError_t launch_bwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                       const float* dout, float* dtable, cudaStream_t s);
+cudaError_t launch_bwd_fixed(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                             const float* dout, long long* acc, const WorkspaceHeader* hdr,
+                             cudaStream_t s);
+cudaError_t launch_indices(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                           uint32_t* idx_out, float* w_out, cudaStream_t s);
+cudaError_t launch_zero(void* ptr, size_t bytes, cudaStream_t s);
+cudaError_t launch_absmax(const float* v, size_t count, WorkspaceHeader* hdr, uint64_t N,
+                          cudaStream_t s);
+cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t count,
+                                  const WorkspaceHeader* hdr, bool overwrite, cudaStream_t s);
+cudaError_t launch_validate(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                            WorkspaceHeader* hdr, cudaStream_t s);
+
+uint64_t launch_counter(bool reset);
+
+}  // namespace dash

@@ -1,0 +1,116 @@
+"""CPU-side checks of the product's C-ABI library: it loads, exports every symbol include/dash_hash4d.h
+declares, validates arguments, and evaluates Eq. 7 (host-only call).  No compute call is made."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import paper_2507_19141_b200 as dh
+from dash_inputs import CONFIGS
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    text = open(os.path.join(ROOT, "include", "dash_hash4d.h")).read()
+    return re.findall(r"DASH_API\s+[\w\s\*]+?\b(dash_hash4d_\w+)\s*\(", text)
+
+
+def test_library_exports_every_declared_symbol():
+    names = _declared()
+    assert len(names) >= 8 and "dash_hash4d_fwd" in names and "dash_hash4d_bwd" in names \
+        and "dash_hash4d_indices" in names
+    lib = C.CDLL(dh.library_path())
+    for n in names:
+        assert hasattr(lib, n), n
+    assert set(dh.exported_symbols()) == set(names)
+
+
+def test_struct_layout_matches_header():
+    assert C.sizeof(dh.Hash4DConfig) == 14 * 4
+
+
+def _rows(path):
+    for line in open(path):
+        line = line.split("#")[0].strip()
+        if line:
+            yield line
+
+
+def test_resolutions_match_printed_lists(golden_dir):
+    for row in _rows(os.path.join(golden_dir, "resolutions.txt")):
+        head, vals = row.split(":")
+        _, n_min, n_max, L = head.split()
+        want = [int(v) for v in vals.split()]
+        cfg = dh.make_config(int(L), 2, 1 << 12, int(n_min), int(n_max), int(n_min), int(n_max))
+        rs, rt, _ = dh.dash_hash4d_resolutions(cfg)
+        assert rs == want and rt == want
+
+
+def test_dense_levels_per_config():
+    want = {"C1": [], "C2": [0, 1], "C3": [0, 1, 2], "C4": [0, 1, 2, 3], "C5": [0, 1, 2]}
+    for name, levels in want.items():
+        cfg = dh.config_from_params(CONFIGS[name].enc)
+        _, _, dn = dh.dash_hash4d_resolutions(cfg)
+        assert [l for l, d in enumerate(dn) if d] == levels
+        cfg = dh.config_from_params(CONFIGS[name].enc, flags=0)
+        assert not any(dh.dash_hash4d_resolutions(cfg)[2])
+
+
+@pytest.mark.parametrize("kw,status", [
+    (dict(L=0), 1), (dict(L=33), 1), (dict(F=3), 2), (dict(F=16), 1), (dict(T=0), 1),
+    (dict(res_s_min=0), 1), (dict(res_s_min=200, res_s_max=100), 1), (dict(res_t_min=9, res_t_max=8), 1),
+    (dict(res_s_max=(1 << 22) + 1), 1), (dict(table_dtype=2), 1), (dict(flags=64), 1), (dict(struct_size=8), 1),
+])
+def test_bad_configs_are_rejected(kw, status):
+    cfg = dh.make_config(4, 2, 4096, 16, 128, 8, 32)
+    for k, v in kw.items():
+        setattr(cfg, k, v)
+    with pytest.raises(dh.Hash4DError) as ei:
+        dh.dash_hash4d_resolutions(cfg)
+    assert ei.value.status == status
+    assert dh.dash_hash4d_last_error() != ""
+    assert dh.dash_hash4d_workspace_bytes(cfg, 10, dh.OP_BWD) == 0
+
+
+def test_workspace_sizes():
+    enc = CONFIGS["C2"].enc
+    cfg = dh.config_from_params(enc)
+    for op in (dh.OP_FWD, dh.OP_BWD, dh.OP_INDICES):
+        assert dh.dash_hash4d_workspace_bytes(cfg, 1000, op) == 0
+    det = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE | dh.FLAG_DETERMINISTIC_BWD)
+    assert dh.dash_hash4d_workspace_bytes(det, 1000, dh.OP_BWD) == 128 + enc.L * enc.T * enc.F * 8
+    assert dh.dash_hash4d_workspace_bytes(det, 1000, dh.OP_FWD) == 0
+    val = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE | dh.FLAG_VALIDATE_INPUTS)
+    assert dh.dash_hash4d_workspace_bytes(val, 1000, dh.OP_FWD) == 128
+
+
+def test_null_and_stride_validation_happens_before_any_cuda_call():
+    lib = C.CDLL(dh.library_path())
+    lib.dash_hash4d_fwd.restype = C.c_int
+    cfg = dh.make_config(4, 2, 4096, 16, 128, 8, 32)
+    u64, u32, vp = C.c_uint64, C.c_uint32, C.c_void_p
+    # N = 0 is OK and a no-op, whatever the pointers
+    assert lib.dash_hash4d_fwd(C.byref(cfg), u64(0), vp(0), u32(3), vp(0), u32(1), vp(0), vp(0), vp(0),
+                               vp(0), C.c_size_t(0), vp(0)) == 0
+    # null xyz
+    assert lib.dash_hash4d_fwd(C.byref(cfg), u64(4), vp(0), u32(3), vp(0), u32(1), vp(0), vp(0), vp(0),
+                               vp(0), C.c_size_t(0), vp(0)) == 1
+    # bad stride (fake non-null, never dereferenced: validation fails first)
+    fake = vp(4096)
+    assert lib.dash_hash4d_fwd(C.byref(cfg), u64(4), fake, u32(5), fake, u32(1), vp(0), fake, fake,
+                               vp(0), C.c_size_t(0), vp(0)) == 1
+    assert lib.dash_hash4d_fwd(C.byref(cfg), u64(4), fake, u32(3), fake, u32(2), vp(0), fake, fake,
+                               vp(0), C.c_size_t(0), vp(0)) == 1
+    # misaligned table
+    assert lib.dash_hash4d_fwd(C.byref(cfg), u64(4), fake, u32(3), fake, u32(1), vp(0), vp(4100), fake,
+                               vp(0), C.c_size_t(0), vp(0)) == 1
+
+
+def test_binding_refuses_cpu_tensors():
+    import torch
+    cfg = dh.make_config(4, 2, 4096, 16, 128, 8, 32)
+    x = torch.zeros(4, 3); t = torch.zeros(4); tab = torch.zeros(4, 4096, 2)
+    with pytest.raises(ValueError):
+        dh.dash_hash4d_fwd(cfg, x, t, tab)
