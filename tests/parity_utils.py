@@ -14,9 +14,21 @@ RTOL_FP32 = 1e-5
 RTOL_FP16 = 2e-3
 
 
-def check_close(got, ref, mag, rtol, L, hits=None, what=""):
+def fixed_point_quantum(n_queries: int, absmax: float) -> float:
+    """Quantum 2^-s of the DETERMINISTIC_BWD fixed-point accumulators (DESIGN.md §3 Q23):
+    s = 61 - e - k with absmax < 2^e and n_queries <= 2^k, clamped to [-100, 100]."""
+    import math
+    e = math.frexp(absmax)[1] if absmax > 0 else 0
+    k = 0
+    while (1 << k) < n_queries:
+        k += 1
+    return 2.0 ** -max(-100, min(100, 61 - e - k))
+
+
+def check_close(got, ref, mag, rtol, L, hits=None, what="", quantum=0.0):
     """got/ref: arrays with a leading or trailing level structure flattened by the caller into
-    shape [L][...]; mag: same shape, the conditioning term A; hits: optional [L][...] counts."""
+    shape [L][...]; mag: same shape, the conditioning term A; hits: optional [L][...] counts;
+    quantum: fixed-point step of the deterministic mode (each of `hits` contributions is rounded to it)."""
     got = np.asarray(got, np.float64).reshape(L, -1)
     ref64 = np.asarray(ref, np.float64).reshape(L, -1)
     mag = np.asarray(mag, np.float64).reshape(L, -1)
@@ -31,7 +43,7 @@ def check_close(got, ref, mag, rtol, L, hits=None, what=""):
         h = np.asarray(hits, np.float64).reshape(L, -1)
         if h.shape[1] != mag.shape[1]:                       # hits per slot, mag per (slot, f)
             h = np.repeat(h, mag.shape[1] // h.shape[1], axis=1)
-        allow = allow * np.maximum(1.0, np.sqrt(h / 1e4))
+        allow = allow * np.maximum(1.0, np.sqrt(h / 1e4)) + 0.5 * quantum * h
     bad = err > allow + 1e-30
     assert not bad.any(), (f"{what}: {bad.sum()} elements out of tolerance; worst ratio "
                            f"{(err / (mag + 1e-300)).max():.3e} (rtol {rtol})")
