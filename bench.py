@@ -327,7 +327,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", default="C4", choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--zero-grad-fused", type=int, default=0,
+    ap.add_argument("--zero-grad-fused", type=int, default=1,
                     help="1: bwd zeroes each level group itself (DASH_HASH4D_FLAG_ZERO_GRAD)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic-bytes", type=float, default=None,

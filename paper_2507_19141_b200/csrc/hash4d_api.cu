@@ -113,10 +113,14 @@ uint32_t env_u32(const char* name) {
     return v ? static_cast<uint32_t>(std::strtoul(v, nullptr, 10)) : 0u;
 }
 
-// Level-group size G (power of two <= 16): as many levels as keep the group's randomly accessed
-// bytes (tables in fwd, fp32 gradient slices in bwd) within a fraction of L2, but at least enough
-// that one lane-quad writes a full 32-byte sector of `out` (G*F*4 >= 32), and without wasting more
-// than a quarter of the lanes when L is not a multiple of G.  DASH_HASH4D_{FWD,BWD}_GROUP override.
+// Level-group size G (power of two <= 8): as many levels as keep the group's randomly accessed
+// bytes (tables in fwd, fp32 gradient slices in bwd) within 0.3 x L2 — measured (profiles/
+// group_sweep_r01.md): B200's 126 MB L2 is two 63 MB halves and read-only lines are replicated in
+// both, so ~40 MB is what stays resident next to the streamed inputs/outputs — but at least enough
+// that a query's slice of `out`/`dout` is one full 32-byte sector (G*F*4 >= 32), and without idling
+// more than a quarter of the lanes when L is not a multiple of G.  G = 16 (one query per warp) is
+// never picked: every warp would then run both the dense and the hashed index path (measured 7-12 %
+// slower than G = 8 at F = 2).  DASH_HASH4D_{FWD,BWD}_GROUP override G (1..16) for sweeps.
 uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, const char* env_name) {
     uint32_t forced = env_u32(env_name);
     if (forced) {
@@ -124,11 +128,11 @@ uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, const c
         while (g * 2 <= forced && g * 2 <= dash::kMaxGroup) g *= 2;
         return g;
     }
-    const size_t budget = l2_bytes() * 6 / 10;
+    const size_t budget = l2_bytes() * 3 / 10;
     uint32_t g_min = 1;
     while (g_min * c->F * 4 < 32 && g_min < dash::kMaxGroup) g_min *= 2;
     uint32_t best = 0;
-    for (uint32_t g = dash::kMaxGroup; g >= 1; g /= 2) {
+    for (uint32_t g = dash::kMaxGroup / 2; g >= 1; g /= 2) {
         const uint32_t groups = (c->L + g - 1) / g;
         const bool efficient = 4 * c->L >= 3 * groups * g;
         const bool resident = g * bytes_per_level <= budget;
