@@ -50,6 +50,16 @@ def algorithmic_bytes(enc, has_index: bool):
     return fwd, bwd, zero
 
 
+def profiled_traffic(config: str, kernel: str):
+    """ncu dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed
+    summary profiles/traffic.json (written by hand from the ncu --set full capture it names)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            return float(json.load(fh)[config][kernel])
+    except Exception:  # noqa: BLE001
+        return None
+
+
 def measured_hbm_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -160,16 +170,14 @@ def run_cuda(args):
     import torch
     import paper_2507_19141_b200 as dh
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
+    from paper_2507_19141_b200.replicas import Replicas
+
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    rep = Replicas(backend="nccl", device=torch.device("cuda", local))
+    world, rank = rep.world, rep.rank
 
     wl = make_workload(args.config)
     enc, N = wl.spec.enc, wl.N
@@ -197,11 +205,7 @@ def run_cuda(args):
         if marks is not None:
             marks[3].record()
 
-    def barrier():
-        torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
+    barrier = rep.barrier
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -220,11 +224,7 @@ def run_cuda(args):
     barrier()
     launches = dh.dash_hash4d_launch_count()
     clocks = sampler.stop() if sampler is not None else None
-    ms_total = start.elapsed_time(stop)
-    if dist is not None:
-        tt = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = rep.max_over_ranks(start.elapsed_time(stop))
     ms_step = ms_total / args.steps
     seg = np.array([[m[0].elapsed_time(m[1]), m[1].elapsed_time(m[2]), m[2].elapsed_time(m[3])]
                     for m in marks])
@@ -238,11 +238,16 @@ def run_cuda(args):
     if dominant == "bwd" and args.zero_grad_fused:
         dom_bytes += b_zero
     dom_ms = ms_bwd if dominant == "bwd" else ms_fwd
+    kernel_name = f"hash4d_{dominant}_kernel"
+    if dominant == "bwd" and args.zero_grad_fused:
+        kernel_name = "hash4d_bwd_kernel+zero_kernel (one dash_hash4d_bwd call, ZERO_GRAD)"
     achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
     step_bytes = (b_fwd + b_bwd) * N + b_zero
     roofline = {
-        "bound": "hbm", "kernel": f"hash4d_{dominant}_kernel", "achieved": achieved, "peak": peak,
-        "unit": "GB/s", "frac": achieved / peak, "traffic": args.traffic_bytes,
+        "bound": "hbm", "kernel": kernel_name, "achieved": achieved, "peak": peak,
+        "unit": "GB/s", "frac": achieved / peak,
+        "traffic": args.traffic_bytes if args.traffic_bytes is not None
+        else profiled_traffic(args.config, kernel_name),
         "peak_source": peak_src,
         "algorithmic_bytes_per_launch": dom_bytes,
         "step": {"algorithmic_bytes": step_bytes, "achieved": step_bytes / (ms_step * 1e-3) / 1e9,
@@ -273,18 +278,13 @@ def run_cuda(args):
         e2e_step()
     e1.record()
     barrier()
-    e2e_ms = e0.elapsed_time(e1) / e2e_steps
-    if dist is not None:
-        tt = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_ms = float(tt.item())
+    e2e_ms = rep.max_over_ranks(e0.elapsed_time(e1) / e2e_steps)
     nbytes = lambda x: 0 if x is None else x.numel() * x.element_size()
     h2d = nbytes(xyz_h) + nbytes(t_h) + nbytes(index_h) + nbytes(dout_h)
     d2h = nbytes(out_h) + nbytes(dtable_h)
 
-    if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
+    if not rep.is_reporter:
+        rep.close()
         return 0
 
     # ---- cpu_baseline: the oracle as it stands, bounded sample, on this box's host cores
@@ -315,8 +315,7 @@ def run_cuda(args):
     if cpu is not None:
         line["cpu_baseline"] = cpu
     print(json.dumps(line), flush=True)
-    if dist is not None:
-        dist.destroy_process_group()
+    rep.close()
     return 0
 
 

@@ -147,3 +147,13 @@ def oracle_half_to_double(h: int) -> float:
     f = lib().dash_oracle_half_to_double
     f.restype = C.c_double
     return float(f(C.c_uint16(h)))
+
+
+def oracle_bwd_input(cfg, N, xyz, t, table, dout, index=None, t_stride=1, want_abs=False):
+    """dq[n] = d<dout[n], G_4D(x_n)>/d(x,y,z,t): [N][4] fp32 (SURVEY §8f NEXT #1; DESIGN.md Q14/Q24)."""
+    xs, ts = _query_args(xyz, t, index, t_stride)
+    dq = np.zeros((N, 4), np.float32)
+    mag = np.zeros((N, 4), np.float64) if want_abs else None
+    _check(lib().dash_oracle_bwd_input(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(t), ts, _p(index),
+                                       _p(table), _p(dout), _p(dq), _p(mag)), "bwd_input")
+    return (dq, mag) if want_abs else dq

@@ -339,3 +339,62 @@ void dash_oracle_locate(float x, uint32_t n, uint32_t *cell, float *frac) {
 }
 
 double dash_oracle_half_to_double(uint16_t h) { return half_to_double(h); }
+
+/* ---- NEXT #1: gradient with respect to the query coordinates -------------------
+ * The paper is silent on whether gradients flow through G_4D into the Gaussian positions
+ * (DESIGN.md §3 Q14); PAPER.md:140-144 makes x both the encoder input and a learnable quantity.
+ * Inside a cell Eq. 9 is multilinear in the fractional offsets w_d = x_d*N_{l,d} - c_d, so
+ *   d out[n][l*F+f] / d x_d = N_{l,d} * sum_k s_d(k) * prod_{d' != d} omega_{d'}(k) * table[l][slot_k][f]
+ * with omega_d(k) = (bit_d(k) ? w_d : 1-w_d), s_d(k) = (bit_d(k) ? +1 : -1), and
+ *   dq[n][d] = sum_{l,f} dout[n][l*F+f] * d out[n][l*F+f] / d x_d.
+ * The derivative is taken on the open cell (one-sided from the right at a vertex, because c = floor);
+ * a coordinate that the Q12 clamp moved (NaN, < 0, > 1-2^-24) has derivative 0.
+ * dq: [N][4] fp32 (x,y,z,t), overwritten.  dq_abs (nullable, [N][4] double): sum of |terms|. */
+int dash_oracle_bwd_input(const dash_oracle_config *c, uint64_t N, const float *xyz,
+                          uint32_t xyz_stride, const float *t, uint32_t t_stride,
+                          const int32_t *index, const void *table, const float *dout, float *dq,
+                          double *dq_abs) {
+    level_plan p;
+    if (!config_ok(c) || make_plan(c, &p)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!args_ok(xyz, xyz_stride, t, t_stride) || !table || !dout || !dq) return ORACLE_INVALID;
+    const uint32_t L = c->L, F = c->F;
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < (int64_t)N; ++n) {
+        float q[4];
+        fetch_query((uint64_t)n, xyz, xyz_stride, t, t_stride, index, q);
+        double acc[4] = {0, 0, 0, 0}, mag[4] = {0, 0, 0, 0};
+        for (uint32_t l = 0; l < L; ++l) {
+            uint32_t cell[4];
+            float frac[4];
+            double res[4];
+            for (int d = 0; d < 4; ++d) {
+                uint32_t nres = (d < 3) ? p.res_s[l] : p.res_t[l];
+                locate(clamp_unit(q[d]), nres, &cell[d], &frac[d]);
+                res[d] = (double)nres;
+            }
+            for (int k = 0; k < 16; ++k) {
+                uint32_t g[4];
+                for (int d = 0; d < 4; ++d) g[d] = cell[d] + (uint32_t)((k >> d) & 1);
+                uint32_t slot = vertex_slot(g, p.pi, c->T, p.dense[l], p.res_s[l]);
+                for (int d = 0; d < 4; ++d) {
+                    double wd = ((k >> d) & 1) ? 1.0 : -1.0; /* d omega_d / d w_d */
+                    for (int e = 0; e < 4; ++e)
+                        if (e != d) wd *= ((k >> e) & 1) ? (double)frac[e] : 1.0 - (double)frac[e];
+                    for (uint32_t f = 0; f < F; ++f) {
+                        double term = (double)dout[(size_t)n * L * F + (size_t)l * F + f] * res[d] *
+                                      wd * table_value(c, table, l, slot, f);
+                        acc[d] += term;
+                        mag[d] += fabs(term);
+                    }
+                }
+            }
+        }
+        for (int d = 0; d < 4; ++d) {
+            int moved = isnan(q[d]) || q[d] < 0.0f || q[d] > 0x1.fffffep-1f;
+            dq[(size_t)n * 4 + d] = moved ? 0.0f : (float)acc[d];
+            if (dq_abs) dq_abs[(size_t)n * 4 + d] = moved ? 0.0 : mag[d];
+        }
+    }
+    return ORACLE_OK;
+}

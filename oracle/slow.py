@@ -96,3 +96,30 @@ def backward(queries, dout, L, F, T, rs_min, rs_max, rt_min, rt_max, dense_coars
                 for f in range(F):
                     g[l, s, f] += w * float(dout[n, l * F + f])
     return g
+
+
+def backward_input(queries, table, dout, L, F, T, rs_min, rs_max, rt_min, rt_max, dense_coarse=True,
+                   primes=DEFAULT_PRIMES):
+    """dq[n][d] = sum_{l,f} dout * N_{l,d} * sum_k s_d(k) prod_{e!=d} omega_e(k) * table  (float64 [n][4]).
+    Coordinates moved by the clamp get 0 (Q24)."""
+    rs, rt, dn = plan(L, T, rs_min, rs_max, rt_min, rt_max, dense_coarse)
+    dq = np.zeros((len(queries), 4))
+    for n, q in enumerate(queries):
+        for l in range(L):
+            res = [rs[l]] * 3 + [rt[l]]
+            cw = [locate(q[d], res[d]) for d in range(4)]
+            for k in range(16):
+                g = [cw[d][0] + ((k >> d) & 1) for d in range(4)]
+                s = slot_of(g, rs[l], T, dn[l], primes)
+                for d in range(4):
+                    w = 1.0 if (k >> d) & 1 else -1.0
+                    for e in range(4):
+                        if e != d:
+                            w *= cw[e][1] if (k >> e) & 1 else 1.0 - cw[e][1]
+                    for f in range(F):
+                        dq[n, d] += float(dout[n, l * F + f]) * res[d] * w * float(table[l, s, f])
+        for d in range(4):
+            v = np.float32(q[d])
+            if np.isnan(v) or v < 0 or float(v) > MAXF:
+                dq[n, d] = 0.0
+    return dq
