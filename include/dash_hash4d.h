@@ -63,7 +63,8 @@ enum dash_hash4d_flags {
                                                instead of accumulating into the caller's contents.          */
 };
 
-enum dash_hash4d_op { DASH_HASH4D_OP_FWD = 0, DASH_HASH4D_OP_BWD = 1, DASH_HASH4D_OP_INDICES = 2 };
+enum dash_hash4d_op { DASH_HASH4D_OP_FWD = 0, DASH_HASH4D_OP_BWD = 1, DASH_HASH4D_OP_INDICES = 2,
+                      DASH_HASH4D_OP_BWD_INPUT = 3 };
 
 /* Encoder hyper-parameters.  POD, passed by pointer (host memory). */
 typedef struct dash_hash4d_config {
@@ -126,6 +127,24 @@ DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N,
                              const float* dout,
                              float* dtable,
                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Coordinate gradient (not in the paper, which is silent on whether gradients reach the Gaussian
+ * positions through G_4D — PAPER.md:140-144 makes x both encoder input and learnable; Q24):
+ *     dq[n][d] = sum_{l,f} dout[n][l*F+f] * d out[n][l*F+f] / d x_d ,   d = 0:x 1:y 2:z 3:t,
+ * with d out / d x_d = N_{l,d} * sum_k s_d(k) prod_{e != d} omega_e(k) table[l][slot_k][f] on the open cell
+ * (the one-sided derivative from the right at a grid vertex).  A coordinate changed by the clamp
+ * (NaN, < 0, > 1-2^-24) gets 0.
+ *   dq         [N][4] fp32, OVERWRITTEN (the library zeroes it, then adds one partial sum per level group).
+ *              Per QUERY, not per xyz row: with an index list the caller reduces rows itself.
+ * Other arguments as in fwd. */
+DASH_API int dash_hash4d_bwd_input(const dash_hash4d_config* cfg, uint64_t N,
+                                   const float* xyz, uint32_t xyz_stride,
+                                   const float* t, uint32_t t_stride,
+                                   const int32_t* index,
+                                   const void* table,
+                                   const float* dout,
+                                   float* dq,
+                                   void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Debug: the 16 table slots and interpolation weights of every (query, level)
  * (Eq. 8).  Corner k: bit d of k set => vertex floor(x_d*N_l)+1 along axis d,

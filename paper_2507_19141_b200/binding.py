@@ -17,12 +17,12 @@ FLAG_DENSE_COARSE = 1
 FLAG_DETERMINISTIC_BWD = 2
 FLAG_VALIDATE_INPUTS = 4
 FLAG_ZERO_GRAD = 8
-OP_FWD, OP_BWD, OP_INDICES = 0, 1, 2
+OP_FWD, OP_BWD, OP_INDICES, OP_BWD_INPUT = 0, 1, 2, 3
 
 _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUDA_ERROR"}
 
 EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4d_fwd",
-           "dash_hash4d_bwd", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
+           "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count"]
 
 
@@ -71,6 +71,8 @@ def _load() -> C.CDLL:
     lib.dash_hash4d_fwd.restype = C.c_int
     lib.dash_hash4d_bwd.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp, sz, vp]
     lib.dash_hash4d_bwd.restype = C.c_int
+    lib.dash_hash4d_bwd_input.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp, vp, sz, vp]
+    lib.dash_hash4d_bwd_input.restype = C.c_int
     lib.dash_hash4d_indices.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp]
     lib.dash_hash4d_indices.restype = C.c_int
     lib.dash_hash4d_zero.argtypes = [cfgp, vp, vp]
@@ -197,6 +199,25 @@ def dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=None, t_stride=None, N=None
     _check(_load().dash_hash4d_bwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
                                    _ptr(dout), _ptr(dtable), _ptr(workspace), wbytes, _stream()))
     return dtable
+
+
+def dash_hash4d_bwd_input(cfg, xyz, t, table, dout, dq=None, index=None, t_stride=None, N=None,
+                          workspace=None):
+    """dq[n] = d<dout[n], G_4D(x_n)>/d(x,y,z,t); returns `dq` ([N][4] fp32, CUDA, overwritten)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(t, torch.float32, "t"); _dev(index, torch.int32, "index")
+    _dev(table, torch.float16 if cfg.table_dtype == 1 else torch.float32, "table")
+    _dev(dout, torch.float32, "dout")
+    xs, ts = _strides(xyz, t, t_stride)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    if dq is None:
+        dq = torch.empty((N, 4), dtype=torch.float32, device=xyz.device)
+    _dev(dq, torch.float32, "dq")
+    workspace, wbytes = _workspace(cfg, N, OP_BWD_INPUT, workspace)
+    _check(_load().dash_hash4d_bwd_input(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
+                                         _ptr(table), _ptr(dout), _ptr(dq), _ptr(workspace), wbytes,
+                                         _stream()))
+    return dq
 
 
 def dash_hash4d_indices(cfg, xyz, t, index=None, t_stride=None, N=None, want_weights=True):

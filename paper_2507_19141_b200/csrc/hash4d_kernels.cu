@@ -38,9 +38,14 @@ __device__ __forceinline__ void locate(float x, float res, uint32_t& cell, float
 }
 
 struct Query {
-    uint32_t c[4];  // cell (floor) per axis x,y,z,t
-    float w[4];     // fractional offset per axis
+    uint32_t c[4];   // cell (floor) per axis x,y,z,t
+    float w[4];      // fractional offset per axis
+    uint32_t moved;  // bit d: the Q12 clamp changed coordinate d (NaN, < 0, > 1-2^-24)
 };
+
+__device__ __forceinline__ uint32_t moved_bit(float v, int d) {
+    return (v >= 0.0f && v <= 0x1.fffffep-1f) ? 0u : (1u << d);  // NaN fails both comparisons
+}
 
 __device__ __forceinline__ Query load_query(const Plan& P, const LevelParams& lp, uint64_t n,
                                             const float* __restrict__ xyz,
@@ -49,10 +54,12 @@ __device__ __forceinline__ Query load_query(const Plan& P, const LevelParams& lp
     const uint64_t row = index ? static_cast<uint64_t>(__ldg(index + n)) : n;
     const float* p = xyz + row * P.xyz_stride;
     Query q;
-    locate(__ldg(p + 0), lp.ns_f, q.c[0], q.w[0]);
-    locate(__ldg(p + 1), lp.ns_f, q.c[1], q.w[1]);
-    locate(__ldg(p + 2), lp.ns_f, q.c[2], q.w[2]);
-    locate(__ldg(t + n * P.t_stride), lp.nt_f, q.c[3], q.w[3]);
+    const float x = __ldg(p + 0), y = __ldg(p + 1), z = __ldg(p + 2), tt = __ldg(t + n * P.t_stride);
+    locate(x, lp.ns_f, q.c[0], q.w[0]);
+    locate(y, lp.ns_f, q.c[1], q.w[1]);
+    locate(z, lp.ns_f, q.c[2], q.w[2]);
+    locate(tt, lp.nt_f, q.c[3], q.w[3]);
+    q.moved = moved_bit(x, 0) | moved_bit(y, 1) | moved_bit(z, 2) | moved_bit(tt, 3);
     return q;
 }
 
@@ -322,6 +329,88 @@ hash4d_bwd_fixed_kernel(const __grid_constant__ Plan P, const float* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------
+// Coordinate gradient (Q24): dq[n][d] = d<dout[n], G_4D(x_n)>/dx_d.
+// Same gathers as the forward.  Per corner the F features collapse to one scalar S_j = <dout, v_j>;
+// the multilinear form is then folded axis by axis (y, z, t), keeping at every fold both the
+// interpolated value and the difference along the folded axis, so each axis derivative costs one
+// extra subtraction per fold instead of a second pass over the 16 corners.
+// ------------------------------------------------------------------------------------------------
+template <int F, bool HALF>
+__global__ void __launch_bounds__(kBlockThreads)
+hash4d_bwd_input_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
+                        const float* __restrict__ t, const int32_t* __restrict__ index,
+                        const void* __restrict__ table, const float* __restrict__ dout,
+                        float* __restrict__ dq) {
+    const Item it = this_item(P);
+    const LevelParams lp = P.lv[it.l];
+    float g[F];
+    load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F,
+                 it.xc, g);
+    const Query q = load_query(P, lp, it.n, xyz, t, index);
+    uint32_t slot[8];
+    float W[8];
+    half_cell(P, lp, q, it.xc, slot, W);  // W unused here; slots shared with fwd
+    constexpr size_t kElem = HALF ? 2 : 4;
+    const char* level_base =
+        static_cast<const char*>(table) + static_cast<size_t>(it.l) * P.T * (F * kElem);
+    float v[8][F];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);
+    float S[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        S[j] = 0.0f;
+#pragma unroll
+        for (int f = 0; f < F; ++f) S[j] = fmaf(g[f], v[j][f], S[j]);
+    }
+    const float wy = q.w[1], wz = q.w[2], wt = q.w[3];
+    // fold y (corner bit 0): value and d/dy for the 4 (z,t) combinations
+    float a[4], ay[4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        ay[m] = S[2 * m + 1] - S[2 * m];
+        a[m] = fmaf(wy, ay[m], S[2 * m]);
+    }
+    // fold z (corner bit 1)
+    float b[2], by[2], bz[2];
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+        bz[m] = a[2 * m + 1] - a[2 * m];
+        b[m] = fmaf(wz, bz[m], a[2 * m]);
+        by[m] = fmaf(wz, ay[2 * m + 1] - ay[2 * m], ay[2 * m]);
+    }
+    // fold t (corner bit 2)
+    const float val = fmaf(wt, b[1] - b[0], b[0]);
+    const float dy = fmaf(wt, by[1] - by[0], by[0]);
+    const float dz = fmaf(wt, bz[1] - bz[0], bz[0]);
+    const float dt = b[1] - b[0];
+    // this lane is x-corner xc: d/dx takes the sign, the other axes the x weight
+    const float wx = it.xc ? q.w[0] : 1.0f - q.w[0];
+    float d4[4] = {it.xc ? val : -val, wx * dy, wx * dz, wx * dt};
+    const float scale[4] = {lp.ns_f, lp.ns_f, lp.ns_f, lp.nt_f};  // dw_d/dx_d = N_{l,d}
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+        d4[d] *= scale[d];
+        if (!it.active || ((q.moved >> d) & 1u)) d4[d] = 0.0f;
+    }
+    // sum the lane pair, then the G levels of this query that sit in this warp (2G adjacent lanes)
+    const uint32_t span = 2u * P.group;
+#pragma unroll
+    for (uint32_t o = 1; o < 32; o <<= 1) {
+        if (o < span) {
+#pragma unroll
+            for (int d = 0; d < 4; ++d) d4[d] += __shfl_xor_sync(0xffffffffu, d4[d], o);
+        }
+    }
+    if (it.active && (threadIdx.x & (span - 1u)) == 0) {
+        float* o = dq + it.n * 4;
+        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(o), "f"(d4[0]),
+                     "f"(d4[1]), "f"(d4[2]), "f"(d4[3])
+                     : "memory");
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Debug: all 16 slots + weights per (query, level)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlockThreads)
@@ -465,6 +554,27 @@ cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const in
         default: return cudaErrorInvalidValue;
     }
 #undef DASH_FWD
+    return after_launch();
+}
+
+cudaError_t launch_bwd_input(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                             const void* table, bool table_half, const float* dout, float* dq,
+                             cudaStream_t s) {
+    const dim3 grid = item_grid(P), block(kBlockThreads);
+#define DASH_BWI(FV, HV) \
+    hash4d_bwd_input_kernel<FV, HV><<<grid, block, 0, s>>>(P, xyz, t, index, table, dout, dq)
+    switch (P.F * 2 + (table_half ? 1 : 0)) {
+        case 2: DASH_BWI(1, false); break;
+        case 3: DASH_BWI(1, true); break;
+        case 4: DASH_BWI(2, false); break;
+        case 5: DASH_BWI(2, true); break;
+        case 8: DASH_BWI(4, false); break;
+        case 9: DASH_BWI(4, true); break;
+        case 16: DASH_BWI(8, false); break;
+        case 17: DASH_BWI(8, true); break;
+        default: return cudaErrorInvalidValue;
+    }
+#undef DASH_BWI
     return after_launch();
 }
 

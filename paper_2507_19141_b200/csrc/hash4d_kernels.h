@@ -21,6 +21,9 @@ static_assert(sizeof(WorkspaceHeader) == 128, "workspace header is 128 bytes");
 
 cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                        const void* table, bool table_half, float* out, cudaStream_t s);
+cudaError_t launch_bwd_input(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                             const void* table, bool table_half, const float* dout, float* dq,
+                             cudaStream_t s);
 cudaError_t launch_bwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                        const float* dout, float* dtable, cudaStream_t s);
 cudaError_t launch_bwd_fixed(const Plan& P, const float* xyz, const float* t, const int32_t* index,

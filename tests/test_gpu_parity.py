@@ -379,3 +379,68 @@ def test_launch_counter_counts_kernels():
     dh.dash_hash4d_launch_count(reset=True)
     dh.dash_hash4d_fwd(gcfg, xyz, t, tab)
     assert dh.dash_hash4d_launch_count() == 1
+
+
+# ----------------------------------------------------------------------------------------------------
+# NEXT #1: coordinate gradient  dq[n][d] = d<dout[n], G_4D(x_n)>/dx_d   (Q24)
+# ----------------------------------------------------------------------------------------------------
+
+def run_bwd_input_parity(enc, xyz, t, table, dout, index=None, t_stride=1, flags=DC, what=""):
+    ocfg, gcfg = both_configs(enc, flags)
+    N = len(index) if index is not None else (len(t) if t_stride else len(xyz))
+    ref, mag = oracle.oracle_bwd_input(ocfg, N, xyz, t, table, dout, index=index, t_stride=t_stride,
+                                       want_abs=True)
+    dq = torch.full((N, 4), 9.0, device="cuda")          # garbage: the call must overwrite
+    dh.dash_hash4d_bwd_input(gcfg, dev(xyz), dev(t), dev(table), dev(dout), dq=dq, index=dev(index),
+                             t_stride=t_stride, N=N)
+    torch.cuda.synchronize()
+    got = dq.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got).all()
+    err = np.abs(got - ref)
+    assert (err <= RTOL_FP32 * mag + 1e-30).all(), \
+        f"{what} bwd_input: worst err/A {(err / (mag + 1e-300)).max():.3e}"
+    for d in range(4):                                     # normwise per axis
+        assert np.linalg.norm(got[:, d] - ref[:, d]) <= RTOL_FP32 * np.linalg.norm(ref[:, d]) + 1e-30
+    return got
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C4", "C5"])
+def test_bwd_input_configs(name):
+    n_over = {"C4": 200_000, "C5": 200_000}.get(name)
+    wl = make_workload(name, n_override=n_over)
+    run_bwd_input_parity(wl.spec.enc, wl.xyz, wl.t, wl.table, wl.dout, index=wl.index, what=name)
+
+
+@pytest.mark.parametrize("L,F,T,rs,rt,dtype,N", VARIANTS)
+def test_bwd_input_variants(L, F, T, rs, rt, dtype, N):
+    enc = EncoderParams(L, F, T, rs[0], rs[1], rt[0], rt[1], dtype)
+    rng = np.random.default_rng(L * 100 + F)
+    xyz, t = make_queries_uniform(L + F, N)
+    table = rng.uniform(-1, 1, (L, T, F)).astype(np.float16 if dtype == "fp16" else np.float32)
+    dout = rng.standard_normal((N, L * F)).astype(np.float32)
+    run_bwd_input_parity(enc, xyz, t, table, dout)
+    run_bwd_input_parity(enc, xyz, t, table, dout, flags=0)
+
+
+@pytest.mark.parametrize("group", [1, 2, 4, 8, 16])
+def test_bwd_input_every_group_size_and_views(group, monkeypatch):
+    monkeypatch.setenv("DASH_HASH4D_FWD_GROUP", str(group))
+    enc = EncoderParams(12, 2, 1 << 14, 16, 1024, 8, 100)
+    rng = np.random.default_rng(group)
+    rows = rng.random((300, 3), dtype=np.float32)
+    index = rng.integers(0, 300, 1111).astype(np.int32)
+    table = rng.uniform(-1, 1, (12, enc.T, 2)).astype(np.float32)
+    dout = rng.standard_normal((1111, 24)).astype(np.float32)
+    run_bwd_input_parity(enc, rows, rng.random(1111, dtype=np.float32), table, dout, index=index)
+    run_bwd_input_parity(enc, rows, np.array([0.7], np.float32), table, dout, index=index, t_stride=0)
+
+
+def test_bwd_input_clamped_coordinates_get_zero():
+    enc = CONFIGS["C1"].enc
+    rng = np.random.default_rng(3)
+    q = rng.random((64, 4), dtype=np.float32)
+    q[0, 0] = -0.5; q[1, 1] = 1.0; q[2, 2] = np.nan; q[3, 3] = 7.0; q[4] = [np.nan, -1, 2, np.inf]
+    table = rng.uniform(-1, 1, (enc.L, enc.T, enc.F)).astype(np.float32)
+    dout = rng.standard_normal((64, enc.L * enc.F)).astype(np.float32)
+    got = run_bwd_input_parity(enc, np.ascontiguousarray(q[:, :3]), np.ascontiguousarray(q[:, 3]), table, dout)
+    assert got[0, 0] == 0 and got[1, 1] == 0 and got[2, 2] == 0 and got[3, 3] == 0 and not got[4].any()
