@@ -191,7 +191,15 @@ def run_cuda(args):
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
+    nbytes = lambda x: 0 if x is None else x.numel() * x.element_size()
+    ws_bytes = nbytes(table) + nbytes(dtable) + nbytes(out) + nbytes(dout) + nbytes(xyz) + nbytes(t)
+    l2_bytes = torch.cuda.get_device_properties(local).L2_cache_size
+    # timing hygiene: inputs larger than L2 (C3-C5), else write a buffer of 2 x L2 between iterations
+    flush = torch.empty(2 * l2_bytes, dtype=torch.uint8, device="cuda") if ws_bytes < 2 * l2_bytes else None
+
     def step(marks=None):
+        if flush is not None:
+            flush.zero_()
         if marks is not None:
             marks[0].record()
         if not args.zero_grad_fused:
@@ -224,11 +232,14 @@ def run_cuda(args):
     barrier()
     launches = dh.dash_hash4d_launch_count()
     clocks = sampler.stop() if sampler is not None else None
-    ms_total = rep.max_over_ranks(start.elapsed_time(stop))
-    ms_step = ms_total / args.steps
     seg = np.array([[m[0].elapsed_time(m[1]), m[1].elapsed_time(m[2]), m[2].elapsed_time(m[3])]
                     for m in marks])
     ms_zero, ms_fwd, ms_bwd = (float(v) for v in seg.mean(0))
+    if flush is None:
+        ms_total = start.elapsed_time(stop)                      # K back-to-back steps, one event pair
+    else:
+        ms_total = float(np.array([m[0].elapsed_time(m[3]) for m in marks]).sum())   # flushes excluded
+    ms_step = rep.max_over_ranks(ms_total) / args.steps
 
     # ---- roofline of the dominant kernel (the bwd scatter), live CUDA-event durations
     b_fwd, b_bwd, b_zero = algorithmic_bytes(enc, index is not None)
@@ -279,7 +290,6 @@ def run_cuda(args):
     e1.record()
     barrier()
     e2e_ms = rep.max_over_ranks(e0.elapsed_time(e1) / e2e_steps)
-    nbytes = lambda x: 0 if x is None else x.numel() * x.element_size()
     h2d = nbytes(xyz_h) + nbytes(t_h) + nbytes(index_h) + nbytes(dout_h)
     d2h = nbytes(out_h) + nbytes(dtable_h)
 
@@ -295,7 +305,11 @@ def run_cuda(args):
                "sample": f"first {n_s} of {N} queries of {args.config}, fwd+bwd once ({sec:.2f} s)"}
 
     value = N * world / (ms_step * 1e-3) / 1e6
-    ws_mb = (nbytes(table) + nbytes(dtable) + nbytes(out) + nbytes(dout) + nbytes(xyz) + nbytes(t)) / 1e6
+    ws_mb = ws_bytes / 1e6
+    l2_note = (f"working set {ws_mb:.0f} MB > 2 x L2 ({l2_bytes / 1e6:.0f} MB): no flush between iterations"
+               if flush is None else
+               f"working set {ws_mb:.0f} MB: a {2 * l2_bytes / 1e6:.0f} MB buffer is written between iterations "
+               f"(outside the timed segments)")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
@@ -304,7 +318,7 @@ def run_cuda(args):
                                f"table {enc.table_dtype}, spatial {enc.res_s_min}->{enc.res_s_max}, "
                                f"temporal {enc.res_t_min}->{enc.res_t_max}; step = zero(dtable)+fwd+bwd",
                    "queries_per_step_per_gpu": N, "parallelism": f"replicas x{world}",
-                   "l2": f"working set {ws_mb:.0f} MB > L2 (126 MB): no flush between iterations",
+                   "l2": l2_note,
                    "zero_grad_fused": bool(args.zero_grad_fused)},
         "roofline": roofline,
         "e2e": {"value": N * world / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": h2d,

@@ -444,3 +444,17 @@ def test_bwd_input_clamped_coordinates_get_zero():
     dout = rng.standard_normal((64, enc.L * enc.F)).astype(np.float32)
     got = run_bwd_input_parity(enc, np.ascontiguousarray(q[:, :3]), np.ascontiguousarray(q[:, 3]), table, dout)
     assert got[0, 0] == 0 and got[1, 1] == 0 and got[2, 2] == 0 and got[3, 3] == 0 and not got[4].any()
+
+
+def test_three_d_special_case_nt1_t0():
+    """G_3D = the 4D kernels with temporal resolution 1 and one timestamp t = 0."""
+    enc = EncoderParams(5, 2, 1 << 12, 4, 64, 1, 1)
+    rng = np.random.default_rng(0)
+    n = 3000
+    xyz, _ = make_queries_uniform(5, n)
+    t0 = np.zeros(1, np.float32)
+    table = rng.uniform(-1, 1, (5, enc.T, 2)).astype(np.float32)
+    dout = rng.standard_normal((n, 10)).astype(np.float32)
+    run_fwd_parity(enc, xyz, t0, table, t_stride=0, what="3d")
+    run_bwd_parity(enc, xyz, t0, dout, t_stride=0, what="3d")
+    run_bwd_input_parity(enc, xyz, t0, table, dout, t_stride=0, what="3d")
