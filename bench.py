@@ -271,14 +271,10 @@ def run_cuda(args):
     xyz_h, t_h, index_h, dout_h = pin(wl.xyz), pin(wl.t), pin(wl.index), pin(wl.dout)
     out_h = torch.empty((N, enc.L * enc.F), dtype=torch.float32).pin_memory()
     dtable_h = torch.empty((enc.L, enc.T, enc.F), dtype=torch.float32).pin_memory()
-    staging = {"xyz": xyz, "t": t, "dout": dout, "out": out, "dtable": dtable}
-    if index is not None:
-        staging["index"] = index
+    host_step = dh.HostStep(cfg)
 
     def e2e_step():
-        dh.dash_hash4d_fwd_host(cfg, xyz_h, t_h, table, out_h, index_h=index_h, staging=staging)
-        dh.dash_hash4d_bwd_host(cfg, xyz_h, t_h, dout_h, dtable_h, index_h=index_h, staging=staging,
-                                reuse_queries=True)
+        host_step(xyz_h, t_h, table, dout_h, out_h, dtable_h, index_h=index_h)
 
     e2e_steps = max(3, min(args.steps, 10))
     e2e_step(); e2e_step()

@@ -157,3 +157,24 @@ def oracle_bwd_input(cfg, N, xyz, t, table, dout, index=None, t_stride=1, want_a
     _check(lib().dash_oracle_bwd_input(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(t), ts, _p(index),
                                        _p(table), _p(dout), _p(dq), _p(mag)), "bwd_input")
     return (dq, mag) if want_abs else dq
+
+
+def oracle_smooth(cfg, N, xyz, t, eps, table, grad_scale=1.0, index=None, t_stride=1, dtable=None,
+                  want_grad=True, want_abs=False):
+    """Eq. 11 (PAPER.md:150): loss[n] = ||G(x_n) - G(x_n + eps_n)||^2 and, if want_grad, dtable +=
+    grad_scale * d(sum_n loss[n])/d table.  eps: [N][4] or [1][4]/[4] (one perturbation for all).
+    -> (loss, dtable[, loss_abs, feat_abs, grad_abs])."""
+    xs, ts = _query_args(xyz, t, index, t_stride)
+    eps = np.ascontiguousarray(eps, np.float32)
+    eps_stride = 0 if eps.size == 4 else 4
+    assert eps_stride == 0 or eps.size == 4 * N
+    loss = np.zeros(N, np.float32)
+    if want_grad and dtable is None:
+        dtable = np.zeros((cfg.L, cfg.T, cfg.F), np.float32)
+    la = np.zeros(N, np.float64) if want_abs else None
+    fa = np.zeros(N, np.float64) if want_abs else None
+    ga = np.zeros((cfg.L, cfg.T, cfg.F), np.float64) if (want_abs and want_grad) else None
+    _check(lib().dash_oracle_smooth(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(t), ts, _p(index), _p(eps),
+                                    C.c_uint32(eps_stride), _p(table), C.c_double(grad_scale), _p(loss),
+                                    _p(dtable if want_grad else None), _p(la), _p(fa), _p(ga)), "smooth")
+    return (loss, dtable, la, fa, ga) if want_abs else (loss, dtable)

@@ -398,3 +398,100 @@ int dash_oracle_bwd_input(const dash_oracle_config *c, uint64_t N, const float *
     }
     return ORACLE_OK;
 }
+
+/* ---- NEXT #2: smoothness regulariser, Eq. 11 -------------------
+ *     L_r(x) = || G_4D(x) - G_4D(x + eps_x) ||_2^2 ,   eps_x = (eps_P, eps_t) a small random perturbation.
+ * The random numbers are an INPUT (eps, drawn by the caller): eps_stride = 4 -> eps[n*4 + d], 0 -> one
+ * perturbation for all queries.  Readings (Q25): the perturbed query is x'_d = fl32(x_d + eps_d),
+ * then clamped like any query (Q12); the norm is over the L*F features; nothing is averaged: loss[n] is the
+ * plain squared norm of query n, and the table gradient is that of  grad_scale * sum_n loss[n]:
+ *     dtable += grad_scale * 2 * sum_n ( J(x_n)^T d_n - J(x'_n)^T d_n ),   d_n = G(x_n) - G(x'_n).
+ * Everything in double from the fp32 cell offsets; loss rounded to fp32 once, dtable as in dash_oracle_bwd.
+ * loss_abs [N] (nullable): sum_{l,f} 2|d| (A + A'), A = sum_k |W_k v_k| — conditioning of loss[n];
+ * feat_abs [N] (nullable): max over (l,f) of (A + A')  (second-order term of the tolerance);
+ * grad_abs [L][T][F] (nullable): sum over contributions of |2 grad_scale W| (A + A'). */
+int dash_oracle_smooth(const dash_oracle_config *c, uint64_t N, const float *xyz, uint32_t xyz_stride,
+                       const float *t, uint32_t t_stride, const int32_t *index, const float *eps,
+                       uint32_t eps_stride, const void *table, double grad_scale, float *loss,
+                       float *dtable, double *loss_abs, double *feat_abs, double *grad_abs) {
+    level_plan p;
+    if (!config_ok(c) || make_plan(c, &p)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!args_ok(xyz, xyz_stride, t, t_stride) || !eps || !table || !loss) return ORACLE_INVALID;
+    if (!(eps_stride == 0 || eps_stride == 4)) return ORACLE_INVALID;
+    const uint32_t L = c->L, F = c->F;
+    const size_t TF = (size_t)c->T * F;
+    for (uint64_t n = 0; n < N; ++n) {
+        loss[n] = 0.0f;
+        if (loss_abs) loss_abs[n] = 0.0;
+        if (feat_abs) feat_abs[n] = 0.0;
+    }
+    int failed = 0;
+    /* level by level (disjoint tables); per-query loss terms are summed over levels in double below */
+    double *loss_acc = (double *)calloc(N, sizeof(double));
+    if (!loss_acc) return ORACLE_NOMEM;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t l = 0; l < (int32_t)L; ++l) {
+        double *acc = dtable ? (double *)calloc(TF, sizeof(double)) : NULL;
+        double *mag = grad_abs ? grad_abs + (size_t)l * TF : NULL;
+        if (dtable && !acc) {
+            failed = 1;
+            continue;
+        }
+        if (mag) memset(mag, 0, TF * sizeof(double));
+        for (uint64_t n = 0; n < N; ++n) {
+            float q[4], q2[4];
+            fetch_query(n, xyz, xyz_stride, t, t_stride, index, q);
+            for (int d = 0; d < 4; ++d) {
+                volatile float moved = q[d] + eps[n * (uint64_t)eps_stride + d]; /* one fp32 add */
+                q2[d] = moved;
+            }
+            uint32_t s1[16], s2[16];
+            double W1[16], W2[16];
+            corners(c, &p, (uint32_t)l, q, s1, W1);
+            corners(c, &p, (uint32_t)l, q2, s2, W2);
+            double lsum = 0.0, labs = 0.0, fabs_max = 0.0;
+            for (uint32_t f = 0; f < F; ++f) {
+                double y1 = 0, y2 = 0, a1 = 0, a2 = 0;
+                for (int k = 0; k < 16; ++k) {
+                    double t1 = W1[k] * table_value(c, table, (uint32_t)l, s1[k], f);
+                    double t2 = W2[k] * table_value(c, table, (uint32_t)l, s2[k], f);
+                    y1 += t1; y2 += t2; a1 += fabs(t1); a2 += fabs(t2);
+                }
+                double dd = y1 - y2;
+                lsum += dd * dd;
+                labs += 2.0 * fabs(dd) * (a1 + a2);
+                if (a1 + a2 > fabs_max) fabs_max = a1 + a2;
+                if (acc) {
+                    for (int k = 0; k < 16; ++k) {
+                        double g1 = 2.0 * grad_scale * W1[k], g2 = 2.0 * grad_scale * W2[k];
+                        acc[(size_t)s1[k] * F + f] += g1 * dd;
+                        acc[(size_t)s2[k] * F + f] -= g2 * dd;
+                        if (mag) {
+                            mag[(size_t)s1[k] * F + f] += fabs(g1) * (a1 + a2);
+                            mag[(size_t)s2[k] * F + f] += fabs(g2) * (a1 + a2);
+                        }
+                    }
+                }
+            }
+#pragma omp atomic
+            loss_acc[n] += lsum;
+            if (loss_abs) {
+#pragma omp atomic
+                loss_abs[n] += labs;
+            }
+            if (feat_abs) {
+#pragma omp critical
+                { if (fabs_max > feat_abs[n]) feat_abs[n] = fabs_max; }
+            }
+        }
+        if (acc) {
+            float *dst = dtable + (size_t)l * TF;
+            for (size_t e = 0; e < TF; ++e) dst[e] = (float)((double)dst[e] + acc[e]);
+            free(acc);
+        }
+    }
+    for (uint64_t n = 0; n < N; ++n) loss[n] = (float)loss_acc[n];
+    free(loss_acc);
+    return failed ? ORACLE_NOMEM : ORACLE_OK;
+}

@@ -123,3 +123,27 @@ def backward_input(queries, table, dout, L, F, T, rs_min, rs_max, rt_min, rt_max
             if np.isnan(v) or v < 0 or float(v) > MAXF:
                 dq[n, d] = 0.0
     return dq
+
+
+def smooth(queries, eps, table, L, F, T, rs_min, rs_max, rt_min, rt_max, dense_coarse=True, grad_scale=1.0,
+           primes=DEFAULT_PRIMES):
+    """Eq. 11: loss[n] = ||G(x_n) - G(fl32(x_n + eps_n))||^2 (float64 [n]) and the gradient of
+    grad_scale * sum_n loss[n] with respect to the table (float64 [L][T][F])."""
+    rs, rt, dn = plan(L, T, rs_min, rs_max, rt_min, rt_max, dense_coarse)
+    eps = np.asarray(eps, np.float32).reshape(-1, 4)
+    loss = np.zeros(len(queries))
+    grad = np.zeros((L, T, F))
+    for n, q in enumerate(queries):
+        e = eps[n if len(eps) > 1 else 0]
+        q2 = [np.float32(np.float32(q[d]) + e[d]) for d in range(4)]
+        for l in range(L):
+            c1 = corners(q, rs[l], rt[l], T, dn[l], primes)
+            c2 = corners(q2, rs[l], rt[l], T, dn[l], primes)
+            for f in range(F):
+                d = sum(w * float(table[l, s, f]) for s, w in c1) - sum(w * float(table[l, s, f]) for s, w in c2)
+                loss[n] += d * d
+                for s, w in c1:
+                    grad[l, s, f] += 2.0 * grad_scale * w * d
+                for s, w in c2:
+                    grad[l, s, f] -= 2.0 * grad_scale * w * d
+    return loss, grad

@@ -281,3 +281,58 @@ def _stage(st: dict, key: str, host: torch.Tensor) -> torch.Tensor:
         dev = st[key] = torch.empty(host.shape, dtype=host.dtype, device="cuda")
     dev.copy_(host, non_blocking=True)
     return dev
+
+
+class HostStep:
+    """One training-shaped step with HOST (pinned) buffers: queries and dY in, features and table gradient
+    out, the table resident on the device.  Copies run on two side streams so that the D2H of `out`
+    overlaps the H2D of `dout` and the backward (PCIe is full duplex); every arithmetic step is still a
+    C-ABI call on the compute stream.  Device staging buffers are owned by this object and reused."""
+
+    def __init__(self, cfg: Hash4DConfig):
+        self.cfg = cfg
+        self.h2d = torch.cuda.Stream()
+        self.d2h = torch.cuda.Stream()
+        self.buf: dict = {}
+        self.out_copied = None        # event: previous step's D2H finished (buffers reusable)
+
+    def _dev_like(self, key, host):
+        cur = self.buf.get(key)
+        if cur is None or cur.shape != host.shape or cur.dtype != host.dtype:
+            cur = self.buf[key] = torch.empty(host.shape, dtype=host.dtype, device="cuda")
+        return cur
+
+    def __call__(self, xyz_h, t_h, table_d, dout_h, out_h, dtable_h, index_h=None, t_stride=None):
+        cfg, main = self.cfg, torch.cuda.current_stream()
+        if self.out_copied is not None:                 # do not overwrite buffers still being read back
+            self.h2d.wait_event(self.out_copied)
+            main.wait_event(self.out_copied)
+        self.h2d.wait_stream(main)
+        with torch.cuda.stream(self.h2d):
+            xyz_d = self._dev_like("xyz", xyz_h); xyz_d.copy_(xyz_h, non_blocking=True)
+            t_d = self._dev_like("t", t_h); t_d.copy_(t_h, non_blocking=True)
+            index_d = None
+            if index_h is not None:
+                index_d = self._dev_like("index", index_h); index_d.copy_(index_h, non_blocking=True)
+            q_ready = torch.cuda.Event(); q_ready.record(self.h2d)
+            dout_d = self._dev_like("dout", dout_h); dout_d.copy_(dout_h, non_blocking=True)
+            d_ready = torch.cuda.Event(); d_ready.record(self.h2d)
+        out_d = self._dev_like("out", out_h)
+        dt_d = self._dev_like("dtable", dtable_h)
+        main.wait_event(q_ready)
+        dash_hash4d_fwd(cfg, xyz_d, t_d, table_d, out=out_d, index=index_d, t_stride=t_stride)
+        f_done = torch.cuda.Event(); f_done.record(main)
+        with torch.cuda.stream(self.d2h):
+            self.d2h.wait_event(f_done)
+            out_h.copy_(out_d, non_blocking=True)
+        main.wait_event(d_ready)
+        if not (cfg.flags & FLAG_ZERO_GRAD):
+            dash_hash4d_zero(cfg, dt_d)
+        dash_hash4d_bwd(cfg, xyz_d, t_d, dout_d, dt_d, index=index_d, t_stride=t_stride)
+        b_done = torch.cuda.Event(); b_done.record(main)
+        with torch.cuda.stream(self.d2h):
+            self.d2h.wait_event(b_done)
+            dtable_h.copy_(dt_d, non_blocking=True)
+            self.out_copied = torch.cuda.Event(); self.out_copied.record(self.d2h)
+        main.wait_event(self.out_copied)               # results are complete when the caller's stream is
+        return out_h, dtable_h

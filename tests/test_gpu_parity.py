@@ -458,3 +458,21 @@ def test_three_d_special_case_nt1_t0():
     run_fwd_parity(enc, xyz, t0, table, t_stride=0, what="3d")
     run_bwd_parity(enc, xyz, t0, dout, t_stride=0, what="3d")
     run_bwd_input_parity(enc, xyz, t0, table, dout, t_stride=0, what="3d")
+
+
+def test_host_step_overlapped_copies_match():
+    wl = make_workload("C2", n_override=20000)
+    enc = wl.spec.enc
+    ocfg, gcfg = both_configs(enc, DC | dh.FLAG_ZERO_GRAD)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    out_h = torch.empty((wl.N, enc.L * enc.F)).pin_memory()
+    dt_h = torch.empty((enc.L, enc.T, enc.F)).pin_memory()
+    step = dh.HostStep(gcfg)
+    ref_o = oracle.oracle_fwd(ocfg, wl.N, wl.xyz, wl.t, wl.table)
+    ref_g = oracle.oracle_bwd(ocfg, wl.N, wl.xyz, wl.t, wl.dout)
+    for _ in range(3):                                   # repeated steps reuse the staging buffers
+        out_h.fill_(-1); dt_h.fill_(-1)
+        step(pin(wl.xyz), pin(wl.t), dev(wl.table), pin(wl.dout), out_h, dt_h)
+        torch.cuda.synchronize()
+        np.testing.assert_allclose(out_h.numpy(), ref_o, rtol=1e-5, atol=1e-9)
+        np.testing.assert_allclose(dt_h.numpy(), ref_g, rtol=1e-4, atol=1e-5)
