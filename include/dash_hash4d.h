@@ -64,7 +64,7 @@ enum dash_hash4d_flags {
 };
 
 enum dash_hash4d_op { DASH_HASH4D_OP_FWD = 0, DASH_HASH4D_OP_BWD = 1, DASH_HASH4D_OP_INDICES = 2,
-                      DASH_HASH4D_OP_BWD_INPUT = 3 };
+                      DASH_HASH4D_OP_BWD_INPUT = 3, DASH_HASH4D_OP_SMOOTH = 4 };
 
 /* Encoder hyper-parameters.  POD, passed by pointer (host memory). */
 typedef struct dash_hash4d_config {
@@ -145,6 +145,29 @@ DASH_API int dash_hash4d_bwd_input(const dash_hash4d_config* cfg, uint64_t N,
                                    const float* dout,
                                    float* dq,
                                    void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Smoothness regulariser, Eq. 11:  L_r = || G_4D(x) - G_4D(x + eps_x) ||_2^2.
+ *   eps        the "small random perturbation" eps_x = (eps_P, eps_t), DRAWN BY THE CALLER: query n reads
+ *              eps[n*eps_stride + d], d = 0..3; eps_stride (in floats) is 4, or 0 for one perturbation shared
+ *              by all queries.  The perturbed query is x'_d = fl32(x_d + eps_d), then clamped like any query.
+ *   loss       [N] fp32, OVERWRITTEN: loss[n] = sum over the L*F features of (G(x_n) - G(x'_n))^2 — the plain
+ *              squared norm, nothing averaged or scaled (reading Q25).
+ *   dtable     nullable; [L][T][F] fp32, ACCUMULATED: += grad_scale * d(sum_n loss[n]) / d table
+ *              = grad_scale * 2 * sum_n (J(x_n)^T d_n - J(x'_n)^T d_n),  d_n = G(x_n) - G(x'_n)
+ *              (pass lambda_r of Eq. 12 as grad_scale; call after dash_hash4d_bwd to add into the same buffer).
+ * One fused pass: where x and x' share a cell (coarse levels, small eps) the 16 corners are gathered once
+ * and scattered once with weight (W - W').  DETERMINISTIC_BWD is not supported here (UNSUPPORTED when
+ * dtable != NULL); ZERO_GRAD is ignored.  Other arguments as in fwd. */
+DASH_API int dash_hash4d_smooth(const dash_hash4d_config* cfg, uint64_t N,
+                                const float* xyz, uint32_t xyz_stride,
+                                const float* t, uint32_t t_stride,
+                                const int32_t* index,
+                                const float* eps, uint32_t eps_stride,
+                                const void* table,
+                                float grad_scale,
+                                float* loss,
+                                float* dtable,
+                                void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Debug: the 16 table slots and interpolation weights of every (query, level)
  * (Eq. 8).  Corner k: bit d of k set => vertex floor(x_d*N_l)+1 along axis d,

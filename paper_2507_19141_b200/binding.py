@@ -17,12 +17,12 @@ FLAG_DENSE_COARSE = 1
 FLAG_DETERMINISTIC_BWD = 2
 FLAG_VALIDATE_INPUTS = 4
 FLAG_ZERO_GRAD = 8
-OP_FWD, OP_BWD, OP_INDICES, OP_BWD_INPUT = 0, 1, 2, 3
+OP_FWD, OP_BWD, OP_INDICES, OP_BWD_INPUT, OP_SMOOTH = 0, 1, 2, 3, 4
 
 _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUDA_ERROR"}
 
 EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4d_fwd",
-           "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
+           "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count"]
 
 
@@ -73,6 +73,8 @@ def _load() -> C.CDLL:
     lib.dash_hash4d_bwd.restype = C.c_int
     lib.dash_hash4d_bwd_input.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp, vp, sz, vp]
     lib.dash_hash4d_bwd_input.restype = C.c_int
+    lib.dash_hash4d_smooth.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, u32, vp, C.c_float, vp, vp, vp, sz, vp]
+    lib.dash_hash4d_smooth.restype = C.c_int
     lib.dash_hash4d_indices.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp]
     lib.dash_hash4d_indices.restype = C.c_int
     lib.dash_hash4d_zero.argtypes = [cfgp, vp, vp]
@@ -218,6 +220,29 @@ def dash_hash4d_bwd_input(cfg, xyz, t, table, dout, dq=None, index=None, t_strid
                                          _ptr(table), _ptr(dout), _ptr(dq), _ptr(workspace), wbytes,
                                          _stream()))
     return dq
+
+
+def dash_hash4d_smooth(cfg, xyz, t, eps, table, grad_scale=1.0, loss=None, dtable=None, index=None,
+                       t_stride=None, N=None, workspace=None):
+    """Eq. 11: loss[n] = ||G(x_n) - G(x_n + eps_n)||^2 ([N] fp32, overwritten) and, if `dtable` is given,
+    dtable += grad_scale * d(sum loss)/d table.  eps: [N][4] CUDA fp32, or 4 values for all queries."""
+    _dev(xyz, torch.float32, "xyz"); _dev(t, torch.float32, "t"); _dev(index, torch.int32, "index")
+    _dev(table, torch.float16 if cfg.table_dtype == 1 else torch.float32, "table")
+    _dev(eps, torch.float32, "eps"); _dev(dtable, torch.float32, "dtable")
+    xs, ts = _strides(xyz, t, t_stride)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    eps_stride = 0 if eps.numel() == 4 else 4
+    if eps_stride and eps.numel() != 4 * N:
+        raise ValueError("eps must hold 4 values, or 4 per query")
+    if loss is None:
+        loss = torch.empty((N,), dtype=torch.float32, device=xyz.device)
+    _dev(loss, torch.float32, "loss")
+    workspace, wbytes = _workspace(cfg, N, OP_SMOOTH, workspace)
+    _check(_load().dash_hash4d_smooth(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index), _ptr(eps),
+                                      eps_stride, _ptr(table), float(grad_scale), _ptr(loss), _ptr(dtable),
+                                      _ptr(workspace), wbytes, _stream()))
+    return loss, dtable
 
 
 def dash_hash4d_indices(cfg, xyz, t, index=None, t_stride=None, N=None, want_weights=True):

@@ -121,7 +121,8 @@ uint32_t env_u32(const char* name) {
 // more than a quarter of the lanes when L is not a multiple of G.  G = 16 (one query per warp) is
 // never picked: every warp would then run both the dense and the hashed index path (measured 7-12 %
 // slower than G = 8 at F = 2).  DASH_HASH4D_{FWD,BWD}_GROUP override G (1..16) for sweeps.
-uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, const char* env_name) {
+uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, const char* env_name,
+                    bool row_sector_rule = true) {
     uint32_t forced = env_u32(env_name);
     if (forced) {
         uint32_t g = 1;
@@ -130,7 +131,7 @@ uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, const c
     }
     const size_t budget = l2_bytes() * 3 / 10;
     uint32_t g_min = 1;
-    while (g_min * c->F * 4 < 32 && g_min < dash::kMaxGroup) g_min *= 2;
+    while (row_sector_rule && g_min * c->F * 4 < 32 && g_min < dash::kMaxGroup) g_min *= 2;
     uint32_t best = 0;
     for (uint32_t g = dash::kMaxGroup / 2; g >= 1; g /= 2) {
         const uint32_t groups = (c->L + g - 1) / g;
@@ -310,6 +311,42 @@ DASH_API int dash_hash4d_bwd_input(const dash_hash4d_config* cfg, uint64_t N, co
     cudaError_t e = dash::launch_zero(dq, static_cast<size_t>(N) * 4 * sizeof(float), s);
     if (e == cudaSuccess) e = dash::launch_bwd_input(P, xyz, t, index, table, half, dout, dq, s);
     if (e != cudaSuccess) return cuda_fail(e, "bwd_input launch");
+    return ok();
+}
+
+DASH_API int dash_hash4d_smooth(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                                uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                                const int32_t* index, const float* eps, uint32_t eps_stride,
+                                const void* table, float grad_scale, float* loss, float* dtable,
+                                void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (int rc = check_config(cfg)) return rc;
+    if (dtable && (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD))
+        return fail(DASH_HASH4D_UNSUPPORTED, "smooth: DETERMINISTIC_BWD is not supported");
+    if (N == 0) return ok();
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
+    if (!eps || !table || !loss) return fail(DASH_HASH4D_INVALID_ARG, "eps, table or loss is NULL");
+    if (!(eps_stride == 0 || eps_stride == 4))
+        return fail(DASH_HASH4D_INVALID_ARG, "eps_stride = %u (want 0 or 4)", eps_stride);
+    if ((reinterpret_cast<uintptr_t>(eps) | reinterpret_cast<uintptr_t>(loss)) & 3u)
+        return fail(DASH_HASH4D_INVALID_ARG, "eps / loss not 4-byte aligned");
+    if (!aligned16(table) || (dtable && !aligned16(dtable)))
+        return fail(DASH_HASH4D_INVALID_ARG, "table / dtable not 16-byte aligned");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const bool half = cfg->table_dtype == DASH_HASH4D_FP16;
+    // a level group keeps its table slice AND (with dtable) its gradient slice in L2; there is no
+    // [N][L*F] row to keep sector-complete, so G may go down to 1
+    const size_t level_bytes =
+        static_cast<size_t>(cfg->T) * cfg->F * ((half ? 2 : 4) + (dtable ? 4 : 0));
+    Plan P;
+    if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
+                           pick_group(cfg, level_bytes, "DASH_HASH4D_SMOOTH_GROUP", false), &P))
+        return rc;
+    if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
+    cudaError_t e = dash::launch_zero(loss, static_cast<size_t>(N) * sizeof(float), s);
+    if (e == cudaSuccess)
+        e = dash::launch_smooth(P, xyz, t, index, eps, eps_stride, table, half, 2.0f * grad_scale,
+                                loss, dtable, s);
+    if (e != cudaSuccess) return cuda_fail(e, "smooth launch");
     return ok();
 }
 

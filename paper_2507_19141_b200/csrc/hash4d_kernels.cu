@@ -47,20 +47,34 @@ __device__ __forceinline__ uint32_t moved_bit(float v, int d) {
     return (v >= 0.0f && v <= 0x1.fffffep-1f) ? 0u : (1u << d);  // NaN fails both comparisons
 }
 
-__device__ __forceinline__ Query load_query(const Plan& P, const LevelParams& lp, uint64_t n,
-                                            const float* __restrict__ xyz,
-                                            const float* __restrict__ t,
-                                            const int32_t* __restrict__ index) {
-    const uint64_t row = index ? static_cast<uint64_t>(__ldg(index + n)) : n;
-    const float* p = xyz + row * P.xyz_stride;
+__device__ __forceinline__ Query make_query(const LevelParams& lp, float x, float y, float z, float tt) {
     Query q;
-    const float x = __ldg(p + 0), y = __ldg(p + 1), z = __ldg(p + 2), tt = __ldg(t + n * P.t_stride);
     locate(x, lp.ns_f, q.c[0], q.w[0]);
     locate(y, lp.ns_f, q.c[1], q.w[1]);
     locate(z, lp.ns_f, q.c[2], q.w[2]);
     locate(tt, lp.nt_f, q.c[3], q.w[3]);
     q.moved = moved_bit(x, 0) | moved_bit(y, 1) | moved_bit(z, 2) | moved_bit(tt, 3);
     return q;
+}
+
+__device__ __forceinline__ void load_coords(const Plan& P, uint64_t n, const float* __restrict__ xyz,
+                                            const float* __restrict__ t,
+                                            const int32_t* __restrict__ index, float c[4]) {
+    const uint64_t row = index ? static_cast<uint64_t>(__ldg(index + n)) : n;
+    const float* p = xyz + row * P.xyz_stride;
+    c[0] = __ldg(p + 0);
+    c[1] = __ldg(p + 1);
+    c[2] = __ldg(p + 2);
+    c[3] = __ldg(t + n * P.t_stride);
+}
+
+__device__ __forceinline__ Query load_query(const Plan& P, const LevelParams& lp, uint64_t n,
+                                            const float* __restrict__ xyz,
+                                            const float* __restrict__ t,
+                                            const int32_t* __restrict__ index) {
+    float c[4];
+    load_coords(P, n, xyz, t, index, c);
+    return make_query(lp, c[0], c[1], c[2], c[3]);
 }
 
 // The 8 (y,z,t) corners that share x-corner `xc` (0: floor, 1: floor+1).  Corner j: bit0 = y, bit1 =
@@ -411,6 +425,117 @@ hash4d_bwd_input_kernel(const __grid_constant__ Plan P, const float* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------
+// Smoothness regulariser, Eq. 11 (Q25):
+//     loss[n] = || G(x_n) - G(x'_n) ||^2 ,  x' = fl32(x + eps),   dtable += 2*scale*(J(x)^T d - J(x')^T d).
+// One pass per (query, level): gather the cell of x; if x' falls in the SAME cell (the common case on
+// coarse levels for a small eps) its 16 corners are the same slots, so the difference is formed directly
+// as sum (W - W') v — no second gather, no cancellation between two large sums — and the scatter is ONE
+// reduction per corner with weight (W - W') instead of two.  Only items whose cell differs pay the second
+// gather and the second set of reductions.
+// ------------------------------------------------------------------------------------------------
+template <int F, bool HALF, bool GRAD>
+__global__ void __launch_bounds__(kBlockThreads)
+hash4d_smooth_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
+                     const float* __restrict__ t, const int32_t* __restrict__ index,
+                     const float* __restrict__ eps, uint32_t eps_stride,
+                     const void* __restrict__ table, float two_scale, float* __restrict__ loss,
+                     float* __restrict__ dtable) {
+    const Item it = this_item(P);
+    const LevelParams lp = P.lv[it.l];
+    float c[4];
+    load_coords(P, it.n, xyz, t, index, c);
+    const float* e = eps + it.n * eps_stride;
+    const Query q1 = make_query(lp, c[0], c[1], c[2], c[3]);
+    const Query q2 = make_query(lp, __fadd_rn(c[0], __ldg(e + 0)), __fadd_rn(c[1], __ldg(e + 1)),
+                                __fadd_rn(c[2], __ldg(e + 2)), __fadd_rn(c[3], __ldg(e + 3)));
+    uint32_t s1[8], s2[8];
+    float W1[8], W2[8];
+    half_cell(P, lp, q1, it.xc, s1, W1);
+    half_cell(P, lp, q2, it.xc, s2, W2);
+    const bool same = q1.c[0] == q2.c[0] && q1.c[1] == q2.c[1] && q1.c[2] == q2.c[2] &&
+                      q1.c[3] == q2.c[3];  // identical for both lanes of the pair
+
+    constexpr size_t kElem = HALF ? 2 : 4;
+    const char* level_base =
+        static_cast<const char*>(table) + static_cast<size_t>(it.l) * P.T * (F * kElem);
+    float d[F];
+    {
+        float v[8][F];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, s1[j], v[j]);
+        float y[F], ds[F];
+#pragma unroll
+        for (int f = 0; f < F; ++f) y[f] = ds[f] = 0.0f;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const float dw = W1[j] - W2[j];
+#pragma unroll
+            for (int f = 0; f < F; ++f) {
+                y[f] = fmaf(W1[j], v[j][f], y[f]);
+                ds[f] = fmaf(dw, v[j][f], ds[f]);
+            }
+        }
+        if (same) {
+#pragma unroll
+            for (int f = 0; f < F; ++f) d[f] = ds[f];
+        } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, s2[j], v[j]);
+#pragma unroll
+            for (int j = 0; j < 8; ++j)
+#pragma unroll
+                for (int f = 0; f < F; ++f) y[f] = fmaf(-W2[j], v[j][f], y[f]);
+#pragma unroll
+            for (int f = 0; f < F; ++f) d[f] = y[f];
+        }
+    }
+#pragma unroll
+    for (int f = 0; f < F; ++f) d[f] += __shfl_xor_sync(0xffffffffu, d[f], 1);  // both x-corners
+
+    // loss: sum_f d^2, once per item (lane xc = 0), summed over the G levels of the query in this warp
+    float lsum = 0.0f;
+    if (it.active && it.xc == 0) {
+#pragma unroll
+        for (int f = 0; f < F; ++f) lsum = fmaf(d[f], d[f], lsum);
+    }
+    const uint32_t span = 2u * P.group;
+#pragma unroll
+    for (uint32_t o = 1; o < 32; o <<= 1)
+        if (o < span) lsum += __shfl_xor_sync(0xffffffffu, lsum, o);
+    if (it.active && (threadIdx.x & (span - 1u)) == 0)
+        asm volatile("red.global.add.f32 [%0], %1;" ::"l"(loss + it.n), "f"(lsum) : "memory");
+
+    if constexpr (GRAD) {
+        if (!it.active) return;
+        float* gbase = dtable + static_cast<size_t>(it.l) * P.T * F;
+        float g[F];
+#pragma unroll
+        for (int f = 0; f < F; ++f) g[f] = two_scale * d[f];
+        if (same) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const float dw = W1[j] - W2[j];
+                float cc[F];
+#pragma unroll
+                for (int f = 0; f < F; ++f) cc[f] = dw * g[f];
+                red_add<F>(gbase + static_cast<size_t>(s1[j]) * F, cc);
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                float cc[F];
+#pragma unroll
+                for (int f = 0; f < F; ++f) cc[f] = W1[j] * g[f];
+                red_add<F>(gbase + static_cast<size_t>(s1[j]) * F, cc);
+#pragma unroll
+                for (int f = 0; f < F; ++f) cc[f] = -W2[j] * g[f];
+                red_add<F>(gbase + static_cast<size_t>(s2[j]) * F, cc);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Debug: all 16 slots + weights per (query, level)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlockThreads)
@@ -576,6 +701,40 @@ cudaError_t launch_bwd_input(const Plan& P, const float* xyz, const float* t, co
     }
 #undef DASH_BWI
     return after_launch();
+}
+
+template <int F, bool HALF>
+static cudaError_t launch_smooth_t(const Plan& P, const float* xyz, const float* t,
+                                   const int32_t* index, const float* eps, uint32_t eps_stride,
+                                   const void* table, float two_scale, float* loss, float* dtable,
+                                   cudaStream_t s) {
+    const dim3 grid = item_grid(P), block(kBlockThreads);
+    if (dtable)
+        hash4d_smooth_kernel<F, HALF, true><<<grid, block, 0, s>>>(P, xyz, t, index, eps, eps_stride,
+                                                                   table, two_scale, loss, dtable);
+    else
+        hash4d_smooth_kernel<F, HALF, false><<<grid, block, 0, s>>>(P, xyz, t, index, eps, eps_stride,
+                                                                    table, two_scale, loss, dtable);
+    return after_launch();
+}
+
+cudaError_t launch_smooth(const Plan& P, const float* xyz, const float* t, const int32_t* index,
+                          const float* eps, uint32_t eps_stride, const void* table, bool table_half,
+                          float two_scale, float* loss, float* dtable, cudaStream_t s) {
+#define DASH_SM(FV, HV) \
+    return launch_smooth_t<FV, HV>(P, xyz, t, index, eps, eps_stride, table, two_scale, loss, dtable, s)
+    switch (P.F * 2 + (table_half ? 1 : 0)) {
+        case 2: DASH_SM(1, false);
+        case 3: DASH_SM(1, true);
+        case 4: DASH_SM(2, false);
+        case 5: DASH_SM(2, true);
+        case 8: DASH_SM(4, false);
+        case 9: DASH_SM(4, true);
+        case 16: DASH_SM(8, false);
+        case 17: DASH_SM(8, true);
+        default: return cudaErrorInvalidValue;
+    }
+#undef DASH_SM
 }
 
 cudaError_t launch_bwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,

@@ -476,3 +476,99 @@ def test_host_step_overlapped_copies_match():
         torch.cuda.synchronize()
         np.testing.assert_allclose(out_h.numpy(), ref_o, rtol=1e-5, atol=1e-9)
         np.testing.assert_allclose(dt_h.numpy(), ref_g, rtol=1e-4, atol=1e-5)
+
+
+# ----------------------------------------------------------------------------------------------------
+# NEXT #2: smoothness regulariser, Eq. 11 (Q25)
+# ----------------------------------------------------------------------------------------------------
+
+def run_smooth_parity(enc, xyz, t, eps, table, index=None, t_stride=1, flags=DC, grad_scale=0.7, what="",
+                      with_grad=True, use_init=True, max_hits=0):
+    ocfg, gcfg = both_configs(enc, flags)
+    N = len(index) if index is not None else (len(t) if t_stride else len(xyz))
+    L, F, T = enc.L, enc.F, enc.T
+    # accumulate semantics: start from a non-zero gradient.  (Not in the degenerate case where ~1000 tiny
+    # terms are added to one slot: each fp32 add then rounds at the ulp of the large start value, an error
+    # of hits * 2^-24 * |init| that has nothing to do with the regulariser.)
+    init = np.random.default_rng(1).standard_normal((L, T, F)).astype(np.float32) * (1e-3 if use_init else 0)
+    ref_l, ref_g, la, fa, ga = oracle.oracle_smooth(ocfg, N, xyz, t, eps, table, grad_scale=grad_scale,
+                                                   index=index, t_stride=t_stride, dtable=init.copy(),
+                                                   want_grad=True, want_abs=True)
+    loss = torch.full((N,), 5.0, device="cuda")                       # garbage: must be overwritten
+    dt = dev(init) if with_grad else None
+    dh.dash_hash4d_smooth(gcfg, dev(xyz), dev(t), dev(eps), dev(table), grad_scale=grad_scale, loss=loss,
+                          dtable=dt, index=dev(index), t_stride=t_stride, N=N)
+    torch.cuda.synchronize()
+    got_l = loss.cpu().numpy().astype(np.float64)
+    assert np.isfinite(got_l).all()
+    # |d| is a difference of two interpolants: its fp32 error is relative to A + A' (oracle's feat_abs),
+    # so the loss tolerance has the first-order term 2|d| err(d) (loss_abs) and the second-order err(d)^2
+    allow = RTOL_FP32 * la + L * F * (RTOL_FP32 * fa) ** 2 + 1e-30
+    err = np.abs(got_l - ref_l)
+    assert (err <= allow).all(), f"{what} smooth loss: worst {np.max(err / allow):.2f} x tolerance"
+    assert abs(got_l.sum() - ref_l.astype(np.float64).sum()) <= RTOL_FP32 * la.sum() + 1e-30
+    if with_grad:
+        got_g = dt.cpu().numpy().astype(np.float64)
+        errg = np.abs(got_g - ref_g)
+        # max_hits: worst-case recursive-summation term (n-1) * 2^-24 * sum|terms| for slots that receive
+        # ~max_hits same-sign fp32 reductions (degenerate inputs only; 0 elsewhere)
+        allow_g = (RTOL_FP32 + max_hits * 2.0 ** -24) * (ga + np.abs(init)) + 1e-30
+        worst = np.unravel_index(np.argmax(errg / allow_g), errg.shape)
+        assert (errg <= allow_g).all(), (f"{what} smooth grad: worst {np.max(errg / allow_g):.2f} x tolerance at "
+                                         f"{worst}: got {got_g[worst]:.6e} ref {ref_g[worst]:.6e} A {ga[worst]:.3e}")
+        for l in range(L):
+            num = np.linalg.norm(got_g[l] - ref_g[l]); den = np.linalg.norm(ref_g[l] - init[l])
+            assert num <= (1e-4 + max_hits * 2.0 ** -24) * den + 1e-12, f"{what} smooth grad level {l}: {num / max(den, 1e-300):.2e}"
+    return got_l
+
+
+@pytest.mark.parametrize("name,scale", [("C1", 1e-3), ("C2", 1e-3), ("C2", 3e-2), ("C4", 5e-4), ("C5", 2e-3)])
+def test_smooth_configs(name, scale):
+    n_over = {"C2": 30_000, "C4": 100_000, "C5": 100_000}.get(name)
+    wl = make_workload(name, n_override=n_over, with_dout=False)
+    eps = np.random.default_rng(9).uniform(-scale, scale, (wl.N, 4)).astype(np.float32)
+    run_smooth_parity(wl.spec.enc, wl.xyz, wl.t, eps, (wl.table.astype(np.float32) * 1e4).astype(wl.table.dtype),
+                      index=wl.index, what=f"{name} eps={scale}")
+
+
+@pytest.mark.parametrize("L,F,T,rs,rt,dtype,N", VARIANTS)
+def test_smooth_variants(L, F, T, rs, rt, dtype, N):
+    enc = EncoderParams(L, F, T, rs[0], rs[1], rt[0], rt[1], dtype)
+    rng = np.random.default_rng(L * 10 + F)
+    xyz, t = make_queries_uniform(L + 3 * F, N)
+    eps = rng.uniform(-4e-3, 4e-3, (N, 4)).astype(np.float32)
+    table = rng.uniform(-1, 1, (L, T, F)).astype(np.float16 if dtype == "fp16" else np.float32)
+    run_smooth_parity(enc, xyz, t, eps, table)
+    run_smooth_parity(enc, xyz, t, eps, table, flags=0, with_grad=False)
+
+
+@pytest.mark.parametrize("group", [1, 2, 4, 8, 16])
+def test_smooth_group_sizes_shared_eps_and_degenerate(group, monkeypatch):
+    monkeypatch.setenv("DASH_HASH4D_SMOOTH_GROUP", str(group))
+    enc = EncoderParams(12, 2, 1 << 14, 16, 1024, 8, 100)
+    rng = np.random.default_rng(group)
+    rows = rng.random((300, 3), dtype=np.float32)
+    index = rng.integers(0, 300, 999).astype(np.int32)
+    t = rng.random(999, dtype=np.float32)
+    table = rng.uniform(-1, 1, (12, enc.T, 2)).astype(np.float32)
+    run_smooth_parity(enc, rows, t, rng.uniform(-2e-3, 2e-3, (999, 4)).astype(np.float32), table, index=index,
+                      what="per-query eps")
+    run_smooth_parity(enc, rows, t, np.array([1e-3, -2e-3, 5e-4, 1e-3], np.float32), table, index=index,
+                      what="shared eps")
+    got = run_smooth_parity(enc, rows, t, np.zeros((999, 4), np.float32), table, index=index, what="eps=0")
+    assert not got.any()                                            # eps = 0: loss exactly 0
+    run_smooth_parity(enc, rows, t, np.full((999, 4), 5.0, np.float32), table, index=index, what="clamped",
+                      use_init=False, max_hits=999)
+    run_smooth_parity(enc, rows, np.array([0.3], np.float32), np.array([1e-3, 0, 0, 2e-3], np.float32), table,
+                      index=index, t_stride=0, what="broadcast t")
+
+
+def test_smooth_rejects_deterministic_flag():
+    enc = CONFIGS["C1"].enc
+    _, gcfg = both_configs(enc, DC | dh.FLAG_DETERMINISTIC_BWD)
+    xyz, t = make_queries_uniform(0, 16)
+    with pytest.raises(dh.Hash4DError) as ei:
+        dh.dash_hash4d_smooth(gcfg, dev(xyz), dev(t), dev(np.zeros(4, np.float32)),
+                              dev(np.zeros((enc.L, enc.T, enc.F), np.float32)),
+                              dtable=torch.zeros((enc.L, enc.T, enc.F), device="cuda"))
+    assert ei.value.status == 2
