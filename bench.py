@@ -289,6 +289,35 @@ def run_cuda(args):
     h2d = nbytes(xyz_h) + nbytes(t_h) + nbytes(index_h) + nbytes(dout_h)
     d2h = nbytes(out_h) + nbytes(dtable_h)
 
+    # ---- extras (information only, not part of the metric): the NEXT-row calls on the same workload
+    extras = None
+    if args.extras:
+        def timed(fn, iters=10):
+            fn(); fn()
+            torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record()
+            for _ in range(iters):
+                fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / iters
+        dq = torch.empty((N, 4), dtype=torch.float32, device="cuda")
+        loss = torch.empty((N,), dtype=torch.float32, device="cuda")
+        cfg_acc = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE)
+        gen = torch.Generator(device="cuda"); gen.manual_seed(1234)
+        extras = {"bwd_input_ms": timed(lambda: dh.dash_hash4d_bwd_input(cfg, xyz, t, table, dout, dq=dq,
+                                                                           index=index))}
+        for delta in (1e-4, 1e-3, 1e-2):
+            eps = (torch.rand((N, 4), device="cuda", generator=gen) * 2 - 1) * delta
+            extras[f"smooth_loss+grad_ms(eps=U(-{delta:g},{delta:g}))"] = timed(
+                lambda: dh.dash_hash4d_smooth(cfg_acc, xyz, t, eps, table, grad_scale=0.1, loss=loss,
+                                              dtable=dtable, index=index))
+        extras["smooth_unfused_equivalent_ms"] = 2 * (ms_fwd + ms_bwd)
+        one_t = t[:1].contiguous()
+        extras["fwd_one_timestamp_ms"] = timed(lambda: dh.dash_hash4d_fwd(cfg, xyz, one_t, table, out=out,
+                                                                           index=index, t_stride=0))
+
     if not rep.is_reporter:
         rep.close()
         return 0
@@ -324,6 +353,8 @@ def run_cuda(args):
     }
     if cpu is not None:
         line["cpu_baseline"] = cpu
+    if extras is not None:
+        line["extras"] = extras
     print(json.dumps(line), flush=True)
     rep.close()
     return 0
@@ -339,6 +370,8 @@ def main():
     ap.add_argument("--zero-grad-fused", type=int, default=1,
                     help="1: bwd zeroes each level group itself (DASH_HASH4D_FLAG_ZERO_GRAD)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extras", type=int, default=1,
+                    help="1: also time bwd_input / smooth / one-timestamp fwd (information only)")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), else null")
     args = ap.parse_args()
