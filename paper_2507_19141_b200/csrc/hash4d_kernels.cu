@@ -117,6 +117,11 @@ __device__ __forceinline__ void half_cell(const Plan& P, const LevelParams& lp, 
 // Table slot access
 // ------------------------------------------------------------------------------------------------
 
+// 8-byte table gather: ld.global.nc with default L1 allocation.  Measured alternatives on C4/C3/C5
+// (profiles/sorted_and_tma_experiments_r01.md §3): L1::no_allocate +41 %/+12 %/+28 % time, ld.global.cg
+// +3 %/+1 %/+5 %, L1::evict_last +-1 %.
+__device__ __forceinline__ uint2 gather8(const void* p) { return __ldg(static_cast<const uint2*>(p)); }
+
 template <int F, bool HALF>
 __device__ __forceinline__ void load_slot(const void* __restrict__ level_base, uint32_t slot,
                                           float v[F]) {
@@ -125,8 +130,8 @@ __device__ __forceinline__ void load_slot(const void* __restrict__ level_base, u
         if constexpr (F == 1) {
             v[0] = __ldg(p);
         } else if constexpr (F == 2) {
-            const float2 a = __ldg(reinterpret_cast<const float2*>(p));
-            v[0] = a.x; v[1] = a.y;
+            const uint2 raw = gather8(p);
+            v[0] = __uint_as_float(raw.x); v[1] = __uint_as_float(raw.y);
         } else if constexpr (F == 4) {
             const float4 a = __ldg(reinterpret_cast<const float4*>(p));
             v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
@@ -146,7 +151,7 @@ __device__ __forceinline__ void load_slot(const void* __restrict__ level_base, u
             const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&raw));
             v[0] = a.x; v[1] = a.y;
         } else if constexpr (F == 4) {
-            const uint2 raw = __ldg(reinterpret_cast<const uint2*>(p));
+            const uint2 raw = gather8(p);
             const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&raw.x));
             const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&raw.y));
             v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
