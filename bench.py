@@ -35,6 +35,7 @@ from dash_inputs import CONFIGS, make_workload  # noqa: E402
 METRIC = "4d_hash_encode_fwd_bwd_mqueries_per_s"
 UNIT = "Mqueries/s"
 REFERENCE_SAMPLE_QUERIES = 100_000     # per step of --impl reference
+REFERENCE_BUDGET_SECONDS = 240.0       # --impl reference stops timing further steps after this long
 CPU_BASELINE_QUERIES = 500_000         # bounded sample of the cpu_baseline leg (~10 s of CPU work)
 
 
@@ -141,22 +142,27 @@ def run_reference(args):
     wl = make_workload(args.config)
     times = []
     n = threads = 0
+    began = time.perf_counter()
     for i in range(args.warmup + args.steps):
         sec, n, threads = time_oracle(wl, REFERENCE_SAMPLE_QUERIES)
         if i >= args.warmup:
             times.append(sec)
+        # the oracle is deliberately slow: never let this arm run longer than a few minutes
+        if times and time.perf_counter() - began > REFERENCE_BUDGET_SECONDS:
+            break
     sec = sum(times) / len(times)
     value = n / sec / 1e6
     enc = wl.spec.enc
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "steps": len(times), "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "steps_requested": args.steps,
         "config": {"workload": f"{args.config}: first {n} of {wl.N} queries per step, L={enc.L} F={enc.F} "
                                f"T=2^{enc.T.bit_length() - 1} table {enc.table_dtype}",
                    "queries_per_step": n},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
-                         "sample": f"first {n} queries of {args.config}, fwd+bwd, mean of {args.steps} steps"},
+                         "sample": f"first {n} queries of {args.config}, fwd+bwd, mean of {len(times)} steps"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -363,8 +369,8 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=None, help="default 200 (cuda arm) / 10 (reference arm)")
+    ap.add_argument("--warmup", type=int, default=None, help="default 20 (cuda arm) / 2 (reference arm)")
     ap.add_argument("--config", default="C4", choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--zero-grad-fused", type=int, default=1,
@@ -375,6 +381,10 @@ def main():
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), else null")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = 10 if args.impl == "reference" else 200
+    if args.warmup is None:
+        args.warmup = 2 if args.impl == "reference" else 20
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)
