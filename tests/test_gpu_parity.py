@@ -572,3 +572,40 @@ def test_smooth_rejects_deterministic_flag():
                               dev(np.zeros((enc.L, enc.T, enc.F), np.float32)),
                               dtable=torch.zeros((enc.L, enc.T, enc.F), device="cuda"))
     assert ei.value.status == 2
+
+
+def test_calls_are_cuda_graph_capturable():
+    """The library only enqueues kernels on the caller's stream (no allocation, no sync), so a whole
+    step can be captured once and replayed — the launch-bound small configs (C1/C2) are run that way."""
+    wl = make_workload("C2", n_override=20000)
+    enc = wl.spec.enc
+    ocfg, gcfg = both_configs(enc, DC | dh.FLAG_ZERO_GRAD)
+    xyz, t, table, dout = dev(wl.xyz), dev(wl.t), dev(wl.table), dev(wl.dout)
+    out = torch.empty((wl.N, enc.L * enc.F), device="cuda")
+    dt = torch.empty((enc.L, enc.T, enc.F), device="cuda")
+    dq = torch.empty((wl.N, 4), device="cuda")
+
+    def step():
+        dh.dash_hash4d_fwd(gcfg, xyz, t, table, out=out)
+        dh.dash_hash4d_bwd(gcfg, xyz, t, dout, dt)
+        dh.dash_hash4d_bwd_input(gcfg, xyz, t, table, dout, dq=dq)
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()                                           # warm-up outside capture
+    torch.cuda.current_stream().wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        step()
+    out.fill_(-1); dt.fill_(-1); dq.fill_(-1)
+    for _ in range(2):
+        graph.replay()
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(out.cpu().numpy(), oracle.oracle_fwd(ocfg, wl.N, wl.xyz, wl.t, wl.table),
+                               rtol=1e-5, atol=1e-9)
+    np.testing.assert_allclose(dt.cpu().numpy(), oracle.oracle_bwd(ocfg, wl.N, wl.xyz, wl.t, wl.dout),
+                               rtol=1e-4, atol=1e-5)
+    np.testing.assert_allclose(dq.cpu().numpy(),
+                               oracle.oracle_bwd_input(ocfg, wl.N, wl.xyz, wl.t, wl.table, wl.dout),
+                               rtol=1e-3, atol=1e-5)
