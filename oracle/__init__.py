@@ -178,3 +178,56 @@ def oracle_smooth(cfg, N, xyz, t, eps, table, grad_scale=1.0, index=None, t_stri
                                     C.c_uint32(eps_stride), _p(table), C.c_double(grad_scale), _p(loss),
                                     _p(dtable if want_grad else None), _p(la), _p(fa), _p(ga)), "smooth")
     return (loss, dtable, la, fa, ga) if want_abs else (loss, dtable)
+
+
+# ---- G_3D (Eq. 3; Q26) ----
+
+def _point_args(xyz, index):
+    assert xyz.dtype == np.float32 and xyz.ndim == 2 and xyz.shape[1] in (3, 4) and xyz.flags.c_contiguous
+    if index is not None:
+        assert index.dtype == np.int32 and index.flags.c_contiguous
+    return C.c_uint32(xyz.shape[1])
+
+
+def oracle3d_resolutions(cfg: OracleConfig):
+    rs, dn = np.zeros(cfg.L, np.uint32), np.zeros(cfg.L, np.uint8)
+    _check(lib().dash_oracle3d_resolutions(C.byref(cfg), _p(rs), _p(dn)), "3d resolutions")
+    return rs, dn.astype(bool)
+
+
+def oracle3d_indices(cfg, N, xyz, index=None, want_weights=True):
+    xs = _point_args(xyz, index)
+    idx = np.zeros((N, cfg.L, 8), np.uint32)
+    w = np.zeros((N, cfg.L, 8), np.float64) if want_weights else None
+    _check(lib().dash_oracle3d_indices(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(index), _p(idx), _p(w)),
+           "3d indices")
+    return idx, w
+
+
+def oracle3d_fwd(cfg, N, xyz, table, index=None, want_abs=False):
+    xs = _point_args(xyz, index)
+    want = np.float16 if cfg.table_dtype == 1 else np.float32
+    assert table.dtype == want and table.flags.c_contiguous and table.size == cfg.L * cfg.T * cfg.F
+    out = np.zeros((N, cfg.L * cfg.F), np.float32)
+    mag = np.zeros((N, cfg.L * cfg.F), np.float64) if want_abs else None
+    _check(lib().dash_oracle3d_fwd(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(index), _p(table), _p(out),
+                                   _p(mag)), "3d fwd")
+    return (out, mag) if want_abs else out
+
+
+def oracle3d_bwd(cfg, N, xyz, dout, index=None, dtable=None, want_abs=False, want_hits=False):
+    xs = _point_args(xyz, index)
+    assert dout.dtype == np.float32 and dout.flags.c_contiguous and dout.size == N * cfg.L * cfg.F
+    if dtable is None:
+        dtable = np.zeros((cfg.L, cfg.T, cfg.F), np.float32)
+    assert dtable.dtype == np.float32 and dtable.flags.c_contiguous
+    mag = np.zeros((cfg.L, cfg.T, cfg.F), np.float64) if want_abs else None
+    hits = np.zeros((cfg.L, cfg.T), np.uint32) if want_hits else None
+    _check(lib().dash_oracle3d_bwd(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(index), _p(dout), _p(dtable),
+                                   _p(mag), _p(hits)), "3d bwd")
+    res = [dtable]
+    if want_abs:
+        res.append(mag)
+    if want_hits:
+        res.append(hits)
+    return res[0] if len(res) == 1 else tuple(res)

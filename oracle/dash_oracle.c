@@ -495,3 +495,177 @@ int dash_oracle_smooth(const dash_oracle_config *c, uint64_t N, const float *xyz
     free(loss_acc);
     return failed ? ORACLE_NOMEM : ORACLE_OK;
 }
+
+/* ---- NEXT #4: the 3D hash encoder G_3D of the decomposition stage -------------------
+ * PAPER.md:97-101, Eq. 3: "we extract spatial features f_3D using a 3D hash encoder G_3D from Instant-NGP
+ * [25]".  The paper gives no separate definition, so G_3D is Eq. 7-9 with d = 3 (Q26): the
+ * spatial resolution schedule Ns_l of Eq. 7, cell floor(p * Ns_l) per axis (one binary32 multiply, Q4),
+ * the 8 vertices of the cell (corner k: bit d set => +1 along d, d = 0:x 1:y 2:z), Eq. 8 over three
+ * coordinates with pi_1..pi_3, trilinear weights, levels concatenated to R^{LF}.  A level is dense iff
+ * (Ns+1)^3 <= T (the d = 3 form of Q10), dense index gx + S(gy + S gz), S = Ns+1.  The temporal fields of
+ * the config are ignored.  Precision as in the 4D functions: weights and sums in double, rounded once. */
+
+static int config3_ok(const dash_oracle_config *c) {
+    if (!c || c->struct_size != sizeof(dash_oracle_config)) return 0;
+    if (c->L < 1 || c->L > ORACLE_MAX_L) return 0;
+    if (!(c->F == 1 || c->F == 2 || c->F == 4 || c->F == 8)) return 0;
+    if (c->T < 1) return 0;
+    if (c->res_s_min < 1 || c->res_s_min > c->res_s_max) return 0;
+    if (c->table_dtype > 1) return 0;
+    return 1;
+}
+
+static int level3_is_dense(const dash_oracle_config *c, uint32_t ns) {
+    if (!(c->flags & 1u)) return 0;
+    long double v = (long double)(ns + 1.0L) * (ns + 1.0L) * (ns + 1.0L);
+    return v <= (long double)c->T;
+}
+
+int dash_oracle3d_resolutions(const dash_oracle_config *c, uint32_t *res_s, uint8_t *is_dense) {
+    if (!config3_ok(c) || !res_s) return ORACLE_INVALID;
+    for (uint32_t l = 0; l < c->L; ++l) {
+        res_s[l] = level_resolution(c->res_s_min, c->res_s_max, l, c->L);
+        if (is_dense) is_dense[l] = (uint8_t)level3_is_dense(c, res_s[l]);
+    }
+    return ORACLE_OK;
+}
+
+/* the 8 slots and 8 trilinear weights of point p at a level of resolution ns */
+static void corners3(const dash_oracle_config *c, const uint32_t pi[4], uint32_t ns, int dense,
+                     const float p[3], uint32_t slot[8], double W[8]) {
+    uint32_t cell[3];
+    float frac[3];
+    for (int d = 0; d < 3; ++d) locate(clamp_unit(p[d]), ns, &cell[d], &frac[d]);
+    for (int k = 0; k < 8; ++k) {
+        uint32_t g[3];
+        double w = 1.0;
+        for (int d = 0; d < 3; ++d) {
+            int up = (k >> d) & 1;
+            g[d] = cell[d] + (uint32_t)up;
+            w *= up ? (double)frac[d] : 1.0 - (double)frac[d];
+        }
+        if (dense) {
+            uint32_t S = ns + 1u;
+            slot[k] = g[0] + S * (g[1] + S * g[2]);
+        } else {
+            uint32_t h = 0;
+            for (int d = 0; d < 3; ++d) h ^= g[d] * pi[d]; /* Eq. 8 with d = 3, uint32 wraparound */
+            slot[k] = h % c->T;
+        }
+        W[k] = w;
+    }
+}
+
+static void fetch_point(uint64_t n, const float *xyz, uint32_t xyz_stride, const int32_t *index,
+                        float p[3]) {
+    uint64_t row = index ? (uint64_t)index[n] : n;
+    for (int d = 0; d < 3; ++d) p[d] = xyz[row * xyz_stride + d];
+}
+
+/* idx_out [N][L][8] u32; w_out [N][L][8] double (nullable). */
+int dash_oracle3d_indices(const dash_oracle_config *c, uint64_t N, const float *xyz,
+                          uint32_t xyz_stride, const int32_t *index, uint32_t *idx_out,
+                          double *w_out) {
+    uint32_t res[ORACLE_MAX_L], pi[4];
+    uint8_t dn[ORACLE_MAX_L];
+    if (dash_oracle3d_resolutions(c, res, dn)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!xyz || !(xyz_stride == 3 || xyz_stride == 4) || !idx_out) return ORACLE_INVALID;
+    get_primes(c, pi);
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < (int64_t)N; ++n) {
+        float p[3];
+        fetch_point((uint64_t)n, xyz, xyz_stride, index, p);
+        for (uint32_t l = 0; l < c->L; ++l) {
+            uint32_t slot[8];
+            double W[8];
+            corners3(c, pi, res[l], dn[l], p, slot, W);
+            size_t base = ((size_t)n * c->L + l) * 8;
+            for (int k = 0; k < 8; ++k) {
+                idx_out[base + k] = slot[k];
+                if (w_out) w_out[base + k] = W[k];
+            }
+        }
+    }
+    return ORACLE_OK;
+}
+
+/* out[n][l*F+f] = sum_{k<8} W_k * table[l][slot_k][f]; out_abs (nullable): sum |terms|. */
+int dash_oracle3d_fwd(const dash_oracle_config *c, uint64_t N, const float *xyz, uint32_t xyz_stride,
+                      const int32_t *index, const void *table, float *out, double *out_abs) {
+    uint32_t res[ORACLE_MAX_L], pi[4];
+    uint8_t dn[ORACLE_MAX_L];
+    if (dash_oracle3d_resolutions(c, res, dn)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!xyz || !(xyz_stride == 3 || xyz_stride == 4) || !table || !out) return ORACLE_INVALID;
+    get_primes(c, pi);
+    const uint32_t L = c->L, F = c->F;
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < (int64_t)N; ++n) {
+        float p[3];
+        fetch_point((uint64_t)n, xyz, xyz_stride, index, p);
+        for (uint32_t l = 0; l < L; ++l) {
+            uint32_t slot[8];
+            double W[8];
+            corners3(c, pi, res[l], dn[l], p, slot, W);
+            for (uint32_t f = 0; f < F; ++f) {
+                double acc = 0.0, mag = 0.0;
+                for (int k = 0; k < 8; ++k) {
+                    double term = W[k] * table_value(c, table, l, slot[k], f);
+                    acc += term;
+                    mag += fabs(term);
+                }
+                size_t o = (size_t)n * L * F + (size_t)l * F + f;
+                out[o] = (float)acc;
+                if (out_abs) out_abs[o] = mag;
+            }
+        }
+    }
+    return ORACLE_OK;
+}
+
+/* dtable[l][slot_k][f] += W_k * dout[n][l*F+f]; accumulators as in dash_oracle_bwd. */
+int dash_oracle3d_bwd(const dash_oracle_config *c, uint64_t N, const float *xyz, uint32_t xyz_stride,
+                      const int32_t *index, const float *dout, float *dtable, double *grad_abs,
+                      uint32_t *hits) {
+    uint32_t res[ORACLE_MAX_L], pi[4];
+    uint8_t dn[ORACLE_MAX_L];
+    if (dash_oracle3d_resolutions(c, res, dn)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!xyz || !(xyz_stride == 3 || xyz_stride == 4) || !dout || !dtable) return ORACLE_INVALID;
+    get_primes(c, pi);
+    const uint32_t L = c->L, F = c->F;
+    const size_t TF = (size_t)c->T * F;
+    int failed = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t l = 0; l < (int32_t)L; ++l) {
+        double *acc = (double *)calloc(TF, sizeof(double));
+        double *mag = grad_abs ? grad_abs + (size_t)l * TF : NULL;
+        uint32_t *cnt = hits ? hits + (size_t)l * c->T : NULL;
+        if (!acc) {
+            failed = 1;
+            continue;
+        }
+        if (mag) memset(mag, 0, TF * sizeof(double));
+        if (cnt) memset(cnt, 0, (size_t)c->T * sizeof(uint32_t));
+        for (uint64_t n = 0; n < N; ++n) {
+            float p[3];
+            uint32_t slot[8];
+            double W[8];
+            fetch_point(n, xyz, xyz_stride, index, p);
+            corners3(c, pi, res[l], dn[l], p, slot, W);
+            for (int k = 0; k < 8; ++k) {
+                for (uint32_t f = 0; f < F; ++f) {
+                    double term = W[k] * (double)dout[(size_t)n * L * F + (size_t)l * F + f];
+                    acc[(size_t)slot[k] * F + f] += term;
+                    if (mag) mag[(size_t)slot[k] * F + f] += fabs(term);
+                }
+                if (cnt) cnt[slot[k]] += 1u;
+            }
+        }
+        float *dst = dtable + (size_t)l * TF;
+        for (size_t e = 0; e < TF; ++e) dst[e] = (float)((double)dst[e] + acc[e]);
+        free(acc);
+    }
+    return failed ? ORACLE_NOMEM : ORACLE_OK;
+}
