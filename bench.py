@@ -323,6 +323,26 @@ def run_cuda(args):
         one_t = t[:1].contiguous()
         extras["fwd_one_timestamp_ms"] = timed(lambda: dh.dash_hash4d_fwd(cfg, xyz, one_t, table, out=out,
                                                                            index=index, t_stride=0))
+        # G_3D of the decomposition stage on its own workload (dash_inputs.G3D_SPEC)
+        from dash_inputs import make_g3d_workload
+        g3 = make_g3d_workload()
+        e3 = g3.spec.enc
+        cfg3 = dh.make_config(e3.L, e3.F, e3.T, e3.res_s_min, e3.res_s_max, 1, 1, e3.table_dtype,
+                              flags=dh.FLAG_DENSE_COARSE | dh.FLAG_ZERO_GRAD)
+        p3, tab3, dy3 = to_dev(g3.xyz), to_dev(g3.table), to_dev(g3.dout)
+        out3 = torch.empty((g3.N, e3.L * e3.F), dtype=torch.float32, device="cuda")
+        dt3 = torch.empty((e3.L, e3.T, e3.F), dtype=torch.float32, device="cuda")
+        t_zero = torch.zeros(1, device="cuda")
+        extras["g3d"] = {
+            "workload": f"N={g3.N} points, L={e3.L} F={e3.F} T=2^{e3.T.bit_length() - 1}, {e3.res_s_min}->{e3.res_s_max}",
+            "fwd_ms": timed(lambda: dh.dash_hash3d_fwd(cfg3, p3, tab3, out=out3)),
+            "bwd_ms": timed(lambda: dh.dash_hash3d_bwd(cfg3, p3, dy3, dt3)),
+            "fwd_ms_via_4d_kernels_nt1_t0": timed(lambda: dh.dash_hash4d_fwd(cfg3, p3, t_zero, tab3, out=out3,
+                                                                               t_stride=0)),
+            "bwd_ms_via_4d_kernels_nt1_t0": timed(lambda: dh.dash_hash4d_bwd(cfg3, p3, t_zero, dy3, dt3,
+                                                                               t_stride=0)),
+        }
+        del p3, tab3, dy3, out3, dt3
 
     if not rep.is_reporter:
         rep.close()

@@ -154,3 +154,27 @@ def make_queries_uniform(seed: int, n: int) -> tuple[np.ndarray, np.ndarray]:
     rng = np.random.default_rng(seed)
     q = rng.random(size=(n, 4), dtype=np.float32)
     return np.ascontiguousarray(q[:, :3]), np.ascontiguousarray(q[:, 3])
+
+
+def make_points_clustered(seed: int, n: int, clusters: int = 64, sigma: float = 0.05) -> np.ndarray:
+    """n points [n][3] fp32 from the clustered recipe of C2-C5 (centres U[0.15,0.85]^3, Gaussian blobs,
+    clamped) — the Gaussian centres p that the 3D encoder G_3D of the decomposition stage sees
+    (ALL Gaussians, static and dynamic)."""
+    return np.ascontiguousarray(_clustered_xyz(np.random.default_rng(seed), n, clusters, sigma))
+
+
+# G_3D workload for bench extras / full-size parity: the 1.5M Gaussians of C5's scene through an
+# Instant-NGP-sized 3D encoder (the paper gives no G_3D hyper-parameters; DESIGN.md Q26).
+G3D_SPEC = WorkloadSpec("G3D", 5, 1_500_000, EncoderParams(16, 2, 1 << 19, 16, 2048, 1, 1), "clustered",
+                        clusters=64, sigma=0.05, note="decomposition stage: every Gaussian, no timestamp")
+
+
+def make_g3d_workload(n_override: Optional[int] = None) -> Workload:
+    spec = G3D_SPEC
+    rng = np.random.default_rng(spec.seed)
+    N = spec.N if n_override is None else int(n_override)
+    xyz = _clustered_xyz(rng, N, spec.clusters, spec.sigma)
+    w = Workload(spec, xyz, np.zeros(N, np.float32), None)
+    w.table = make_table(rng, spec.enc)
+    w.dout = rng.standard_normal(size=(N, spec.enc.L * spec.enc.F), dtype=np.float32)
+    return w

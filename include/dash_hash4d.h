@@ -179,6 +179,34 @@ DASH_API int dash_hash4d_indices(const dash_hash4d_config* cfg, uint64_t N,
                                  const int32_t* index,
                                  uint32_t* idx_out, float* w_out, void* cuda_stream);
 
+/* ---- G_3D: the 3D hash encoder of the decomposition stage (Eq. 3: "a 3D hash encoder
+ * G_3D from Instant-NGP"; Q26) -------------------------------------------------------------------
+ * Eq. 7-9 with d = 3: per level the cell floor(p * Ns_l) of a point p = (x,y,z), its 8 vertices hashed with
+ * pi_x, pi_y, pi_z (Eq. 8) or, where (Ns_l+1)^3 <= T and DENSE_COARSE is set, indexed gx + S(gy + S gz),
+ * S = Ns_l+1; trilinear weights; levels concatenated to R^{L*F}.  The same config struct is used; its temporal
+ * fields (res_t_min, res_t_max, primes[3]) are ignored.  Same kernels as the 4D path with 4 instead of 8
+ * corners per lane, same level-group-major schedule, flags (ZERO_GRAD, DETERMINISTIC_BWD, VALIDATE_INPUTS),
+ * alignment, ownership, error and N == 0 behaviour as dash_hash4d_fwd / _bwd / _indices.
+ *   idx_out / w_out of dash_hash3d_indices: [N][L][8], corner k bit d => +1 along axis d (0:x 1:y 2:z).
+ *   dash_hash3d_resolutions: res_s [L] host (written), is_dense [L] host, nullable.  Needs no GPU. */
+DASH_API int dash_hash3d_resolutions(const dash_hash4d_config* cfg, uint32_t* res_s, uint8_t* is_dense);
+DASH_API int dash_hash3d_fwd(const dash_hash4d_config* cfg, uint64_t N,
+                             const float* xyz, uint32_t xyz_stride,
+                             const int32_t* index,
+                             const void* table,
+                             float* out,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+DASH_API int dash_hash3d_bwd(const dash_hash4d_config* cfg, uint64_t N,
+                             const float* xyz, uint32_t xyz_stride,
+                             const int32_t* index,
+                             const float* dout,
+                             float* dtable,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+DASH_API int dash_hash3d_indices(const dash_hash4d_config* cfg, uint64_t N,
+                                 const float* xyz, uint32_t xyz_stride,
+                                 const int32_t* index,
+                                 uint32_t* idx_out, float* w_out, void* cuda_stream);
+
 /* dtable <- 0 for the whole [L][T][F] fp32 gradient buffer (the accumulation's initial state), with the
  * library's own fill kernel on `cuda_stream`. */
 DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream);

@@ -23,7 +23,8 @@ _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUD
 
 EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4d_fwd",
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
-           "dash_hash4d_launch_count"]
+           "dash_hash4d_launch_count",
+           "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices"]
 
 
 class Hash4DError(RuntimeError):
@@ -81,6 +82,14 @@ def _load() -> C.CDLL:
     lib.dash_hash4d_zero.restype = C.c_int
     lib.dash_hash4d_last_error.argtypes = []
     lib.dash_hash4d_last_error.restype = C.c_char_p
+    lib.dash_hash3d_resolutions.argtypes = [cfgp, vp, vp]
+    lib.dash_hash3d_resolutions.restype = C.c_int
+    lib.dash_hash3d_fwd.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp, sz, vp]
+    lib.dash_hash3d_fwd.restype = C.c_int
+    lib.dash_hash3d_bwd.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp, sz, vp]
+    lib.dash_hash3d_bwd.restype = C.c_int
+    lib.dash_hash3d_indices.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp]
+    lib.dash_hash3d_indices.restype = C.c_int
     lib.dash_hash4d_launch_count.argtypes = [C.c_int]
     lib.dash_hash4d_launch_count.restype = u64
     _lib = lib
@@ -262,6 +271,64 @@ def dash_hash4d_zero(cfg, dtable):
     _dev(dtable, torch.float32, "dtable")
     _check(_load().dash_hash4d_zero(C.byref(cfg), _ptr(dtable), _stream()))
     return dtable
+
+
+# ---- G_3D (Eq. 3): the same encoder with d = 3; temporal config fields ignored -------
+
+def _xyz_stride(xyz: torch.Tensor) -> int:
+    if xyz.dim() != 2 or xyz.shape[1] not in (3, 4):
+        raise ValueError("xyz must be [rows][3] or [rows][4]")
+    return int(xyz.shape[1])
+
+
+def dash_hash3d_resolutions(cfg: Hash4DConfig):
+    """-> (res_s, is_dense) as Python lists (host only; needs no GPU)."""
+    L = max(int(cfg.L), 1)
+    rs, dn = (C.c_uint32 * L)(), (C.c_uint8 * L)()
+    _check(_load().dash_hash3d_resolutions(C.byref(cfg), rs, dn))
+    return list(rs), [bool(v) for v in dn]
+
+
+def dash_hash3d_fwd(cfg, xyz, table, out=None, index=None, N=None, workspace=None):
+    """out[n][l*F+f] = sum_{k<8} W_k table[l][slot_k][f]; returns `out` ([N][L*F] fp32, CUDA)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index")
+    _dev(table, torch.float16 if cfg.table_dtype == 1 else torch.float32, "table")
+    xs = _xyz_stride(xyz)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    if out is None:
+        out = torch.empty((N, cfg.L * cfg.F), dtype=torch.float32, device=xyz.device)
+    _dev(out, torch.float32, "out")
+    workspace, wbytes = _workspace(cfg, N, OP_FWD, workspace)
+    _check(_load().dash_hash3d_fwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(table), _ptr(out),
+                                   _ptr(workspace), wbytes, _stream()))
+    return out
+
+
+def dash_hash3d_bwd(cfg, xyz, dout, dtable, index=None, N=None, workspace=None):
+    """dtable[l][slot_k][f] += W_k dout[n][l*F+f] over the 8 corners; returns `dtable`."""
+    _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index")
+    _dev(dout, torch.float32, "dout"); _dev(dtable, torch.float32, "dtable")
+    xs = _xyz_stride(xyz)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    workspace, wbytes = _workspace(cfg, N, OP_BWD, workspace)
+    _check(_load().dash_hash3d_bwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(dout), _ptr(dtable),
+                                   _ptr(workspace), wbytes, _stream()))
+    return dtable
+
+
+def dash_hash3d_indices(cfg, xyz, index=None, N=None, want_weights=True):
+    """-> (idx [N][L][8] int32-viewed uint32, w [N][L][8] fp32 or None)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index")
+    xs = _xyz_stride(xyz)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    idx = torch.empty((N, cfg.L, 8), dtype=torch.int32, device=xyz.device)
+    w = torch.empty((N, cfg.L, 8), dtype=torch.float32, device=xyz.device) if want_weights else None
+    _check(_load().dash_hash3d_indices(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(idx), _ptr(w),
+                                       _stream()))
+    return idx, w
 
 
 # ---- host-buffer entry points (bench.py "e2e"): copies in, C-ABI calls, copies out -----------------

@@ -39,7 +39,7 @@ const uint32_t kDefaultPrimes[4] = {1u, 2654435761u, 805459861u, 3674653429u};  
 constexpr uint32_t kMaxResolution = 1u << 22;
 constexpr size_t kHeaderBytes = sizeof(WorkspaceHeader);
 
-int check_config(const dash_hash4d_config* c) {
+int check_config(const dash_hash4d_config* c, int dims = 4) {
     if (!c) return fail(DASH_HASH4D_INVALID_ARG, "config is NULL");
     if (c->struct_size != sizeof(dash_hash4d_config))
         return fail(DASH_HASH4D_INVALID_ARG, "struct_size %u != %zu", c->struct_size,
@@ -53,7 +53,7 @@ int check_config(const dash_hash4d_config* c) {
     if (c->res_s_min < 1 || c->res_s_min > c->res_s_max || c->res_s_max > kMaxResolution)
         return fail(DASH_HASH4D_INVALID_ARG, "spatial resolution range [%u, %u] invalid",
                     c->res_s_min, c->res_s_max);
-    if (c->res_t_min < 1 || c->res_t_min > c->res_t_max || c->res_t_max > kMaxResolution)
+    if (dims == 4 && (c->res_t_min < 1 || c->res_t_min > c->res_t_max || c->res_t_max > kMaxResolution))
         return fail(DASH_HASH4D_INVALID_ARG, "temporal resolution range [%u, %u] invalid",
                     c->res_t_min, c->res_t_max);
     if (c->table_dtype != DASH_HASH4D_FP32 && c->table_dtype != DASH_HASH4D_FP16)
@@ -81,17 +81,24 @@ bool fits_dense(uint32_t ns, uint32_t nt, uint32_t T) {  // (Ns+1)^3 (Nt+1) <= T
     return v <= T;
 }
 
+bool fits_dense3(uint32_t ns, uint32_t T) {  // (Ns+1)^3 <= T: the d = 3 form of reading Q10 (Q26)
+    const unsigned long long S = static_cast<unsigned long long>(ns) + 1ull;
+    const unsigned long long v = S * S;
+    return v <= T && v * S <= T;
+}
+
 struct Schedule {
     uint32_t res_s[dash::kMaxLevels], res_t[dash::kMaxLevels];
     uint8_t dense[dash::kMaxLevels];
 };
 
-void make_schedule(const dash_hash4d_config* c, Schedule* s) {
+void make_schedule(const dash_hash4d_config* c, Schedule* s, int dims = 4) {
     for (uint32_t l = 0; l < c->L; ++l) {
         s->res_s[l] = geometric_level(c->res_s_min, c->res_s_max, l, c->L);
-        s->res_t[l] = geometric_level(c->res_t_min, c->res_t_max, l, c->L);
+        s->res_t[l] = dims == 4 ? geometric_level(c->res_t_min, c->res_t_max, l, c->L) : 1u;
         s->dense[l] = (c->flags & DASH_HASH4D_FLAG_DENSE_COARSE) &&
-                      fits_dense(s->res_s[l], s->res_t[l], c->T);
+                      (dims == 4 ? fits_dense(s->res_s[l], s->res_t[l], c->T)
+                                 : fits_dense3(s->res_s[l], c->T));
     }
 }
 
@@ -146,10 +153,11 @@ uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, const c
 }
 
 int fill_plan(const dash_hash4d_config* c, uint64_t N, uint32_t xyz_stride, uint32_t t_stride,
-              uint32_t group, Plan* P) {
+              uint32_t group, Plan* P, int dims = 4) {
     Schedule s;
-    make_schedule(c, &s);
+    make_schedule(c, &s, dims);
     std::memset(P, 0, sizeof(*P));
+    P->dims = static_cast<uint32_t>(dims);
     P->N = N;
     P->L = c->L;
     P->F = c->F;
@@ -176,7 +184,7 @@ int fill_plan(const dash_hash4d_config* c, uint64_t N, uint32_t xyz_stride, uint
             lp.m[0] = 1;
             lp.m[1] = S;
             lp.m[2] = S * S;
-            lp.m[3] = S * S * S;
+            lp.m[3] = dims == 4 ? S * S * S : 0u;
         } else {
             for (int d = 0; d < 4; ++d) lp.m[d] = defaults ? kDefaultPrimes[d] : c->primes[d];
         }
@@ -191,8 +199,8 @@ int fill_plan(const dash_hash4d_config* c, uint64_t N, uint32_t xyz_stride, uint
 }
 
 int check_queries(const float* xyz, uint32_t xyz_stride, const float* t, uint32_t t_stride,
-                  const int32_t* index) {
-    if (!xyz || !t) return fail(DASH_HASH4D_INVALID_ARG, "xyz or t is NULL");
+                  const int32_t* index, int dims = 4) {
+    if (!xyz || (dims == 4 && !t)) return fail(DASH_HASH4D_INVALID_ARG, "xyz or t is NULL");
     if (!(xyz_stride == 3 || xyz_stride == 4))
         return fail(DASH_HASH4D_INVALID_ARG, "xyz_stride = %u (want 3 or 4)", xyz_stride);
     if (!(t_stride == 0 || t_stride == 1 || t_stride == 4))
@@ -254,25 +262,29 @@ DASH_API int dash_hash4d_resolutions(const dash_hash4d_config* cfg, uint32_t* re
     return ok();
 }
 
-DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op) {
-    (void)N;
-    if (check_config(cfg)) return 0;
+static size_t workspace_need(const dash_hash4d_config* cfg, int op) {
     size_t bytes = 0;
     if ((cfg->flags & DASH_HASH4D_FLAG_VALIDATE_INPUTS) && op != DASH_HASH4D_OP_INDICES)
         bytes = kHeaderBytes;
     if (op == DASH_HASH4D_OP_BWD && (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD))
         bytes = kHeaderBytes + table_elems(cfg) * sizeof(long long);
-    g_error[0] = '\0';
     return bytes;
 }
 
-DASH_API int dash_hash4d_fwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
-                             uint32_t xyz_stride, const float* t, uint32_t t_stride,
-                             const int32_t* index, const void* table, float* out, void* workspace,
-                             size_t workspace_bytes, void* cuda_stream) {
-    if (int rc = check_config(cfg)) return rc;
+DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op) {
+    (void)N;
+    if (check_config(cfg, 3)) return 0;  // the temporal range is not needed to size a workspace
+    g_error[0] = '\0';
+    return workspace_need(cfg, op);
+}
+
+static int fwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                    uint32_t xyz_stride, const float* t, uint32_t t_stride, const int32_t* index,
+                    const void* table, float* out, void* workspace, size_t workspace_bytes,
+                    void* cuda_stream) {
+    if (int rc = check_config(cfg, dims)) return rc;
     if (N == 0) return ok();
-    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index, dims)) return rc;
     if (!table || !out) return fail(DASH_HASH4D_INVALID_ARG, "table or out is NULL");
     if (!aligned16(table) || !aligned16(out))
         return fail(DASH_HASH4D_INVALID_ARG, "table / out not 16-byte aligned");
@@ -281,12 +293,28 @@ DASH_API int dash_hash4d_fwd(const dash_hash4d_config* cfg, uint64_t N, const fl
     const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * (half ? 2 : 4);
     Plan P;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
-                           pick_group(cfg, level_bytes, "DASH_HASH4D_FWD_GROUP"), &P))
+                           pick_group(cfg, level_bytes, "DASH_HASH4D_FWD_GROUP"), &P, dims))
         return rc;
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
     cudaError_t e = dash::launch_fwd(P, xyz, t, index, table, half, out, s);
     if (e != cudaSuccess) return cuda_fail(e, "fwd launch");
     return ok();
+}
+
+DASH_API int dash_hash4d_fwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                             uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                             const int32_t* index, const void* table, float* out, void* workspace,
+                             size_t workspace_bytes, void* cuda_stream) {
+    return fwd_impl(4, cfg, N, xyz, xyz_stride, t, t_stride, index, table, out, workspace,
+                    workspace_bytes, cuda_stream);
+}
+
+DASH_API int dash_hash3d_fwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                             uint32_t xyz_stride, const int32_t* index, const void* table,
+                             float* out, void* workspace, size_t workspace_bytes,
+                             void* cuda_stream) {
+    return fwd_impl(3, cfg, N, xyz, xyz_stride, nullptr, 0, index, table, out, workspace,
+                    workspace_bytes, cuda_stream);
 }
 
 DASH_API int dash_hash4d_bwd_input(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
@@ -350,11 +378,11 @@ DASH_API int dash_hash4d_smooth(const dash_hash4d_config* cfg, uint64_t N, const
     return ok();
 }
 
-DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
-                             uint32_t xyz_stride, const float* t, uint32_t t_stride,
-                             const int32_t* index, const float* dout, float* dtable,
-                             void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    if (int rc = check_config(cfg)) return rc;
+static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                    uint32_t xyz_stride, const float* t, uint32_t t_stride, const int32_t* index,
+                    const float* dout, float* dtable, void* workspace, size_t workspace_bytes,
+                    void* cuda_stream) {
+    if (int rc = check_config(cfg, dims)) return rc;
     if (!dtable && (N || (cfg->flags & DASH_HASH4D_FLAG_ZERO_GRAD)))
         return fail(DASH_HASH4D_INVALID_ARG, "dtable is NULL");
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -369,12 +397,12 @@ DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N, const fl
         }
         return ok();
     }
-    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index, dims)) return rc;
     if (!dout) return fail(DASH_HASH4D_INVALID_ARG, "dout is NULL");
     if (!aligned16(dout) || !aligned16(dtable))
         return fail(DASH_HASH4D_INVALID_ARG, "dout / dtable not 16-byte aligned");
     const bool fixed = (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD) != 0;
-    const size_t need = dash_hash4d_workspace_bytes(cfg, N, DASH_HASH4D_OP_BWD);
+    const size_t need = workspace_need(cfg, DASH_HASH4D_OP_BWD);
     if (need && (!workspace || workspace_bytes < need))
         return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "bwd needs %zu workspace bytes, got %zu", need,
                     workspace_bytes);
@@ -383,7 +411,7 @@ DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N, const fl
     Plan P;
     const size_t scatter_bytes = fixed ? 2 * level_bytes : level_bytes;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
-                           pick_group(cfg, scatter_bytes, "DASH_HASH4D_BWD_GROUP"), &P))
+                           pick_group(cfg, scatter_bytes, "DASH_HASH4D_BWD_GROUP"), &P, dims))
         return rc;
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
 
@@ -423,26 +451,67 @@ DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N, const fl
     return ok();
 }
 
-DASH_API int dash_hash4d_indices(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
-                                 uint32_t xyz_stride, const float* t, uint32_t t_stride,
-                                 const int32_t* index, uint32_t* idx_out, float* w_out,
-                                 void* cuda_stream) {
-    if (int rc = check_config(cfg)) return rc;
+DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                             uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                             const int32_t* index, const float* dout, float* dtable,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    return bwd_impl(4, cfg, N, xyz, xyz_stride, t, t_stride, index, dout, dtable, workspace,
+                    workspace_bytes, cuda_stream);
+}
+
+DASH_API int dash_hash3d_bwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                             uint32_t xyz_stride, const int32_t* index, const float* dout,
+                             float* dtable, void* workspace, size_t workspace_bytes,
+                             void* cuda_stream) {
+    return bwd_impl(3, cfg, N, xyz, xyz_stride, nullptr, 0, index, dout, dtable, workspace,
+                    workspace_bytes, cuda_stream);
+}
+
+static int indices_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                        uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                        const int32_t* index, uint32_t* idx_out, float* w_out, void* cuda_stream) {
+    if (int rc = check_config(cfg, dims)) return rc;
     if (N == 0) return ok();
-    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index, dims)) return rc;
     if (!idx_out) return fail(DASH_HASH4D_INVALID_ARG, "idx_out is NULL");
     if (N * cfg->L > 0x7fffffffull * dash::kBlockThreads)
         return fail(DASH_HASH4D_UNSUPPORTED, "N*L too large for one launch");
     Plan P;
-    if (int rc = fill_plan(cfg, N, xyz_stride, t_stride, 1, &P)) return rc;
+    if (int rc = fill_plan(cfg, N, xyz_stride, t_stride, 1, &P, dims)) return rc;
     cudaError_t e = dash::launch_indices(P, xyz, t, index, idx_out, w_out,
                                          static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return cuda_fail(e, "indices launch");
     return ok();
 }
 
+DASH_API int dash_hash4d_indices(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                                 uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                                 const int32_t* index, uint32_t* idx_out, float* w_out,
+                                 void* cuda_stream) {
+    return indices_impl(4, cfg, N, xyz, xyz_stride, t, t_stride, index, idx_out, w_out, cuda_stream);
+}
+
+DASH_API int dash_hash3d_indices(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                                 uint32_t xyz_stride, const int32_t* index, uint32_t* idx_out,
+                                 float* w_out, void* cuda_stream) {
+    return indices_impl(3, cfg, N, xyz, xyz_stride, nullptr, 0, index, idx_out, w_out, cuda_stream);
+}
+
+DASH_API int dash_hash3d_resolutions(const dash_hash4d_config* cfg, uint32_t* res_s,
+                                     uint8_t* is_dense) {
+    if (int rc = check_config(cfg, 3)) return rc;
+    if (!res_s) return fail(DASH_HASH4D_INVALID_ARG, "res_s is NULL");
+    Schedule s;
+    make_schedule(cfg, &s, 3);
+    for (uint32_t l = 0; l < cfg->L; ++l) {
+        res_s[l] = s.res_s[l];
+        if (is_dense) is_dense[l] = s.dense[l];
+    }
+    return ok();
+}
+
 DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream) {
-    if (int rc = check_config(cfg)) return rc;
+    if (int rc = check_config(cfg, 3)) return rc;  // only L, T, F matter here (serves G_3D tables too)
     if (!dtable) return fail(DASH_HASH4D_INVALID_ARG, "dtable is NULL");
     if (!aligned16(dtable)) return fail(DASH_HASH4D_INVALID_ARG, "dtable not 16-byte aligned");
     cudaError_t e = dash::launch_zero(dtable, table_elems(cfg) * sizeof(float),

@@ -47,16 +47,24 @@ __device__ __forceinline__ uint32_t moved_bit(float v, int d) {
     return (v >= 0.0f && v <= 0x1.fffffep-1f) ? 0u : (1u << d);  // NaN fails both comparisons
 }
 
+template <int D = 4>
 __device__ __forceinline__ Query make_query(const LevelParams& lp, float x, float y, float z, float tt) {
     Query q;
     locate(x, lp.ns_f, q.c[0], q.w[0]);
     locate(y, lp.ns_f, q.c[1], q.w[1]);
     locate(z, lp.ns_f, q.c[2], q.w[2]);
-    locate(tt, lp.nt_f, q.c[3], q.w[3]);
-    q.moved = moved_bit(x, 0) | moved_bit(y, 1) | moved_bit(z, 2) | moved_bit(tt, 3);
+    q.moved = moved_bit(x, 0) | moved_bit(y, 1) | moved_bit(z, 2);
+    if constexpr (D == 4) {
+        locate(tt, lp.nt_f, q.c[3], q.w[3]);
+        q.moved |= moved_bit(tt, 3);
+    } else {  // G_3D: no temporal axis
+        q.c[3] = 0u;
+        q.w[3] = 0.0f;
+    }
     return q;
 }
 
+template <int D = 4>
 __device__ __forceinline__ void load_coords(const Plan& P, uint64_t n, const float* __restrict__ xyz,
                                             const float* __restrict__ t,
                                             const int32_t* __restrict__ index, float c[4]) {
@@ -65,52 +73,72 @@ __device__ __forceinline__ void load_coords(const Plan& P, uint64_t n, const flo
     c[0] = __ldg(p + 0);
     c[1] = __ldg(p + 1);
     c[2] = __ldg(p + 2);
-    c[3] = __ldg(t + n * P.t_stride);
+    if constexpr (D == 4) c[3] = __ldg(t + n * P.t_stride);
+    else c[3] = 0.0f;
 }
 
+template <int D = 4>
 __device__ __forceinline__ Query load_query(const Plan& P, const LevelParams& lp, uint64_t n,
                                             const float* __restrict__ xyz,
                                             const float* __restrict__ t,
                                             const int32_t* __restrict__ index) {
     float c[4];
-    load_coords(P, n, xyz, t, index, c);
-    return make_query(lp, c[0], c[1], c[2], c[3]);
+    load_coords<D>(P, n, xyz, t, index, c);
+    return make_query<D>(lp, c[0], c[1], c[2], c[3]);
 }
 
-// The 8 (y,z,t) corners that share x-corner `xc` (0: floor, 1: floor+1).  Corner j: bit0 = y, bit1 =
-// z, bit2 = t, i.e. full corner number k = xc | (j << 1) (reading Q6).  Hashed level: slot = (XOR of
-// g_d*pi_d) mod T (Eq. 8, uint32 wraparound, Q8/Q9); dense level: slot = sum of g_d*stride_d (Q10).
+// The 2^(D-1) corners that share x-corner `xc` (0: floor, 1: floor+1).  Corner j: bit0 = y, bit1 = z,
+// bit2 = t (D = 4 only), i.e. full corner number k = xc | (j << 1) (reading Q6).  Hashed level: slot =
+// (XOR of g_d*pi_d) mod T (Eq. 8, uint32 wraparound, Q8/Q9); dense level: slot = sum of g_d*stride_d (Q10).
+// D = 3 is G_3D of the decomposition stage (Eq. 3; Q26): 4 (y,z) corners.
+template <int D = 4>
 __device__ __forceinline__ void half_cell(const Plan& P, const LevelParams& lp, const Query& q,
-                                          uint32_t xc, uint32_t slot[8], float W[8]) {
+                                          uint32_t xc, uint32_t* __restrict__ slot,
+                                          float* __restrict__ W) {
+    constexpr int NC = 1 << (D - 1);
     const uint32_t ax = (q.c[0] + xc) * lp.m[0];
     const uint32_t ay0 = q.c[1] * lp.m[1], ay1 = ay0 + lp.m[1];
     const uint32_t az0 = q.c[2] * lp.m[2], az1 = az0 + lp.m[2];
-    const uint32_t at0 = q.c[3] * lp.m[3], at1 = at0 + lp.m[3];
     if (lp.dense) {
         const uint32_t p0 = ax + ay0, p1 = ax + ay1;
-        const uint32_t q0 = az0 + at0, q1 = az1 + at0, q2 = az0 + at1, q3 = az1 + at1;
-        slot[0] = p0 + q0; slot[1] = p1 + q0; slot[2] = p0 + q1; slot[3] = p1 + q1;
-        slot[4] = p0 + q2; slot[5] = p1 + q2; slot[6] = p0 + q3; slot[7] = p1 + q3;
+        if constexpr (D == 4) {
+            const uint32_t at0 = q.c[3] * lp.m[3], at1 = at0 + lp.m[3];
+            const uint32_t q0 = az0 + at0, q1 = az1 + at0, q2 = az0 + at1, q3 = az1 + at1;
+            slot[0] = p0 + q0; slot[1] = p1 + q0; slot[2] = p0 + q1; slot[3] = p1 + q1;
+            slot[4] = p0 + q2; slot[5] = p1 + q2; slot[6] = p0 + q3; slot[7] = p1 + q3;
+        } else {
+            slot[0] = p0 + az0; slot[1] = p1 + az0; slot[2] = p0 + az1; slot[3] = p1 + az1;
+        }
     } else {
         const uint32_t p0 = ax ^ ay0, p1 = ax ^ ay1;
-        const uint32_t q0 = az0 ^ at0, q1 = az1 ^ at0, q2 = az0 ^ at1, q3 = az1 ^ at1;
-        slot[0] = p0 ^ q0; slot[1] = p1 ^ q0; slot[2] = p0 ^ q1; slot[3] = p1 ^ q1;
-        slot[4] = p0 ^ q2; slot[5] = p1 ^ q2; slot[6] = p0 ^ q3; slot[7] = p1 ^ q3;
+        if constexpr (D == 4) {
+            const uint32_t at0 = q.c[3] * lp.m[3], at1 = at0 + lp.m[3];
+            const uint32_t q0 = az0 ^ at0, q1 = az1 ^ at0, q2 = az0 ^ at1, q3 = az1 ^ at1;
+            slot[0] = p0 ^ q0; slot[1] = p1 ^ q0; slot[2] = p0 ^ q1; slot[3] = p1 ^ q1;
+            slot[4] = p0 ^ q2; slot[5] = p1 ^ q2; slot[6] = p0 ^ q3; slot[7] = p1 ^ q3;
+        } else {
+            slot[0] = p0 ^ az0; slot[1] = p1 ^ az0; slot[2] = p0 ^ az1; slot[3] = p1 ^ az1;
+        }
         if (P.t_pow2) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) slot[j] &= P.t_mask;
+            for (int j = 0; j < NC; ++j) slot[j] &= P.t_mask;
         } else {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) slot[j] %= P.T;
+            for (int j = 0; j < NC; ++j) slot[j] %= P.T;
         }
     }
-    // quadrilinear weights: W = prod_d (corner bit ? w_d : 1 - w_d), fp32
+    // multilinear weights: W = prod_d (corner bit ? w_d : 1 - w_d), fp32
     const float wx = xc ? q.w[0] : 1.0f - q.w[0];
     const float py0 = wx * (1.0f - q.w[1]), py1 = wx * q.w[1];
-    const float z0 = 1.0f - q.w[2], z1 = q.w[2], t0 = 1.0f - q.w[3], t1 = q.w[3];
-    const float r0 = z0 * t0, r1 = z1 * t0, r2 = z0 * t1, r3 = z1 * t1;
-    W[0] = py0 * r0; W[1] = py1 * r0; W[2] = py0 * r1; W[3] = py1 * r1;
-    W[4] = py0 * r2; W[5] = py1 * r2; W[6] = py0 * r3; W[7] = py1 * r3;
+    const float z0 = 1.0f - q.w[2], z1 = q.w[2];
+    if constexpr (D == 4) {
+        const float t0 = 1.0f - q.w[3], t1 = q.w[3];
+        const float r0 = z0 * t0, r1 = z1 * t0, r2 = z0 * t1, r3 = z1 * t1;
+        W[0] = py0 * r0; W[1] = py1 * r0; W[2] = py0 * r1; W[3] = py1 * r1;
+        W[4] = py0 * r2; W[5] = py1 * r2; W[6] = py0 * r3; W[7] = py1 * r3;
+    } else {
+        W[0] = py0 * z0; W[1] = py1 * z0; W[2] = py0 * z1; W[3] = py1 * z1;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -213,29 +241,30 @@ __device__ __forceinline__ Item this_item(const Plan& P) {
 // ------------------------------------------------------------------------------------------------
 // Forward: gather + quadrilinear interpolation (Eq. 9)
 // ------------------------------------------------------------------------------------------------
-template <int F, bool HALF>
+template <int F, bool HALF, int D>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_fwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                   const float* __restrict__ t, const int32_t* __restrict__ index,
                   const void* __restrict__ table, float* __restrict__ out) {
+    constexpr int NC = 1 << (D - 1);
     const Item it = this_item(P);
     const LevelParams lp = P.lv[it.l];
-    const Query q = load_query(P, lp, it.n, xyz, t, index);
-    uint32_t slot[8];
-    float W[8];
-    half_cell(P, lp, q, it.xc, slot, W);
+    const Query q = load_query<D>(P, lp, it.n, xyz, t, index);
+    uint32_t slot[NC];
+    float W[NC];
+    half_cell<D>(P, lp, q, it.xc, slot, W);
 
     constexpr size_t kElem = HALF ? 2 : 4;
     const char* level_base =
         static_cast<const char*>(table) + static_cast<size_t>(it.l) * P.T * (F * kElem);
-    float v[8][F];
+    float v[NC][F];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);  // 8 loads in flight
+    for (int j = 0; j < NC; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);  // NC loads in flight
     float acc[F];
 #pragma unroll
     for (int f = 0; f < F; ++f) acc[f] = 0.0f;
 #pragma unroll
-    for (int j = 0; j < 8; ++j)
+    for (int j = 0; j < NC; ++j)
 #pragma unroll
         for (int f = 0; f < F; ++f) acc[f] = fmaf(W[j], v[j][f], acc[f]);
 #pragma unroll
@@ -290,24 +319,25 @@ __device__ __forceinline__ void load_dout(const float* __restrict__ d, uint32_t 
 // ------------------------------------------------------------------------------------------------
 // Backward: scatter-add of W_k * dY into the table gradient (transpose of Eq. 9)
 // ------------------------------------------------------------------------------------------------
-template <int F>
+template <int F, int D>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_bwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                   const float* __restrict__ t, const int32_t* __restrict__ index,
                   const float* __restrict__ dout, float* __restrict__ dtable) {
+    constexpr int NC = 1 << (D - 1);
     const Item it = this_item(P);
     const LevelParams lp = P.lv[it.l];
     float g[F];
     load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F,
                  it.xc, g);
-    const Query q = load_query(P, lp, it.n, xyz, t, index);
-    uint32_t slot[8];
-    float W[8];
-    half_cell(P, lp, q, it.xc, slot, W);  // recomputed, never cached from fwd (128 B per item)
+    const Query q = load_query<D>(P, lp, it.n, xyz, t, index);
+    uint32_t slot[NC];
+    float W[NC];
+    half_cell<D>(P, lp, q, it.xc, slot, W);  // recomputed, never cached from fwd (128 B per item)
     if (!it.active) return;
     float* level_base = dtable + static_cast<size_t>(it.l) * P.T * F;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < NC; ++j) {
         float c[F];
 #pragma unroll
         for (int f = 0; f < F; ++f) c[f] = W[j] * g[f];
@@ -317,27 +347,28 @@ hash4d_bwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
 
 // Deterministic variant: 64-bit fixed-point accumulation.  Integer addition is associative, so the
 // sums do not depend on the order in which the L2 applies the reductions.
-template <int F>
+template <int F, int D>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_bwd_fixed_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                         const float* __restrict__ t, const int32_t* __restrict__ index,
                         const float* __restrict__ dout, long long* __restrict__ acc,
                         const WorkspaceHeader* __restrict__ hdr) {
+    constexpr int NC = 1 << (D - 1);
     const Item it = this_item(P);
     const LevelParams lp = P.lv[it.l];
     float g[F];
     load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F,
                  it.xc, g);
-    const Query q = load_query(P, lp, it.n, xyz, t, index);
-    uint32_t slot[8];
-    float W[8];
-    half_cell(P, lp, q, it.xc, slot, W);
+    const Query q = load_query<D>(P, lp, it.n, xyz, t, index);
+    uint32_t slot[NC];
+    float W[NC];
+    half_cell<D>(P, lp, q, it.xc, slot, W);
     if (!it.active) return;
     const float scale = hdr->scale;  // power of two: the products below are exact rescalings
     unsigned long long* level_base =
         reinterpret_cast<unsigned long long*>(acc) + static_cast<size_t>(it.l) * P.T * F;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < NC; ++j) {
 #pragma unroll
         for (int f = 0; f < F; ++f) {
             const long long fx = __float2ll_rn(__fmul_rn(__fmul_rn(W[j], g[f]), scale));
@@ -543,25 +574,27 @@ hash4d_smooth_kernel(const __grid_constant__ Plan P, const float* __restrict__ x
 // ------------------------------------------------------------------------------------------------
 // Debug: all 16 slots + weights per (query, level)
 // ------------------------------------------------------------------------------------------------
+template <int D>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_indices_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                       const float* __restrict__ t, const int32_t* __restrict__ index,
                       uint32_t* __restrict__ idx_out, float* __restrict__ w_out) {
+    constexpr int NC = 1 << (D - 1);
     const uint64_t i = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x;
     if (i >= P.N * P.L) return;
     const uint64_t n = i / P.L;
     const uint32_t l = static_cast<uint32_t>(i - n * P.L);
     const LevelParams lp = P.lv[l];
-    const Query q = load_query(P, lp, n, xyz, t, index);
+    const Query q = load_query<D>(P, lp, n, xyz, t, index);
 #pragma unroll
     for (uint32_t xc = 0; xc < 2; ++xc) {
-        uint32_t slot[8];
-        float W[8];
-        half_cell(P, lp, q, xc, slot, W);
+        uint32_t slot[NC];
+        float W[NC];
+        half_cell<D>(P, lp, q, xc, slot, W);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            idx_out[i * 16 + (xc | (j << 1))] = slot[j];
-            if (w_out) w_out[i * 16 + (xc | (j << 1))] = W[j];
+        for (int j = 0; j < NC; ++j) {
+            idx_out[i * (2 * NC) + (xc | (j << 1))] = slot[j];
+            if (w_out) w_out[i * (2 * NC) + (xc | (j << 1))] = W[j];
         }
     }
 }
@@ -630,7 +663,7 @@ validate_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
          n += stride) {
         const uint64_t row = index ? static_cast<uint64_t>(index[n]) : n;
         const float* p = xyz + row * P.xyz_stride;
-        const float c[4] = {p[0], p[1], p[2], t[n * P.t_stride]};
+        const float c[4] = {p[0], p[1], p[2], P.dims == 3 ? 0.0f : t[n * P.t_stride]};
 #pragma unroll
         for (int d = 0; d < 4; ++d) bad += !(c[d] >= 0.0f && c[d] < 1.0f);  // NaN fails both
     }
@@ -670,8 +703,13 @@ uint64_t launch_counter(bool reset) {
 cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                        const void* table, bool table_half, float* out, cudaStream_t s) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
-#define DASH_FWD(FV, HV) \
-    hash4d_fwd_kernel<FV, HV><<<grid, block, 0, s>>>(P, xyz, t, index, table, out)
+#define DASH_FWD(FV, HV)                                                                       \
+    do {                                                                                       \
+        if (P.dims == 3)                                                                       \
+            hash4d_fwd_kernel<FV, HV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, table, out); \
+        else                                                                                   \
+            hash4d_fwd_kernel<FV, HV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, table, out); \
+    } while (0)
     switch (P.F * 2 + (table_half ? 1 : 0)) {
         case 2: DASH_FWD(1, false); break;
         case 3: DASH_FWD(1, true); break;
@@ -745,13 +783,21 @@ cudaError_t launch_smooth(const Plan& P, const float* xyz, const float* t, const
 cudaError_t launch_bwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                        const float* dout, float* dtable, cudaStream_t s) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
+#define DASH_BWD(FV)                                                                         \
+    do {                                                                                     \
+        if (P.dims == 3)                                                                     \
+            hash4d_bwd_kernel<FV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); \
+        else                                                                                 \
+            hash4d_bwd_kernel<FV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); \
+    } while (0)
     switch (P.F) {
-        case 1: hash4d_bwd_kernel<1><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); break;
-        case 2: hash4d_bwd_kernel<2><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); break;
-        case 4: hash4d_bwd_kernel<4><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); break;
-        case 8: hash4d_bwd_kernel<8><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); break;
+        case 1: DASH_BWD(1); break;
+        case 2: DASH_BWD(2); break;
+        case 4: DASH_BWD(4); break;
+        case 8: DASH_BWD(8); break;
         default: return cudaErrorInvalidValue;
     }
+#undef DASH_BWD
     return after_launch();
 }
 
@@ -759,13 +805,21 @@ cudaError_t launch_bwd_fixed(const Plan& P, const float* xyz, const float* t, co
                              const float* dout, long long* acc, const WorkspaceHeader* hdr,
                              cudaStream_t s) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
+#define DASH_BWDF(FV)                                                                               \
+    do {                                                                                            \
+        if (P.dims == 3)                                                                            \
+            hash4d_bwd_fixed_kernel<FV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); \
+        else                                                                                        \
+            hash4d_bwd_fixed_kernel<FV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); \
+    } while (0)
     switch (P.F) {
-        case 1: hash4d_bwd_fixed_kernel<1><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); break;
-        case 2: hash4d_bwd_fixed_kernel<2><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); break;
-        case 4: hash4d_bwd_fixed_kernel<4><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); break;
-        case 8: hash4d_bwd_fixed_kernel<8><<<grid, block, 0, s>>>(P, xyz, t, index, dout, acc, hdr); break;
+        case 1: DASH_BWDF(1); break;
+        case 2: DASH_BWDF(2); break;
+        case 4: DASH_BWDF(4); break;
+        case 8: DASH_BWDF(8); break;
         default: return cudaErrorInvalidValue;
     }
+#undef DASH_BWDF
     return after_launch();
 }
 
@@ -773,8 +827,12 @@ cudaError_t launch_indices(const Plan& P, const float* xyz, const float* t, cons
                            uint32_t* idx_out, float* w_out, cudaStream_t s) {
     const uint64_t items = P.N * P.L;
     const uint64_t blocks = (items + kBlockThreads - 1) / kBlockThreads;
-    hash4d_indices_kernel<<<static_cast<unsigned>(blocks), kBlockThreads, 0, s>>>(P, xyz, t, index,
-                                                                                 idx_out, w_out);
+    if (P.dims == 3)
+        hash4d_indices_kernel<3><<<static_cast<unsigned>(blocks), kBlockThreads, 0, s>>>(
+            P, xyz, t, index, idx_out, w_out);
+    else
+        hash4d_indices_kernel<4><<<static_cast<unsigned>(blocks), kBlockThreads, 0, s>>>(
+            P, xyz, t, index, idx_out, w_out);
     return after_launch();
 }
 

@@ -13,14 +13,19 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _declared():
-    text = open(os.path.join(ROOT, "include", "dash_hash4d.h")).read()
-    return re.findall(r"DASH_API\s+[\w\s\*]+?\b(dash_hash4d_\w+)\s*\(", text)
+    names = []
+    inc = os.path.join(ROOT, "include")
+    for fn in sorted(os.listdir(inc)):
+        if fn.endswith(".h"):
+            text = open(os.path.join(inc, fn)).read()
+            names += re.findall(r"DASH_API\s+[\w\s\*]+?\b(dash_\w+)\s*\(", text)
+    return names
 
 
 def test_library_exports_every_declared_symbol():
     names = _declared()
     assert len(names) >= 8 and "dash_hash4d_fwd" in names and "dash_hash4d_bwd" in names \
-        and "dash_hash4d_indices" in names
+        and "dash_hash4d_indices" in names and "dash_hash3d_fwd" in names
     lib = C.CDLL(dh.library_path())
     for n in names:
         assert hasattr(lib, n), n
