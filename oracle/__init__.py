@@ -231,3 +231,55 @@ def oracle3d_bwd(cfg, N, xyz, dout, index=None, dtable=None, want_abs=False, wan
     if want_hits:
         res.append(hits)
     return res[0] if len(res) == 1 else tuple(res)
+
+
+# ---- phi_d + multi-head deformation decoder (Eq. 9-10; Q27) ----
+
+MLP_QUANT_BF16 = 1
+
+
+class OracleMlpConfig(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_layers", C.c_uint32), ("width", C.c_uint32 * 5),
+                ("flags", C.c_uint32)]
+
+
+def make_mlp_config(widths, quant_bf16=False) -> OracleMlpConfig:
+    """widths = [inputs, out_1, ..., out_n], 1 <= n <= 4."""
+    assert 2 <= len(widths) <= 5
+    m = OracleMlpConfig()
+    m.struct_size = C.sizeof(OracleMlpConfig)
+    m.n_layers = len(widths) - 1
+    m.width = (C.c_uint32 * 5)(*(list(widths) + [0] * (5 - len(widths))))
+    m.flags = MLP_QUANT_BF16 if quant_bf16 else 0
+    return m
+
+
+def mlp_param_count(widths) -> int:
+    return sum(widths[l] * widths[l - 1] + widths[l] for l in range(1, len(widths)))
+
+
+def oracle_to_bf16(v: float) -> float:
+    f = lib().dash_oracle_to_bf16
+    f.restype = C.c_double
+    return float(f(C.c_double(v)))
+
+
+def oracle_mlp(mcfg: OracleMlpConfig, feat, params, base=None, want_abs=False):
+    """out = base + MLP(feat): [N][width_n] fp32 (+ the propagated magnitude bound, double)."""
+    widths = list(mcfg.width)[:mcfg.n_layers + 1]
+    assert feat.dtype == np.float32 and feat.flags.c_contiguous and feat.ndim == 2 and feat.shape[1] == widths[0]
+    assert params.dtype == np.float32 and params.flags.c_contiguous and params.size == mlp_param_count(widths)
+    N = feat.shape[0]
+    if base is not None:
+        assert base.dtype == np.float32 and base.flags.c_contiguous and base.shape == (N, widths[-1])
+    out = np.zeros((N, widths[-1]), np.float32)
+    mag = np.zeros((N, widths[-1]), np.float64) if want_abs else None
+    _check(lib().dash_oracle_mlp(C.byref(mcfg), C.c_uint64(N), _p(feat), _p(params), _p(base), _p(out), _p(mag)),
+           "mlp")
+    return (out, mag) if want_abs else out
+
+
+def oracle_deform(cfg, mcfg, N, xyz, t, table, params, base=None, index=None, t_stride=1, want_abs=False):
+    """Eq. 9-10: out = base + MLP(G_4D(x)); the features are the fp32 outputs of oracle_fwd."""
+    feat = oracle_fwd(cfg, N, xyz, t, table, index=index, t_stride=t_stride)
+    return oracle_mlp(mcfg, feat, params, base=base, want_abs=want_abs)

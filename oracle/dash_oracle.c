@@ -669,3 +669,102 @@ int dash_oracle3d_bwd(const dash_oracle_config *c, uint64_t N, const float *xyz,
     }
     return failed ? ORACLE_NOMEM : ORACLE_OK;
 }
+
+/* ---- NEXT #3: the tiny MLP phi_d and the multi-head deformation decoder ---------------
+ * "quadrilinear interpolation ..., followed by a tiny MLP phi_d", f_4D = phi_d(f_h) (Eq. 9);
+ * "a multi-head deformation decoder D = {phi_x, phi_r, phi_s}": dx = phi_x(f_4D), dr = phi_r(f_4D),
+ * ds = phi_s(f_4D), and (x', r', s') = (x + dx, r + dr, s + ds) (Eq. 10).  Layer sizes and activation are
+ * not in the paper (Q27): the decoder is taken as ONE chain of dense layers
+ *     a_0 = f_h;   a_l = relu(W_l a_{l-1} + b_l), l < n;   delta = W_n a_{n-1} + b_n;   out = base + delta
+ * (the three heads are the row blocks of the last layer(s); a block-diagonal matrix expresses separate
+ * hidden layers per head).  params = [W_1 (width1 x width0, row-major) | b_1 | W_2 | b_2 | ...], fp32.
+ * Arithmetic: double.  flags bit0 (QUANT_BF16): the operands of every product — the weights and each
+ * layer's input vector — are first rounded to bfloat16 (round-to-nearest-even), which is the precision the
+ * CUDA path feeds its tensor cores with (Q27); biases, sums and the output stay unrounded.
+ * out_abs (nullable, [N][width_n] double): |b_n| + sum_k |W_n[j][k]| * A_k with A the same bound propagated
+ * from the input (A_0 = |a_0|, A_l = |b_l| + |W_l| A_{l-1}) — the conditioning term of the tolerance. */
+
+typedef struct dash_oracle_mlp_config {
+    uint32_t struct_size;
+    uint32_t n_layers; /* 1..4 */
+    uint32_t width[5]; /* width[0] inputs, width[l] outputs of layer l */
+    uint32_t flags;    /* bit0: round product operands to bf16 */
+} dash_oracle_mlp_config;
+
+/* round-to-nearest-even to the 8-bit-significand bfloat16 grid, from double via one fp32 rounding */
+static double to_bf16(double v) {
+    float f = (float)v;
+    uint32_t u;
+    memcpy(&u, &f, 4);
+    if ((u & 0x7f800000u) == 0x7f800000u) return (double)f; /* inf / nan unchanged */
+    uint32_t lsb = (u >> 16) & 1u;
+    u += 0x7fffu + lsb;
+    u &= 0xffff0000u;
+    memcpy(&f, &u, 4);
+    return (double)f;
+}
+
+double dash_oracle_to_bf16(double v) { return to_bf16(v); }
+
+int dash_oracle_mlp(const dash_oracle_mlp_config *m, uint64_t N, const float *in, const float *params,
+                    const float *base, float *out, double *out_abs) {
+    if (!m || m->struct_size != sizeof(*m) || m->n_layers < 1 || m->n_layers > 4) return ORACLE_INVALID;
+    for (uint32_t l = 0; l <= m->n_layers; ++l)
+        if (m->width[l] < 1 || m->width[l] > 4096) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!in || !params || !out) return ORACLE_INVALID;
+    const int quant = (m->flags & 1u) != 0;
+    const uint32_t n_out = m->width[m->n_layers];
+    uint32_t wmax = 0;
+    for (uint32_t l = 0; l <= m->n_layers; ++l)
+        if (m->width[l] > wmax) wmax = m->width[l];
+    int failed = 0;
+#pragma omp parallel
+    {
+        double *a = (double *)malloc(sizeof(double) * wmax * 4);
+        if (!a) {
+#pragma omp atomic write
+            failed = 1;
+        }
+        double *A = a ? a + wmax : NULL, *z = a ? a + 2 * wmax : NULL, *Z = a ? a + 3 * wmax : NULL;
+#pragma omp for schedule(static)
+        for (int64_t n = 0; n < (int64_t)N; ++n) {
+            if (!a) continue;
+            for (uint32_t k = 0; k < m->width[0]; ++k) {
+                a[k] = (double)in[(size_t)n * m->width[0] + k];
+                A[k] = fabs(a[k]);
+            }
+            const float *p = params;
+            for (uint32_t l = 1; l <= m->n_layers; ++l) {
+                const uint32_t K = m->width[l - 1], J = m->width[l];
+                const float *W = p, *b = p + (size_t)J * K;
+                for (uint32_t j = 0; j < J; ++j) {
+                    double s = (double)b[j], S = fabs((double)b[j]);
+                    for (uint32_t k = 0; k < K; ++k) {
+                        double w = (double)W[(size_t)j * K + k], x = a[k];
+                        if (quant) {
+                            w = to_bf16(w);
+                            x = to_bf16(x);
+                        }
+                        s += w * x;
+                        S += fabs(w) * A[k];
+                    }
+                    z[j] = (l < m->n_layers && s < 0.0) ? 0.0 : s; /* relu on hidden layers */
+                    Z[j] = S;
+                }
+                for (uint32_t j = 0; j < J; ++j) {
+                    a[j] = z[j];
+                    A[j] = Z[j];
+                }
+                p = b + J;
+            }
+            for (uint32_t j = 0; j < n_out; ++j) {
+                double v = a[j] + (base ? (double)base[(size_t)n * n_out + j] : 0.0);
+                out[(size_t)n * n_out + j] = (float)v;
+                if (out_abs) out_abs[(size_t)n * n_out + j] = A[j] + (base ? fabs((double)base[(size_t)n * n_out + j]) : 0.0);
+            }
+        }
+        free(a);
+    }
+    return failed ? ORACLE_NOMEM : ORACLE_OK;
+}
