@@ -178,3 +178,16 @@ def make_g3d_workload(n_override: Optional[int] = None) -> Workload:
     w.table = make_table(rng, spec.enc)
     w.dout = rng.standard_normal(size=(N, spec.enc.L * spec.enc.F), dtype=np.float32)
     return w
+
+
+def make_mlp_params(seed: int, widths) -> np.ndarray:
+    """Packed fp32 parameters [W_1 | b_1 | W_2 | b_2 | ...] of a dense-layer chain (phi_d + heads, PAPER.md:133-142;
+    sizes are not in the paper): W_l, b_l iid U(-1/sqrt(K_l), 1/sqrt(K_l)), K_l the layer's input width — the
+    default initialisation of a linear layer, so activations keep the scale of the features."""
+    rng = np.random.default_rng(seed)
+    parts = []
+    for l in range(1, len(widths)):
+        k = 1.0 / np.sqrt(widths[l - 1])
+        parts.append(rng.uniform(-k, k, size=widths[l] * widths[l - 1]))
+        parts.append(rng.uniform(-k, k, size=widths[l]))
+    return np.concatenate(parts).astype(np.float32)

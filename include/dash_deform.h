@@ -1,0 +1,78 @@
+/*
+ * dash_deform.h — C ABI of the render path of DASH's 4D hash deformation field (arxiv 2507.19141, §4.2,
+ * lines 133-142):
+ *
+ *     f_h = G_4D(x)                          Eq. 9, the hash encoder of dash_hash4d.h
+ *     f_4D = phi_d(f_h)                      "followed by a tiny MLP phi_d"
+ *     dx = phi_x(f_4D), dr = phi_r(f_4D), ds = phi_s(f_4D)      multi-head deformation decoder
+ *     (x', r', s') = (x + dx, r + dr, s + ds)                   Eq. 10
+ *
+ * The paper gives neither layer sizes nor the activation.  Reading (Q27): phi_d and the heads form ONE
+ * chain of n <= 4 dense layers with relu between them and none after the last,
+ *     a_0 = f_h;  a_l = relu(W_l a_{l-1} + b_l) for l < n;  delta = W_n a_{n-1} + b_n;  out = base + delta,
+ * the three heads being row blocks of the last layer (a block-diagonal W expresses per-head hidden layers).
+ *
+ * Arithmetic: the products run on the tensor cores (tcgen05.mma kind::f16): weights and each layer's input
+ * vector are rounded to bfloat16 (round-to-nearest-even), products and sums are fp32, biases / base / out fp32.
+ * The features f_h are formed in fp32 exactly as dash_hash4d_fwd forms them, then rounded to bf16 as the first
+ * layer's input.
+ *
+ * Conventions as in dash_hash4d.h: device pointers, caller-owned buffers, nothing allocated or kept, work is
+ * enqueued on `cuda_stream`, return codes of dash_hash4d_status, N == 0 is a no-op, no CPU fallback.
+ */
+#ifndef DASH_DEFORM_H_
+#define DASH_DEFORM_H_
+
+#include "dash_hash4d.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* The dense-layer chain.  POD, passed by pointer (host memory). */
+typedef struct dash_mlp_config {
+    uint32_t struct_size; /* = sizeof(dash_mlp_config)                                                       */
+    uint32_t n_layers;    /* 1..4                                                                            */
+    uint32_t width[5];    /* width[0]: inputs (must equal L*F in dash_deform_fwd); width[l]: outputs of layer
+                             l, l = 1..n_layers; each 1..256 (internally padded to multiples of 16)          */
+    uint32_t flags;       /* reserved, 0                                                                     */
+} dash_mlp_config;
+
+/* Number of floats in the packed parameter buffer [W_1 | b_1 | W_2 | b_2 | ...], W_l row-major
+ * [width[l]][width[l-1]] (the layout of a torch.nn.Linear weight), b_l [width[l]].  0 on a bad config. */
+DASH_API size_t dash_mlp_param_count(const dash_mlp_config* mlp);
+
+/* out[n][j] = (base ? base[n][j] : 0) + MLP(feat[n])[j].
+ *   feat    [N][width[0]] fp32.     params  packed fp32 parameters (see dash_mlp_param_count).
+ *   base    nullable, [N][width[n_layers]] fp32 (the Gaussian attributes x, r, s of Eq. 10, concatenated).
+ *   out     [N][width[n_layers]] fp32, written.
+ * UNSUPPORTED when the bf16 weights and tile buffers of the chain exceed one SM's 227 KB of shared memory. */
+DASH_API int dash_mlp_fwd(const dash_mlp_config* mlp, uint64_t N,
+                          const float* feat, const float* params, const float* base,
+                          float* out, void* cuda_stream);
+
+/* Device workspace dash_deform_fwd needs: 0 when the fused kernel applies (the table fits L2 as one level
+ * group), else N * L*F * 4 bytes for the feature matrix of the two-pass path. */
+DASH_API size_t dash_deform_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp,
+                                            uint64_t N);
+
+/* out[n] = base[n] + MLP(G_4D(x_n)): Eq. 9-10 in one call.
+ * Query arguments (xyz, xyz_stride, t, t_stride, index) and `table` as in dash_hash4d_fwd; t_stride = 0 is the
+ * render path's one timestamp per frame.  mlp->width[0] must equal enc->L * enc->F.
+ * Fused kernel (default when L*T*F*sizeof(table element) <= 0.55 x L2): per 128-query tile the gathers write the
+ * features as bf16 into shared memory, tcgen05.mma runs the layers out of shared / tensor memory, only `out`
+ * goes to HBM.  Otherwise: dash_hash4d_fwd into `workspace`, then the same kernel in feature-matrix mode.
+ * enc->flags: DENSE_COARSE honoured; the other flags must be clear (INVALID_ARG). */
+DASH_API int dash_deform_fwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
+                             const float* xyz, uint32_t xyz_stride,
+                             const float* t, uint32_t t_stride,
+                             const int32_t* index,
+                             const void* table,
+                             const float* params, const float* base,
+                             float* out,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DASH_DEFORM_H_ */

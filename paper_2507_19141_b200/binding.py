@@ -24,7 +24,8 @@ _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUD
 EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4d_fwd",
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count",
-           "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices"]
+           "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
+           "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd"]
 
 
 class Hash4DError(RuntimeError):
@@ -39,6 +40,12 @@ class Hash4DConfig(C.Structure):
                 ("res_s_min", C.c_uint32), ("res_s_max", C.c_uint32),
                 ("res_t_min", C.c_uint32), ("res_t_max", C.c_uint32),
                 ("primes", C.c_uint32 * 4), ("table_dtype", C.c_uint32), ("flags", C.c_uint32)]
+
+
+class MlpConfig(C.Structure):
+    """Mirror of `struct dash_mlp_config` (include/dash_deform.h)."""
+    _fields_ = [("struct_size", C.c_uint32), ("n_layers", C.c_uint32), ("width", C.c_uint32 * 5),
+                ("flags", C.c_uint32)]
 
 
 _lib: Optional[C.CDLL] = None
@@ -90,6 +97,15 @@ def _load() -> C.CDLL:
     lib.dash_hash3d_bwd.restype = C.c_int
     lib.dash_hash3d_indices.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp]
     lib.dash_hash3d_indices.restype = C.c_int
+    mlpp = C.POINTER(MlpConfig)
+    lib.dash_mlp_param_count.argtypes = [mlpp]
+    lib.dash_mlp_param_count.restype = sz
+    lib.dash_mlp_fwd.argtypes = [mlpp, u64, vp, vp, vp, vp, vp]
+    lib.dash_mlp_fwd.restype = C.c_int
+    lib.dash_deform_workspace_bytes.argtypes = [cfgp, mlpp, u64]
+    lib.dash_deform_workspace_bytes.restype = sz
+    lib.dash_deform_fwd.argtypes = [cfgp, mlpp, u64, vp, u32, vp, u32, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.dash_deform_fwd.restype = C.c_int
     lib.dash_hash4d_launch_count.argtypes = [C.c_int]
     lib.dash_hash4d_launch_count.restype = u64
     _lib = lib
@@ -329,6 +345,63 @@ def dash_hash3d_indices(cfg, xyz, index=None, N=None, want_weights=True):
     _check(_load().dash_hash3d_indices(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(idx), _ptr(w),
                                        _stream()))
     return idx, w
+
+
+# ---- render path: G_4D -> phi_d -> heads (include/dash_deform.h; Eq. 9-10) -------------
+
+def make_mlp_config(widths) -> MlpConfig:
+    """widths = [inputs, out_1, ..., out_n], 1 <= n <= 4."""
+    if not 2 <= len(widths) <= 5:
+        raise ValueError("an MLP chain has 1..4 layers")
+    m = MlpConfig()
+    m.struct_size = C.sizeof(MlpConfig)
+    m.n_layers = len(widths) - 1
+    m.width = (C.c_uint32 * 5)(*(list(widths) + [0] * (5 - len(widths))))
+    m.flags = 0
+    return m
+
+
+def dash_mlp_param_count(mlp: MlpConfig) -> int:
+    return int(_load().dash_mlp_param_count(C.byref(mlp)))
+
+
+def dash_mlp_fwd(mlp, feat, params, base=None, out=None):
+    """out = base + MLP(feat): [N][width_n] fp32 (tcgen05 bf16 x bf16 -> fp32)."""
+    _dev(feat, torch.float32, "feat"); _dev(params, torch.float32, "params"); _dev(base, torch.float32, "base")
+    N = int(feat.shape[0])
+    n_out = int(mlp.width[mlp.n_layers])
+    if out is None:
+        out = torch.empty((N, n_out), dtype=torch.float32, device=feat.device)
+    _dev(out, torch.float32, "out")
+    _check(_load().dash_mlp_fwd(C.byref(mlp), N, _ptr(feat), _ptr(params), _ptr(base), _ptr(out), _stream()))
+    return out
+
+
+def dash_deform_workspace_bytes(cfg, mlp, N: int) -> int:
+    return int(_load().dash_deform_workspace_bytes(C.byref(cfg), C.byref(mlp), N))
+
+
+def dash_deform_fwd(cfg, mlp, xyz, t, table, params, base=None, out=None, index=None, t_stride=None, N=None,
+                    workspace=None):
+    """out[n] = base[n] + MLP(G_4D(x_n)) (Eq. 9-10) in one call; returns `out` ([N][width_n] fp32, CUDA)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(t, torch.float32, "t"); _dev(index, torch.int32, "index")
+    _dev(table, torch.float16 if cfg.table_dtype == 1 else torch.float32, "table")
+    _dev(params, torch.float32, "params"); _dev(base, torch.float32, "base")
+    xs, ts = _strides(xyz, t, t_stride)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    n_out = int(mlp.width[mlp.n_layers])
+    if out is None:
+        out = torch.empty((N, n_out), dtype=torch.float32, device=xyz.device)
+    _dev(out, torch.float32, "out")
+    need = dash_deform_workspace_bytes(cfg, mlp, N)
+    if need and workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+    wbytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    _check(_load().dash_deform_fwd(C.byref(cfg), C.byref(mlp), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
+                                   _ptr(table), _ptr(params), _ptr(base), _ptr(out), _ptr(workspace), wbytes,
+                                   _stream()))
+    return out
 
 
 # ---- host-buffer entry points (bench.py "e2e"): copies in, C-ABI calls, copies out -----------------

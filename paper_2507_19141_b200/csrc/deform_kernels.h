@@ -1,0 +1,50 @@
+// deform_kernels.h — launch plan and host-callable launchers of the fused deformation kernel (deform_kernels.cu).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+
+#include "hash4d_plan.h"
+
+namespace dash {
+
+constexpr uint32_t kDeformTileM = 128;      // queries per tile = rows of one tcgen05.mma (M = 128, cta_group::1)
+constexpr uint32_t kDeformEncWarps = 24;    // producer warps (multiple of 4 so that the epilogue warps that follow
+                                            // have warp % 4 = 0..3, the TMEM lane quarter each may read)
+constexpr uint32_t kDeformEpiWarps = 4;
+constexpr uint32_t kDeformMmaWarp = kDeformEncWarps + kDeformEpiWarps;
+constexpr uint32_t kDeformThreads = (kDeformEncWarps + kDeformEpiWarps + 1) * 32;
+constexpr uint32_t kMlpMaxLayers = 4;
+constexpr uint32_t kMlpMaxWidth = 256;      // one tcgen05.mma covers N <= 256
+constexpr uint32_t kDeformSmemLimit = 227u * 1024u;
+
+// Dense-layer chain: widths, padded operand shapes and the shared-memory map of one CTA.
+struct MlpPlan {
+    uint64_t N;                  // rows (queries)
+    uint32_t num_tiles;          // ceil(N / 128)
+    uint32_t n_layers;
+    uint32_t width[kMlpMaxLayers + 1];  // width[0] inputs, width[l] outputs of layer l (as given)
+    uint32_t kpad[kMlpMaxLayers];       // K of layer l: its input width rounded up to 16
+    uint32_t npad[kMlpMaxLayers];       // N of layer l: its output width rounded up to 16
+    uint32_t p_off[kMlpMaxLayers];      // float offset of W_l in the packed parameter buffer (b_l follows W_l)
+    uint32_t w_off[kMlpMaxLayers];      // byte offset of the bf16 operand copy of W_l in shared memory
+    uint32_t b_off[kMlpMaxLayers];      // byte offset of the fp32 bias of layer l in shared memory
+    uint32_t a0_off;             // two A buffers of the first layer, 128 x kpad[0] bf16 each
+    uint32_t act_off;            // activations between layers, 128 x max(kpad[1..]) bf16
+    uint32_t smem_bytes;
+    uint32_t tmem_cols;          // power of two >= max npad, >= 32
+    uint32_t n_out;              // width[n_layers]
+};
+
+cudaError_t launch_deform_fused(const Plan& P, const MlpPlan& M, const float* xyz, const float* t,
+                                const int32_t* index, const void* table, bool table_half,
+                                const float* params, const float* base, float* out, int sms,
+                                cudaStream_t s);
+cudaError_t launch_mlp(const MlpPlan& M, const float* feat, const float* params, const float* base,
+                       float* out, int sms, cudaStream_t s);
+
+void count_launch();   // bumps the per-thread launch counter kept in hash4d_kernels.cu
+int device_sm_count();
+
+}  // namespace dash

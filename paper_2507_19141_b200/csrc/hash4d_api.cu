@@ -11,7 +11,9 @@
 #include <cstdlib>
 #include <cstring>
 
+#include "../../include/dash_deform.h"
 #include "../../include/dash_hash4d.h"
+#include "deform_kernels.h"
 #include "hash4d_kernels.h"
 #include "hash4d_plan.h"
 
@@ -517,6 +519,169 @@ DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void
     cudaError_t e = dash::launch_zero(dtable, table_elems(cfg) * sizeof(float),
                                       static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return cuda_fail(e, "zero launch");
+    return ok();
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------
+// Render path: G_4D -> phi_d -> heads (include/dash_deform.h; Eq. 9-10; Q27)
+// ------------------------------------------------------------------------------------------------------------
+namespace {
+
+int check_mlp(const dash_mlp_config* m) {
+    if (!m) return fail(DASH_HASH4D_INVALID_ARG, "mlp config is NULL");
+    if (m->struct_size != sizeof(dash_mlp_config))
+        return fail(DASH_HASH4D_INVALID_ARG, "mlp struct_size %u != %zu", m->struct_size,
+                    sizeof(dash_mlp_config));
+    if (m->n_layers < 1 || m->n_layers > dash::kMlpMaxLayers)
+        return fail(DASH_HASH4D_INVALID_ARG, "n_layers = %u outside 1..%u", m->n_layers,
+                    dash::kMlpMaxLayers);
+    for (uint32_t l = 0; l <= m->n_layers; ++l)
+        if (m->width[l] < 1 || m->width[l] > dash::kMlpMaxWidth)
+            return fail(DASH_HASH4D_INVALID_ARG, "width[%u] = %u outside 1..%u", l, m->width[l],
+                        dash::kMlpMaxWidth);
+    if (m->flags) return fail(DASH_HASH4D_INVALID_ARG, "unknown mlp flag bits 0x%x", m->flags);
+    return DASH_HASH4D_OK;
+}
+
+uint32_t round_up(uint32_t v, uint32_t m) { return (v + m - 1) / m * m; }
+
+// Shared-memory map of one CTA: [barriers + TMEM slot: 128 B][biases][weights][A0 x 2][activations]
+int fill_mlp_plan(const dash_mlp_config* m, uint64_t N, dash::MlpPlan* M) {
+    std::memset(M, 0, sizeof(*M));
+    M->N = N;
+    const uint64_t tiles = (N + dash::kDeformTileM - 1) / dash::kDeformTileM;
+    if (tiles > 0x7fffffffull) return fail(DASH_HASH4D_UNSUPPORTED, "N too large for one launch");
+    M->num_tiles = static_cast<uint32_t>(tiles);
+    M->n_layers = m->n_layers;
+    for (uint32_t l = 0; l <= m->n_layers; ++l) M->width[l] = m->width[l];
+    M->n_out = m->width[m->n_layers];
+    uint32_t off = 128, p = 0, nmax = 0, kmax = 0;
+    for (uint32_t l = 0; l < m->n_layers; ++l) {
+        M->kpad[l] = round_up(m->width[l], 16);
+        M->npad[l] = round_up(m->width[l + 1], 16);
+        M->p_off[l] = p;
+        p += m->width[l + 1] * m->width[l] + m->width[l + 1];
+        if (M->npad[l] > nmax) nmax = M->npad[l];
+        if (l > 0 && M->kpad[l] > kmax) kmax = M->kpad[l];
+    }
+    for (uint32_t l = 0; l < m->n_layers; ++l) {
+        M->b_off[l] = off;
+        off += M->npad[l] * 4;
+    }
+    off = round_up(off, 128);
+    for (uint32_t l = 0; l < m->n_layers; ++l) {
+        M->w_off[l] = off;
+        off += M->npad[l] * M->kpad[l] * 2;
+    }
+    off = round_up(off, 128);
+    M->a0_off = off;
+    off += 2 * dash::kDeformTileM * M->kpad[0] * 2;
+    M->act_off = off;
+    off += dash::kDeformTileM * kmax * 2;
+    M->smem_bytes = off;
+    uint32_t cols = 32;
+    while (cols < nmax) cols *= 2;
+    M->tmem_cols = cols;
+    if (M->smem_bytes > dash::kDeformSmemLimit)
+        return fail(DASH_HASH4D_UNSUPPORTED,
+                    "this layer chain needs %u bytes of shared memory per CTA (limit %u)", M->smem_bytes,
+                    dash::kDeformSmemLimit);
+    return DASH_HASH4D_OK;
+}
+
+size_t mlp_params(const dash_mlp_config* m) {
+    size_t p = 0;
+    for (uint32_t l = 0; l < m->n_layers; ++l)
+        p += static_cast<size_t>(m->width[l + 1]) * m->width[l] + m->width[l + 1];
+    return p;
+}
+
+// the fused kernel walks all L levels per tile: the whole table must stay L2-resident
+bool deform_fused_applies(const dash_hash4d_config* enc) {
+    const char* v = std::getenv("DASH_DEFORM_FUSED");
+    if (v) return std::atoi(v) != 0;
+    const size_t elem = enc->table_dtype == DASH_HASH4D_FP16 ? 2 : 4;
+    const size_t table_bytes = static_cast<size_t>(enc->L) * enc->T * enc->F * elem;
+    return table_bytes <= l2_bytes() / 100 * 55;
+}
+
+}  // namespace
+
+extern "C" {
+
+DASH_API size_t dash_mlp_param_count(const dash_mlp_config* mlp) {
+    if (check_mlp(mlp)) return 0;
+    g_error[0] = '\0';
+    return mlp_params(mlp);
+}
+
+DASH_API int dash_mlp_fwd(const dash_mlp_config* mlp, uint64_t N, const float* feat,
+                          const float* params, const float* base, float* out, void* cuda_stream) {
+    if (int rc = check_mlp(mlp)) return rc;
+    dash::MlpPlan M;
+    if (int rc = fill_mlp_plan(mlp, N, &M)) return rc;
+    if (N == 0) return ok();
+    if (!feat || !params || !out) return fail(DASH_HASH4D_INVALID_ARG, "feat, params or out is NULL");
+    if ((reinterpret_cast<uintptr_t>(feat) | reinterpret_cast<uintptr_t>(params) |
+         reinterpret_cast<uintptr_t>(base) | reinterpret_cast<uintptr_t>(out)) & 3u)
+        return fail(DASH_HASH4D_INVALID_ARG, "feat / params / base / out not 4-byte aligned");
+    cudaError_t e = dash::launch_mlp(M, feat, params, base, out, dash::device_sm_count(),
+                                     static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "mlp launch");
+    return ok();
+}
+
+DASH_API size_t dash_deform_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp,
+                                            uint64_t N) {
+    if (check_config(enc) || check_mlp(mlp)) return 0;
+    g_error[0] = '\0';
+    if (deform_fused_applies(enc)) return 0;
+    return static_cast<size_t>(N) * enc->L * enc->F * sizeof(float);
+}
+
+DASH_API int dash_deform_fwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
+                             const float* xyz, uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                             const int32_t* index, const void* table, const float* params,
+                             const float* base, float* out, void* workspace, size_t workspace_bytes,
+                             void* cuda_stream) {
+    if (int rc = check_config(enc)) return rc;
+    if (int rc = check_mlp(mlp)) return rc;
+    if (enc->flags & ~static_cast<uint32_t>(DASH_HASH4D_FLAG_DENSE_COARSE))
+        return fail(DASH_HASH4D_INVALID_ARG, "deform_fwd: only DENSE_COARSE may be set in enc->flags");
+    if (mlp->width[0] != enc->L * enc->F)
+        return fail(DASH_HASH4D_INVALID_ARG, "mlp width[0] = %u != L*F = %u", mlp->width[0],
+                    enc->L * enc->F);
+    dash::MlpPlan M;
+    if (int rc = fill_mlp_plan(mlp, N, &M)) return rc;
+    if (N == 0) return ok();
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
+    if (!table || !params || !out) return fail(DASH_HASH4D_INVALID_ARG, "table, params or out is NULL");
+    if (!aligned16(table)) return fail(DASH_HASH4D_INVALID_ARG, "table not 16-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(params) | reinterpret_cast<uintptr_t>(base) |
+         reinterpret_cast<uintptr_t>(out)) & 3u)
+        return fail(DASH_HASH4D_INVALID_ARG, "params / base / out not 4-byte aligned");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const bool half = enc->table_dtype == DASH_HASH4D_FP16;
+    if (deform_fused_applies(enc)) {
+        Plan P;
+        if (int rc = fill_plan(enc, N, xyz_stride, t_stride, 1, &P)) return rc;
+        cudaError_t e = dash::launch_deform_fused(P, M, xyz, t, index, table, half, params, base, out,
+                                                  dash::device_sm_count(), s);
+        if (e != cudaSuccess) return cuda_fail(e, "deform launch");
+        return ok();
+    }
+    const size_t need = static_cast<size_t>(N) * enc->L * enc->F * sizeof(float);
+    if (!workspace || workspace_bytes < need)
+        return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "deform_fwd (two-pass) needs %zu workspace bytes, got %zu",
+                    need, workspace_bytes);
+    if (!aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
+    float* feat = static_cast<float*>(workspace);
+    if (int rc = fwd_impl(4, enc, N, xyz, xyz_stride, t, t_stride, index, table, feat, nullptr, 0, cuda_stream))
+        return rc;
+    cudaError_t e = dash::launch_mlp(M, feat, params, base, out, dash::device_sm_count(), s);
+    if (e != cudaSuccess) return cuda_fail(e, "mlp launch");
     return ok();
 }
 
