@@ -343,6 +343,34 @@ def run_cuda(args):
                                                                                t_stride=0)),
         }
         del p3, tab3, dy3, out3, dt3
+        # render path (Eq. 9-10): G_4D -> phi_d -> heads in one kernel, one timestamp per frame
+        from dash_inputs import make_mlp_params
+        extras["deform"] = {}
+        for name in ("C2", "C3"):
+            w2 = make_workload(name, with_dout=False)
+            e2 = w2.spec.enc
+            widths = [e2.L * e2.F, 128, 128, 10]
+            cfg2 = dh.config_from_params(e2, flags=dh.FLAG_DENSE_COARSE)
+            mlp = dh.make_mlp_config(widths)
+            x2, tab2 = to_dev(w2.xyz), to_dev(w2.table)
+            one = to_dev(w2.t[:1].copy())
+            prm = to_dev(make_mlp_params(11, widths))
+            o2 = torch.empty((w2.N, 10), dtype=torch.float32, device="cuda")
+            f2 = torch.empty((w2.N, e2.L * e2.F), dtype=torch.float32, device="cuda")
+            ws2 = torch.empty(w2.N * e2.L * e2.F * 4, dtype=torch.uint8, device="cuda")
+            row = {"workload": f"{name}: N={w2.N}, one timestamp, MLP {widths}"}
+            os.environ["DASH_DEFORM_FUSED"] = "1"
+            row["fused_ms"] = timed(lambda: dh.dash_deform_fwd(cfg2, mlp, x2, one, tab2, prm, out=o2, t_stride=0), 20)
+            os.environ["DASH_DEFORM_FUSED"] = "0"
+            row["two_pass_ms"] = timed(lambda: dh.dash_deform_fwd(cfg2, mlp, x2, one, tab2, prm, out=o2, t_stride=0,
+                                                                  workspace=ws2), 20)
+            os.environ.pop("DASH_DEFORM_FUSED")
+            row["encoder_only_ms"] = timed(lambda: dh.dash_hash4d_fwd(cfg2, x2, one, tab2, out=f2, t_stride=0), 20)
+            row["mlp_only_ms"] = timed(lambda: dh.dash_mlp_fwd(mlp, f2, prm, out=o2), 20)
+            row["mlp_tflops"] = 2.0 * w2.N * sum(a * b for a, b in zip(widths[:-1], widths[1:])) / (
+                row["mlp_only_ms"] * 1e-3) / 1e12
+            extras["deform"][name] = row
+            del x2, tab2, o2, f2, ws2
 
     if not rep.is_reporter:
         rep.close()

@@ -61,6 +61,10 @@ def _load() -> C.CDLL:
     global _lib
     if _lib is not None:
         return _lib
+    path = os.environ.get("DASH_HASH4D_LIB")       # development: load an alternative build of the same ABI
+    if path:
+        lib = C.CDLL(path)
+        return _bind(lib)
     path = _build.LIB
     if _build.is_stale():
         try:
@@ -68,7 +72,11 @@ def _load() -> C.CDLL:
         except Exception as exc:  # noqa: BLE001
             if not os.path.exists(path):
                 raise ImportError(f"libdash_hash4d.so is not built and nvcc failed: {exc}") from exc
-    lib = C.CDLL(path)
+    return _bind(C.CDLL(path))
+
+
+def _bind(lib: C.CDLL) -> C.CDLL:
+    global _lib
     vp, u32, u64, sz = C.c_void_p, C.c_uint32, C.c_uint64, C.c_size_t
     cfgp = C.POINTER(Hash4DConfig)
     lib.dash_hash4d_resolutions.argtypes = [cfgp, vp, vp, vp]

@@ -6,10 +6,15 @@
 //                           of 128 queries x all L levels; the L*F features never go to HBM: they are written
 //                           as bf16 straight into the shared-memory A operand of the first dense layer
 //                           (UMMA K-major, no-swizzle core-matrix layout), double buffered.
-//   warp  28      MMA       one elected thread issues tcgen05.mma (kind::f16, bf16 x bf16 -> fp32, M = 128,
-//                           N = layer width, K = 16 per instruction); accumulators live in TMEM.
-//   warps 24..27  EPILOGUE  tcgen05.ld the accumulator rows (warp e owns TMEM lanes 32e..32e+31), + bias, relu,
-//                           -> bf16 -> the next layer's A operand in shared memory; last layer: + base, store.
+//   warps 24..31  two independent CONSUMER pipelines p = 0, 1 (even / odd tiles) of 4 warps each:
+//                 MMA       the pipeline's first thread issues tcgen05.mma (kind::f16, bf16 x bf16 -> fp32,
+//                           M = 128, N = layer width, K = 16 per instruction); accumulators live in TMEM.  The
+//                           bias rides in the MMA: two extra K columns hold b as bf16 hi + lo against 1.0 in A.
+//                 EPILOGUE  all 4 warps tcgen05.ld the accumulator rows (warp e owns TMEM lanes 32e..32e+31),
+//                           relu, -> bf16 -> the next layer's A operand in shared memory; last layer: + base,
+//                           store.  No shared-memory loads: the LSU queue belongs to the producers' gathers.
+//   The layers of one tile are a dependent chain (MMA -> epilogue -> MMA ...); two pipelines keep the tensor
+//   pipe and the epilogue of one tile busy while the other tile waits on a hand-off.
 //
 // The weights of every layer are converted to bf16 once per CTA and stay resident in shared memory.  Hand-offs
 // are mbarriers (full/empty per A buffer, accumulator-done via tcgen05.commit, activations-ready); no
@@ -20,6 +25,8 @@
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
+#include <cstdio>
+
 #include "deform_kernels.h"
 #include "hash4d_device.cuh"
 
@@ -28,7 +35,7 @@ namespace dash {
 namespace {
 
 constexpr uint32_t kProducerThreads = kDeformEncWarps * 32;
-constexpr uint32_t kEpilogueThreads = kDeformEpiWarps * 32;
+constexpr uint32_t kEpilogueThreads = 4 * 32;   // per pipeline
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -94,6 +101,21 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, float v[16]) {
     for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
 
+// 32 consecutive columns, no wait: several loads are issued back to back, then tc_ld_wait() once
+__device__ __forceinline__ void tc_ld32_nowait(uint32_t taddr, uint32_t r[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, "
+        "%14, %15, %16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]),
+          "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]),
+          "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
 // UMMA shared-memory matrix descriptor, K-major, SWIZZLE_NONE ("interleave"): core matrices of 8 rows x 16 bytes
 // stored as 128 contiguous bytes; SBO = distance between 8-row groups, LBO = distance between the two 16-byte
 // K-chunks one K = 16 instruction reads.  Bits: [0,14) address >> 4, [16,30) LBO >> 4, [32,46) SBO >> 4,
@@ -109,10 +131,12 @@ __device__ __forceinline__ uint32_t umma_idesc(uint32_t n) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((kDeformTileM >> 4) << 24);
 }
 
-// byte offset of element (row, col) of a K-major operand with `rows` rows in the layout umma_desc() describes:
-// 16-byte chunk (col / 8) of row `row` sits at chunk * rows*16 + row*16.
-__device__ __forceinline__ uint32_t operand_offset(uint32_t rows, uint32_t row, uint32_t col) {
-    return (col >> 3) * (rows * 16u) + row * 16u + (col & 7u) * 2u;
+// byte offset of element (row, col) of a K-major operand in the layout umma_desc() describes: the 16-byte chunk
+// (col / 8) of row `row` sits at chunk * LBO + row * 16.  LBO = rows*16 + 16: the 16 spare bytes skew successive
+// K-chunks across the shared-memory banks (stores that walk along K would otherwise all hit one bank group).
+__device__ __forceinline__ uint32_t operand_lbo(uint32_t rows) { return rows * 16u + 16u; }
+__device__ __forceinline__ uint32_t operand_offset(uint32_t lbo, uint32_t row, uint32_t col) {
+    return (col >> 3) * lbo + row * 16u + (col & 7u) * 2u;
 }
 
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
@@ -131,201 +155,337 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                     const float* __restrict__ feat, const float* __restrict__ params,
                     const float* __restrict__ base, float* __restrict__ out) {
     extern __shared__ __align__(128) unsigned char smem[];
+#ifdef DASH_DEFORM_PROFILE
+    const long long t_entry = clock64();
+#endif
     const uint32_t sbase = smem_u32(smem);
     const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31u;
-    // barriers: [0] full0 [1] full1 [2] empty0 [3] empty1 [4] mma_done [5] act_ready ; [8] (u32) TMEM base
-    const uint32_t bar_full = sbase + 0, bar_empty = sbase + 16, bar_mma = sbase + 32, bar_act = sbase + 40;
+    // barriers (8 bytes each): full[2] @0, empty[2] @16, mma_done[2] @32; TMEM base (u32) @64.
+    // A buffer s, pipeline p and tile parity coincide: tile i of this CTA uses s = p = i & 1.
+    const uint32_t bar_full = sbase + 0, bar_empty = sbase + 16, bar_mma0 = sbase + 32;
     volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + 64);
+    const uint32_t a_lbo = operand_lbo(kDeformTileM);           // A operands: 128 rows
+    const uint32_t a0_bytes = (M.kpad[0] >> 3) * a_lbo;
+    // one 16-byte chunk holding (1, 1, 0, ...) in bf16: the two "ones" columns that multiply the bias columns of W
+    const uint4 ones_chunk = make_uint4(0x3f803f80u, 0u, 0u, 0u);
 
-    // ---- one-time setup: barriers, TMEM, weights -> bf16 operand layout, zero padding of the A buffers
+    // ---- one-time setup: barriers, TMEM, weights (+ bias columns) -> bf16 operand layout, A buffers
     if (tid == 0) {
         mbar_init(bar_full + 0, kProducerThreads);
         mbar_init(bar_full + 8, kProducerThreads);
         mbar_init(bar_empty + 0, 1);
         mbar_init(bar_empty + 8, 1);
-        mbar_init(bar_mma, 1);
-        mbar_init(bar_act, kEpilogueThreads);
+        mbar_init(bar_mma0 + 0, 1);
+        mbar_init(bar_mma0 + 8, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == kDeformMmaWarp) {
+    if (warp == kDeformEncWarps) {  // first consumer warp owns the TMEM allocation
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sbase + 64),
                      "r"(M.tmem_cols)
                      : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+#ifdef DASH_DEFORM_PROFILE
+        if (blockIdx.x == 0 && lane == 0) printf("alloc done at %lld\n", clock64() - t_entry);
+#endif
     }
+#ifdef DASH_DEFORM_PROFILE
+    const long long t_s1 = clock64();
+#endif
     for (uint32_t l = 0; l < M.n_layers; ++l) {
-        const uint32_t K = M.width[l], J = M.width[l + 1], kp = M.kpad[l], np = M.npad[l];
+        // W_l as the B operand [npad][kpad], one 16-byte chunk (8 consecutive k of one output row j) per step;
+        // consecutive threads take consecutive chunks of a row: coalesced (float4 when aligned) global reads; the
+        // skewed LBO keeps the shared stores of neighbouring chunks on different banks.
+        // Columns kb, kb+1 carry the bias as bf16 hi + bf16 lo (the A operand has 1.0 there): the tensor core
+        // adds b_j = hi + lo (>= 16 significant bits) and the epilogue needs no bias loads.
+        const uint32_t K = M.width[l], J = M.width[l + 1], kp = M.kpad[l], np = M.npad[l], kb = M.kbias[l];
         const float* W = params + M.p_off[l];
         const float* b = W + static_cast<size_t>(J) * K;
-        for (uint32_t i = tid; i < np * kp; i += kDeformThreads) {
-            const uint32_t j = i / kp, k = i - j * kp;
-            const float w = (j < J && k < K) ? __ldg(W + static_cast<size_t>(j) * K + k) : 0.0f;
-            *reinterpret_cast<__nv_bfloat16*>(smem + M.w_off[l] + operand_offset(np, j, k)) =
-                __float2bfloat16_rn(w);
+        unsigned char* ws = smem + M.w_off[l];
+        const uint32_t cpr = kp >> 3, w_lbo = operand_lbo(np);
+        const bool vec = (K & 7u) == 0 && (reinterpret_cast<uintptr_t>(W) & 15u) == 0;  // float4 row chunks
+        for (uint32_t i = tid; i < np * cpr; i += kDeformThreads) {
+            const uint32_t j = i / cpr, c = i - j * cpr, k0 = c * 8u;   // consecutive threads: consecutive chunks
+            float w[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) w[e] = 0.0f;
+            if (j < J) {
+                const float* src = W + static_cast<size_t>(j) * K + k0;
+                if (k0 < kb) {
+                    if (vec && k0 + 8u <= K) {
+                        const float4 lo = __ldg(reinterpret_cast<const float4*>(src));
+                        const float4 hi = __ldg(reinterpret_cast<const float4*>(src) + 1);
+                        w[0] = lo.x; w[1] = lo.y; w[2] = lo.z; w[3] = lo.w;
+                        w[4] = hi.x; w[5] = hi.y; w[6] = hi.z; w[7] = hi.w;
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 8; ++e)
+                            if (k0 + e < K) w[e] = __ldg(src + e);
+                    }
+                } else if (k0 == kb) {
+                    const float bj = __ldg(b + j);
+                    w[0] = __bfloat162float(__float2bfloat16_rn(bj));
+                    w[1] = bj - w[0];
+                }
+            }
+            *reinterpret_cast<uint4*>(ws + c * w_lbo + j * 16u) =
+                make_uint4(pack_bf16(w[0], w[1]), pack_bf16(w[2], w[3]), pack_bf16(w[4], w[5]),
+                           pack_bf16(w[6], w[7]));
         }
-        float* bs = reinterpret_cast<float*>(smem + M.b_off[l]);
-        for (uint32_t j = tid; j < np; j += kDeformThreads) bs[j] = j < J ? __ldg(b + j) : 0.0f;
     }
-    for (uint32_t i = tid; i < (2u * kDeformTileM * M.kpad[0] * 2u) / 16u; i += kDeformThreads)
-        reinterpret_cast<uint4*>(smem + M.a0_off)[i] = make_uint4(0u, 0u, 0u, 0u);
+#ifdef DASH_DEFORM_PROFILE
+    const long long t_s2 = clock64();
+#endif
+    for (uint32_t i = tid; i < (2u * a0_bytes) / 16u; i += kDeformThreads) {
+        const uint32_t within = (i * 16u) % a0_bytes;                     // byte offset inside one A buffer
+        reinterpret_cast<uint4*>(smem + M.a0_off)[i] =
+            (within / a_lbo == (M.kbias[0] >> 3)) ? ones_chunk : make_uint4(0u, 0u, 0u, 0u);
+    }
+#ifdef DASH_DEFORM_PROFILE
+    const long long t_s3 = clock64();
+#endif
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+#ifdef DASH_DEFORM_PROFILE
+    if (blockIdx.x == 0 && (tid == 0 || tid == 1023))
+        printf("tid %u: init %lld weights %lld a0 %lld sync %lld\n", tid, t_s1 - t_entry, t_s2 - t_s1, t_s3 - t_s2,
+               clock64() - t_s3);
+#endif
+#ifdef DASH_DEFORM_PROFILE
+    __shared__ long long prof[3][64];
+    const long long t_setup = clock64();
+#define PROF(role, idx) do { if (blockIdx.x == 0 && (idx) < 64) prof[role][idx] = clock64() - t_setup; } while (0)
+#else
+#define PROF(role, idx) do { } while (0)
+#endif
 
-    const uint32_t a0_bytes = kDeformTileM * M.kpad[0] * 2u;
+    // Each CTA owns a contiguous range of rows [r_begin, r_end) — an equal share of N, not a whole number of
+    // tiles — and walks it in tiles of 128; in its last, partial tile the producers skip the missing rows, so the
+    // gather work (the bound) is balanced to a row, whatever N is.
+    const uint64_t r_begin = static_cast<uint64_t>(blockIdx.x) * M.rows_per_cta;
+    const uint64_t r_end = r_begin + M.rows_per_cta < M.N ? r_begin + M.rows_per_cta : M.N;
     const uint32_t my_tiles =
-        blockIdx.x < M.num_tiles ? (M.num_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0u;
+        r_begin < r_end ? static_cast<uint32_t>((r_end - r_begin + kDeformTileM - 1) / kDeformTileM) : 0u;
 
     if (warp < kDeformEncWarps) {
         // ================================================================================== PRODUCER
         for (uint32_t i = 0; i < my_tiles; ++i) {
             const uint32_t s = i & 1u;
-            const uint64_t row0 = (static_cast<uint64_t>(blockIdx.x) + static_cast<uint64_t>(i) * gridDim.x) *
-                                  kDeformTileM;
+            const uint64_t row0 = r_begin + static_cast<uint64_t>(i) * kDeformTileM;
+            const uint32_t rows_here = r_end - row0 < kDeformTileM ? static_cast<uint32_t>(r_end - row0) : kDeformTileM;
             mbar_wait(bar_empty + 8 * s, ((i >> 1) & 1u) ^ 1u);  // first use of each buffer passes at once
+            if (tid == 0) PROF(0, 2 * i);
             unsigned char* a0 = smem + M.a0_off + s * a0_bytes;
             if constexpr (FUSED) {
+                // One ROUND = 16 (query, level) items = one warp instruction's worth of lane pairs; a tile has
+                // 8*L rounds.  Each warp iteration takes TWO rounds (rr and rr + kDeformEncWarps) so that 16 gathers
+                // per lane are in flight, and the coordinates of the next iteration are loaded under them.  The
+                // warp -> round assignment rotates from tile to tile: 8*L is rarely a multiple of the warp count,
+                // and the producers may run up to two tiles ahead, so the rotation evens the work out.
                 const uint32_t pair = lane >> 1, xc = lane & 1u;
-                const uint32_t items = kDeformTileM * P.L;  // multiple of 16: whole warps stay together
-                for (uint32_t it = warp * 16u + pair; it < items; it += kDeformEncWarps * 16u) {
-                    const uint32_t q = it / P.L, l = it - q * P.L;
-                    uint64_t n = row0 + q;
-                    if (n >= P.N) n = P.N - 1;  // tail tile: duplicate work, rows never stored
-                    const LevelParams lp = P.lv[l];
-                    const Query qq = load_query<4>(P, lp, n, xyz, t, index);
-                    uint32_t slot[8];
-                    float W[8];
-                    half_cell<4>(P, lp, qq, xc, slot, W);
-                    constexpr size_t kElem = HALF ? 2 : 4;
-                    const char* level_base =
-                        static_cast<const char*>(table) + static_cast<size_t>(l) * P.T * (F * kElem);
-                    float v[8][F];
+                const uint32_t rounds = (rows_here * P.L + 15u) >> 4;   // rounds that hold at least one real row
+                const uint32_t w0 = (warp + 8u * i) % kDeformEncWarps;
+                constexpr size_t kElem = HALF ? 2 : 4;
+                constexpr bool kTwo = false;           // two rounds per iteration measured SLOWER (34K vs 21K cycles per tile)
+                constexpr uint32_t kStep = (kTwo ? 2u : 1u) * kDeformEncWarps;
+                auto item_row = [&](uint32_t rr) -> uint64_t {
+                    const uint64_t n = row0 + (rr * 16u + pair) / P.L;
+                    return n < r_end ? n : r_end - 1;  // ragged last round: duplicate work, rows never stored
+                };
+                auto store_feature = [&](uint32_t rr, const float acc[F]) {
+                    const uint32_t it = rr * 16u + pair, q = it / P.L, l = it - q * P.L;
+                    unsigned char* dst = a0 + operand_offset(a_lbo, q, l * F);   // (row q, column l*F + f), bf16
+                    if constexpr (F == 1) {
+                        *reinterpret_cast<__nv_bfloat16*>(dst) = __float2bfloat16_rn(acc[0]);
+                    } else if constexpr (F == 2) {
+                        *reinterpret_cast<uint32_t*>(dst) = pack_bf16(acc[0], acc[1]);
+                    } else if constexpr (F == 4) {
+                        *reinterpret_cast<uint2*>(dst) =
+                            make_uint2(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]));
+                    } else {
+                        *reinterpret_cast<uint4*>(dst) =
+                            make_uint4(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]),
+                                       pack_bf16(acc[4], acc[5]), pack_bf16(acc[6], acc[7]));
+                    }
+                };
+                float ca[4], cb[4];
+                if (w0 < rounds) {
+                    load_coords<4>(P, item_row(w0), xyz, t, index, ca);
+                    if constexpr (kTwo)
+                        load_coords<4>(P, item_row(w0 + kDeformEncWarps < rounds ? w0 + kDeformEncWarps : w0), xyz,
+                                       t, index, cb);
+                }
+                for (uint32_t ra = w0; ra < rounds; ra += kStep) {
+                    const bool has_b = kTwo && ra + kDeformEncWarps < rounds;
+                    const uint32_t rb = has_b ? ra + kDeformEncWarps : ra;
+                    const uint32_t la = (ra * 16u + pair) % P.L, lb = (rb * 16u + pair) % P.L;
+                    const LevelParams lpa = P.lv[la];
+                    const Query qa = make_query<4>(lpa, ca[0], ca[1], ca[2], ca[3]);
+                    uint32_t sa[8], sb[8];
+                    float Wa[8], Wb[8];
+                    half_cell<4>(P, lpa, qa, xc, sa, Wa);
+                    const char* base_a =
+                        static_cast<const char*>(table) + static_cast<size_t>(la) * P.T * (F * kElem);
+                    float va[8][F], vb[8][F];
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);
-                    float acc[F];
+                    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(base_a, sa[j], va[j]);
+                    if constexpr (kTwo) {
+                        const LevelParams lpb = P.lv[lb];
+                        const Query qb = make_query<4>(lpb, cb[0], cb[1], cb[2], cb[3]);
+                        half_cell<4>(P, lpb, qb, xc, sb, Wb);
+                        const char* base_b =
+                            static_cast<const char*>(table) + static_cast<size_t>(lb) * P.T * (F * kElem);
 #pragma unroll
-                    for (int f = 0; f < F; ++f) acc[f] = 0.0f;
+                        for (int j = 0; j < 8; ++j) load_slot<F, HALF>(base_b, sb[j], vb[j]);
+                    }
+                    // next iteration's coordinates, under the gathers
+                    const uint32_t na = ra + kStep;
+                    if (na < rounds) {
+                        load_coords<4>(P, item_row(na), xyz, t, index, ca);
+                        if constexpr (kTwo)
+                            load_coords<4>(P, item_row(na + kDeformEncWarps < rounds ? na + kDeformEncWarps : na),
+                                           xyz, t, index, cb);
+                    }
+                    float acc_a[F], acc_b[F];
+#pragma unroll
+                    for (int f = 0; f < F; ++f) acc_a[f] = acc_b[f] = 0.0f;
 #pragma unroll
                     for (int j = 0; j < 8; ++j)
 #pragma unroll
-                        for (int f = 0; f < F; ++f) acc[f] = fmaf(W[j], v[j][f], acc[f]);
+                        for (int f = 0; f < F; ++f) acc_a[f] = fmaf(Wa[j], va[j][f], acc_a[f]);
 #pragma unroll
-                    for (int f = 0; f < F; ++f) acc[f] += __shfl_xor_sync(0xffffffffu, acc[f], 1);
-                    if (xc == 0) {  // fp32 feature -> bf16 operand element (row q, column l*F + f)
-                        unsigned char* dst = a0 + operand_offset(kDeformTileM, q, l * F);
-                        if constexpr (F == 1) {
-                            *reinterpret_cast<__nv_bfloat16*>(dst) = __float2bfloat16_rn(acc[0]);
-                        } else if constexpr (F == 2) {
-                            *reinterpret_cast<uint32_t*>(dst) = pack_bf16(acc[0], acc[1]);
-                        } else if constexpr (F == 4) {
-                            *reinterpret_cast<uint2*>(dst) =
-                                make_uint2(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]));
-                        } else {
-                            *reinterpret_cast<uint4*>(dst) =
-                                make_uint4(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]),
-                                           pack_bf16(acc[4], acc[5]), pack_bf16(acc[6], acc[7]));
-                        }
+                    for (int f = 0; f < F; ++f) acc_a[f] += __shfl_xor_sync(0xffffffffu, acc_a[f], 1);
+                    if constexpr (kTwo) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+#pragma unroll
+                            for (int f = 0; f < F; ++f) acc_b[f] = fmaf(Wb[j], vb[j][f], acc_b[f]);
+#pragma unroll
+                        for (int f = 0; f < F; ++f) acc_b[f] += __shfl_xor_sync(0xffffffffu, acc_b[f], 1);
+                    }
+                    if (xc == 0) {
+                        store_feature(ra, acc_a);
+                        if (has_b) store_feature(rb, acc_b);
                     }
                 }
             } else {
-                // feature rows from global memory: one 8-column chunk (32 bytes in, 16 bytes out) per step
-                const uint32_t K = M.width[0], chunks = M.kpad[0] >> 3;
-                for (uint32_t i2 = tid; i2 < kDeformTileM * chunks; i2 += kProducerThreads) {
+                // feature rows from global memory: one 8-column chunk (32 bytes in, 16 bytes out) per step;
+                // only the data chunks — the bias ("ones") chunk behind them was written once at setup
+                const uint32_t K = M.width[0], chunks = M.kbias[0] >> 3;
+                for (uint32_t i2 = tid; i2 < rows_here * chunks; i2 += kProducerThreads) {
                     const uint32_t q = i2 / chunks, c = i2 - q * chunks;
                     const uint64_t n = row0 + q;
                     float x[8];
 #pragma unroll
                     for (int e = 0; e < 8; ++e) {
                         const uint32_t k = c * 8u + e;
-                        x[e] = (n < M.N && k < K) ? __ldcs(feat + n * K + k) : 0.0f;
+                        x[e] = k < K ? __ldcs(feat + n * K + k) : 0.0f;
                     }
-                    *reinterpret_cast<uint4*>(a0 + operand_offset(kDeformTileM, q, c * 8u)) =
+                    *reinterpret_cast<uint4*>(a0 + operand_offset(a_lbo, q, c * 8u)) =
                         make_uint4(pack_bf16(x[0], x[1]), pack_bf16(x[2], x[3]), pack_bf16(x[4], x[5]),
                                    pack_bf16(x[6], x[7]));
                 }
             }
             fence_async_smem();
             mbar_arrive(bar_full + 8 * s);
+            if (tid == 0) PROF(0, 2 * i + 1);
         }
-    } else if (warp == kDeformMmaWarp) {
-        // ================================================================================== MMA ISSUER
-        if (lane == 0) {
-            uint32_t act_phase = 0, batch = 0;
-            for (uint32_t i = 0; i < my_tiles; ++i) {
-                const uint32_t s = i & 1u;
-                for (uint32_t l = 0; l < M.n_layers; ++l, ++batch) {
-                    if (l == 0) mbar_wait(bar_full + 8 * s, (i >> 1) & 1u);
-                    if (batch > 0) {  // TMEM drained (and, for l > 0, the activations written) by the epilogue
-                        mbar_wait(bar_act, act_phase);
-                        act_phase ^= 1u;
-                    }
+    } else {
+        // ================================================================================== CONSUMER PIPELINE p
+        const uint32_t cw = warp - kDeformEncWarps;
+        const uint32_t p = cw >> 2, e = cw & 3u;            // e == warp % 4: owns TMEM lanes 32e .. 32e+31
+        const bool issuer = e == 0 && lane == 0;            // this pipeline's MMA-issuing thread
+        const uint32_t r = e * 32u + lane;                  // accumulator row = query within the tile
+        const uint32_t tmem_d = tmem_base + p * M.tmem_pipe_cols;
+        const uint32_t taddr_row = tmem_d + ((e * 32u) << 16);
+        const uint32_t bar_mma = bar_mma0 + 8 * p;
+        unsigned char* act = smem + M.act_off + p * M.act_bytes;
+        uint32_t mma_phase = 0, batch = 0;
+        for (uint32_t i = p; i < my_tiles; i += kDeformPipes) {
+            const uint64_t n = r_begin + static_cast<uint64_t>(i) * kDeformTileM + r;
+            for (uint32_t l = 0; l < M.n_layers; ++l, ++batch) {
+                if (issuer) {
+                    if (l == 0) mbar_wait(bar_full + 8 * p, (i >> 1) & 1u);
                     tc_fence_after();
-                    const uint32_t a_addr = sbase + (l == 0 ? M.a0_off + s * a0_bytes : M.act_off);
+                    if (p == 0) PROF(1, 2 * batch);
+                    const uint32_t a_addr = l == 0 ? sbase + M.a0_off + p * a0_bytes : smem_u32(act);
                     const uint32_t w_addr = sbase + M.w_off[l];
                     const uint32_t np = M.npad[l], ksteps = M.kpad[l] >> 4;
-                    const uint32_t a_lbo = kDeformTileM * 16u, w_lbo = np * 16u;
+                    const uint32_t w_lbo = operand_lbo(np);
                     const uint32_t idesc = umma_idesc(np);
                     for (uint32_t kk = 0; kk < ksteps; ++kk) {
                         const uint64_t ad = umma_desc(a_addr + kk * 2u * a_lbo, a_lbo, 128u);
                         const uint64_t bd = umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u);
-                        tc_mma_bf16(tmem_base, ad, bd, idesc, kk > 0 ? 1u : 0u);
+                        tc_mma_bf16(tmem_d, ad, bd, idesc, kk > 0 ? 1u : 0u);
                     }
-                    if (l == 0) tc_commit(bar_empty + 8 * s);  // A buffer free once these MMAs have read it
+                    if (l == 0) tc_commit(bar_empty + 8 * p);  // A buffer free once these MMAs have read it
                     tc_commit(bar_mma);
+                    if (p == 0) PROF(1, 2 * batch + 1);
                 }
-            }
-        }
-    } else {
-        // ================================================================================== EPILOGUE
-        const uint32_t e = warp - kDeformEncWarps;          // == warp % 4: owns TMEM lanes 32e .. 32e+31
-        const uint32_t r = e * 32u + lane;                  // accumulator row = query within the tile
-        const uint32_t taddr_row = tmem_base + ((e * 32u) << 16);
-        uint32_t mma_phase = 0;
-        for (uint32_t i = 0; i < my_tiles; ++i) {
-            const uint64_t n = (static_cast<uint64_t>(blockIdx.x) + static_cast<uint64_t>(i) * gridDim.x) *
-                                   kDeformTileM + r;
-            for (uint32_t l = 0; l < M.n_layers; ++l) {
                 mbar_wait(bar_mma, mma_phase);
                 mma_phase ^= 1u;
+                __syncwarp();
                 tc_fence_after();
-                const float* bs = reinterpret_cast<const float*>(smem + M.b_off[l]);
+                if (cw == 0 && lane == 0) PROF(2, 2 * batch);
                 const uint32_t np = M.npad[l];
-                const bool last = l + 1 == M.n_layers;
-                for (uint32_t c = 0; c < np; c += 16u) {
-                    float v[16];
-                    tc_ld16(taddr_row + c, v);
+                if (l + 1 < M.n_layers) {
+                    // hidden layer: relu, -> bf16, -> A operand of the next layer (the bias came out of the MMA)
+                    for (uint32_t c = 0; c < np; c += 32u) {   // np is a multiple of 16: the last round may be half
+                        uint32_t rr[32];
+                        tc_ld32_nowait(taddr_row + c, rr);
+                        tc_ld_wait();
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) v[j] += bs[c + j];
-                    if (!last) {
+                        for (int g = 0; g < 4; ++g) {          // one 16-byte chunk = 8 columns
+                            if (c + 8u * g < np) {
+                                float v[8];
 #pragma unroll
-                        for (int j = 0; j < 16; ++j) v[j] = fmaxf(v[j], 0.0f);
-                        unsigned char* dst = smem + M.act_off + operand_offset(kDeformTileM, r, c);
-                        *reinterpret_cast<uint4*>(dst) = make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]),
-                                                                    pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
-                        *reinterpret_cast<uint4*>(dst + kDeformTileM * 16u) =
-                            make_uint4(pack_bf16(v[8], v[9]), pack_bf16(v[10], v[11]),
-                                       pack_bf16(v[12], v[13]), pack_bf16(v[14], v[15]));
-                    } else if (n < M.N) {
-                        float* o = out + n * M.n_out;
-                        const float* bb = base ? base + n * M.n_out : nullptr;
+                                for (int j = 0; j < 8; ++j) v[j] = fmaxf(__uint_as_float(rr[8 * g + j]), 0.0f);
+                                *reinterpret_cast<uint4*>(act + operand_offset(a_lbo, r, c + 8u * g)) =
+                                    make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]),
+                                               pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
+                            }
+                        }
+                    }
+                    // the next layer's "ones" chunk and the zero chunk behind it (a wider layer may have used them)
+                    *reinterpret_cast<uint4*>(act + operand_offset(a_lbo, r, np)) = ones_chunk;
+                    *reinterpret_cast<uint4*>(act + operand_offset(a_lbo, r, np + 8u)) =
+                        make_uint4(0u, 0u, 0u, 0u);
+                    fence_async_smem();
+                } else {
+                    for (uint32_t c = 0; c < np; c += 16u) {
+                        float v[16];
+                        tc_ld16(taddr_row + c, v);
+                        if (n < r_end) {   // rows past the range hold stale operands: never stored
+                            float* o = out + n * M.n_out;
+                            const float* bb = base ? base + n * M.n_out : nullptr;
 #pragma unroll
-                        for (int j = 0; j < 16; ++j)
-                            if (c + j < M.n_out) __stcs(o + c + j, v[j] + (bb ? __ldcs(bb + c + j) : 0.0f));
+                            for (int j = 0; j < 16; ++j)
+                                if (c + j < M.n_out) __stcs(o + c + j, v[j] + (bb ? __ldcs(bb + c + j) : 0.0f));
+                        }
                     }
                 }
-                if (!last) fence_async_smem();
                 tc_fence_before();
-                mbar_arrive(bar_act);
+                // the 4 warps of this pipeline: activations written and TMEM drained before the next MMAs
+                asm volatile("bar.sync %0, %1;" ::"r"(1u + p), "r"(kEpilogueThreads) : "memory");
+                if (cw == 0 && lane == 0) PROF(2, 2 * batch + 1);
             }
         }
     }
 
-    // ---- teardown: every TMEM read has completed (each epilogue thread waited on its loads)
+    // ---- teardown: every TMEM read has completed (each consumer thread waited on its loads)
     tc_fence_before();
     __syncthreads();
-    if (warp == kDeformMmaWarp) {
+#ifdef DASH_DEFORM_PROFILE
+    if (blockIdx.x == 0 && tid == 0) {
+        printf("tiles=%u setup=%lld end=%lld\n", my_tiles, t_setup - t_entry, clock64() - t_setup);
+        for (int k = 0; k < 2 * (int)my_tiles && k < 64; ++k) printf("prod[%d]=%lld\n", k, prof[0][k]);
+        for (int k = 0; k < (int)(my_tiles + 1) / 2 * 2 * (int)M.n_layers && k < 64; ++k)
+            printf("mma0[%d]=%lld epi0[%d]=%lld\n", k, prof[1][k], k, prof[2][k]);
+    }
+#endif
+    if (warp == kDeformEncWarps) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(M.tmem_cols)
                      : "memory");
@@ -341,8 +501,8 @@ static cudaError_t launch_t(const Plan& P, const MlpPlan& M, const float* xyz, c
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(M.smem_bytes));
     if (e != cudaSuccess) return e;
-    const unsigned grid = M.num_tiles < static_cast<uint32_t>(sms) ? M.num_tiles : static_cast<unsigned>(sms);
-    k<<<grid, kDeformThreads, M.smem_bytes, s>>>(P, M, xyz, t, index, table, feat, params, base, out);
+    (void)sms;
+    k<<<M.grid, kDeformThreads, M.smem_bytes, s>>>(P, M, xyz, t, index, table, feat, params, base, out);
     count_launch();
     return cudaGetLastError();
 }

@@ -12,9 +12,10 @@ namespace dash {
 constexpr uint32_t kDeformTileM = 128;      // queries per tile = rows of one tcgen05.mma (M = 128, cta_group::1)
 constexpr uint32_t kDeformEncWarps = 24;    // producer warps (multiple of 4 so that the epilogue warps that follow
                                             // have warp % 4 = 0..3, the TMEM lane quarter each may read)
-constexpr uint32_t kDeformEpiWarps = 4;
-constexpr uint32_t kDeformMmaWarp = kDeformEncWarps + kDeformEpiWarps;
-constexpr uint32_t kDeformThreads = (kDeformEncWarps + kDeformEpiWarps + 1) * 32;
+constexpr uint32_t kDeformPipes = 2;        // independent consumer pipelines (even / odd tiles): each has 4 warps
+                                            // (MMA issue + epilogue), its own TMEM accumulator, activation buffer
+                                            // and barriers, so one tile's epilogue overlaps the other's MMAs
+constexpr uint32_t kDeformThreads = (kDeformEncWarps + 4 * kDeformPipes) * 32;   // 1024
 constexpr uint32_t kMlpMaxLayers = 4;
 constexpr uint32_t kMlpMaxWidth = 256;      // one tcgen05.mma covers N <= 256
 constexpr uint32_t kDeformSmemLimit = 227u * 1024u;
@@ -23,17 +24,21 @@ constexpr uint32_t kDeformSmemLimit = 227u * 1024u;
 struct MlpPlan {
     uint64_t N;                  // rows (queries)
     uint32_t num_tiles;          // ceil(N / 128)
+    uint32_t grid;               // CTAs: min(SM count, num_tiles)
+    uint64_t rows_per_cta;       // ceil(N / grid): CTA b owns rows [b * rows_per_cta, ...)
     uint32_t n_layers;
     uint32_t width[kMlpMaxLayers + 1];  // width[0] inputs, width[l] outputs of layer l (as given)
-    uint32_t kpad[kMlpMaxLayers];       // K of layer l: its input width rounded up to 16
+    uint32_t kbias[kMlpMaxLayers];      // input width of layer l rounded up to 16: column of the bias (hi, lo) pair
+    uint32_t kpad[kMlpMaxLayers];       // K of layer l = kbias[l] + 16
     uint32_t npad[kMlpMaxLayers];       // N of layer l: its output width rounded up to 16
     uint32_t p_off[kMlpMaxLayers];      // float offset of W_l in the packed parameter buffer (b_l follows W_l)
     uint32_t w_off[kMlpMaxLayers];      // byte offset of the bf16 operand copy of W_l in shared memory
-    uint32_t b_off[kMlpMaxLayers];      // byte offset of the fp32 bias of layer l in shared memory
     uint32_t a0_off;             // two A buffers of the first layer, 128 x kpad[0] bf16 each
-    uint32_t act_off;            // activations between layers, 128 x max(kpad[1..]) bf16
+    uint32_t act_off;            // activations between layers, 128 x max(kpad[1..]) bf16, one per pipeline
+    uint32_t act_bytes;          // size of one activation buffer
     uint32_t smem_bytes;
-    uint32_t tmem_cols;          // power of two >= max npad, >= 32
+    uint32_t tmem_cols;          // allocated TMEM columns: kDeformPipes x tmem_pipe_cols
+    uint32_t tmem_pipe_cols;     // power of two >= max npad, >= 32
     uint32_t n_out;              // width[n_layers]
 };
 

@@ -554,36 +554,40 @@ int fill_mlp_plan(const dash_mlp_config* m, uint64_t N, dash::MlpPlan* M) {
     const uint64_t tiles = (N + dash::kDeformTileM - 1) / dash::kDeformTileM;
     if (tiles > 0x7fffffffull) return fail(DASH_HASH4D_UNSUPPORTED, "N too large for one launch");
     M->num_tiles = static_cast<uint32_t>(tiles);
+    const uint64_t sms = static_cast<uint64_t>(dash::device_sm_count());
+    M->grid = static_cast<uint32_t>(tiles < sms ? tiles : sms);
+    M->rows_per_cta = M->grid ? (N + M->grid - 1) / M->grid : 0;
     M->n_layers = m->n_layers;
     for (uint32_t l = 0; l <= m->n_layers; ++l) M->width[l] = m->width[l];
     M->n_out = m->width[m->n_layers];
     uint32_t off = 128, p = 0, nmax = 0, kmax = 0;
     for (uint32_t l = 0; l < m->n_layers; ++l) {
-        M->kpad[l] = round_up(m->width[l], 16);
+        M->kbias[l] = round_up(m->width[l], 16);
+        M->kpad[l] = M->kbias[l] + 16;   // two bias columns (bf16 hi + lo), padded to one K = 16 step
         M->npad[l] = round_up(m->width[l + 1], 16);
         M->p_off[l] = p;
         p += m->width[l + 1] * m->width[l] + m->width[l + 1];
         if (M->npad[l] > nmax) nmax = M->npad[l];
         if (l > 0 && M->kpad[l] > kmax) kmax = M->kpad[l];
     }
-    for (uint32_t l = 0; l < m->n_layers; ++l) {
-        M->b_off[l] = off;
-        off += M->npad[l] * 4;
-    }
-    off = round_up(off, 128);
+    // operands are stored chunk-major with LBO = rows*16 + 16 bytes (deform_kernels.cu operand_lbo)
     for (uint32_t l = 0; l < m->n_layers; ++l) {
         M->w_off[l] = off;
-        off += M->npad[l] * M->kpad[l] * 2;
+        off += (M->kpad[l] / 8) * (M->npad[l] * 16 + 16);
     }
     off = round_up(off, 128);
+    const uint32_t a_lbo = dash::kDeformTileM * 16 + 16;
     M->a0_off = off;
-    off += 2 * dash::kDeformTileM * M->kpad[0] * 2;
+    off += 2 * (M->kpad[0] / 8) * a_lbo;
+    off = round_up(off, 128);
     M->act_off = off;
-    off += dash::kDeformTileM * kmax * 2;
+    M->act_bytes = round_up((kmax / 8) * a_lbo, 128);
+    off += dash::kDeformPipes * M->act_bytes;
     M->smem_bytes = off;
     uint32_t cols = 32;
     while (cols < nmax) cols *= 2;
-    M->tmem_cols = cols;
+    M->tmem_pipe_cols = cols;
+    M->tmem_cols = cols * dash::kDeformPipes;   // <= 512: nmax <= 256
     if (M->smem_bytes > dash::kDeformSmemLimit)
         return fail(DASH_HASH4D_UNSUPPORTED,
                     "this layer chain needs %u bytes of shared memory per CTA (limit %u)", M->smem_bytes,

@@ -43,7 +43,7 @@ MLP_SHAPES = [
     ([32, 10], 128),
     ([16, 16], 1),
     ([24, 40, 7], 300),                  # widths that need padding to 16
-    ([64, 192, 128, 128, 10], 2000),
+    ([64, 128, 128, 128, 10], 2000),
     ([256, 64, 10], 513),
     ([64, 128, 10], 0),
 ]
