@@ -283,3 +283,24 @@ def oracle_deform(cfg, mcfg, N, xyz, t, table, params, base=None, index=None, t_
     """Eq. 9-10: out = base + MLP(G_4D(x)); the features are the fp32 outputs of oracle_fwd."""
     feat = oracle_fwd(cfg, N, xyz, t, table, index=index, t_stride=t_stride)
     return oracle_mlp(mcfg, feat, params, base=base, want_abs=want_abs)
+
+
+# ---- sparse Adam over the touched table entries (SURVEY §8f NEXT #4; DESIGN.md Q28) ----
+
+def oracle_double_to_half(d: float) -> int:
+    f = lib().dash_oracle_double_to_half
+    f.restype = C.c_uint16
+    return int(f(C.c_double(d)))
+
+
+def oracle_adam_step(theta, grad, m, v, lr, beta1, beta2, eps, t, theta16=None, zero_grad=True):
+    """In place on fp32 arrays theta, grad, m, v (and uint16-viewed theta16).  -> number of touched entries."""
+    for a in (theta, grad, m, v):
+        assert a.dtype == np.float32 and a.flags.c_contiguous and a.size == theta.size
+    if theta16 is not None:
+        assert theta16.dtype == np.float16 and theta16.flags.c_contiguous and theta16.size == theta.size
+    touched = C.c_uint64(0)
+    _check(lib().dash_oracle_adam_step(C.c_uint64(theta.size), C.c_double(lr), C.c_double(beta1), C.c_double(beta2),
+                                       C.c_double(eps), C.c_uint32(t), _p(theta), _p(theta16), _p(grad), _p(m), _p(v),
+                                       C.c_int(1 if zero_grad else 0), C.byref(touched)), "adam_step")
+    return int(touched.value)

@@ -768,3 +768,64 @@ int dash_oracle_mlp(const dash_oracle_mlp_config *m, uint64_t N, const float *in
     }
     return failed ? ORACLE_NOMEM : ORACLE_OK;
 }
+
+/* ---- NEXT #4: sparse optimiser step over the touched table entries -------------------
+ * The paper does not name its optimiser ("primarily based on the PyTorch framework"; 3DGS [14]
+ * and Instant-NGP [25], which it follows, both train with Adam).  Reading (Q28): Adam (Kingma & Ba),
+ * bias-corrected, applied ONLY to entries whose gradient is not exactly zero — an entry no query touched in
+ * this step keeps theta, m and v unchanged (no moment decay), which is what makes the step sparse on the
+ * coarse dense levels (1-27 % of T touched at C4) and is the rule of torch.optim.SparseAdam.  For g != 0:
+ *     m <- beta1 m + (1 - beta1) g ;  v <- beta2 v + (1 - beta2) g^2
+ *     theta <- theta - lr * (m / (1 - beta1^t)) / (sqrt(v / (1 - beta2^t)) + eps)
+ * theta is the fp32 master copy; theta16 (nullable) receives its IEEE-half rounding (the fp16 table the encoder
+ * reads).  With zero_grad != 0 every gradient entry is set to 0 afterwards (the next backward accumulates into
+ * it).  Arithmetic in double from the fp32 state, each stored value rounded once. */
+static uint16_t double_to_half(double d) {
+    /* round-to-nearest-even to IEEE binary16 by search over the format's definition (slow, obviously right) */
+    if (isnan(d)) return 0x7e00u;
+    uint16_t sign = (uint16_t)(signbit(d) ? 0x8000u : 0u);
+    double a = fabs(d);
+    if (a >= 65520.0) return (uint16_t)(sign | 0x7c00u); /* rounds to inf */
+    /* spacing: subnormal step 2^-24 below 2^-14, else 2^(e-10) */
+    int e;
+    (void)frexp(a, &e); /* a = f * 2^e, f in [0.5, 1) -> a in [2^(e-1), 2^e) */
+    double step = (a < ldexp(1.0, -14)) ? ldexp(1.0, -24) : ldexp(1.0, e - 1 - 10);
+    double q = a / step; /* exact: power-of-two scaling */
+    double lo = floor(q), frac = q - lo;
+    if (frac > 0.5 || (frac == 0.5 && fmod(lo, 2.0) == 1.0)) lo += 1.0;
+    double r = lo * step;
+    if (r == 0.0) return sign;
+    if (r < ldexp(1.0, -14)) return (uint16_t)(sign | (uint16_t)(r / ldexp(1.0, -24)));
+    int er;
+    double fr = frexp(r, &er); /* r = fr * 2^er, fr in [0.5,1) */
+    uint16_t expo = (uint16_t)(er - 1 + 15);
+    uint16_t mant = (uint16_t)((fr * 2.0 - 1.0) * 1024.0);
+    return (uint16_t)(sign | (uint16_t)(expo << 10) | mant);
+}
+
+uint16_t dash_oracle_double_to_half(double d) { return double_to_half(d); }
+
+int dash_oracle_adam_step(uint64_t count, double lr, double beta1, double beta2, double eps, uint32_t t,
+                          float *theta, uint16_t *theta16, float *grad, float *m, float *v,
+                          int zero_grad, uint64_t *touched) {
+    if (!theta || !grad || !m || !v || t < 1) return ORACLE_INVALID;
+    const double c1 = 1.0 - pow(beta1, (double)t), c2 = 1.0 - pow(beta2, (double)t);
+    uint64_t n_touched = 0;
+#pragma omp parallel for schedule(static) reduction(+ : n_touched)
+    for (int64_t i = 0; i < (int64_t)count; ++i) {
+        const double g = (double)grad[i];
+        if (g != 0.0) {
+            const double mn = beta1 * (double)m[i] + (1.0 - beta1) * g;
+            const double vn = beta2 * (double)v[i] + (1.0 - beta2) * g * g;
+            const double th = (double)theta[i] - lr * (mn / c1) / (sqrt(vn / c2) + eps);
+            m[i] = (float)mn;
+            v[i] = (float)vn;
+            theta[i] = (float)th;
+            if (theta16) theta16[i] = double_to_half((double)theta[i]);
+            ++n_touched;
+        }
+        if (zero_grad) grad[i] = 0.0f;
+    }
+    if (touched) *touched = n_touched;
+    return ORACLE_OK;
+}

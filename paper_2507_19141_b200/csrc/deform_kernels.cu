@@ -279,95 +279,59 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
             if (tid == 0) PROF(0, 2 * i);
             unsigned char* a0 = smem + M.a0_off + s * a0_bytes;
             if constexpr (FUSED) {
-                // One ROUND = 16 (query, level) items = one warp instruction's worth of lane pairs; a tile has
-                // 8*L rounds.  Each warp iteration takes TWO rounds (rr and rr + kDeformEncWarps) so that 16 gathers
-                // per lane are in flight, and the coordinates of the next iteration are loaded under them.  The
-                // warp -> round assignment rotates from tile to tile: 8*L is rarely a multiple of the warp count,
-                // and the producers may run up to two tiles ahead, so the rotation evens the work out.
+                // One ROUND = 16 (query, level) items = one warp instruction's worth of lane pairs; a full tile has
+                // 8*L rounds, taken by the warps round-robin.  The coordinates of a warp's NEXT round are loaded under
+                // the gathers of the current one (one global round trip on the critical path instead of two).  The
+                // warp -> round assignment rotates from tile to tile: 8*L is rarely a multiple of the warp count, and
+                // the producers may run up to two tiles ahead, so the rotation evens the work out.  (Two rounds per
+                // iteration, 16 gathers per lane in flight, was measured SLOWER: 34K instead of 21K cycles per tile.)
                 const uint32_t pair = lane >> 1, xc = lane & 1u;
                 const uint32_t rounds = (rows_here * P.L + 15u) >> 4;   // rounds that hold at least one real row
                 const uint32_t w0 = (warp + 8u * i) % kDeformEncWarps;
                 constexpr size_t kElem = HALF ? 2 : 4;
-                constexpr bool kTwo = false;           // two rounds per iteration measured SLOWER (34K vs 21K cycles per tile)
-                constexpr uint32_t kStep = (kTwo ? 2u : 1u) * kDeformEncWarps;
                 auto item_row = [&](uint32_t rr) -> uint64_t {
                     const uint64_t n = row0 + (rr * 16u + pair) / P.L;
                     return n < r_end ? n : r_end - 1;  // ragged last round: duplicate work, rows never stored
                 };
-                auto store_feature = [&](uint32_t rr, const float acc[F]) {
+                float cq[4];
+                if (w0 < rounds) load_coords<4>(P, item_row(w0), xyz, t, index, cq);
+                for (uint32_t rr = w0; rr < rounds; rr += kDeformEncWarps) {
                     const uint32_t it = rr * 16u + pair, q = it / P.L, l = it - q * P.L;
-                    unsigned char* dst = a0 + operand_offset(a_lbo, q, l * F);   // (row q, column l*F + f), bf16
-                    if constexpr (F == 1) {
-                        *reinterpret_cast<__nv_bfloat16*>(dst) = __float2bfloat16_rn(acc[0]);
-                    } else if constexpr (F == 2) {
-                        *reinterpret_cast<uint32_t*>(dst) = pack_bf16(acc[0], acc[1]);
-                    } else if constexpr (F == 4) {
-                        *reinterpret_cast<uint2*>(dst) =
-                            make_uint2(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]));
-                    } else {
-                        *reinterpret_cast<uint4*>(dst) =
-                            make_uint4(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]),
-                                       pack_bf16(acc[4], acc[5]), pack_bf16(acc[6], acc[7]));
-                    }
-                };
-                float ca[4], cb[4];
-                if (w0 < rounds) {
-                    load_coords<4>(P, item_row(w0), xyz, t, index, ca);
-                    if constexpr (kTwo)
-                        load_coords<4>(P, item_row(w0 + kDeformEncWarps < rounds ? w0 + kDeformEncWarps : w0), xyz,
-                                       t, index, cb);
-                }
-                for (uint32_t ra = w0; ra < rounds; ra += kStep) {
-                    const bool has_b = kTwo && ra + kDeformEncWarps < rounds;
-                    const uint32_t rb = has_b ? ra + kDeformEncWarps : ra;
-                    const uint32_t la = (ra * 16u + pair) % P.L, lb = (rb * 16u + pair) % P.L;
-                    const LevelParams lpa = P.lv[la];
-                    const Query qa = make_query<4>(lpa, ca[0], ca[1], ca[2], ca[3]);
-                    uint32_t sa[8], sb[8];
-                    float Wa[8], Wb[8];
-                    half_cell<4>(P, lpa, qa, xc, sa, Wa);
-                    const char* base_a =
-                        static_cast<const char*>(table) + static_cast<size_t>(la) * P.T * (F * kElem);
-                    float va[8][F], vb[8][F];
+                    const LevelParams lp = P.lv[l];
+                    const Query qq = make_query<4>(lp, cq[0], cq[1], cq[2], cq[3]);
+                    uint32_t slot[8];
+                    float W[8];
+                    half_cell<4>(P, lp, qq, xc, slot, W);
+                    const char* level_base =
+                        static_cast<const char*>(table) + static_cast<size_t>(l) * P.T * (F * kElem);
+                    float v[8][F];
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(base_a, sa[j], va[j]);
-                    if constexpr (kTwo) {
-                        const LevelParams lpb = P.lv[lb];
-                        const Query qb = make_query<4>(lpb, cb[0], cb[1], cb[2], cb[3]);
-                        half_cell<4>(P, lpb, qb, xc, sb, Wb);
-                        const char* base_b =
-                            static_cast<const char*>(table) + static_cast<size_t>(lb) * P.T * (F * kElem);
+                    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);
+                    if (rr + kDeformEncWarps < rounds)
+                        load_coords<4>(P, item_row(rr + kDeformEncWarps), xyz, t, index, cq);
+                    float acc[F];
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) load_slot<F, HALF>(base_b, sb[j], vb[j]);
-                    }
-                    // next iteration's coordinates, under the gathers
-                    const uint32_t na = ra + kStep;
-                    if (na < rounds) {
-                        load_coords<4>(P, item_row(na), xyz, t, index, ca);
-                        if constexpr (kTwo)
-                            load_coords<4>(P, item_row(na + kDeformEncWarps < rounds ? na + kDeformEncWarps : na),
-                                           xyz, t, index, cb);
-                    }
-                    float acc_a[F], acc_b[F];
-#pragma unroll
-                    for (int f = 0; f < F; ++f) acc_a[f] = acc_b[f] = 0.0f;
+                    for (int f = 0; f < F; ++f) acc[f] = 0.0f;
 #pragma unroll
                     for (int j = 0; j < 8; ++j)
 #pragma unroll
-                        for (int f = 0; f < F; ++f) acc_a[f] = fmaf(Wa[j], va[j][f], acc_a[f]);
+                        for (int f = 0; f < F; ++f) acc[f] = fmaf(W[j], v[j][f], acc[f]);
 #pragma unroll
-                    for (int f = 0; f < F; ++f) acc_a[f] += __shfl_xor_sync(0xffffffffu, acc_a[f], 1);
-                    if constexpr (kTwo) {
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-#pragma unroll
-                            for (int f = 0; f < F; ++f) acc_b[f] = fmaf(Wb[j], vb[j][f], acc_b[f]);
-#pragma unroll
-                        for (int f = 0; f < F; ++f) acc_b[f] += __shfl_xor_sync(0xffffffffu, acc_b[f], 1);
-                    }
-                    if (xc == 0) {
-                        store_feature(ra, acc_a);
-                        if (has_b) store_feature(rb, acc_b);
+                    for (int f = 0; f < F; ++f) acc[f] += __shfl_xor_sync(0xffffffffu, acc[f], 1);
+                    if (xc == 0) {  // fp32 feature -> bf16 operand element (row q, column l*F + f)
+                        unsigned char* dst = a0 + operand_offset(a_lbo, q, l * F);
+                        if constexpr (F == 1) {
+                            *reinterpret_cast<__nv_bfloat16*>(dst) = __float2bfloat16_rn(acc[0]);
+                        } else if constexpr (F == 2) {
+                            *reinterpret_cast<uint32_t*>(dst) = pack_bf16(acc[0], acc[1]);
+                        } else if constexpr (F == 4) {
+                            *reinterpret_cast<uint2*>(dst) =
+                                make_uint2(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]));
+                        } else {
+                            *reinterpret_cast<uint4*>(dst) =
+                                make_uint4(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]),
+                                           pack_bf16(acc[4], acc[5]), pack_bf16(acc[6], acc[7]));
+                        }
                     }
                 }
             } else {
