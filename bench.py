@@ -343,6 +343,33 @@ def run_cuda(args):
                                                                                t_stride=0)),
         }
         del p3, tab3, dy3, out3, dt3
+        # sparse Adam over the touched entries of the step's own gradient (dtable as the timed bwd left it)
+        th32 = table.float().contiguous()
+        m1, v1 = torch.zeros_like(th32), torch.zeros_like(th32)
+        t16 = table if enc.table_dtype == "fp16" else None
+        g_keep = dtable.clone()
+        touched = int((g_keep != 0).sum())
+        def adam_once():
+            dtable.copy_(g_keep)
+        def adam_timed(iters=5):
+            tot = 0.0
+            for k in range(iters + 1):
+                dtable.copy_(g_keep)
+                a, b = ev(), ev()
+                a.record()
+                dh.dash_hash4d_adam_step(cfg, th32, dtable, m1, v1, k + 1, table16=t16)
+                b.record()
+                torch.cuda.synchronize()
+                if k:
+                    tot += a.elapsed_time(b)
+            return tot / iters
+        ms_adam = adam_timed()
+        n_el = th32.numel()
+        adam_bytes = 4 * n_el + touched * (12 + 12 + 4 + (2 if t16 is not None else 0))
+        extras["adam_step"] = {"ms": ms_adam, "touched_fraction": touched / n_el,
+                               "algorithmic_GBps": adam_bytes / (ms_adam * 1e-3) / 1e9,
+                               "frac_of_hbm_peak": adam_bytes / (ms_adam * 1e-3) / 1e9 / peak}
+        del th32, m1, v1, g_keep
         # render path (Eq. 9-10): G_4D -> phi_d -> heads in one kernel, one timestamp per frame
         from dash_inputs import make_mlp_params
         extras["deform"] = {}

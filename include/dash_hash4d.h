@@ -207,6 +207,31 @@ DASH_API int dash_hash3d_indices(const dash_hash4d_config* cfg, uint64_t N,
                                  const int32_t* index,
                                  uint32_t* idx_out, float* w_out, void* cuda_stream);
 
+/* ---- Sparse optimiser step over the touched table entries (Q28) -------------------
+ * The paper does not name its optimiser; 3DGS [14] and Instant-NGP [25], which it builds on, train with Adam.
+ * Adam (bias-corrected) applied only to entries whose gradient is not exactly zero; an entry no query touched
+ * keeps theta, m and v unchanged (the rule of torch.optim.SparseAdam), and is not even read beyond its gradient:
+ *     m <- beta1 m + (1-beta1) g;  v <- beta2 v + (1-beta2) g^2;
+ *     theta <- theta - lr * (m / (1-beta1^t)) / (sqrt(v / (1-beta2^t)) + eps)          (fp32 arithmetic). */
+typedef struct dash_adam_config {
+    uint32_t struct_size; /* = sizeof(dash_adam_config)                                                     */
+    uint32_t step;        /* t >= 1, the global step count of the bias correction                           */
+    float lr, beta1, beta2, eps;
+    uint32_t flags;       /* bit0 DASH_ADAM_ZERO_GRAD: set every touched gradient entry to 0 afterwards, so
+                             the buffer is all-zero again and the next backward can accumulate into it      */
+} dash_adam_config;
+enum dash_adam_flags { DASH_ADAM_ZERO_GRAD = 1u };
+
+/*   theta    [L][T][F] fp32 master parameters (read/written).  For a fp32 table this IS the table.
+ *   table16  nullable; [L][T][F] IEEE half: receives the rounding of every updated theta (the fp16 table the
+ *            encoder reads).  Untouched entries are not rewritten.
+ *   dtable   [L][T][F] fp32 gradient (read; zeroed where touched under DASH_ADAM_ZERO_GRAD).
+ *   m, v     [L][T][F] fp32 first / second moments (read/written where touched).
+ * All five 16-byte aligned.  Only cfg->L, T, F are used. */
+DASH_API int dash_hash4d_adam_step(const dash_hash4d_config* cfg, const dash_adam_config* opt,
+                                   float* theta, void* table16, float* dtable, float* m, float* v,
+                                   void* cuda_stream);
+
 /* dtable <- 0 for the whole [L][T][F] fp32 gradient buffer (the accumulation's initial state), with the
  * library's own fill kernel on `cuda_stream`. */
 DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream);

@@ -25,7 +25,7 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
-           "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd"]
+           "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd"]
 
 
 class Hash4DError(RuntimeError):
@@ -40,6 +40,15 @@ class Hash4DConfig(C.Structure):
                 ("res_s_min", C.c_uint32), ("res_s_max", C.c_uint32),
                 ("res_t_min", C.c_uint32), ("res_t_max", C.c_uint32),
                 ("primes", C.c_uint32 * 4), ("table_dtype", C.c_uint32), ("flags", C.c_uint32)]
+
+
+class AdamConfig(C.Structure):
+    """Mirror of `struct dash_adam_config` (include/dash_hash4d.h)."""
+    _fields_ = [("struct_size", C.c_uint32), ("step", C.c_uint32), ("lr", C.c_float), ("beta1", C.c_float),
+                ("beta2", C.c_float), ("eps", C.c_float), ("flags", C.c_uint32)]
+
+
+ADAM_ZERO_GRAD = 1
 
 
 class MlpConfig(C.Structure):
@@ -105,6 +114,8 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_hash3d_bwd.restype = C.c_int
     lib.dash_hash3d_indices.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp]
     lib.dash_hash3d_indices.restype = C.c_int
+    lib.dash_hash4d_adam_step.argtypes = [cfgp, C.POINTER(AdamConfig), vp, vp, vp, vp, vp, vp]
+    lib.dash_hash4d_adam_step.restype = C.c_int
     mlpp = C.POINTER(MlpConfig)
     lib.dash_mlp_param_count.argtypes = [mlpp]
     lib.dash_mlp_param_count.restype = sz
@@ -353,6 +364,21 @@ def dash_hash3d_indices(cfg, xyz, index=None, N=None, want_weights=True):
     _check(_load().dash_hash3d_indices(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(idx), _ptr(w),
                                        _stream()))
     return idx, w
+
+
+def dash_hash4d_adam_step(cfg, theta, dtable, m, v, step, lr=1e-2, beta1=0.9, beta2=0.99, eps=1e-15, table16=None,
+                          zero_grad=True):
+    """Sparse Adam over the entries with a non-zero gradient (in place on theta, m, v[, table16], dtable)."""
+    for name, a in (("theta", theta), ("dtable", dtable), ("m", m), ("v", v)):
+        _dev(a, torch.float32, name)
+    _dev(table16, torch.float16, "table16")
+    opt = AdamConfig()
+    opt.struct_size = C.sizeof(AdamConfig)
+    opt.step, opt.lr, opt.beta1, opt.beta2, opt.eps = int(step), lr, beta1, beta2, eps
+    opt.flags = ADAM_ZERO_GRAD if zero_grad else 0
+    _check(_load().dash_hash4d_adam_step(C.byref(cfg), C.byref(opt), _ptr(theta), _ptr(table16), _ptr(dtable),
+                                         _ptr(m), _ptr(v), _stream()))
+    return theta
 
 
 # ---- render path: G_4D -> phi_d -> heads (include/dash_deform.h; PAPER.md:133-142, Eq. 9-10) -------------

@@ -512,6 +512,29 @@ DASH_API int dash_hash3d_resolutions(const dash_hash4d_config* cfg, uint32_t* re
     return ok();
 }
 
+DASH_API int dash_hash4d_adam_step(const dash_hash4d_config* cfg, const dash_adam_config* opt,
+                                   float* theta, void* table16, float* dtable, float* m, float* v,
+                                   void* cuda_stream) {
+    if (int rc = check_config(cfg, 3)) return rc;
+    if (!opt || opt->struct_size != sizeof(dash_adam_config))
+        return fail(DASH_HASH4D_INVALID_ARG, "adam config NULL or wrong struct_size");
+    if (opt->step < 1) return fail(DASH_HASH4D_INVALID_ARG, "adam step must be >= 1");
+    if (!(opt->beta1 >= 0.0f && opt->beta1 < 1.0f && opt->beta2 >= 0.0f && opt->beta2 < 1.0f) ||
+        !(opt->eps >= 0.0f) || !(opt->lr == opt->lr))
+        return fail(DASH_HASH4D_INVALID_ARG, "adam hyper-parameters out of range");
+    if (opt->flags & ~static_cast<uint32_t>(DASH_ADAM_ZERO_GRAD))
+        return fail(DASH_HASH4D_INVALID_ARG, "unknown adam flag bits 0x%x", opt->flags);
+    if (!theta || !dtable || !m || !v) return fail(DASH_HASH4D_INVALID_ARG, "theta, dtable, m or v is NULL");
+    if (!aligned16(theta) || !aligned16(dtable) || !aligned16(m) || !aligned16(v) ||
+        (table16 && !aligned16(table16)))
+        return fail(DASH_HASH4D_INVALID_ARG, "adam buffers not 16-byte aligned");
+    cudaError_t e = dash::launch_adam(table_elems(cfg), opt->lr, opt->beta1, opt->beta2, opt->eps, opt->step,
+                                      (opt->flags & DASH_ADAM_ZERO_GRAD) != 0, theta, table16, dtable, m, v,
+                                      static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "adam launch");
+    return ok();
+}
+
 DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream) {
     if (int rc = check_config(cfg, 3)) return rc;  // only L, T, F matter here (serves G_3D tables too)
     if (!dtable) return fail(DASH_HASH4D_INVALID_ARG, "dtable is NULL");

@@ -14,6 +14,8 @@
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
+#include <cmath>
+
 #include "hash4d_device.cuh"
 #include "deform_kernels.h"
 #include "hash4d_kernels.h"
@@ -477,6 +479,68 @@ validate_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
     if (bad) atomicAdd(&hdr->bad_inputs, bad);
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// Sparse Adam over the touched table entries (Q28): entries whose gradient is
+// exactly zero are skipped — theta, m, v untouched, and (four at a time) not even read.  Streaming, HBM-bound:
+// 4 B per untouched entry, 34-36 B per touched one (g, m, v, theta in; m, v, theta, [half copy], g = 0 out).
+// ------------------------------------------------------------------------------------------------
+struct AdamParams {
+    float lr, beta1, beta2, eps;
+    float omb1, omb2;      // 1 - beta1, 1 - beta2
+    float inv_c1, inv_c2;  // 1 / (1 - beta1^t), 1 / (1 - beta2^t), evaluated in double on the host
+    int zero_grad;
+};
+
+__device__ __forceinline__ void adam_one(const AdamParams& A, float g, float& th, float& m, float& v) {
+    if (g != 0.0f) {
+        m = fmaf(A.beta1, m, A.omb1 * g);
+        v = fmaf(A.beta2, v, A.omb2 * g * g);
+        th -= __fdiv_rn(A.lr * (m * A.inv_c1), sqrtf(v * A.inv_c2) + A.eps);
+    }
+}
+
+__global__ void __launch_bounds__(kBlockThreads)
+adam_step_kernel(const AdamParams A, size_t n4, size_t count, float* __restrict__ theta,
+                 __half* __restrict__ theta16, float* __restrict__ grad, float* __restrict__ m,
+                 float* __restrict__ v) {
+    const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
+    for (size_t i = static_cast<size_t>(blockIdx.x) * kBlockThreads + threadIdx.x; i < n4; i += stride) {
+        const float4 g = reinterpret_cast<const float4*>(grad)[i];
+        if (g.x == 0.0f && g.y == 0.0f && g.z == 0.0f && g.w == 0.0f) continue;  // untouched: 16 bytes read
+        float4 th = reinterpret_cast<float4*>(theta)[i];
+        float4 mm = reinterpret_cast<float4*>(m)[i];
+        float4 vv = reinterpret_cast<float4*>(v)[i];
+        adam_one(A, g.x, th.x, mm.x, vv.x);
+        adam_one(A, g.y, th.y, mm.y, vv.y);
+        adam_one(A, g.z, th.z, mm.z, vv.z);
+        adam_one(A, g.w, th.w, mm.w, vv.w);
+        reinterpret_cast<float4*>(theta)[i] = th;
+        reinterpret_cast<float4*>(m)[i] = mm;
+        reinterpret_cast<float4*>(v)[i] = vv;
+        if (theta16) {
+            const __half2 lo = __floats2half2_rn(th.x, th.y), hi = __floats2half2_rn(th.z, th.w);
+            uint2 packed;
+            packed.x = *reinterpret_cast<const uint32_t*>(&lo);
+            packed.y = *reinterpret_cast<const uint32_t*>(&hi);
+            reinterpret_cast<uint2*>(theta16)[i] = packed;
+        }
+        if (A.zero_grad) reinterpret_cast<float4*>(grad)[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    }
+    // the last count % 4 entries
+    if (blockIdx.x == 0 && threadIdx.x < count - n4 * 4) {
+        const size_t e = n4 * 4 + threadIdx.x;
+        const float g = grad[e];
+        if (g != 0.0f) {
+            float th = theta[e], mm = m[e], vv = v[e];
+            adam_one(A, g, th, mm, vv);
+            theta[e] = th; m[e] = mm; v[e] = vv;
+            if (theta16) theta16[e] = __float2half_rn(th);
+            if (A.zero_grad) grad[e] = 0.0f;
+        }
+    }
+}
+
 int sm_count() {
     static int sms = 0;
     if (!sms) {
@@ -677,6 +741,28 @@ cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t co
     const size_t cap = static_cast<size_t>(sm_count()) * 16;
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
     fixed_finalize_kernel<<<blocks, kBlockThreads, 0, s>>>(acc, dtable, count, hdr, overwrite ? 1 : 0);
+    return after_launch();
+}
+
+cudaError_t launch_adam(size_t count, double lr, double beta1, double beta2, double eps, uint32_t step,
+                        bool zero_grad, float* theta, void* theta16, float* grad, float* m, float* v,
+                        cudaStream_t s) {
+    AdamParams A;
+    A.lr = static_cast<float>(lr);
+    A.beta1 = static_cast<float>(beta1);
+    A.beta2 = static_cast<float>(beta2);
+    A.eps = static_cast<float>(eps);
+    A.omb1 = static_cast<float>(1.0 - beta1);
+    A.omb2 = static_cast<float>(1.0 - beta2);
+    A.inv_c1 = static_cast<float>(1.0 / (1.0 - std::pow(beta1, static_cast<double>(step))));
+    A.inv_c2 = static_cast<float>(1.0 / (1.0 - std::pow(beta2, static_cast<double>(step))));
+    A.zero_grad = zero_grad ? 1 : 0;
+    const size_t n4 = count / 4;
+    const size_t want = (n4 + kBlockThreads - 1) / kBlockThreads;
+    const size_t cap = static_cast<size_t>(sm_count()) * 8;
+    const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
+    adam_step_kernel<<<blocks, kBlockThreads, 0, s>>>(A, n4, count, theta, static_cast<__half*>(theta16), grad,
+                                                      m, v);
     return after_launch();
 }
 
