@@ -162,3 +162,48 @@ def test_deform_errors():
         dh.dash_mlp_fwd(big, torch.zeros((4, 256), device="cuda"), torch.zeros(dh.dash_mlp_param_count(big),
                                                                                 device="cuda"))
     assert e.value.status == 2
+
+
+def test_render_and_train_calls_are_cuda_graph_capturable():
+    """dash_deform_fwd (fused), dash_hash3d_fwd and dash_hash4d_adam_step only enqueue kernels: a render frame and an
+    optimiser step replay from one CUDA graph and give the directly launched results bit for bit."""
+    wl = make_workload("C2", n_override=20_000)
+    enc, N = wl.spec.enc, wl.N
+    gcfg = dh.config_from_params(enc, flags=DC | dh.FLAG_ZERO_GRAD)
+    cfg_plain = dh.config_from_params(enc)
+    widths = [enc.L * enc.F, 64, 10]
+    m = dh.make_mlp_config(widths)
+    xyz, t, dout = dev(wl.xyz), dev(wl.t), dev(wl.dout)
+    table, prm = dev(wl.table * 1e4), dev(make_mlp_params(1, widths))
+    out = torch.empty((N, 10), device="cuda")
+    f3 = torch.empty((N, enc.L * enc.F), device="cuda")
+    dt = torch.empty((enc.L, enc.T, enc.F), device="cuda")
+    theta = table.clone()
+    m1, v1 = torch.zeros_like(theta), torch.zeros_like(theta)
+
+    def step():
+        dh.dash_deform_fwd(cfg_plain, m, xyz, t, table, prm, out=out)
+        dh.dash_hash3d_fwd(cfg_plain, xyz, table, out=f3)
+        dh.dash_hash4d_bwd(gcfg, xyz, t, dout, dt)
+        dh.dash_hash4d_adam_step(gcfg, theta, dt, m1, v1, 1)
+
+    step()
+    torch.cuda.synchronize()
+    want = [a.clone() for a in (out, f3, theta, m1, v1)]
+    theta.copy_(table); m1.zero_(); v1.zero_(); out.fill_(-1); f3.fill_(-1)
+    graph = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()
+    torch.cuda.current_stream().wait_stream(side)
+    theta.copy_(table); m1.zero_(); v1.zero_()
+    with torch.cuda.graph(graph):
+        step()
+    theta.copy_(table); m1.zero_(); v1.zero_(); out.fill_(-1); f3.fill_(-1)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, want[0]) and torch.equal(f3, want[1])
+    # the scatter order varies run to run (fp32 reductions): the optimiser state agrees to rounding, not bitwise
+    torch.testing.assert_close(theta, want[2], rtol=1e-4, atol=1e-6)
+    assert float(dt.abs().max()) == 0.0
