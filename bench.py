@@ -394,10 +394,15 @@ def run_cuda(args):
             os.environ.pop("DASH_DEFORM_FUSED")
             row["encoder_only_ms"] = timed(lambda: dh.dash_hash4d_fwd(cfg2, x2, one, tab2, out=f2, t_stride=0), 20)
             row["mlp_only_ms"] = timed(lambda: dh.dash_mlp_fwd(mlp, f2, prm, out=o2), 20)
+            sl2 = torch.empty((e2.L, e2.T, e2.F), dtype=torch.float32, device="cuda")
+            row["slice_t_ms"] = timed(lambda: dh.dash_hash4d_slice_t(cfg2, one, tab2, slice_out=sl2), 20)
+            row["slice_encoder_only_ms"] = timed(lambda: dh.dash_hash4d_slice_fwd(cfg2, x2, sl2, out=f2), 20)
+            row["slice_fused_ms"] = timed(lambda: dh.dash_deform_slice_fwd(cfg2, mlp, x2, sl2, prm, out=o2), 20)
+            row["frame_ms_slice_path"] = row["slice_t_ms"] + row["slice_fused_ms"]
             row["mlp_tflops"] = 2.0 * w2.N * sum(a * b for a, b in zip(widths[:-1], widths[1:])) / (
                 row["mlp_only_ms"] * 1e-3) / 1e12
             extras["deform"][name] = row
-            del x2, tab2, o2, f2, ws2
+            del x2, tab2, o2, f2, ws2, sl2
 
     if not rep.is_reporter:
         rep.close()

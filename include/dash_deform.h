@@ -72,6 +72,30 @@ DASH_API int dash_deform_fwd(const dash_hash4d_config* enc, const dash_mlp_confi
                              float* out,
                              void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- Time slice: the render path at ONE timestamp (the rendered frame has one t; Q29) -----
+ * For a fixed t, Eq. 9 factors: the two t-layers of every level are blended ONCE per frame,
+ *     hashed level (power-of-two T):  slice[l][u]  = (1-w_t) table[l][u ^ a] + w_t table[l][u ^ b],
+ *                                     a = (c_t pi_t) mod T, b = ((c_t+1) pi_t) mod T      (mod 2^k commutes with XOR)
+ *     dense level:                    slice[l][s3] = (1-w_t) table[l][s3 + S^3 c_t] + w_t table[l][s3 + S^3 (c_t+1)]
+ * and every query then interpolates 8 instead of 16 vertices, at slot (g_x pi_x ^ g_y pi_y ^ g_z pi_z) mod T resp.
+ * g_x + S(g_y + S g_z).  Same value as dash_hash4d_fwd with t_stride = 0 up to fp32 rounding; half the gathers.
+ * Pays when N is not small against T (the blend streams 3 * L*T*F entries).
+ *   t       DEVICE pointer to the one timestamp.       slice   [L][T][F] fp32 (written; 16-byte aligned).
+ * UNSUPPORTED when a hashed level exists and T is not a power of two.  cfg->flags: DENSE_COARSE only. */
+DASH_API int dash_hash4d_slice_t(const dash_hash4d_config* cfg, const float* t, const void* table,
+                                 float* slice, void* cuda_stream);
+
+/* out[n][l*F+f] = G_4D(xyz_n, t)[l*F+f] from a slice made by dash_hash4d_slice_t with the same cfg ([N][L*F] fp32). */
+DASH_API int dash_hash4d_slice_fwd(const dash_hash4d_config* cfg, uint64_t N,
+                                   const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                   const float* slice, float* out, void* cuda_stream);
+
+/* dash_deform_fwd on a slice: out[n] = base[n] + MLP(G_4D(xyz_n, t)), the fused kernel with 8-corner gathers. */
+DASH_API int dash_deform_slice_fwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
+                                   const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                   const float* slice, const float* params, const float* base,
+                                   float* out, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

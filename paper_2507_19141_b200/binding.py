@@ -25,7 +25,8 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
-           "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd"]
+           "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd",
+           "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd"]
 
 
 class Hash4DError(RuntimeError):
@@ -125,6 +126,12 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_deform_workspace_bytes.restype = sz
     lib.dash_deform_fwd.argtypes = [cfgp, mlpp, u64, vp, u32, vp, u32, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.dash_deform_fwd.restype = C.c_int
+    lib.dash_hash4d_slice_t.argtypes = [cfgp, vp, vp, vp, vp]
+    lib.dash_hash4d_slice_t.restype = C.c_int
+    lib.dash_hash4d_slice_fwd.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp]
+    lib.dash_hash4d_slice_fwd.restype = C.c_int
+    lib.dash_deform_slice_fwd.argtypes = [cfgp, mlpp, u64, vp, u32, vp, vp, vp, vp, vp, vp]
+    lib.dash_deform_slice_fwd.restype = C.c_int
     lib.dash_hash4d_launch_count.argtypes = [C.c_int]
     lib.dash_hash4d_launch_count.restype = u64
     _lib = lib
@@ -435,6 +442,48 @@ def dash_deform_fwd(cfg, mlp, xyz, t, table, params, base=None, out=None, index=
     _check(_load().dash_deform_fwd(C.byref(cfg), C.byref(mlp), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
                                    _ptr(table), _ptr(params), _ptr(base), _ptr(out), _ptr(workspace), wbytes,
                                    _stream()))
+    return out
+
+
+# ---- time slice: the render path at one timestamp (include/dash_deform.h; Q29) -----------------
+
+def dash_hash4d_slice_t(cfg, t, table, slice_out=None):
+    """slice[l][u] = blend of the two t-layers of level l at the one timestamp t ([L][T][F] fp32, CUDA)."""
+    _dev(t, torch.float32, "t")
+    _dev(table, torch.float16 if cfg.table_dtype == 1 else torch.float32, "table")
+    if slice_out is None:
+        slice_out = torch.empty((cfg.L, cfg.T, cfg.F), dtype=torch.float32, device=table.device)
+    _dev(slice_out, torch.float32, "slice")
+    _check(_load().dash_hash4d_slice_t(C.byref(cfg), _ptr(t), _ptr(table), _ptr(slice_out), _stream()))
+    return slice_out
+
+
+def dash_hash4d_slice_fwd(cfg, xyz, slice_t, out=None, index=None, N=None):
+    """G_4D(xyz_n, t) from a slice: 8-corner lookups; returns `out` ([N][L*F] fp32)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index"); _dev(slice_t, torch.float32, "slice")
+    xs = _xyz_stride(xyz)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    if out is None:
+        out = torch.empty((N, cfg.L * cfg.F), dtype=torch.float32, device=xyz.device)
+    _dev(out, torch.float32, "out")
+    _check(_load().dash_hash4d_slice_fwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(slice_t), _ptr(out),
+                                         _stream()))
+    return out
+
+
+def dash_deform_slice_fwd(cfg, mlp, xyz, slice_t, params, base=None, out=None, index=None, N=None):
+    """out[n] = base[n] + MLP(G_4D(xyz_n, t)) from a slice, fused kernel with 8-corner gathers."""
+    _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index"); _dev(slice_t, torch.float32, "slice")
+    _dev(params, torch.float32, "params"); _dev(base, torch.float32, "base")
+    xs = _xyz_stride(xyz)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    if out is None:
+        out = torch.empty((N, int(mlp.width[mlp.n_layers])), dtype=torch.float32, device=xyz.device)
+    _dev(out, torch.float32, "out")
+    _check(_load().dash_deform_slice_fwd(C.byref(cfg), C.byref(mlp), N, _ptr(xyz), xs, _ptr(index), _ptr(slice_t),
+                                         _ptr(params), _ptr(base), _ptr(out), _stream()))
     return out
 
 

@@ -147,7 +147,7 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------------------
-template <int F, bool HALF, bool FUSED>
+template <int F, bool HALF, bool FUSED, int D>
 __global__ void __launch_bounds__(kDeformThreads, 1)
 deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpPlan M,
                     const float* __restrict__ xyz, const float* __restrict__ t,
@@ -293,27 +293,28 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                     const uint64_t n = row0 + (rr * 16u + pair) / P.L;
                     return n < r_end ? n : r_end - 1;  // ragged last round: duplicate work, rows never stored
                 };
+                constexpr int NC = 1 << (D - 1);   // D = 3: lookups in a time slice (8 corners), D = 4: Eq. 9 as is
                 float cq[4];
-                if (w0 < rounds) load_coords<4>(P, item_row(w0), xyz, t, index, cq);
+                if (w0 < rounds) load_coords<D>(P, item_row(w0), xyz, t, index, cq);
                 for (uint32_t rr = w0; rr < rounds; rr += kDeformEncWarps) {
                     const uint32_t it = rr * 16u + pair, q = it / P.L, l = it - q * P.L;
                     const LevelParams lp = P.lv[l];
-                    const Query qq = make_query<4>(lp, cq[0], cq[1], cq[2], cq[3]);
-                    uint32_t slot[8];
-                    float W[8];
-                    half_cell<4>(P, lp, qq, xc, slot, W);
+                    const Query qq = make_query<D>(lp, cq[0], cq[1], cq[2], cq[3]);
+                    uint32_t slot[NC];
+                    float W[NC];
+                    half_cell<D>(P, lp, qq, xc, slot, W);
                     const char* level_base =
                         static_cast<const char*>(table) + static_cast<size_t>(l) * P.T * (F * kElem);
-                    float v[8][F];
+                    float v[NC][F];
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);
+                    for (int j = 0; j < NC; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);
                     if (rr + kDeformEncWarps < rounds)
-                        load_coords<4>(P, item_row(rr + kDeformEncWarps), xyz, t, index, cq);
+                        load_coords<D>(P, item_row(rr + kDeformEncWarps), xyz, t, index, cq);
                     float acc[F];
 #pragma unroll
                     for (int f = 0; f < F; ++f) acc[f] = 0.0f;
 #pragma unroll
-                    for (int j = 0; j < 8; ++j)
+                    for (int j = 0; j < NC; ++j)
 #pragma unroll
                         for (int f = 0; f < F; ++f) acc[f] = fmaf(W[j], v[j][f], acc[f]);
 #pragma unroll
@@ -457,11 +458,11 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
 }
 
 // ------------------------------------------------------------------------------------------------------------
-template <int F, bool HALF, bool FUSED>
+template <int F, bool HALF, bool FUSED, int D>
 static cudaError_t launch_t(const Plan& P, const MlpPlan& M, const float* xyz, const float* t,
                             const int32_t* index, const void* table, const float* feat, const float* params,
                             const float* base, float* out, int sms, cudaStream_t s) {
-    auto* k = deform_fused_kernel<F, HALF, FUSED>;
+    auto* k = deform_fused_kernel<F, HALF, FUSED, D>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(M.smem_bytes));
     if (e != cudaSuccess) return e;
@@ -476,7 +477,19 @@ cudaError_t launch_deform_fused(const Plan& P, const MlpPlan& M, const float* xy
                                 const float* params, const float* base, float* out, int sms,
                                 cudaStream_t s) {
 #define DASH_DF(FV, HV) \
-    return launch_t<FV, HV, true>(P, M, xyz, t, index, table, nullptr, params, base, out, sms, s)
+    return launch_t<FV, HV, true, 4>(P, M, xyz, t, index, table, nullptr, params, base, out, sms, s)
+#define DASH_DF3(FV) \
+    return launch_t<FV, false, true, 3>(P, M, xyz, t, index, table, nullptr, params, base, out, sms, s)
+    if (P.dims == 3) {  // lookups in a time slice (fp32, Q29) or a G_3D table
+        if (table_half) return cudaErrorInvalidValue;
+        switch (P.F) {
+            case 1: DASH_DF3(1);
+            case 2: DASH_DF3(2);
+            case 4: DASH_DF3(4);
+            case 8: DASH_DF3(8);
+            default: return cudaErrorInvalidValue;
+        }
+    }
     switch (P.F * 2 + (table_half ? 1 : 0)) {
         case 2: DASH_DF(1, false);
         case 3: DASH_DF(1, true);
@@ -489,12 +502,13 @@ cudaError_t launch_deform_fused(const Plan& P, const MlpPlan& M, const float* xy
         default: return cudaErrorInvalidValue;
     }
 #undef DASH_DF
+#undef DASH_DF3
 }
 
 cudaError_t launch_mlp(const MlpPlan& M, const float* feat, const float* params, const float* base,
                        float* out, int sms, cudaStream_t s) {
     Plan P{};  // unused by the non-fused instantiation
-    return launch_t<1, false, false>(P, M, nullptr, nullptr, nullptr, nullptr, feat, params, base, out, sms,
+    return launch_t<1, false, false, 4>(P, M, nullptr, nullptr, nullptr, nullptr, feat, params, base, out, sms,
                                      s);
 }
 

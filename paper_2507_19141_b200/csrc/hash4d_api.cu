@@ -713,3 +713,95 @@ DASH_API int dash_deform_fwd(const dash_hash4d_config* enc, const dash_mlp_confi
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------
+// Time slice (render path; Q29): collapse the tables at one timestamp, then 8-corner lookups
+// ------------------------------------------------------------------------------------------------------------
+namespace {
+
+// the plan of the D = 3 kernels on a slice: the 4D schedule's dense/hashed decision per level, three axes
+int fill_slice_plan(const dash_hash4d_config* cfg, uint64_t N, uint32_t xyz_stride, uint32_t group, Plan* P) {
+    if (int rc = fill_plan(cfg, N, xyz_stride, 0, group, P, 4)) return rc;
+    P->dims = 3;
+    for (uint32_t l = 0; l < cfg->L; ++l) P->lv[l].m[3] = 0;
+    return DASH_HASH4D_OK;
+}
+
+int check_sliceable(const dash_hash4d_config* cfg) {
+    if (int rc = check_config(cfg)) return rc;
+    if (cfg->flags & ~static_cast<uint32_t>(DASH_HASH4D_FLAG_DENSE_COARSE))
+        return fail(DASH_HASH4D_INVALID_ARG, "slice calls: only DENSE_COARSE may be set in cfg->flags");
+    if ((cfg->T & (cfg->T - 1)) != 0) {
+        Schedule s;
+        make_schedule(cfg, &s);
+        for (uint32_t l = 0; l < cfg->L; ++l)
+            if (!s.dense[l])
+                return fail(DASH_HASH4D_UNSUPPORTED,
+                            "time slice needs a power-of-two T on hashed levels (level %u, T = %u)", l, cfg->T);
+    }
+    return DASH_HASH4D_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+DASH_API int dash_hash4d_slice_t(const dash_hash4d_config* cfg, const float* t, const void* table,
+                                 float* slice, void* cuda_stream) {
+    if (int rc = check_sliceable(cfg)) return rc;
+    if (!t || !table || !slice) return fail(DASH_HASH4D_INVALID_ARG, "t, table or slice is NULL");
+    if (!aligned16(table) || !aligned16(slice))
+        return fail(DASH_HASH4D_INVALID_ARG, "table / slice not 16-byte aligned");
+    Plan P;
+    if (int rc = fill_plan(cfg, 1, 3, 0, 1, &P, 4)) return rc;
+    cudaError_t e = dash::launch_slice_t(P, t, table, cfg->table_dtype == DASH_HASH4D_FP16, slice,
+                                         static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "slice launch");
+    return ok();
+}
+
+DASH_API int dash_hash4d_slice_fwd(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                                   uint32_t xyz_stride, const int32_t* index, const float* slice,
+                                   float* out, void* cuda_stream) {
+    if (int rc = check_sliceable(cfg)) return rc;
+    if (N == 0) return ok();
+    if (int rc = check_queries(xyz, xyz_stride, nullptr, 0, index, 3)) return rc;
+    if (!slice || !out) return fail(DASH_HASH4D_INVALID_ARG, "slice or out is NULL");
+    if (!aligned16(slice) || !aligned16(out))
+        return fail(DASH_HASH4D_INVALID_ARG, "slice / out not 16-byte aligned");
+    const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * sizeof(float);
+    Plan P;
+    if (int rc = fill_slice_plan(cfg, N, xyz_stride, pick_group(cfg, level_bytes, "DASH_HASH4D_FWD_GROUP"), &P))
+        return rc;
+    cudaError_t e = dash::launch_fwd(P, xyz, nullptr, index, slice, false, out,
+                                     static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "slice fwd launch");
+    return ok();
+}
+
+DASH_API int dash_deform_slice_fwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
+                                   const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                   const float* slice, const float* params, const float* base, float* out,
+                                   void* cuda_stream) {
+    if (int rc = check_sliceable(enc)) return rc;
+    if (int rc = check_mlp(mlp)) return rc;
+    if (mlp->width[0] != enc->L * enc->F)
+        return fail(DASH_HASH4D_INVALID_ARG, "mlp width[0] = %u != L*F = %u", mlp->width[0], enc->L * enc->F);
+    dash::MlpPlan M;
+    if (int rc = fill_mlp_plan(mlp, N, &M)) return rc;
+    if (N == 0) return ok();
+    if (int rc = check_queries(xyz, xyz_stride, nullptr, 0, index, 3)) return rc;
+    if (!slice || !params || !out) return fail(DASH_HASH4D_INVALID_ARG, "slice, params or out is NULL");
+    if (!aligned16(slice)) return fail(DASH_HASH4D_INVALID_ARG, "slice not 16-byte aligned");
+    if ((reinterpret_cast<uintptr_t>(params) | reinterpret_cast<uintptr_t>(base) |
+         reinterpret_cast<uintptr_t>(out)) & 3u)
+        return fail(DASH_HASH4D_INVALID_ARG, "params / base / out not 4-byte aligned");
+    Plan P;
+    if (int rc = fill_slice_plan(enc, N, xyz_stride, 1, &P)) return rc;
+    cudaError_t e = dash::launch_deform_fused(P, M, xyz, nullptr, index, slice, false, params, base, out,
+                                              dash::device_sm_count(), static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "deform slice launch");
+    return ok();
+}
+
+}  // extern "C"

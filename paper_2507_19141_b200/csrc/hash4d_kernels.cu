@@ -541,6 +541,50 @@ adam_step_kernel(const AdamParams A, size_t n4, size_t count, float* __restrict_
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Time slice of the tables at ONE timestamp (render path, "one timestamp per rendered frame";
+// DESIGN.md Q29).  For a fixed t the 16-corner interpolation of Eq. 9 factors into a blend of the two
+// t-layers, done here once per frame over the whole level, and an 8-corner lookup per query (the D = 3
+// kernels on the slice):  hashed level, power-of-two T:  slice[u] = (1-w) tab[u ^ a] + w tab[u ^ b],
+// a = (c_t pi_4) mod T, b = ((c_t+1) pi_4) mod T ("mod 2^k" commutes with XOR);  dense level:
+// slice[s3] = (1-w) tab[s3 + S^3 c_t] + w tab[s3 + S^3 (c_t+1)], s3 < S^3.  Streaming: 2 reads, 1 write.
+// ------------------------------------------------------------------------------------------------
+template <int F, bool HALF>
+__global__ void __launch_bounds__(kBlockThreads)
+slice_t_kernel(const __grid_constant__ Plan P, const float* __restrict__ t,
+               const void* __restrict__ table, float* __restrict__ slice) {
+    const uint32_t l = blockIdx.y;
+    const LevelParams lp = P.lv[l];
+    uint32_t ct;
+    float wt;
+    locate(__ldg(t), lp.nt_f, ct, wt);
+    const uint32_t count = lp.dense ? lp.m[3] : P.T;           // dense: m[3] = S^3 vertices per t-layer
+    const uint32_t a = lp.dense ? lp.m[3] * ct : (ct * lp.m[3]) & P.t_mask;
+    const uint32_t b = lp.dense ? a + lp.m[3] : ((ct + 1u) * lp.m[3]) & P.t_mask;
+    constexpr size_t kElem = HALF ? 2 : 4;
+    const char* level_base = static_cast<const char*>(table) + static_cast<size_t>(l) * P.T * (F * kElem);
+    float* dst = slice + static_cast<size_t>(l) * P.T * F;
+    const float w0 = 1.0f - wt;
+    for (uint32_t u = blockIdx.x * kBlockThreads + threadIdx.x; u < count; u += gridDim.x * kBlockThreads) {
+        float v0[F], v1[F], r[F];
+        load_slot<F, HALF>(level_base, lp.dense ? u + a : u ^ a, v0);
+        load_slot<F, HALF>(level_base, lp.dense ? u + b : u ^ b, v1);
+#pragma unroll
+        for (int f = 0; f < F; ++f) r[f] = fmaf(wt, v1[f], w0 * v0[f]);
+        float* o = dst + static_cast<size_t>(u) * F;
+        if constexpr (F == 1) {
+            o[0] = r[0];
+        } else if constexpr (F == 2) {
+            *reinterpret_cast<float2*>(o) = make_float2(r[0], r[1]);
+        } else if constexpr (F == 4) {
+            *reinterpret_cast<float4*>(o) = make_float4(r[0], r[1], r[2], r[3]);
+        } else {
+            *reinterpret_cast<float4*>(o) = make_float4(r[0], r[1], r[2], r[3]);
+            *(reinterpret_cast<float4*>(o) + 1) = make_float4(r[4], r[5], r[6], r[7]);
+        }
+    }
+}
+
 int sm_count() {
     static int sms = 0;
     if (!sms) {
@@ -741,6 +785,27 @@ cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t co
     const size_t cap = static_cast<size_t>(sm_count()) * 16;
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
     fixed_finalize_kernel<<<blocks, kBlockThreads, 0, s>>>(acc, dtable, count, hdr, overwrite ? 1 : 0);
+    return after_launch();
+}
+
+cudaError_t launch_slice_t(const Plan& P, const float* t, const void* table, bool table_half, float* slice,
+                           cudaStream_t s) {
+    const unsigned per_level = (P.T + kBlockThreads - 1) / kBlockThreads;
+    const unsigned cap = static_cast<unsigned>(sm_count()) * 8u / (P.L < 8 ? 1u : P.L / 8u);
+    const dim3 grid(per_level < cap ? per_level : (cap ? cap : 1u), P.L, 1), block(kBlockThreads);
+#define DASH_SL(FV, HV) slice_t_kernel<FV, HV><<<grid, block, 0, s>>>(P, t, table, slice)
+    switch (P.F * 2 + (table_half ? 1 : 0)) {
+        case 2: DASH_SL(1, false); break;
+        case 3: DASH_SL(1, true); break;
+        case 4: DASH_SL(2, false); break;
+        case 5: DASH_SL(2, true); break;
+        case 8: DASH_SL(4, false); break;
+        case 9: DASH_SL(4, true); break;
+        case 16: DASH_SL(8, false); break;
+        case 17: DASH_SL(8, true); break;
+        default: return cudaErrorInvalidValue;
+    }
+#undef DASH_SL
     return after_launch();
 }
 
