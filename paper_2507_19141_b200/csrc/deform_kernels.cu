@@ -11,8 +11,9 @@
 //                           M = 128, N = layer width, K = 16 per instruction); accumulators live in TMEM.  The
 //                           bias rides in the MMA: two extra K columns hold b as bf16 hi + lo against 1.0 in A.
 //                 EPILOGUE  all 4 warps tcgen05.ld the accumulator rows (warp e owns TMEM lanes 32e..32e+31),
-//                           relu, -> bf16 -> the next layer's A operand in shared memory; last layer: + base,
-//                           store.  No shared-memory loads: the LSU queue belongs to the producers' gathers.
+//                           relu, -> bf16 -> tcgen05.st into the TMEM A operand of the next layer (TS-form MMA);
+//                           last layer: + base, store.  No shared-memory traffic at all between layers: the
+//                           SM's LSU queue belongs to the producers' gathers.
 //   The layers of one tile are a dependent chain (MMA -> epilogue -> MMA ...); two pipelines keep the tensor
 //   pipe and the epilogue of one tile busy while the other tile waits on a hand-off.
 //
@@ -86,6 +87,35 @@ __device__ __forceinline__ void tc_mma_bf16(uint32_t tmem_d, uint64_t adesc, uin
         "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// D[tmem] (+)= A[tmem] * B[smem]^T ; A: 128 lanes x 8 columns, each 32-bit column two bf16 along K (even k low)
+__device__ __forceinline__ void tc_mma_bf16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc,
+                                               uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
+        "}" ::"r"(tmem_d),
+        "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// registers -> 16 / 8 consecutive 32-bit columns of this thread's TMEM lane
+__device__ __forceinline__ void tc_st16(uint32_t taddr, const uint32_t r[16]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, "
+        "%14, %15, %16};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+        "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+__device__ __forceinline__ void tc_st8(uint32_t taddr, const uint32_t r[8]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
+        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+        : "memory");
+}
+__device__ __forceinline__ void tc_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
 // 16 consecutive fp32 accumulator columns of this thread's TMEM lane
 __device__ __forceinline__ void tc_ld16(uint32_t taddr, float v[16]) {
     uint32_t r[16];
@@ -139,6 +169,22 @@ __device__ __forceinline__ uint32_t operand_offset(uint32_t lbo, uint32_t row, u
     return (col >> 3) * lbo + row * 16u + (col & 7u) * 2u;
 }
 
+// Explicit shared-space stores on 32-bit shared addresses.  Stores through generic pointers into `extern
+// __shared__` made the compiler rebuild the shared window base (S2UR SR_CgaCtaId + ULEA) in the hot loop: 25 % of
+// the producers' stall samples were short-scoreboard waits on that chain (profiles/ncu_deform_adam_r01c.md).
+__device__ __forceinline__ void sts16(uint32_t a, uint16_t v) {
+    asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(v) : "memory");
+}
+__device__ __forceinline__ void sts32(uint32_t a, uint32_t v) {
+    asm volatile("st.shared.b32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ void sts64(uint32_t a, uint32_t x, uint32_t y) {
+    asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(a), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);  // .x = lo (low 16 bits)
     return *reinterpret_cast<const uint32_t*>(&h);
@@ -158,7 +204,8 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
 #ifdef DASH_DEFORM_PROFILE
     const long long t_entry = clock64();
 #endif
-    const uint32_t sbase = smem_u32(smem);
+    uint32_t sbase = smem_u32(smem);
+    asm volatile("" : "+r"(sbase));   // opaque: keep it in a register instead of re-deriving the shared window base
     const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31u;
     // barriers (8 bytes each): full[2] @0, empty[2] @16, mma_done[2] @32; TMEM base (u32) @64.
     // A buffer s, pipeline p and tile parity coincide: tile i of this CTA uses s = p = i & 1.
@@ -184,13 +231,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                      "r"(M.tmem_cols)
                      : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-#ifdef DASH_DEFORM_PROFILE
-        if (blockIdx.x == 0 && lane == 0) printf("alloc done at %lld\n", clock64() - t_entry);
-#endif
     }
-#ifdef DASH_DEFORM_PROFILE
-    const long long t_s1 = clock64();
-#endif
     for (uint32_t l = 0; l < M.n_layers; ++l) {
         // W_l as the B operand [npad][kpad], one 16-byte chunk (8 consecutive k of one output row j) per step;
         // consecutive threads take consecutive chunks of a row: coalesced (float4 when aligned) global reads; the
@@ -232,30 +273,23 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                            pack_bf16(w[6], w[7]));
         }
     }
-#ifdef DASH_DEFORM_PROFILE
-    const long long t_s2 = clock64();
-#endif
     for (uint32_t i = tid; i < (2u * a0_bytes) / 16u; i += kDeformThreads) {
         const uint32_t within = (i * 16u) % a0_bytes;                     // byte offset inside one A buffer
         reinterpret_cast<uint4*>(smem + M.a0_off)[i] =
             (within / a_lbo == (M.kbias[0] >> 3)) ? ones_chunk : make_uint4(0u, 0u, 0u, 0u);
     }
-#ifdef DASH_DEFORM_PROFILE
-    const long long t_s3 = clock64();
-#endif
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
-#ifdef DASH_DEFORM_PROFILE
-    if (blockIdx.x == 0 && (tid == 0 || tid == 1023))
-        printf("tid %u: init %lld weights %lld a0 %lld sync %lld\n", tid, t_s1 - t_entry, t_s2 - t_s1, t_s3 - t_s2,
-               clock64() - t_s3);
-#endif
+
 #ifdef DASH_DEFORM_PROFILE
     __shared__ long long prof[3][64];
-    const long long t_setup = clock64();
+    __shared__ long long prof_t0;
+    if (tid == 0) { prof_t0 = clock64(); prof[0][40] = prof[0][41] = prof[0][42] = 0; }
+    __syncthreads();
+    const long long t_setup = prof_t0;   // one time base for all roles (SM clock)
 #define PROF(role, idx) do { if (blockIdx.x == 0 && (idx) < 64) prof[role][idx] = clock64() - t_setup; } while (0)
 #else
 #define PROF(role, idx) do { } while (0)
@@ -277,7 +311,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
             const uint32_t rows_here = r_end - row0 < kDeformTileM ? static_cast<uint32_t>(r_end - row0) : kDeformTileM;
             mbar_wait(bar_empty + 8 * s, ((i >> 1) & 1u) ^ 1u);  // first use of each buffer passes at once
             if (tid == 0) PROF(0, 2 * i);
-            unsigned char* a0 = smem + M.a0_off + s * a0_bytes;
+            const uint32_t a0 = sbase + M.a0_off + s * a0_bytes;   // shared-space address of this tile's A buffer
             if constexpr (FUSED) {
                 // One ROUND = 16 (query, level) items = one warp instruction's worth of lane pairs; a full tile has
                 // 8*L rounds, taken by the warps round-robin.  The coordinates of a warp's NEXT round are loaded under
@@ -290,48 +324,96 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                 const uint32_t w0 = (warp + 8u * i) % kDeformEncWarps;
                 constexpr size_t kElem = HALF ? 2 : 4;
                 auto item_row = [&](uint32_t rr) -> uint64_t {
-                    const uint64_t n = row0 + (rr * 16u + pair) / P.L;
+                    const uint32_t it = rr * 16u + pair;
+                    const uint64_t n = row0 + ((P.L & (P.L - 1u)) == 0u ? it >> (31u - __clz(P.L)) : it / P.L);
                     return n < r_end ? n : r_end - 1;  // ragged last round: duplicate work, rows never stored
                 };
                 constexpr int NC = 1 << (D - 1);   // D = 3: lookups in a time slice (8 corners), D = 4: Eq. 9 as is
-                float cq[4];
-                if (w0 < rounds) load_coords<D>(P, item_row(w0), xyz, t, index, cq);
-                for (uint32_t rr = w0; rr < rounds; rr += kDeformEncWarps) {
-                    const uint32_t it = rr * 16u + pair, q = it / P.L, l = it - q * P.L;
-                    const LevelParams lp = P.lv[l];
-                    const Query qq = make_query<D>(lp, cq[0], cq[1], cq[2], cq[3]);
-                    uint32_t slot[NC];
-                    float W[NC];
-                    half_cell<D>(P, lp, qq, xc, slot, W);
-                    const char* level_base =
-                        static_cast<const char*>(table) + static_cast<size_t>(l) * P.T * (F * kElem);
-                    float v[NC][F];
+                // Gathers in flight set the rate: the SM's load queue is served at ~1 wavefront per cycle behind a
+                // fixed ~1.2K-cycle L2 round trip, so throughput ~ W / (W + 1.2K) with W the queued wavefronts
+                // (24 warps x 8 loads x 17 lines = 3.3K -> 0.73, measured).  R rounds per warp iteration: R = 2 was
+                // measured slower for both D = 4 (34K vs 21K cycles per tile) and D = 3 (87 vs 75 us at C2), so R = 1.
+                constexpr int R = 1;
+                constexpr uint32_t kStep = R * kDeformEncWarps;
+                // When L divides 16 a lane pair serves the SAME level in every round (l = pair mod L): its level
+                // constants and table base are then fetched once, not per round — the indexed constant loads and
+                // the integer divisions were 2K of the ~3.2K cycles a round took (clock64 phase timers).
+                const bool fixed_level = (16u % P.L) == 0u;
+                const uint32_t l_shift = 31u - __clz(P.L);           // valid when L is a power of two
+                LevelParams lp_fix = P.lv[pair % P.L];
+                const char* base_fix =
+                    static_cast<const char*>(table) + static_cast<size_t>(pair % P.L) * P.T * (F * kElem);
+                float cq[R][4];
 #pragma unroll
-                    for (int j = 0; j < NC; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);
-                    if (rr + kDeformEncWarps < rounds)
-                        load_coords<D>(P, item_row(rr + kDeformEncWarps), xyz, t, index, cq);
-                    float acc[F];
+                for (int k = 0; k < R; ++k) {
+                    const uint32_t rk = w0 + k * kDeformEncWarps;
+                    if (w0 < rounds) load_coords<D>(P, item_row(rk < rounds ? rk : w0), xyz, t, index, cq[k]);
+                }
+                for (uint32_t ra = w0; ra < rounds; ra += kStep) {
+#ifdef DASH_DEFORM_PROFILE
+                    const long long q0 = clock64();
+#endif
+                    uint32_t rk[R];
+                    uint32_t slot[R][NC];
+                    float W[R][NC];
+                    float v[R][NC][F];
 #pragma unroll
-                    for (int f = 0; f < F; ++f) acc[f] = 0.0f;
+                    for (int k = 0; k < R; ++k) {
+                        rk[k] = ra + k * kDeformEncWarps < rounds ? ra + k * kDeformEncWarps : ra;  // past the end:
+                        LevelParams lp = lp_fix;                                         // redo round ra, no store
+                        const char* level_base = base_fix;
+                        if (!fixed_level) {
+                            const uint32_t l = (rk[k] * 16u + pair) % P.L;
+                            lp = P.lv[l];
+                            level_base = static_cast<const char*>(table) + static_cast<size_t>(l) * P.T * (F * kElem);
+                        }
+                        const Query qq = make_query<D>(lp, cq[k][0], cq[k][1], cq[k][2], cq[k][3]);
+                        half_cell<D>(P, lp, qq, xc, slot[k], W[k]);
 #pragma unroll
-                    for (int j = 0; j < NC; ++j)
+                        for (int j = 0; j < NC; ++j) load_slot<F, HALF>(level_base, slot[k][j], v[k][j]);
+                    }
+#ifdef DASH_DEFORM_PROFILE
+                    const long long q1 = clock64();
+#endif
+                    if (ra + kStep < rounds) {   // next iteration's coordinates, under the gathers
 #pragma unroll
-                        for (int f = 0; f < F; ++f) acc[f] = fmaf(W[j], v[j][f], acc[f]);
+                        for (int k = 0; k < R; ++k) {
+                            const uint32_t rn = ra + kStep + k * kDeformEncWarps;
+                            load_coords<D>(P, item_row(rn < rounds ? rn : ra + kStep), xyz, t, index, cq[k]);
+                        }
+                    }
 #pragma unroll
-                    for (int f = 0; f < F; ++f) acc[f] += __shfl_xor_sync(0xffffffffu, acc[f], 1);
-                    if (xc == 0) {  // fp32 feature -> bf16 operand element (row q, column l*F + f)
-                        unsigned char* dst = a0 + operand_offset(a_lbo, q, l * F);
-                        if constexpr (F == 1) {
-                            *reinterpret_cast<__nv_bfloat16*>(dst) = __float2bfloat16_rn(acc[0]);
-                        } else if constexpr (F == 2) {
-                            *reinterpret_cast<uint32_t*>(dst) = pack_bf16(acc[0], acc[1]);
-                        } else if constexpr (F == 4) {
-                            *reinterpret_cast<uint2*>(dst) =
-                                make_uint2(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]));
-                        } else {
-                            *reinterpret_cast<uint4*>(dst) =
-                                make_uint4(pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]),
-                                           pack_bf16(acc[4], acc[5]), pack_bf16(acc[6], acc[7]));
+                    for (int k = 0; k < R; ++k) {
+                        float acc[F];
+#pragma unroll
+                        for (int f = 0; f < F; ++f) acc[f] = 0.0f;
+#pragma unroll
+                        for (int j = 0; j < NC; ++j)
+#pragma unroll
+                            for (int f = 0; f < F; ++f) acc[f] = fmaf(W[k][j], v[k][j][f], acc[f]);
+#pragma unroll
+                        for (int f = 0; f < F; ++f) acc[f] += __shfl_xor_sync(0xffffffffu, acc[f], 1);
+#ifdef DASH_DEFORM_PROFILE
+                        if (blockIdx.x == 0 && tid == 0) {
+                            const long long q2 = clock64();
+                            prof[0][40] += q1 - q0; prof[0][41] += q2 - q1; prof[0][42] += 1;
+                        }
+#endif
+                        if (xc == 0 && (k == 0 || rk[k] != ra)) {
+                            // fp32 feature -> bf16 operand element (row q, column l*F + f)
+                            const uint32_t it = rk[k] * 16u + pair;
+                            const uint32_t q = (P.L & (P.L - 1u)) == 0u ? it >> l_shift : it / P.L, l = it - q * P.L;
+                            const uint32_t dst = a0 + operand_offset(a_lbo, q, l * F);
+                            if constexpr (F == 1) {
+                                sts16(dst, __bfloat16_as_ushort(__float2bfloat16_rn(acc[0])));
+                            } else if constexpr (F == 2) {
+                                sts32(dst, pack_bf16(acc[0], acc[1]));
+                            } else if constexpr (F == 4) {
+                                sts64(dst, pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]));
+                            } else {
+                                sts128(dst, pack_bf16(acc[0], acc[1]), pack_bf16(acc[2], acc[3]),
+                                       pack_bf16(acc[4], acc[5]), pack_bf16(acc[6], acc[7]));
+                            }
                         }
                     }
                 }
@@ -348,9 +430,8 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                         const uint32_t k = c * 8u + e;
                         x[e] = k < K ? __ldcs(feat + n * K + k) : 0.0f;
                     }
-                    *reinterpret_cast<uint4*>(a0 + operand_offset(a_lbo, q, c * 8u)) =
-                        make_uint4(pack_bf16(x[0], x[1]), pack_bf16(x[2], x[3]), pack_bf16(x[4], x[5]),
-                                   pack_bf16(x[6], x[7]));
+                    sts128(a0 + operand_offset(a_lbo, q, c * 8u), pack_bf16(x[0], x[1]), pack_bf16(x[2], x[3]),
+                           pack_bf16(x[4], x[5]), pack_bf16(x[6], x[7]));
                 }
             }
             fence_async_smem();
@@ -359,33 +440,46 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
         }
     } else {
         // ================================================================================== CONSUMER PIPELINE p
+        // Tile i of this CTA: A buffer s = i & 1, pipeline p = i % npipes.  Layer 1 reads its A operand from shared
+        // memory (written by the producers); the hidden activations go accumulator -> registers -> TENSOR MEMORY
+        // (tcgen05.st) and the next layer's MMA reads its A operand from there (TS form).  A consumer thread touches
+        // shared memory only to wait on an mbarrier: everything that goes through the SM's LSU queue waits behind
+        // the producers' gathers (measured: 6-14K cycles per layer with shared-memory activations, profiles/).
         const uint32_t cw = warp - kDeformEncWarps;
         const uint32_t p = cw >> 2, e = cw & 3u;            // e == warp % 4: owns TMEM lanes 32e .. 32e+31
         const bool issuer = e == 0 && lane == 0;            // this pipeline's MMA-issuing thread
         const uint32_t r = e * 32u + lane;                  // accumulator row = query within the tile
-        const uint32_t tmem_d = tmem_base + p * M.tmem_pipe_cols;
-        const uint32_t taddr_row = tmem_d + ((e * 32u) << 16);
+        const uint32_t tmem_d = tmem_base + p * M.tmem_pipe_cols;        // accumulator columns of this pipeline
+        const uint32_t tmem_a = tmem_d + M.tmem_a_off;                   // bf16 A operand of layers 2..n
+        const uint32_t lane_off = (e * 32u) << 16;
         const uint32_t bar_mma = bar_mma0 + 8 * p;
-        unsigned char* act = smem + M.act_off + p * M.act_bytes;
         uint32_t mma_phase = 0, batch = 0;
-        for (uint32_t i = p; i < my_tiles; i += kDeformPipes) {
+        for (uint32_t i = p; i < my_tiles && p < M.npipes; i += M.npipes) {
+            const uint32_t s = i & 1u;
             const uint64_t n = r_begin + static_cast<uint64_t>(i) * kDeformTileM + r;
             for (uint32_t l = 0; l < M.n_layers; ++l, ++batch) {
                 if (issuer) {
-                    if (l == 0) mbar_wait(bar_full + 8 * p, (i >> 1) & 1u);
+                    if (l == 0) mbar_wait(bar_full + 8 * s, (i >> 1) & 1u);
                     tc_fence_after();
                     if (p == 0) PROF(1, 2 * batch);
-                    const uint32_t a_addr = l == 0 ? sbase + M.a0_off + p * a0_bytes : smem_u32(act);
                     const uint32_t w_addr = sbase + M.w_off[l];
                     const uint32_t np = M.npad[l], ksteps = M.kpad[l] >> 4;
                     const uint32_t w_lbo = operand_lbo(np);
                     const uint32_t idesc = umma_idesc(np);
-                    for (uint32_t kk = 0; kk < ksteps; ++kk) {
-                        const uint64_t ad = umma_desc(a_addr + kk * 2u * a_lbo, a_lbo, 128u);
-                        const uint64_t bd = umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u);
-                        tc_mma_bf16(tmem_d, ad, bd, idesc, kk > 0 ? 1u : 0u);
+                    if (l == 0) {
+                        const uint32_t a_addr = sbase + M.a0_off + s * a0_bytes;
+                        for (uint32_t kk = 0; kk < ksteps; ++kk) {
+                            const uint64_t ad = umma_desc(a_addr + kk * 2u * a_lbo, a_lbo, 128u);
+                            const uint64_t bd = umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u);
+                            tc_mma_bf16(tmem_d, ad, bd, idesc, kk > 0 ? 1u : 0u);
+                        }
+                        tc_commit(bar_empty + 8 * s);  // A buffer free once these MMAs have read it
+                    } else {
+                        for (uint32_t kk = 0; kk < ksteps; ++kk) {   // K = 16 per instruction = 8 TMEM columns of A
+                            const uint64_t bd = umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u);
+                            tc_mma_bf16_ts(tmem_d, tmem_a + kk * 8u, bd, idesc, kk > 0 ? 1u : 0u);
+                        }
                     }
-                    if (l == 0) tc_commit(bar_empty + 8 * p);  // A buffer free once these MMAs have read it
                     tc_commit(bar_mma);
                     if (p == 0) PROF(1, 2 * batch + 1);
                 }
@@ -396,32 +490,30 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                 if (cw == 0 && lane == 0) PROF(2, 2 * batch);
                 const uint32_t np = M.npad[l];
                 if (l + 1 < M.n_layers) {
-                    // hidden layer: relu, -> bf16, -> A operand of the next layer (the bias came out of the MMA)
+                    // hidden layer: relu, -> bf16 pairs, -> tensor memory (the bias came out of the MMA)
                     for (uint32_t c = 0; c < np; c += 32u) {   // np is a multiple of 16: the last round may be half
                         uint32_t rr[32];
-                        tc_ld32_nowait(taddr_row + c, rr);
+                        tc_ld32_nowait(tmem_d + lane_off + c, rr);
                         tc_ld_wait();
+                        uint32_t w[16];
 #pragma unroll
-                        for (int g = 0; g < 4; ++g) {          // one 16-byte chunk = 8 columns
-                            if (c + 8u * g < np) {
-                                float v[8];
-#pragma unroll
-                                for (int j = 0; j < 8; ++j) v[j] = fmaxf(__uint_as_float(rr[8 * g + j]), 0.0f);
-                                *reinterpret_cast<uint4*>(act + operand_offset(a_lbo, r, c + 8u * g)) =
-                                    make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]),
-                                               pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
-                            }
+                        for (int j = 0; j < 16; ++j)
+                            w[j] = pack_bf16(fmaxf(__uint_as_float(rr[2 * j]), 0.0f),
+                                             fmaxf(__uint_as_float(rr[2 * j + 1]), 0.0f));
+                        if (c + 16u < np) {
+                            tc_st16(tmem_a + lane_off + (c >> 1), w);
+                        } else {
+                            tc_st8(tmem_a + lane_off + (c >> 1), w);
                         }
                     }
-                    // the next layer's "ones" chunk and the zero chunk behind it (a wider layer may have used them)
-                    *reinterpret_cast<uint4*>(act + operand_offset(a_lbo, r, np)) = ones_chunk;
-                    *reinterpret_cast<uint4*>(act + operand_offset(a_lbo, r, np + 8u)) =
-                        make_uint4(0u, 0u, 0u, 0u);
-                    fence_async_smem();
+                    // the "ones" pair that multiplies the next layer's bias columns, zeros behind it
+                    const uint32_t tail[8] = {0x3f803f80u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+                    tc_st8(tmem_a + lane_off + (np >> 1), tail);
+                    tc_st_wait();
                 } else {
                     for (uint32_t c = 0; c < np; c += 16u) {
                         float v[16];
-                        tc_ld16(taddr_row + c, v);
+                        tc_ld16(tmem_d + lane_off + c, v);
                         if (n < r_end) {   // rows past the range hold stale operands: never stored
                             float* o = out + n * M.n_out;
                             const float* bb = base ? base + n * M.n_out : nullptr;
@@ -445,6 +537,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
 #ifdef DASH_DEFORM_PROFILE
     if (blockIdx.x == 0 && tid == 0) {
         printf("tiles=%u setup=%lld end=%lld\n", my_tiles, t_setup - t_entry, clock64() - t_setup);
+        printf("warp0 rounds=%lld issue_cycles=%lld wait_cycles=%lld\n", prof[0][42], prof[0][40], prof[0][41]);
         for (int k = 0; k < 2 * (int)my_tiles && k < 64; ++k) printf("prod[%d]=%lld\n", k, prof[0][k]);
         for (int k = 0; k < (int)(my_tiles + 1) / 2 * 2 * (int)M.n_layers && k < 64; ++k)
             printf("mma0[%d]=%lld epi0[%d]=%lld\n", k, prof[1][k], k, prof[2][k]);

@@ -34,11 +34,11 @@ struct MlpPlan {
     uint32_t p_off[kMlpMaxLayers];      // float offset of W_l in the packed parameter buffer (b_l follows W_l)
     uint32_t w_off[kMlpMaxLayers];      // byte offset of the bf16 operand copy of W_l in shared memory
     uint32_t a0_off;             // two A buffers of the first layer, 128 x kpad[0] bf16 each
-    uint32_t act_off;            // activations between layers, 128 x max(kpad[1..]) bf16, one per pipeline
-    uint32_t act_bytes;          // size of one activation buffer
     uint32_t smem_bytes;
-    uint32_t tmem_cols;          // allocated TMEM columns: kDeformPipes x tmem_pipe_cols
-    uint32_t tmem_pipe_cols;     // power of two >= max npad, >= 32
+    uint32_t tmem_cols;          // allocated TMEM columns: power of two >= npipes * tmem_pipe_cols, >= 32
+    uint32_t tmem_pipe_cols;     // per pipeline: accumulator (max npad) + bf16 A operand of layers 2..n (max kpad/2)
+    uint32_t tmem_a_off;         // column offset of the A operand inside a pipeline's region (= max npad)
+    uint32_t npipes;             // consumer pipelines in use: 2 when both fit the 512 TMEM columns, else 1
     uint32_t n_out;              // width[n_layers]
 };
 

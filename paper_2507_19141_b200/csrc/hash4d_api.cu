@@ -602,15 +602,15 @@ int fill_mlp_plan(const dash_mlp_config* m, uint64_t N, dash::MlpPlan* M) {
     const uint32_t a_lbo = dash::kDeformTileM * 16 + 16;
     M->a0_off = off;
     off += 2 * (M->kpad[0] / 8) * a_lbo;
-    off = round_up(off, 128);
-    M->act_off = off;
-    M->act_bytes = round_up((kmax / 8) * a_lbo, 128);
-    off += dash::kDeformPipes * M->act_bytes;
     M->smem_bytes = off;
+    // tensor memory per pipeline: fp32 accumulator (nmax columns) + the bf16 A operand of layers 2..n (two
+    // elements per 32-bit column: kmax / 2 columns).  Two pipelines when both fit the SM's 512 columns.
+    M->tmem_a_off = nmax;
+    M->tmem_pipe_cols = nmax + kmax / 2;
+    M->npipes = (2 * M->tmem_pipe_cols <= 512) ? dash::kDeformPipes : 1;
     uint32_t cols = 32;
-    while (cols < nmax) cols *= 2;
-    M->tmem_pipe_cols = cols;
-    M->tmem_cols = cols * dash::kDeformPipes;   // <= 512: nmax <= 256
+    while (cols < M->npipes * M->tmem_pipe_cols) cols *= 2;
+    M->tmem_cols = cols;
     if (M->smem_bytes > dash::kDeformSmemLimit)
         return fail(DASH_HASH4D_UNSUPPORTED,
                     "this layer chain needs %u bytes of shared memory per CTA (limit %u)", M->smem_bytes,
