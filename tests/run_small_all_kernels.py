@@ -36,6 +36,35 @@ def main():
                 torch.cuda.synchronize()
                 assert torch.isfinite(out).all() and torch.isfinite(dt).all() and torch.isfinite(dq).all()
                 assert int(idx.view(torch.int32).max()) < T
+        # smoothness regulariser, G_3D, sparse Adam, render path (fused / two-pass / MLP alone), time slice
+        cfg = dh.config_from_params(enc)
+        x, tt, tab = d(xyz), d(t), d(table)
+        eps = d((rng.random((n, 4), dtype=np.float32) - 0.5) * 1e-2)
+        dt = torch.zeros((L, T, F), device="cuda")
+        loss, _ = dh.dash_hash4d_smooth(cfg, x, tt, eps, tab, grad_scale=0.1, dtable=dt)
+        o3 = dh.dash_hash3d_fwd(cfg, x, tab)
+        dh.dash_hash3d_bwd(dh.with_flags(cfg, dh.FLAG_DENSE_COARSE | dh.FLAG_ZERO_GRAD), x, d(dout), dt)
+        i3, _ = dh.dash_hash3d_indices(cfg, x)
+        theta = tab.float().contiguous()
+        m1, v1 = torch.zeros_like(theta), torch.zeros_like(theta)
+        dh.dash_hash4d_adam_step(cfg, theta, dt, m1, v1, 1, table16=tab if dtype == "fp16" else None)
+        widths = [L * F, 24, 10]
+        mlp = dh.make_mlp_config(widths)
+        prm = d(rng.uniform(-0.3, 0.3, dh.dash_mlp_param_count(mlp)).astype(np.float32))
+        outs = []
+        for fused in ("1", "0"):
+            os.environ["DASH_DEFORM_FUSED"] = fused
+            outs.append(dh.dash_deform_fwd(cfg, mlp, x, tt, tab, prm))
+        os.environ.pop("DASH_DEFORM_FUSED")
+        outs.append(dh.dash_mlp_fwd(mlp, dh.dash_hash4d_fwd(cfg, x, tt, tab), prm))
+        if T & (T - 1) == 0:
+            sl = dh.dash_hash4d_slice_t(cfg, tt[:1].contiguous(), tab)
+            outs.append(dh.dash_hash4d_slice_fwd(cfg, x, sl))
+            outs.append(dh.dash_deform_slice_fwd(cfg, mlp, x, sl, prm))
+        torch.cuda.synchronize()
+        for a in [loss, o3, theta, m1, v1] + outs:
+            assert torch.isfinite(a).all()
+        assert int(i3.max()) < T
     print("all kernels ran")
 
 
