@@ -17,11 +17,13 @@
 //   The layers of one tile are a dependent chain (MMA -> epilogue -> MMA ...); two pipelines keep the tensor
 //   pipe and the epilogue of one tile busy while the other tile waits on a hand-off.
 //
-// The weights of every layer are converted to bf16 once per CTA and stay resident in shared memory.  Hand-offs
-// are mbarriers (full/empty per A buffer, accumulator-done via tcgen05.commit, activations-ready); no
-// __syncthreads in the steady state.  The gathers are the bound (L1 wavefronts, as in the forward kernel); the
-// tensor pipe and the epilogue run underneath them.  With FUSED = false the producer warps read a feature
-// matrix from global memory instead (two-pass path for tables that do not fit L2 in one level group).
+// The weights of every layer are converted to bf16 once per CTA and stay resident in shared memory.  Hand-offs:
+// mbarriers full/empty per A buffer, accumulator-done via tcgen05.commit, a 128-thread named barrier inside a
+// pipeline; no __syncthreads in the steady state.  The gathers are the bound (issue + latency of 24 warps; L1 at
+// ~70 % of its wavefront rate); the tensor pipe (~4 % busy) and the epilogue run underneath them.  D = 3: 8-corner
+// gathers in a per-frame time slice of the tables (Q29).  FUSED = false: the producer warps read a
+// feature matrix from global memory instead (two-pass path for tables that do not fit L2 in one level group).
+// Build with -DDASH_DEFORM_PROFILE for clock64() phase timers printed by CTA 0 (development only).
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
