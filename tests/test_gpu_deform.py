@@ -207,3 +207,25 @@ def test_render_and_train_calls_are_cuda_graph_capturable():
     # the scatter order varies run to run (fp32 reductions): the optimiser state agrees to rounding, not bitwise
     torch.testing.assert_close(theta, want[2], rtol=1e-4, atol=1e-6)
     assert float(dt.abs().max()) == 0.0
+
+
+def test_deform_two_pass_on_a_table_beyond_l2_c4_sample():
+    """C4's 268 MB fp16 table does not fit L2 as one level group: dash_deform_fwd must take the two-pass route
+    (level-group-major forward into the caller's workspace, then the MLP kernel) and ask for that workspace."""
+    wl = make_workload("C4", n_override=150_000, with_dout=False)
+    enc, N = wl.spec.enc, wl.N
+    widths = [enc.L * enc.F, 128, 10]
+    params = make_mlp_params(5, widths)
+    ocfg, gcfg = oracle.config_from_params(enc), dh.config_from_params(enc)
+    m = dh.make_mlp_config(widths)
+    need = dh.dash_deform_workspace_bytes(gcfg, m, N)
+    assert need == N * enc.L * enc.F * 4
+    table = (wl.table.astype(np.float32) * 1e4).astype(np.float16)
+    with pytest.raises(dh.Hash4DError) as e:                                  # no workspace: status 3
+        dh.dash_deform_fwd(gcfg, m, dev(wl.xyz), dev(wl.t), dev(table), dev(params),
+                           workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.status == 3
+    out = dh.dash_deform_fwd(gcfg, m, dev(wl.xyz), dev(wl.t), dev(table), dev(params))
+    torch.cuda.synchronize()
+    feat = oracle.oracle_fwd(ocfg, N, wl.xyz, wl.t, table)
+    check_mlp_out(out.cpu().numpy(), feat, params, widths, None, "C4 sample two-pass")
