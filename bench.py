@@ -386,12 +386,12 @@ def run_cuda(args):
             f2 = torch.empty((w2.N, e2.L * e2.F), dtype=torch.float32, device="cuda")
             ws2 = torch.empty(w2.N * e2.L * e2.F * 4, dtype=torch.uint8, device="cuda")
             row = {"workload": f"{name}: N={w2.N}, one timestamp, MLP {widths}"}
-            os.environ["DASH_DEFORM_FUSED"] = "1"
+            dh.dash_hash4d_set_debug(dh.DEBUG_DEFORM_PATH, 1)
             row["fused_ms"] = timed(lambda: dh.dash_deform_fwd(cfg2, mlp, x2, one, tab2, prm, out=o2, t_stride=0), 20)
-            os.environ["DASH_DEFORM_FUSED"] = "0"
+            dh.dash_hash4d_set_debug(dh.DEBUG_DEFORM_PATH, 2)
             row["two_pass_ms"] = timed(lambda: dh.dash_deform_fwd(cfg2, mlp, x2, one, tab2, prm, out=o2, t_stride=0,
                                                                   workspace=ws2), 20)
-            os.environ.pop("DASH_DEFORM_FUSED")
+            dh.dash_hash4d_set_debug(dh.DEBUG_DEFORM_PATH, 0)
             row["encoder_only_ms"] = timed(lambda: dh.dash_hash4d_fwd(cfg2, x2, one, tab2, out=f2, t_stride=0), 20)
             row["mlp_only_ms"] = timed(lambda: dh.dash_mlp_fwd(mlp, f2, prm, out=o2), 20)
             sl2 = torch.empty((e2.L, e2.T, e2.F), dtype=torch.float32, device="cuda")

@@ -243,6 +243,24 @@ DASH_API const char* dash_hash4d_last_error(void);
  * (used by bench.py for "gpu_launches"). */
 DASH_API uint64_t dash_hash4d_launch_count(int reset);
 
+/* Hash of the sources the library was built from (never NULL).  The Python binding compares it with the sources
+ * beside it and refuses (rebuilds, else raises) a library that is out of date. */
+DASH_API const char* dash_hash4d_build_id(void);
+
+/* Tuning overrides for sweeps and A/B measurements (bench.py --sweep, tests).  Process-wide; value 0 restores the
+ * library's own choice; the library reads NO environment variable.  Not part of the method: every setting computes
+ * the same result.  Returns INVALID_ARG for an unknown key or a negative value. */
+enum dash_debug_key {
+    DASH_DEBUG_FWD_GROUP = 0,    /* levels per level group G of fwd / bwd_input / slice_fwd (1..16, power of two) */
+    DASH_DEBUG_BWD_GROUP = 1,    /* ... of bwd */
+    DASH_DEBUG_SMOOTH_GROUP = 2, /* ... of smooth */
+    DASH_DEBUG_DEFORM_PATH = 3,  /* dash_deform_fwd: 1 = fused kernel, 2 = two-pass (encoder -> workspace -> MLP) */
+    DASH_DEBUG_BWD_VARIANT = 4,  /* bwd scatter variant, see hash4d_api.cu bwd_impl (0 = default) */
+    DASH_DEBUG_FWD_VARIANT = 5,  /* fwd gather variant (0 = default) */
+    DASH_DEBUG_KEY_COUNT = 6
+};
+DASH_API int dash_hash4d_set_debug(int key, int64_t value);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUD
 
 EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4d_fwd",
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
-           "dash_hash4d_launch_count",
+           "dash_hash4d_launch_count", "dash_hash4d_set_debug", "dash_hash4d_build_id",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
            "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd",
            "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd"]
@@ -71,17 +71,14 @@ def _load() -> C.CDLL:
     global _lib
     if _lib is not None:
         return _lib
-    path = os.environ.get("DASH_HASH4D_LIB")       # development: load an alternative build of the same ABI
-    if path:
-        lib = C.CDLL(path)
-        return _bind(lib)
     path = _build.LIB
     if _build.is_stale():
+        # never run old kernels against new sources: a stale library that cannot be rebuilt is an error
         try:
             _build.build()
         except Exception as exc:  # noqa: BLE001
-            if not os.path.exists(path):
-                raise ImportError(f"libdash_hash4d.so is not built and nvcc failed: {exc}") from exc
+            raise ImportError(f"libdash_hash4d.so is missing or older than its sources and the nvcc build "
+                              f"failed: {exc}") from exc
     return _bind(C.CDLL(path))
 
 
@@ -134,6 +131,10 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_deform_slice_fwd.restype = C.c_int
     lib.dash_hash4d_launch_count.argtypes = [C.c_int]
     lib.dash_hash4d_launch_count.restype = u64
+    lib.dash_hash4d_build_id.argtypes = []
+    lib.dash_hash4d_build_id.restype = C.c_char_p
+    lib.dash_hash4d_set_debug.argtypes = [C.c_int, C.c_int64]
+    lib.dash_hash4d_set_debug.restype = C.c_int
     _lib = lib
     return lib
 
@@ -190,6 +191,47 @@ def _dev(t: Optional[torch.Tensor], dtype, what: str):
         raise ValueError(f"{what} must be contiguous {dtype}")
 
 
+def _at_least(t: Optional[torch.Tensor], count: int, what: str):
+    """The C ABI takes raw pointers and cannot know the allocation sizes: check them here."""
+    if t is not None and t.numel() < count:
+        raise ValueError(f"{what} holds {t.numel()} elements, the call needs {count}")
+
+
+def _exactly(t: Optional[torch.Tensor], count: int, what: str):
+    if t is not None and t.numel() != count:
+        raise ValueError(f"{what} holds {t.numel()} elements, the config says {count}")
+
+
+def _one_device(*tensors):
+    devs = {t.device for t in tensors if t is not None}
+    if len(devs) > 1:
+        raise ValueError(f"all tensors of a call must live on one device, got {sorted(map(str, devs))}")
+    dev = next(iter(devs))
+    if dev != torch.device("cuda", torch.cuda.current_device()):
+        raise ValueError(f"tensors live on {dev} but the current device is cuda:{torch.cuda.current_device()} "
+                         "(the call enqueues on the current stream)")
+
+
+def _check_queries(cfg, xyz, t, index, ts: int, N: int):
+    """Sizes of the query arrays for N queries; under VALIDATE_INPUTS also the range of the index list."""
+    if N < 0:
+        raise ValueError("N < 0")
+    if index is not None:
+        _at_least(index, N, "index")
+        if (cfg.flags & FLAG_VALIDATE_INPUTS) and N:
+            lo, hi = int(index[:N].min()), int(index[:N].max())
+            if lo < 0 or hi >= xyz.shape[0]:
+                raise ValueError(f"index values span [{lo}, {hi}] but xyz has {xyz.shape[0]} rows")
+    elif xyz.shape[0] < N:
+        raise ValueError(f"xyz has {xyz.shape[0]} rows, the call needs {N}")
+    if t is not None and N:
+        _at_least(t, (N - 1) * ts + 1, "t")
+
+
+def _table_elems(cfg) -> int:
+    return int(cfg.L) * int(cfg.T) * int(cfg.F)
+
+
 def _strides(xyz: torch.Tensor, t: torch.Tensor, t_stride: Optional[int]):
     if xyz.dim() != 2 or xyz.shape[1] not in (3, 4):
         raise ValueError("xyz must be [rows][3] or [rows][4]")
@@ -206,6 +248,14 @@ def dash_hash4d_launch_count(reset: bool = False) -> int:
     return int(_load().dash_hash4d_launch_count(1 if reset else 0))
 
 
+DEBUG_FWD_GROUP, DEBUG_BWD_GROUP, DEBUG_SMOOTH_GROUP, DEBUG_DEFORM_PATH, DEBUG_BWD_VARIANT, DEBUG_FWD_VARIANT = range(6)
+
+
+def dash_hash4d_set_debug(key: int, value: int) -> None:
+    """Tuning override for sweeps (include/dash_hash4d.h `dash_debug_key`); 0 restores the library's choice."""
+    _check(_load().dash_hash4d_set_debug(int(key), int(value)))
+
+
 def dash_hash4d_resolutions(cfg: Hash4DConfig):
     """-> (res_s, res_t, is_dense) as Python lists (host only; needs no GPU)."""
     L = max(int(cfg.L), 1)
@@ -218,10 +268,12 @@ def dash_hash4d_workspace_bytes(cfg: Hash4DConfig, N: int, op: int) -> int:
     return int(_load().dash_hash4d_workspace_bytes(C.byref(cfg), N, op))
 
 
-def _workspace(cfg, N, op, workspace):
+def _workspace(cfg, N, op, workspace, device):
     need = dash_hash4d_workspace_bytes(cfg, N, op)
     if need and workspace is None:
-        workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+        workspace = torch.empty(need, dtype=torch.uint8, device=device)
+    if workspace is not None and not workspace.is_cuda:
+        raise ValueError("workspace must be a CUDA tensor")
     return workspace, (0 if workspace is None else workspace.numel() * workspace.element_size())
 
 
@@ -235,7 +287,10 @@ def dash_hash4d_fwd(cfg, xyz, t, table, out=None, index=None, t_stride=None, N=N
     if out is None:
         out = torch.empty((N, cfg.L * cfg.F), dtype=torch.float32, device=xyz.device)
     _dev(out, torch.float32, "out")
-    workspace, wbytes = _workspace(cfg, N, OP_FWD, workspace)
+    _check_queries(cfg, xyz, t, index, ts, N)
+    _exactly(table, _table_elems(cfg), "table"); _at_least(out, N * cfg.L * cfg.F, "out")
+    _one_device(xyz, t, index, table, out, workspace)
+    workspace, wbytes = _workspace(cfg, N, OP_FWD, workspace, xyz.device)
     _check(_load().dash_hash4d_fwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
                                    _ptr(table), _ptr(out), _ptr(workspace), wbytes, _stream()))
     return out
@@ -248,7 +303,10 @@ def dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=None, t_stride=None, N=None
     xs, ts = _strides(xyz, t, t_stride)
     if N is None:
         N = int(index.numel()) if index is not None else int(xyz.shape[0])
-    workspace, wbytes = _workspace(cfg, N, OP_BWD, workspace)
+    _check_queries(cfg, xyz, t, index, ts, N)
+    _at_least(dout, N * cfg.L * cfg.F, "dout"); _exactly(dtable, _table_elems(cfg), "dtable")
+    _one_device(xyz, t, index, dout, dtable, workspace)
+    workspace, wbytes = _workspace(cfg, N, OP_BWD, workspace, xyz.device)
     _check(_load().dash_hash4d_bwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
                                    _ptr(dout), _ptr(dtable), _ptr(workspace), wbytes, _stream()))
     return dtable
@@ -266,7 +324,10 @@ def dash_hash4d_bwd_input(cfg, xyz, t, table, dout, dq=None, index=None, t_strid
     if dq is None:
         dq = torch.empty((N, 4), dtype=torch.float32, device=xyz.device)
     _dev(dq, torch.float32, "dq")
-    workspace, wbytes = _workspace(cfg, N, OP_BWD_INPUT, workspace)
+    _check_queries(cfg, xyz, t, index, ts, N)
+    _exactly(table, _table_elems(cfg), "table"); _at_least(dout, N * cfg.L * cfg.F, "dout")
+    _at_least(dq, 4 * N, "dq"); _one_device(xyz, t, index, table, dout, dq, workspace)
+    workspace, wbytes = _workspace(cfg, N, OP_BWD_INPUT, workspace, xyz.device)
     _check(_load().dash_hash4d_bwd_input(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
                                          _ptr(table), _ptr(dout), _ptr(dq), _ptr(workspace), wbytes,
                                          _stream()))
@@ -289,7 +350,10 @@ def dash_hash4d_smooth(cfg, xyz, t, eps, table, grad_scale=1.0, loss=None, dtabl
     if loss is None:
         loss = torch.empty((N,), dtype=torch.float32, device=xyz.device)
     _dev(loss, torch.float32, "loss")
-    workspace, wbytes = _workspace(cfg, N, OP_SMOOTH, workspace)
+    _check_queries(cfg, xyz, t, index, ts, N)
+    _exactly(table, _table_elems(cfg), "table"); _exactly(dtable, _table_elems(cfg), "dtable")
+    _at_least(loss, N, "loss"); _one_device(xyz, t, index, eps, table, loss, dtable, workspace)
+    workspace, wbytes = _workspace(cfg, N, OP_SMOOTH, workspace, xyz.device)
     _check(_load().dash_hash4d_smooth(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index), _ptr(eps),
                                       eps_stride, _ptr(table), float(grad_scale), _ptr(loss), _ptr(dtable),
                                       _ptr(workspace), wbytes, _stream()))
@@ -302,6 +366,7 @@ def dash_hash4d_indices(cfg, xyz, t, index=None, t_stride=None, N=None, want_wei
     xs, ts = _strides(xyz, t, t_stride)
     if N is None:
         N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    _check_queries(cfg, xyz, t, index, ts, N); _one_device(xyz, t, index)
     idx = torch.empty((N, cfg.L, 16), dtype=torch.int32, device=xyz.device)   # bits are uint32
     w = torch.empty((N, cfg.L, 16), dtype=torch.float32, device=xyz.device) if want_weights else None
     _check(_load().dash_hash4d_indices(C.byref(cfg), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
@@ -311,6 +376,7 @@ def dash_hash4d_indices(cfg, xyz, t, index=None, t_stride=None, N=None, want_wei
 
 def dash_hash4d_zero(cfg, dtable):
     _dev(dtable, torch.float32, "dtable")
+    _exactly(dtable, _table_elems(cfg), "dtable"); _one_device(dtable)
     _check(_load().dash_hash4d_zero(C.byref(cfg), _ptr(dtable), _stream()))
     return dtable
 
@@ -341,7 +407,10 @@ def dash_hash3d_fwd(cfg, xyz, table, out=None, index=None, N=None, workspace=Non
     if out is None:
         out = torch.empty((N, cfg.L * cfg.F), dtype=torch.float32, device=xyz.device)
     _dev(out, torch.float32, "out")
-    workspace, wbytes = _workspace(cfg, N, OP_FWD, workspace)
+    _check_queries(cfg, xyz, None, index, 0, N)
+    _exactly(table, _table_elems(cfg), "table"); _at_least(out, N * cfg.L * cfg.F, "out")
+    _one_device(xyz, index, table, out, workspace)
+    workspace, wbytes = _workspace(cfg, N, OP_FWD, workspace, xyz.device)
     _check(_load().dash_hash3d_fwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(table), _ptr(out),
                                    _ptr(workspace), wbytes, _stream()))
     return out
@@ -354,7 +423,10 @@ def dash_hash3d_bwd(cfg, xyz, dout, dtable, index=None, N=None, workspace=None):
     xs = _xyz_stride(xyz)
     if N is None:
         N = int(index.numel()) if index is not None else int(xyz.shape[0])
-    workspace, wbytes = _workspace(cfg, N, OP_BWD, workspace)
+    _check_queries(cfg, xyz, None, index, 0, N)
+    _at_least(dout, N * cfg.L * cfg.F, "dout"); _exactly(dtable, _table_elems(cfg), "dtable")
+    _one_device(xyz, index, dout, dtable, workspace)
+    workspace, wbytes = _workspace(cfg, N, OP_BWD, workspace, xyz.device)
     _check(_load().dash_hash3d_bwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(dout), _ptr(dtable),
                                    _ptr(workspace), wbytes, _stream()))
     return dtable
@@ -366,6 +438,7 @@ def dash_hash3d_indices(cfg, xyz, index=None, N=None, want_weights=True):
     xs = _xyz_stride(xyz)
     if N is None:
         N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    _check_queries(cfg, xyz, None, index, 0, N); _one_device(xyz, index)
     idx = torch.empty((N, cfg.L, 8), dtype=torch.int32, device=xyz.device)
     w = torch.empty((N, cfg.L, 8), dtype=torch.float32, device=xyz.device) if want_weights else None
     _check(_load().dash_hash3d_indices(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(idx), _ptr(w),
@@ -379,6 +452,9 @@ def dash_hash4d_adam_step(cfg, theta, dtable, m, v, step, lr=1e-2, beta1=0.9, be
     for name, a in (("theta", theta), ("dtable", dtable), ("m", m), ("v", v)):
         _dev(a, torch.float32, name)
     _dev(table16, torch.float16, "table16")
+    for name, a in (("theta", theta), ("dtable", dtable), ("m", m), ("v", v), ("table16", table16)):
+        _exactly(a, _table_elems(cfg), name)
+    _one_device(theta, dtable, m, v, table16)
     opt = AdamConfig()
     opt.struct_size = C.sizeof(AdamConfig)
     opt.step, opt.lr, opt.beta1, opt.beta2, opt.eps = int(step), lr, beta1, beta2, eps
@@ -414,6 +490,8 @@ def dash_mlp_fwd(mlp, feat, params, base=None, out=None):
     if out is None:
         out = torch.empty((N, n_out), dtype=torch.float32, device=feat.device)
     _dev(out, torch.float32, "out")
+    _exactly(feat, N * int(mlp.width[0]), "feat"); _exactly(params, dash_mlp_param_count(mlp), "params")
+    _at_least(base, N * n_out, "base"); _at_least(out, N * n_out, "out"); _one_device(feat, params, base, out)
     _check(_load().dash_mlp_fwd(C.byref(mlp), N, _ptr(feat), _ptr(params), _ptr(base), _ptr(out), _stream()))
     return out
 
@@ -435,9 +513,13 @@ def dash_deform_fwd(cfg, mlp, xyz, t, table, params, base=None, out=None, index=
     if out is None:
         out = torch.empty((N, n_out), dtype=torch.float32, device=xyz.device)
     _dev(out, torch.float32, "out")
+    _check_queries(cfg, xyz, t, index, ts, N)
+    _exactly(table, _table_elems(cfg), "table"); _exactly(params, dash_mlp_param_count(mlp), "params")
+    _at_least(base, N * n_out, "base"); _at_least(out, N * n_out, "out")
+    _one_device(xyz, t, index, table, params, base, out, workspace)
     need = dash_deform_workspace_bytes(cfg, mlp, N)
     if need and workspace is None:
-        workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+        workspace = torch.empty(need, dtype=torch.uint8, device=xyz.device)
     wbytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     _check(_load().dash_deform_fwd(C.byref(cfg), C.byref(mlp), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index),
                                    _ptr(table), _ptr(params), _ptr(base), _ptr(out), _ptr(workspace), wbytes,
@@ -454,6 +536,8 @@ def dash_hash4d_slice_t(cfg, t, table, slice_out=None):
     if slice_out is None:
         slice_out = torch.empty((cfg.L, cfg.T, cfg.F), dtype=torch.float32, device=table.device)
     _dev(slice_out, torch.float32, "slice")
+    _at_least(t, 1, "t"); _exactly(table, _table_elems(cfg), "table"); _exactly(slice_out, _table_elems(cfg), "slice")
+    _one_device(t, table, slice_out)
     _check(_load().dash_hash4d_slice_t(C.byref(cfg), _ptr(t), _ptr(table), _ptr(slice_out), _stream()))
     return slice_out
 
@@ -467,6 +551,9 @@ def dash_hash4d_slice_fwd(cfg, xyz, slice_t, out=None, index=None, N=None):
     if out is None:
         out = torch.empty((N, cfg.L * cfg.F), dtype=torch.float32, device=xyz.device)
     _dev(out, torch.float32, "out")
+    _check_queries(cfg, xyz, None, index, 0, N)
+    _exactly(slice_t, _table_elems(cfg), "slice"); _at_least(out, N * cfg.L * cfg.F, "out")
+    _one_device(xyz, index, slice_t, out)
     _check(_load().dash_hash4d_slice_fwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(slice_t), _ptr(out),
                                          _stream()))
     return out
@@ -482,6 +569,11 @@ def dash_deform_slice_fwd(cfg, mlp, xyz, slice_t, params, base=None, out=None, i
     if out is None:
         out = torch.empty((N, int(mlp.width[mlp.n_layers])), dtype=torch.float32, device=xyz.device)
     _dev(out, torch.float32, "out")
+    n_out = int(mlp.width[mlp.n_layers])
+    _check_queries(cfg, xyz, None, index, 0, N)
+    _exactly(slice_t, _table_elems(cfg), "slice"); _exactly(params, dash_mlp_param_count(mlp), "params")
+    _at_least(base, N * n_out, "base"); _at_least(out, N * n_out, "out")
+    _one_device(xyz, index, slice_t, params, base, out)
     _check(_load().dash_deform_slice_fwd(C.byref(cfg), C.byref(mlp), N, _ptr(xyz), xs, _ptr(index), _ptr(slice_t),
                                          _ptr(params), _ptr(base), _ptr(out), _stream()))
     return out
@@ -497,7 +589,7 @@ def dash_hash4d_fwd_host(cfg, xyz_h, t_h, table_d, out_h, index_h=None, t_stride
     index_d = _stage(st, "index", index_h) if index_h is not None else None
     out_d = st.get("out")
     if out_d is None or out_d.shape != out_h.shape:
-        out_d = st["out"] = torch.empty(out_h.shape, dtype=torch.float32, device="cuda")
+        out_d = st["out"] = torch.empty(out_h.shape, dtype=torch.float32, device=torch.device("cuda", torch.cuda.current_device()))
     dash_hash4d_fwd(cfg, xyz_d, t_d, table_d, out=out_d, index=index_d, t_stride=t_stride)
     out_h.copy_(out_d, non_blocking=True)
     return out_h
@@ -515,7 +607,7 @@ def dash_hash4d_bwd_host(cfg, xyz_h, t_h, dout_h, dtable_h, index_h=None, t_stri
     dout_d = _stage(st, "dout", dout_h)
     dt_d = st.get("dtable")
     if dt_d is None or dt_d.shape != dtable_h.shape:
-        dt_d = st["dtable"] = torch.empty(dtable_h.shape, dtype=torch.float32, device="cuda")
+        dt_d = st["dtable"] = torch.empty(dtable_h.shape, dtype=torch.float32, device=torch.device("cuda", torch.cuda.current_device()))
     if not (cfg.flags & FLAG_ZERO_GRAD):
         dash_hash4d_zero(cfg, dt_d)
     dash_hash4d_bwd(cfg, xyz_d, t_d, dout_d, dt_d, index=index_d, t_stride=t_stride)
@@ -526,7 +618,7 @@ def dash_hash4d_bwd_host(cfg, xyz_h, t_h, dout_h, dtable_h, index_h=None, t_stri
 def _stage(st: dict, key: str, host: torch.Tensor) -> torch.Tensor:
     dev = st.get(key)
     if dev is None or dev.shape != host.shape or dev.dtype != host.dtype:
-        dev = st[key] = torch.empty(host.shape, dtype=host.dtype, device="cuda")
+        dev = st[key] = torch.empty(host.shape, dtype=host.dtype, device=torch.device("cuda", torch.cuda.current_device()))
     dev.copy_(host, non_blocking=True)
     return dev
 
@@ -547,7 +639,7 @@ class HostStep:
     def _dev_like(self, key, host):
         cur = self.buf.get(key)
         if cur is None or cur.shape != host.shape or cur.dtype != host.dtype:
-            cur = self.buf[key] = torch.empty(host.shape, dtype=host.dtype, device="cuda")
+            cur = self.buf[key] = torch.empty(host.shape, dtype=host.dtype, device=torch.device("cuda", torch.cuda.current_device()))
         return cur
 
     def __call__(self, xyz_h, t_h, table_d, dout_h, out_h, dtable_h, index_h=None, t_stride=None):

@@ -4,6 +4,7 @@ Run:  python -m paper_2507_19141_b200.build [--force]
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
@@ -25,17 +26,38 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+_ID_MARK = b"DASH_BUILD_ID="
+
+
+def source_hash() -> str:
+    """sha256 over the bytes of every source and header the library is built from (mtimes do not survive rsync)."""
+    h = hashlib.sha256()
+    for d in sorted(DEPS):
+        with open(os.path.join(CSRC, d), "rb") as fh:
+            h.update(d.encode() + b"\0" + fh.read() + b"\0")
+    return h.hexdigest()[:32]
+
+
+def built_id(path: str = LIB):
+    """The source hash baked into the library (`dash_hash4d_build_id`), read from the file without loading it."""
+    try:
+        with open(path, "rb") as fh:
+            blob = fh.read()
+    except OSError:
+        return None
+    at = blob.find(_ID_MARK)
+    return None if at < 0 else blob[at + len(_ID_MARK): at + len(_ID_MARK) + 32].decode("ascii", "replace")
+
+
 def is_stale() -> bool:
-    if not os.path.exists(LIB):
-        return True
-    built = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, d)) > built for d in DEPS)
+    return built_id() != source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
     cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+          [f'-DDASH_BUILD_ID_STRING="{source_hash()}"'] + \
           [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB + ".tmp"]
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)

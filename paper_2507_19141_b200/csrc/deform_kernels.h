@@ -50,6 +50,7 @@ cudaError_t launch_mlp(const MlpPlan& M, const float* feat, const float* params,
                        float* out, int sms, cudaStream_t s);
 
 void count_launch();   // bumps the per-thread launch counter kept in hash4d_kernels.cu
-int device_sm_count();
+int device_sm_count();      // of the current device, cached per device ordinal
+size_t device_l2_bytes();
 
 }  // namespace dash

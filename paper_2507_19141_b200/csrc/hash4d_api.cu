@@ -5,6 +5,7 @@
 // no synchronisation (except VALIDATE_INPUTS), no state kept between calls.
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -104,23 +105,13 @@ void make_schedule(const dash_hash4d_config* c, Schedule* s, int dims = 4) {
     }
 }
 
-size_t l2_bytes() {
-    static size_t cached = 0;
-    if (!cached) {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&v, cudaDevAttrL2CacheSize, dev) == cudaSuccess && v > 0)
-            cached = static_cast<size_t>(v);
-        else
-            cached = 64u << 20;
-    }
-    return cached;
-}
+size_t l2_bytes() { return dash::device_l2_bytes(); }  // current device, cached per ordinal
 
-uint32_t env_u32(const char* name) {
-    const char* v = std::getenv(name);
-    return v ? static_cast<uint32_t>(std::strtoul(v, nullptr, 10)) : 0u;
-}
+// Tuning overrides for sweeps (dash_hash4d_set_debug): process-wide, 0 = the library decides.  No environment
+// variable is ever read.
+std::atomic<int64_t> g_debug[DASH_DEBUG_KEY_COUNT];
+
+uint32_t debug_u32(int key) { return static_cast<uint32_t>(g_debug[key].load(std::memory_order_relaxed)); }
 
 // Level-group size G (power of two <= 8): as many levels as keep the group's randomly accessed
 // bytes (tables in fwd, fp32 gradient slices in bwd) within 0.3 x L2 — measured (profiles/
@@ -129,10 +120,10 @@ uint32_t env_u32(const char* name) {
 // that a query's slice of `out`/`dout` is one full 32-byte sector (G*F*4 >= 32), and without idling
 // more than a quarter of the lanes when L is not a multiple of G.  G = 16 (one query per warp) is
 // never picked: every warp would then run both the dense and the hashed index path (measured 7-12 %
-// slower than G = 8 at F = 2).  DASH_HASH4D_{FWD,BWD}_GROUP override G (1..16) for sweeps.
-uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, const char* env_name,
+// slower than G = 8 at F = 2).  dash_hash4d_set_debug(DASH_DEBUG_{FWD,BWD,SMOOTH}_GROUP, G) overrides G (1..16).
+uint32_t pick_group(const dash_hash4d_config* c, size_t bytes_per_level, int debug_key,
                     bool row_sector_rule = true) {
-    uint32_t forced = env_u32(env_name);
+    uint32_t forced = debug_u32(debug_key);
     if (forced) {
         uint32_t g = 1;
         while (g * 2 <= forced && g * 2 <= dash::kMaxGroup) g *= 2;
@@ -248,7 +239,24 @@ extern "C" {
 
 DASH_API const char* dash_hash4d_last_error(void) { return g_error; }
 
+#ifndef DASH_BUILD_ID_STRING
+#define DASH_BUILD_ID_STRING "unknown"
+#endif
+// hash of the sources this library was built from (paper_2507_19141_b200/build.py); the binding refuses a
+// library whose id differs from the sources beside it
+DASH_API const char* dash_hash4d_build_id(void) {
+    static const char id[] = "DASH_BUILD_ID=" DASH_BUILD_ID_STRING;
+    return id + 14;
+}
+
 DASH_API uint64_t dash_hash4d_launch_count(int reset) { return dash::launch_counter(reset != 0); }
+
+DASH_API int dash_hash4d_set_debug(int key, int64_t value) {
+    if (key < 0 || key >= DASH_DEBUG_KEY_COUNT) return fail(DASH_HASH4D_INVALID_ARG, "debug key %d unknown", key);
+    if (value < 0) return fail(DASH_HASH4D_INVALID_ARG, "debug value must be >= 0");
+    g_debug[key].store(value, std::memory_order_relaxed);
+    return ok();
+}
 
 DASH_API int dash_hash4d_resolutions(const dash_hash4d_config* cfg, uint32_t* res_s,
                                      uint32_t* res_t, uint8_t* is_dense) {
@@ -294,10 +302,10 @@ static int fwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
     const bool half = cfg->table_dtype == DASH_HASH4D_FP16;
     const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * (half ? 2 : 4);
     Plan P;
-    uint32_t group = pick_group(cfg, level_bytes, "DASH_HASH4D_FWD_GROUP");
+    uint32_t group = pick_group(cfg, level_bytes, DASH_DEBUG_FWD_GROUP);
     // 8-corner gathers: 4 levels per group measured best (G_3D workload: 0.423 ms at G = 4, 0.476 at G = 8,
     // 0.454 at G = 2) as long as a query's row slice stays a full 32-byte sector
-    if (dims == 3 && group > 4 && 4 * cfg->F * sizeof(float) >= 32 && !std::getenv("DASH_HASH4D_FWD_GROUP"))
+    if (dims == 3 && group > 4 && 4 * cfg->F * sizeof(float) >= 32 && !debug_u32(DASH_DEBUG_FWD_GROUP))
         group = 4;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride, group, &P, dims)) return rc;
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
@@ -338,7 +346,7 @@ DASH_API int dash_hash4d_bwd_input(const dash_hash4d_config* cfg, uint64_t N, co
     const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * (half ? 2 : 4);
     Plan P;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
-                           pick_group(cfg, level_bytes, "DASH_HASH4D_FWD_GROUP"), &P))
+                           pick_group(cfg, level_bytes, DASH_DEBUG_FWD_GROUP), &P))
         return rc;
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
     cudaError_t e = dash::launch_zero(dq, static_cast<size_t>(N) * 4 * sizeof(float), s);
@@ -372,7 +380,7 @@ DASH_API int dash_hash4d_smooth(const dash_hash4d_config* cfg, uint64_t N, const
         static_cast<size_t>(cfg->T) * cfg->F * ((half ? 2 : 4) + (dtable ? 4 : 0));
     Plan P;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
-                           pick_group(cfg, level_bytes, "DASH_HASH4D_SMOOTH_GROUP", false), &P))
+                           pick_group(cfg, level_bytes, DASH_DEBUG_SMOOTH_GROUP, false), &P))
         return rc;
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
     cudaError_t e = dash::launch_zero(loss, static_cast<size_t>(N) * sizeof(float), s);
@@ -416,7 +424,7 @@ static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
     Plan P;
     const size_t scatter_bytes = fixed ? 2 * level_bytes : level_bytes;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
-                           pick_group(cfg, scatter_bytes, "DASH_HASH4D_BWD_GROUP"), &P, dims))
+                           pick_group(cfg, scatter_bytes, DASH_DEBUG_BWD_GROUP), &P, dims))
         return rc;
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
 
@@ -630,8 +638,7 @@ size_t mlp_params(const dash_mlp_config* m) {
 
 // the fused kernel walks all L levels per tile: the whole table must stay L2-resident
 bool deform_fused_applies(const dash_hash4d_config* enc) {
-    const char* v = std::getenv("DASH_DEFORM_FUSED");
-    if (v) return std::atoi(v) != 0;
+    if (const uint32_t forced = debug_u32(DASH_DEBUG_DEFORM_PATH)) return forced == 1;  // 1 fused, 2 two-pass
     const size_t elem = enc->table_dtype == DASH_HASH4D_FP16 ? 2 : 4;
     const size_t table_bytes = static_cast<size_t>(enc->L) * enc->T * enc->F * elem;
     return table_bytes <= l2_bytes() / 100 * 55;
@@ -774,8 +781,8 @@ DASH_API int dash_hash4d_slice_fwd(const dash_hash4d_config* cfg, uint64_t N, co
         return fail(DASH_HASH4D_INVALID_ARG, "slice / out not 16-byte aligned");
     const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * sizeof(float);
     Plan P;
-    uint32_t group = pick_group(cfg, level_bytes, "DASH_HASH4D_FWD_GROUP");
-    if (group > 4 && 4 * cfg->F * sizeof(float) >= 32 && !std::getenv("DASH_HASH4D_FWD_GROUP")) group = 4;
+    uint32_t group = pick_group(cfg, level_bytes, DASH_DEBUG_FWD_GROUP);
+    if (group > 4 && 4 * cfg->F * sizeof(float) >= 32 && !debug_u32(DASH_DEBUG_FWD_GROUP)) group = 4;
     if (int rc = fill_slice_plan(cfg, N, xyz_stride, group, &P)) return rc;
     cudaError_t e = dash::launch_fwd(P, xyz, nullptr, index, slice, false, out,
                                      static_cast<cudaStream_t>(cuda_stream));

@@ -585,17 +585,32 @@ slice_t_kernel(const __grid_constant__ Plan P, const float* __restrict__ t,
     }
 }
 
-int sm_count() {
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-            sms <= 0)
+// SM count / L2 bytes of the CURRENT device, cached per device ordinal (a process may drive several GPUs).
+struct DeviceInfo {
+    int sms;
+    size_t l2;
+};
+
+const DeviceInfo& device_info() {
+    constexpr int kMaxDevices = 64;
+    static DeviceInfo cache[kMaxDevices] = {};  // sms == 0: not queried yet; races write identical values
+    static thread_local DeviceInfo scratch;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) dev = -1;
+    DeviceInfo* slot = (dev >= 0 && dev < kMaxDevices) ? &cache[dev] : &scratch;
+    if (slot == &scratch || slot->sms == 0) {
+        int sms = 0, l2 = 0;
+        if (dev < 0 || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
             sms = 148;
+        if (dev < 0 || cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) != cudaSuccess || l2 <= 0)
+            l2 = 64 << 20;
+        slot->l2 = static_cast<size_t>(l2);
+        slot->sms = sms;
     }
-    return sms;
+    return *slot;
 }
+
+int sm_count() { return device_info().sms; }
 
 inline cudaError_t after_launch() {
     ++g_launches;
@@ -612,6 +627,8 @@ inline dim3 item_grid(const Plan& P) {
 void count_launch() { ++g_launches; }
 
 int device_sm_count() { return sm_count(); }
+
+size_t device_l2_bytes() { return device_info().l2; }
 
 uint64_t launch_counter(bool reset) {
     const uint64_t v = g_launches;

@@ -21,3 +21,18 @@ def pytest_collection_modifyitems(config, items):
 @pytest.fixture(scope="session")
 def golden_dir():
     return os.path.join(ROOT, "tests", "golden")
+
+
+@pytest.fixture
+def set_debug():
+    """dash_hash4d_set_debug(key, value) for one test; every touched key is reset to 0 (library default) after."""
+    import paper_2507_19141_b200 as dh
+    used = []
+
+    def _set(key, value):
+        dh.dash_hash4d_set_debug(key, value)
+        used.append(key)
+
+    yield _set
+    for key in used:
+        dh.dash_hash4d_set_debug(key, 0)

@@ -119,3 +119,24 @@ def test_binding_refuses_cpu_tensors():
     x = torch.zeros(4, 3); t = torch.zeros(4); tab = torch.zeros(4, 4096, 2)
     with pytest.raises(ValueError):
         dh.dash_hash4d_fwd(cfg, x, t, tab)
+
+
+def test_build_id_is_the_hash_of_the_sources_beside_the_library():
+    from paper_2507_19141_b200 import build as b
+    lib = C.CDLL(dh.library_path())
+    lib.dash_hash4d_build_id.restype = C.c_char_p
+    assert lib.dash_hash4d_build_id().decode() == b.source_hash() == b.built_id()
+    assert not b.is_stale()
+
+
+def test_set_debug_validates_and_reads_no_environment(monkeypatch):
+    """Overrides go through dash_hash4d_set_debug only; the old environment knobs are dead."""
+    assert dh.dash_hash4d_set_debug(dh.DEBUG_FWD_GROUP, 4) is None
+    dh.dash_hash4d_set_debug(dh.DEBUG_FWD_GROUP, 0)
+    with pytest.raises(dh.Hash4DError):
+        dh.dash_hash4d_set_debug(99, 1)
+    with pytest.raises(dh.Hash4DError):
+        dh.dash_hash4d_set_debug(dh.DEBUG_BWD_GROUP, -1)
+    src = "".join(open(os.path.join(ROOT, "paper_2507_19141_b200", "csrc", f)).read()
+                  for f in os.listdir(os.path.join(ROOT, "paper_2507_19141_b200", "csrc")))
+    assert "getenv" not in src

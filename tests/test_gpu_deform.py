@@ -89,8 +89,8 @@ ENC_CASES = [
 
 @pytest.mark.parametrize("L,F,T,rs,rt,dtype,N,widths,t_stride", ENC_CASES)
 @pytest.mark.parametrize("fused", [1, 0])
-def test_deform_fwd_parity(L, F, T, rs, rt, dtype, N, widths, t_stride, fused, monkeypatch):
-    monkeypatch.setenv("DASH_DEFORM_FUSED", str(fused))
+def test_deform_fwd_parity(L, F, T, rs, rt, dtype, N, widths, t_stride, fused, set_debug):
+    set_debug(dh.DEBUG_DEFORM_PATH, 1 if fused else 2)
     enc = EncoderParams(L, F, T, rs[0], rs[1], rt[0], rt[1], dtype)
     ocfg, gcfg = oracle.config_from_params(enc), dh.config_from_params(enc)
     rng = np.random.default_rng(L * 7 + F + N)

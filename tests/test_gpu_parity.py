@@ -146,10 +146,10 @@ def test_variants(L, F, T, rs, rt, dtype, N, flags):
 
 
 @pytest.mark.parametrize("group", [1, 2, 4, 8, 16])
-def test_every_level_group_size(group, monkeypatch):
+def test_every_level_group_size(group, set_debug):
     """The scheduler's level-group size only changes the launch shape, never the result."""
-    monkeypatch.setenv("DASH_HASH4D_FWD_GROUP", str(group))
-    monkeypatch.setenv("DASH_HASH4D_BWD_GROUP", str(group))
+    set_debug(dh.DEBUG_FWD_GROUP, group)
+    set_debug(dh.DEBUG_BWD_GROUP, group)
     for (L, F, dtype) in [(16, 2, "fp32"), (16, 4, "fp16"), (6, 2, "fp32")]:
         enc = EncoderParams(L, F, 1 << 14, 16, 1024, 8, 100, dtype)
         rng = np.random.default_rng(group)
@@ -423,8 +423,8 @@ def test_bwd_input_variants(L, F, T, rs, rt, dtype, N):
 
 
 @pytest.mark.parametrize("group", [1, 2, 4, 8, 16])
-def test_bwd_input_every_group_size_and_views(group, monkeypatch):
-    monkeypatch.setenv("DASH_HASH4D_FWD_GROUP", str(group))
+def test_bwd_input_every_group_size_and_views(group, set_debug):
+    set_debug(dh.DEBUG_FWD_GROUP, group)
     enc = EncoderParams(12, 2, 1 << 14, 16, 1024, 8, 100)
     rng = np.random.default_rng(group)
     rows = rng.random((300, 3), dtype=np.float32)
@@ -543,8 +543,8 @@ def test_smooth_variants(L, F, T, rs, rt, dtype, N):
 
 
 @pytest.mark.parametrize("group", [1, 2, 4, 8, 16])
-def test_smooth_group_sizes_shared_eps_and_degenerate(group, monkeypatch):
-    monkeypatch.setenv("DASH_HASH4D_SMOOTH_GROUP", str(group))
+def test_smooth_group_sizes_shared_eps_and_degenerate(group, set_debug):
+    set_debug(dh.DEBUG_SMOOTH_GROUP, group)
     enc = EncoderParams(12, 2, 1 << 14, 16, 1024, 8, 100)
     rng = np.random.default_rng(group)
     rows = rng.random((300, 3), dtype=np.float32)
