@@ -36,7 +36,8 @@ METRIC = "4d_hash_encode_fwd_bwd_mqueries_per_s"
 UNIT = "Mqueries/s"
 REFERENCE_SAMPLE_QUERIES = 100_000     # per step of --impl reference
 REFERENCE_BUDGET_SECONDS = 240.0       # --impl reference stops timing further steps after this long
-CPU_BASELINE_QUERIES = 500_000         # bounded sample of the cpu_baseline leg (~10 s of CPU work)
+CPU_BASELINE_QUERIES = 1_000_000       # bounded sample of the cpu_baseline leg (3 runs, ~10 s of CPU work)
+CPU_BASELINE_QUERIES_1T = 100_000      # ... of its single-thread run
 
 
 # ------------------------------------------------------------------------------------------ helpers
@@ -51,14 +52,46 @@ def algorithmic_bytes(enc, has_index: bool):
     return fwd, bwd, zero
 
 
-def profiled_traffic(config: str, kernel: str):
-    """ncu dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed
-    summary profiles/traffic.json (written by hand from the ncu --set full capture it names)."""
+def profiled_traffic(config: str, key: str):
+    """ncu dram__bytes_read.sum + dram__bytes_write.sum, from the committed summary profiles/traffic.json —
+    written by `python -m paper_2507_19141_b200.ncu_summary` from the raw-page CSV of the ncu capture it names.
+    Keys: "fwd_call", "bwd_call" (all launches of one C-ABI call), "step"."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            return float(json.load(fh)[config][kernel])
+            return float(json.load(fh)[config][key])
     except Exception:  # noqa: BLE001
         return None
+
+
+def compulsory_bytes(dh, torch, cfg, enc, N, xyz, t, index):
+    """B_min of SURVEY.md §8d: HBM bytes an ideal cache would still move.  fwd: query inputs once + every TOUCHED
+    32-byte table sector once + `out` once; bwd: query inputs + `dout` once + the whole gradient buffer written
+    once.  The touched sectors are counted exactly, from the library's own corner indices (dash_hash4d_indices)."""
+    s_table = 2 if enc.table_dtype == "fp16" else 4
+    slot_bytes = enc.F * s_table
+    n_sectors = (enc.L * enc.T * slot_bytes + 31) // 32
+    seen = torch.zeros(n_sectors, dtype=torch.bool, device=xyz.device)
+    level_base = (torch.arange(enc.L, device=xyz.device, dtype=torch.int64) * enc.T).view(1, enc.L, 1)
+    chunk = 1 << 16
+    rows_seen = torch.zeros(xyz.shape[0], dtype=torch.bool, device=xyz.device) if index is not None else None
+    for a in range(0, N, chunk):
+        z = min(N, a + chunk)
+        if index is not None:
+            idx, _ = dh.dash_hash4d_indices(cfg, xyz, t[a:z], index=index[a:z], want_weights=False)
+            rows_seen[index[a:z].long()] = True
+        else:
+            idx, _ = dh.dash_hash4d_indices(cfg, xyz[a:z], t[a:z], want_weights=False)
+        slot = idx.long() & 0xffffffff
+        seen[((slot + level_base) * slot_bytes) // 32] = True
+    table_touched = int(seen.sum()) * 32
+    if index is not None:
+        inputs = N * 4 + N * 4 + int(rows_seen.sum()) * 12          # index + t + touched xyz rows
+    else:
+        inputs = N * 16
+    row = enc.L * enc.F * 4
+    fwd = inputs + table_touched + N * row
+    bwd = inputs + N * row + enc.L * enc.T * enc.F * 4
+    return {"fwd": fwd, "bwd": bwd, "step": fwd + bwd, "table_sectors_touched_bytes": table_touched}
 
 
 def measured_hbm_peak():
@@ -170,6 +203,99 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ launcher
+
+def launch_replicas(args):
+    """`python bench.py --gpus N` without torchrun: re-exec this command under torch.distributed.run with N ranks
+    on this node (one process per GPU).  Refuses N above the number of visible devices."""
+    import socket
+    if args.impl != "plumbing":
+        import torch
+        have = torch.cuda.device_count()
+        if args.gpus > have:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) are visible")
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")            # communicator lines: the driver's rank check reads them
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
+def run_plumbing(args):
+    """Launcher self-test (CPU, gloo): every rank joins, barriers, contributes a fake per-rank time; rank 0 prints
+    the rank count it really saw.  No kernel runs and no number here is a measurement."""
+    from paper_2507_19141_b200.replicas import Replicas
+    rep = Replicas(backend="gloo")
+    rep.barrier()
+    ms = rep.max_over_ranks(1.0 + rep.rank)
+    if rep.is_reporter:
+        print(json.dumps({"impl": "plumbing", "n_gpus": rep.world, "max_over_ranks_ms": ms,
+                          "config": {"parallelism": f"replicas x{rep.world}"}}), flush=True)
+    rep.close()
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ ceilings / sweeps
+
+def run_ceilings(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --ceilings: no CUDA device")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    from paper_2507_19141_b200 import ceilings
+    print(json.dumps({"ceilings": ceilings.full()}), flush=True)
+    return 0
+
+
+def run_group_sweep(args):
+    """ms per call of fwd, zero+bwd and bwd(ZERO_GRAD) for G = 1..16 on --config (reproduces profiles/group_sweep_*)."""
+    import torch
+    import paper_2507_19141_b200 as dh
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --sweep-groups: no CUDA device")
+    wl = make_workload(args.config)
+    enc, N = wl.spec.enc, wl.N
+    cfg = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE)
+    cfg_z = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE | dh.FLAG_ZERO_GRAD)
+    to_dev = lambda a: None if a is None else torch.from_numpy(a).cuda()
+    xyz, t, index, table, dout = (to_dev(a) for a in (wl.xyz, wl.t, wl.index, wl.table, wl.dout))
+    out = torch.empty((N, enc.L * enc.F), dtype=torch.float32, device="cuda")
+    dtable = torch.empty((enc.L, enc.T, enc.F), dtype=torch.float32, device="cuda")
+
+    def timed(fn, iters=20):
+        for _ in range(3):
+            fn()
+        a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(iters):
+            fn()
+        z.record(); z.synchronize()
+        return a.elapsed_time(z) / iters
+
+    rows = {}
+    for g in (1, 2, 4, 8, 16):
+        dh.dash_hash4d_set_debug(dh.DEBUG_FWD_GROUP, g)
+        dh.dash_hash4d_set_debug(dh.DEBUG_BWD_GROUP, g)
+        rows[f"G={g}"] = {
+            "fwd_ms": timed(lambda: dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index)),
+            "zero+bwd_ms": timed(lambda: (dh.dash_hash4d_zero(cfg, dtable),
+                                          dh.dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=index))),
+            "bwd_zero_grad_ms": timed(lambda: dh.dash_hash4d_bwd(cfg_z, xyz, t, dout, dtable, index=index)),
+        }
+    dh.dash_hash4d_set_debug(dh.DEBUG_FWD_GROUP, 0)
+    dh.dash_hash4d_set_debug(dh.DEBUG_BWD_GROUP, 0)
+    rows["library_choice"] = {
+        "fwd_ms": timed(lambda: dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index)),
+        "bwd_zero_grad_ms": timed(lambda: dh.dash_hash4d_bwd(cfg_z, xyz, t, dout, dtable, index=index)),
+    }
+    print(json.dumps({"group_sweep": {"config": args.config, "rows": rows}}), flush=True)
+    return 0
+
+
 # ------------------------------------------------------------------------------------------ CUDA arm
 
 def run_cuda(args):
@@ -264,13 +390,57 @@ def run_cuda(args):
         "bound": "hbm", "kernel": kernel_name, "achieved": achieved, "peak": peak,
         "unit": "GB/s", "frac": achieved / peak,
         "traffic": args.traffic_bytes if args.traffic_bytes is not None
-        else profiled_traffic(args.config, kernel_name),
+        else profiled_traffic(args.config, "bwd_call" if dominant == "bwd" else "fwd_call"),
         "peak_source": peak_src,
         "algorithmic_bytes_per_launch": dom_bytes,
         "step": {"algorithmic_bytes": step_bytes, "achieved": step_bytes / (ms_step * 1e-3) / 1e9,
                  "frac": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
                  "ms": {"zero": ms_zero, "fwd": ms_fwd, "bwd": ms_bwd}},
     }
+
+    # ---- the stricter figures of SURVEY.md §8d, beside the algorithmic-bytes fraction
+    bmin = compulsory_bytes(dh, torch, dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE), enc, N, xyz, t, index)
+    roofline["b_min"] = {"bytes": bmin, "step_GBps": bmin["step"] / (ms_step * 1e-3) / 1e9,
+                         "step_frac_of_hbm_peak": bmin["step"] / (ms_step * 1e-3) / 1e9 / peak,
+                         "note": "compulsory HBM bytes with an ideal cache; touched table sectors counted exactly"}
+    roofline["traffic_step"] = profiled_traffic(args.config, "step")
+    roofline["traffic_fwd_call"] = profiled_traffic(args.config, "fwd_call")
+    from paper_2507_19141_b200 import ceilings as ceil_mod
+    ceil = ceil_mod.quick()
+    lane_ops = 16 * enc.L * N                                    # corner gathers (fwd) / corner reductions (bwd)
+    red_key = "red16_pair_xcorner_L2" if enc.F * 4 >= 16 else "red8_pair_xcorner_L2"
+    roofline["ceilings"] = {
+        "gather_G_lane_loads_per_s": ceil["gather8_pair_xcorner_L2"]["G_lane_ops_per_s"],
+        "red_G_lane_reds_per_s": ceil[red_key]["G_lane_ops_per_s"], "red_kernel": red_key,
+        "fwd_G_lane_loads_per_s": lane_ops / (ms_fwd * 1e-3) / 1e9,
+        "bwd_G_lane_reds_per_s": lane_ops / (ms_bwd * 1e-3) / 1e9,
+        "fwd_frac_of_gather_ceiling": lane_ops / (ms_fwd * 1e-3) / 1e9 / ceil["gather8_pair_xcorner_L2"]["G_lane_ops_per_s"],
+        "bwd_frac_of_red_ceiling": lane_ops / (ms_bwd * 1e-3) / 1e9 / ceil[red_key]["G_lane_ops_per_s"],
+        "note": "microbenchmarks of include/dash_ceilings.h run in this process (L2-resident 32 MiB footprint, "
+                "x-corner lane pairs, 8 accesses in flight per lane); bwd time includes the fused zero passes",
+    }
+
+    # ---- deterministic mode (DETERMINISTIC_BWD, 64-bit fixed point): what it costs on this workload
+    det_ms = None
+    if args.deterministic_leg:
+        cfg_det = dh.config_from_params(enc, flags=flags | dh.FLAG_DETERMINISTIC_BWD)
+        need = dh.dash_hash4d_workspace_bytes(cfg_det, N, dh.OP_BWD)
+        try:
+            ws_det = torch.empty(need, dtype=torch.uint8, device="cuda")
+            run_det = lambda: dh.dash_hash4d_bwd(cfg_det, xyz, t, dout, dtable, index=index, workspace=ws_det)
+            run_det(); run_det()
+            torch.cuda.synchronize()
+            d0, d1 = ev(), ev()
+            d0.record()
+            for _ in range(5):
+                run_det()
+            d1.record()
+            torch.cuda.synchronize()
+            det_ms = d0.elapsed_time(d1) / 5
+            del ws_det
+        except torch.OutOfMemoryError:
+            det_ms = None
+    roofline["deterministic_bwd_ms"] = det_ms
 
     # ---- e2e: HOST (pinned) buffers through the binding's *_host calls, copies inside the timed region
     pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory()
@@ -411,9 +581,15 @@ def run_cuda(args):
     # ---- cpu_baseline: the oracle as it stands, bounded sample, on this box's host cores
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        sec, n_s, threads = time_oracle(wl, CPU_BASELINE_QUERIES)
+        import oracle
+        sec, n_s, threads = time_oracle(wl, CPU_BASELINE_QUERIES, repeats=3)
+        oracle.set_threads(1)
+        sec1, n_1, _ = time_oracle(wl, CPU_BASELINE_QUERIES_1T)
+        oracle.set_threads(threads)
         cpu = {"value": n_s / sec / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
-               "sample": f"first {n_s} of {N} queries of {args.config}, fwd+bwd once ({sec:.2f} s)"}
+               "sample": f"first {n_s} of {N} queries of {args.config}, fwd+bwd, best of 3 ({sec:.2f} s)",
+               "one_thread": {"value": n_1 / sec1 / 1e6, "unit": UNIT, "cores": 1,
+                              "sample": f"first {n_1} queries, fwd+bwd once ({sec1:.2f} s)"}}
 
     value = N * world / (ms_step * 1e-3) / 1e6
     ws_mb = ws_bytes / 1e6
@@ -452,15 +628,35 @@ def main():
     ap.add_argument("--steps", type=int, default=None, help="default 200 (cuda arm) / 10 (reference arm)")
     ap.add_argument("--warmup", type=int, default=None, help="default 20 (cuda arm) / 2 (reference arm)")
     ap.add_argument("--config", default="C4", choices=sorted(CONFIGS))
-    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference", "plumbing"],
+                    help="cuda: the product; reference: the CPU oracle; plumbing: launcher/rank self-test on gloo "
+                         "(no kernels, no measurement; tests/test_replicas_gloo.py)")
     ap.add_argument("--zero-grad-fused", type=int, default=1,
                     help="1: bwd zeroes each level group itself (DASH_HASH4D_FLAG_ZERO_GRAD)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", type=int, default=1,
                     help="1: also time bwd_input / smooth / one-timestamp fwd (information only)")
+    ap.add_argument("--deterministic-leg", type=int, default=1,
+                    help="1: also time dash_hash4d_bwd with DETERMINISTIC_BWD (information only)")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), else null")
+    ap.add_argument("--ceilings", action="store_true",
+                    help="run the microbenchmarks of include/dash_ceilings.h and print their JSON line instead")
+    ap.add_argument("--sweep-groups", action="store_true",
+                    help="time fwd / bwd for every level-group size G (dash_hash4d_set_debug) and print a JSON line")
     args = ap.parse_args()
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    if args.impl in ("cuda", "plumbing") and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return launch_replicas(args)
+    if "WORLD_SIZE" in os.environ and int(os.environ["WORLD_SIZE"]) != args.gpus:
+        ap.error(f"--gpus {args.gpus} but the launcher started WORLD_SIZE={os.environ['WORLD_SIZE']} ranks")
+    if args.impl == "plumbing":
+        return run_plumbing(args)
+    if args.ceilings:
+        return run_ceilings(args)
+    if args.sweep_groups:
+        return run_group_sweep(args)
     if args.steps is None:
         args.steps = 10 if args.impl == "reference" else 200
     if args.warmup is None:

@@ -26,7 +26,7 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4
            "dash_hash4d_launch_count", "dash_hash4d_set_debug", "dash_hash4d_build_id",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
            "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd",
-           "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd"]
+           "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch"]
 
 
 class Hash4DError(RuntimeError):
@@ -57,6 +57,16 @@ class MlpConfig(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_layers", C.c_uint32), ("width", C.c_uint32 * 5),
                 ("flags", C.c_uint32)]
 
+
+class CeilingParams(C.Structure):
+    """Mirror of `struct dash_ceiling_params` (include/dash_ceilings.h)."""
+    _fields_ = [("struct_size", C.c_uint32), ("kind", C.c_uint32), ("width", C.c_uint32), ("pattern", C.c_uint32),
+                ("footprint_bytes", C.c_uint64), ("grid", C.c_uint32), ("block", C.c_uint32),
+                ("dyn_smem", C.c_uint32), ("iters", C.c_uint32), ("seed", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+CEIL_COPY, CEIL_GATHER, CEIL_RED, CEIL_SMEM_ATOMIC, CEIL_TMA_GATHER, CEIL_SMEM_ATOMIC_U64 = range(6)
+CEIL_INDEPENDENT, CEIL_PAIR_ALIGNED, CEIL_PAIR_XCORNER = range(3)
 
 _lib: Optional[C.CDLL] = None
 
@@ -131,6 +141,8 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_deform_slice_fwd.restype = C.c_int
     lib.dash_hash4d_launch_count.argtypes = [C.c_int]
     lib.dash_hash4d_launch_count.restype = u64
+    lib.dash_ceiling_launch.argtypes = [C.POINTER(CeilingParams), vp, vp, C.POINTER(C.c_uint64), vp]
+    lib.dash_ceiling_launch.restype = C.c_int
     lib.dash_hash4d_build_id.argtypes = []
     lib.dash_hash4d_build_id.restype = C.c_char_p
     lib.dash_hash4d_set_debug.argtypes = [C.c_int, C.c_int64]
@@ -676,3 +688,23 @@ class HostStep:
             self.out_copied = torch.cuda.Event(); self.out_copied.record(self.d2h)
         main.wait_event(self.out_copied)               # results are complete when the caller's stream is
         return out_h, dtable_h
+
+
+# ---- chip-ceiling microbenchmarks (include/dash_ceilings.h; bench.py --ceilings) --------------------------
+
+def dash_ceiling_launch(kind, buf, sink, width=8, pattern=CEIL_INDEPENDENT, footprint_bytes=None, grid=0, block=0,
+                        dyn_smem=0, iters=16, seed=1) -> int:
+    """One launch of a microbenchmark kernel on the current stream; returns its number of lane accesses."""
+    _dev(buf, torch.uint8, "buf"); _dev(sink, torch.uint8, "sink"); _one_device(buf, sink)
+    p = CeilingParams()
+    p.struct_size = C.sizeof(CeilingParams)
+    p.kind, p.width, p.pattern = int(kind), int(width), int(pattern)
+    p.footprint_bytes = int(buf.numel() if footprint_bytes is None else footprint_bytes)
+    if p.footprint_bytes > buf.numel() or sink.numel() < (p.footprint_bytes if kind == CEIL_COPY else 16):
+        raise ValueError("buf / sink smaller than the footprint")
+    p.grid, p.block, p.dyn_smem, p.iters, p.seed = int(grid), int(block), int(dyn_smem), int(iters), int(seed)
+    ops = C.c_uint64(0)
+    rc = _load().dash_ceiling_launch(C.byref(p), _ptr(buf), _ptr(sink), C.byref(ops), _stream())
+    if rc != 0:
+        raise Hash4DError(rc, "dash_ceiling_launch: bad parameters or launch failure")
+    return int(ops.value)

@@ -51,3 +51,31 @@ def test_single_process_is_identity():
     rate, ms = rep.whole_job_rate(500, 2.0)
     assert ms == 2.0 and rate == 500 / 2e-3
     rep.barrier()
+
+
+def test_bench_launcher_starts_n_ranks_itself():
+    """`python bench.py --gpus 2` with no torchrun wrapper must start 2 ranks.  The launcher path
+    is the product's; `--impl plumbing` swaps the CUDA step for a gloo barrier so it runs on the CPU box."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR",
+                                                              "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "plumbing"],
+                         env=env, capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [json.loads(l) for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                          # rank 0 alone prints
+    assert lines[0]["n_gpus"] == 2 and lines[0]["config"]["parallelism"] == "replicas x2"
+    assert lines[0]["max_over_ranks_ms"] == 2.0                     # rank 1's value won the MAX
+
+
+def test_bench_refuses_a_rank_count_that_contradicts_gpus():
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "plumbing"],
+                         env=env, capture_output=True, text=True, timeout=120)
+    assert res.returncode != 0 and "WORLD_SIZE" in res.stderr
