@@ -311,6 +311,13 @@ def run_cuda(args):
     rep = Replicas(backend="nccl", device=torch.device("cuda", local))
     world, rank = rep.world, rep.rank
 
+    debug_keys = {"fwd_group": dh.DEBUG_FWD_GROUP, "bwd_group": dh.DEBUG_BWD_GROUP,
+                  "smooth_group": dh.DEBUG_SMOOTH_GROUP, "deform_path": dh.DEBUG_DEFORM_PATH,
+                  "bwd_variant": dh.DEBUG_BWD_VARIANT, "fwd_variant": dh.DEBUG_FWD_VARIANT}
+    for item in args.set_debug:
+        key, _, val = item.partition("=")
+        dh.dash_hash4d_set_debug(debug_keys[key], int(val))
+
     wl = make_workload(args.config)
     enc, N = wl.spec.enc, wl.N
     flags = dh.FLAG_DENSE_COARSE | (dh.FLAG_ZERO_GRAD if args.zero_grad_fused else 0)
@@ -606,7 +613,8 @@ def run_cuda(args):
                                f"temporal {enc.res_t_min}->{enc.res_t_max}; step = zero(dtable)+fwd+bwd",
                    "queries_per_step_per_gpu": N, "parallelism": f"replicas x{world}",
                    "l2": l2_note,
-                   "zero_grad_fused": bool(args.zero_grad_fused)},
+                   "zero_grad_fused": bool(args.zero_grad_fused),
+                   **({"debug_overrides": args.set_debug} if args.set_debug else {})},
         "roofline": roofline,
         "e2e": {"value": N * world / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps},
@@ -640,6 +648,9 @@ def main():
                     help="1: also time dash_hash4d_bwd with DETERMINISTIC_BWD (information only)")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), else null")
+    ap.add_argument("--set-debug", action="append", default=[], metavar="KEY=VALUE",
+                    help="dash_hash4d_set_debug override for A/B runs, e.g. bwd_group=1, bwd_variant=2 "
+                         "(keys: fwd_group bwd_group smooth_group deform_path bwd_variant fwd_variant)")
     ap.add_argument("--ceilings", action="store_true",
                     help="run the microbenchmarks of include/dash_ceilings.h and print their JSON line instead")
     ap.add_argument("--sweep-groups", action="store_true",

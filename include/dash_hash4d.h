@@ -255,7 +255,7 @@ enum dash_debug_key {
     DASH_DEBUG_BWD_GROUP = 1,    /* ... of bwd */
     DASH_DEBUG_SMOOTH_GROUP = 2, /* ... of smooth */
     DASH_DEBUG_DEFORM_PATH = 3,  /* dash_deform_fwd: 1 = fused kernel, 2 = two-pass (encoder -> workspace -> MLP) */
-    DASH_DEBUG_BWD_VARIANT = 4,  /* bwd scatter variant, see hash4d_api.cu bwd_impl (0 = default) */
+    DASH_DEBUG_BWD_VARIANT = 4,  /* bwd with ZERO_GRAD: 1 = no L2 eviction hints on the zero stores / reductions */
     DASH_DEBUG_FWD_VARIANT = 5,  /* fwd gather variant (0 = default) */
     DASH_DEBUG_KEY_COUNT = 6
 };

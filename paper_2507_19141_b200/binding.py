@@ -210,7 +210,8 @@ def _at_least(t: Optional[torch.Tensor], count: int, what: str):
 
 
 def _exactly(t: Optional[torch.Tensor], count: int, what: str):
-    if t is not None and t.numel() != count:
+    """count == 0 means the config itself is invalid: let the C ABI report that with its own status code."""
+    if t is not None and count and t.numel() != count:
         raise ValueError(f"{what} holds {t.numel()} elements, the config says {count}")
 
 

@@ -447,18 +447,24 @@ static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
         return ok();
     }
     // ZERO_GRAD: zero one level group, scatter into it while the zeros are still in L2, next group.
+    // (A one-launch variant whose tail CTAs zero the next group's slice was built and measured in round 2: slower,
+    // profiles/experiments_r02.md §1.)
     const uint32_t groups = P.num_groups;
     for (uint32_t g = 0; g < groups; ++g) {
         const uint32_t l0 = g * P.group;
         const uint32_t l1 = (l0 + P.group < cfg->L) ? l0 + P.group : cfg->L;
         char* base = reinterpret_cast<char*>(dtable) + static_cast<size_t>(l0) * level_bytes;
         const size_t bytes = static_cast<size_t>(l1 - l0) * level_bytes;
-        e = dash::launch_zero(base, bytes, s);  // handles slices that are only 4-byte aligned
+        // L2 evict_last hints on the zero stores and the reductions keep the group's slice resident against the
+        // streamed dout / coordinates: C4 bwd 1.190 -> 1.168 ms, DRAM bytes per call 2.76 -> 1.54 GB (ncu,
+        // profiles/experiments_r02.md §2).  DASH_DEBUG_BWD_VARIANT = 1 turns the hints off for A/B runs.
+        const bool hint = debug_u32(DASH_DEBUG_BWD_VARIANT) != 1;
+        e = dash::launch_zero(base, bytes, s, hint);  // handles slices that are only 4-byte aligned
         if (e != cudaSuccess) return cuda_fail(e, "zero launch");
         Plan Pg = P;
         Pg.level_begin = l0;
         Pg.num_groups = 1;
-        e = dash::launch_bwd(Pg, xyz, t, index, dout, dtable, s);
+        e = dash::launch_bwd(Pg, xyz, t, index, dout, dtable, s, hint);
         if (e != cudaSuccess) return cuda_fail(e, "bwd launch");
     }
     return ok();

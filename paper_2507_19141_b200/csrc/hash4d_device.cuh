@@ -208,5 +208,30 @@ __device__ __forceinline__ void red_add(float* p, const float v[F]) {
     }
 }
 
+// The same reductions carrying an L2 eviction-priority hint (createpolicy): experiment of round 2 on keeping a level
+// group's gradient slice resident against the streamed dout / coordinates.
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+
+template <int F>
+__device__ __forceinline__ void red_add_hint(float* p, const float v[F], uint64_t pol) {
+    if constexpr (F == 1) {
+        asm volatile("red.global.add.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(p), "f"(v[0]), "l"(pol) : "memory");
+    } else if constexpr (F == 2) {
+        asm volatile("red.global.add.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v[0]), "f"(v[1]),
+                     "l"(pol)
+                     : "memory");
+    } else {
+#pragma unroll
+        for (int h = 0; h < F / 4; ++h)
+            asm volatile("red.global.add.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p + 4 * h),
+                         "f"(v[4 * h]), "f"(v[4 * h + 1]), "f"(v[4 * h + 2]), "f"(v[4 * h + 3]), "l"(pol)
+                         : "memory");
+    }
+}
+
 }  // namespace
 }  // namespace dash

@@ -35,17 +35,19 @@ struct Item {
     bool active;
 };
 
-__device__ __forceinline__ Item this_item(const Plan& P) {
+__device__ __forceinline__ Item this_item(const Plan& P, uint32_t tile, uint32_t grp) {
     const uint32_t pair = threadIdx.x >> 1;
     Item it;
     it.xc = threadIdx.x & 1u;
-    it.n = static_cast<uint64_t>(blockIdx.x) * P.q_per_block + (pair >> P.group_log2);
-    it.l = P.level_begin + blockIdx.y * P.group + (pair & (P.group - 1u));
+    it.n = static_cast<uint64_t>(tile) * P.q_per_block + (pair >> P.group_log2);
+    it.l = P.level_begin + grp * P.group + (pair & (P.group - 1u));
     it.active = (it.n < P.N) && (it.l < P.L);
     if (it.n >= P.N) it.n = P.N - 1;
     if (it.l >= P.L) it.l = P.L - 1;
     return it;
 }
+
+__device__ __forceinline__ Item this_item(const Plan& P) { return this_item(P, blockIdx.x, blockIdx.y); }
 
 // ------------------------------------------------------------------------------------------------
 // Forward: gather + quadrilinear interpolation (Eq. 9)
@@ -128,7 +130,7 @@ __device__ __forceinline__ void load_dout(const float* __restrict__ d, uint32_t 
 // ------------------------------------------------------------------------------------------------
 // Backward: scatter-add of W_k * dY into the table gradient (transpose of Eq. 9)
 // ------------------------------------------------------------------------------------------------
-template <int F, int D>
+template <int F, int D, bool HINT = false>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_bwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                   const float* __restrict__ t, const int32_t* __restrict__ index,
@@ -145,12 +147,15 @@ hash4d_bwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
     half_cell<D>(P, lp, q, it.xc, slot, W);  // recomputed, never cached from fwd (128 B per item)
     if (!it.active) return;
     float* level_base = dtable + static_cast<size_t>(it.l) * P.T * F;
+    uint64_t pol = 0;
+    if constexpr (HINT) pol = l2_policy_evict_last();
 #pragma unroll
     for (int j = 0; j < NC; ++j) {
         float c[F];
 #pragma unroll
         for (int f = 0; f < F; ++f) c[f] = W[j] * g[f];
-        red_add<F>(level_base + static_cast<size_t>(slot[j]) * F, c);
+        if constexpr (HINT) red_add_hint<F>(level_base + static_cast<size_t>(slot[j]) * F, c, pol);
+        else red_add<F>(level_base + static_cast<size_t>(slot[j]) * F, c);
     }
 }
 
@@ -411,14 +416,23 @@ hash4d_indices_kernel(const __grid_constant__ Plan P, const float* __restrict__ 
 // ------------------------------------------------------------------------------------------------
 // Small helpers: fill, |dout| max, fixed-point finalize, input validation
 // ------------------------------------------------------------------------------------------------
+template <bool HINT>
 __global__ void __launch_bounds__(kBlockThreads)
 zero_kernel(unsigned char* __restrict__ base, size_t head, size_t n16, size_t tail) {
     // [base, base+head) bytes up to 16-byte alignment, then n16 aligned 16-byte stores, then tail bytes
     uint4* body = reinterpret_cast<uint4*>(base + head);
     const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
+    uint64_t pol = 0;
+    if constexpr (HINT) pol = l2_policy_evict_last();
     for (size_t i = static_cast<size_t>(blockIdx.x) * kBlockThreads + threadIdx.x; i < n16;
-         i += stride)
-        body[i] = make_uint4(0u, 0u, 0u, 0u);
+         i += stride) {
+        if constexpr (HINT)
+            asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1, %1, %1, %1}, %2;" ::"l"(body + i), "r"(0u),
+                         "l"(pol)
+                         : "memory");
+        else
+            body[i] = make_uint4(0u, 0u, 0u, 0u);
+    }
     if (blockIdx.x == 0) {
         if (threadIdx.x < head) base[threadIdx.x] = 0;
         if (threadIdx.x < tail) base[head + n16 * 16 + threadIdx.x] = 0;
@@ -717,14 +731,18 @@ cudaError_t launch_smooth(const Plan& P, const float* xyz, const float* t, const
 }
 
 cudaError_t launch_bwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
-                       const float* dout, float* dtable, cudaStream_t s) {
+                       const float* dout, float* dtable, cudaStream_t s, bool l2_hint) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
-#define DASH_BWD(FV)                                                                         \
-    do {                                                                                     \
-        if (P.dims == 3)                                                                     \
-            hash4d_bwd_kernel<FV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); \
-        else                                                                                 \
-            hash4d_bwd_kernel<FV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable); \
+#define DASH_BWD(FV)                                                                                 \
+    do {                                                                                             \
+        if (P.dims == 3 && l2_hint)                                                                  \
+            hash4d_bwd_kernel<FV, 3, true><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable);   \
+        else if (P.dims == 3)                                                                        \
+            hash4d_bwd_kernel<FV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable);         \
+        else if (l2_hint)                                                                            \
+            hash4d_bwd_kernel<FV, 4, true><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable);   \
+        else                                                                                         \
+            hash4d_bwd_kernel<FV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, dout, dtable);         \
     } while (0)
     switch (P.F) {
         case 1: DASH_BWD(1); break;
@@ -772,7 +790,7 @@ cudaError_t launch_indices(const Plan& P, const float* xyz, const float* t, cons
     return after_launch();
 }
 
-cudaError_t launch_zero(void* ptr, size_t bytes, cudaStream_t s) {
+cudaError_t launch_zero(void* ptr, size_t bytes, cudaStream_t s, bool l2_hint) {
     if (bytes == 0) return cudaSuccess;
     size_t head = (16 - (reinterpret_cast<uintptr_t>(ptr) & 15u)) & 15u;
     if (head > bytes) head = bytes;
@@ -780,7 +798,10 @@ cudaError_t launch_zero(void* ptr, size_t bytes, cudaStream_t s) {
     const size_t want = (n16 + kBlockThreads - 1) / kBlockThreads;
     const size_t cap = static_cast<size_t>(sm_count()) * 16;
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
-    zero_kernel<<<blocks, kBlockThreads, 0, s>>>(static_cast<unsigned char*>(ptr), head, n16, tail);
+    if (l2_hint)
+        zero_kernel<true><<<blocks, kBlockThreads, 0, s>>>(static_cast<unsigned char*>(ptr), head, n16, tail);
+    else
+        zero_kernel<false><<<blocks, kBlockThreads, 0, s>>>(static_cast<unsigned char*>(ptr), head, n16, tail);
     return after_launch();
 }
 

@@ -28,13 +28,13 @@ cudaError_t launch_smooth(const Plan& P, const float* xyz, const float* t, const
                           const float* eps, uint32_t eps_stride, const void* table, bool table_half,
                           float two_scale, float* loss, float* dtable, cudaStream_t s);
 cudaError_t launch_bwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
-                       const float* dout, float* dtable, cudaStream_t s);
+                       const float* dout, float* dtable, cudaStream_t s, bool l2_hint = false);
 cudaError_t launch_bwd_fixed(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                              const float* dout, long long* acc, const WorkspaceHeader* hdr,
                              cudaStream_t s);
 cudaError_t launch_indices(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                            uint32_t* idx_out, float* w_out, cudaStream_t s);
-cudaError_t launch_zero(void* ptr, size_t bytes, cudaStream_t s);
+cudaError_t launch_zero(void* ptr, size_t bytes, cudaStream_t s, bool l2_hint = false);
 cudaError_t launch_absmax(const float* v, size_t count, WorkspaceHeader* hdr, uint64_t N,
                           cudaStream_t s);
 cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t count,

@@ -609,3 +609,74 @@ def test_calls_are_cuda_graph_capturable():
     np.testing.assert_allclose(dq.cpu().numpy(),
                                oracle.oracle_bwd_input(ocfg, wl.N, wl.xyz, wl.t, wl.table, wl.dout),
                                rtol=1e-3, atol=1e-5)
+
+
+def test_binding_rejects_buffers_that_do_not_match_the_config():
+    """The C ABI takes raw pointers; the binding is where allocation sizes are known: a short table /
+    out / dout / dtable / t / index, rows < N, or an out-of-range index under VALIDATE_INPUTS must raise, not corrupt."""
+    enc = EncoderParams(4, 2, 1 << 10, 8, 64, 4, 16)
+    cfg = dh.config_from_params(enc)
+    n = 100
+    xyz, t = torch.rand((n, 3), device="cuda"), torch.rand(n, device="cuda")
+    table = torch.zeros((enc.L, enc.T, enc.F), device="cuda")
+    dout = torch.zeros((n, enc.L * enc.F), device="cuda")
+    dtable = torch.zeros_like(table)
+    dh.dash_hash4d_fwd(cfg, xyz, t, table)                                        # the well-formed call passes
+    with pytest.raises(ValueError, match="table"):
+        dh.dash_hash4d_fwd(cfg, xyz, t, table[:-1].contiguous())
+    with pytest.raises(ValueError, match="out"):
+        dh.dash_hash4d_fwd(cfg, xyz, t, table, out=torch.empty((n - 1, enc.L * enc.F), device="cuda"))
+    with pytest.raises(ValueError, match="t holds"):
+        dh.dash_hash4d_fwd(cfg, xyz, t[:50].contiguous(), table, t_stride=1)
+    with pytest.raises(ValueError, match="rows"):
+        dh.dash_hash4d_fwd(cfg, xyz, t, table, N=n + 1)
+    with pytest.raises(ValueError, match="dout"):
+        dh.dash_hash4d_bwd(cfg, xyz, t, dout[:-1].contiguous(), dtable)
+    with pytest.raises(ValueError, match="dtable"):
+        dh.dash_hash4d_bwd(cfg, xyz, t, dout, dtable[:, :-1].contiguous())
+    index = torch.arange(n, device="cuda", dtype=torch.int32)
+    with pytest.raises(ValueError, match="index"):
+        dh.dash_hash4d_fwd(cfg, xyz, t, table, index=index[:10].contiguous(), N=n)
+    bad = index.clone(); bad[7] = n + 5
+    cfg_v = dh.config_from_params(enc, flags=DC | dh.FLAG_VALIDATE_INPUTS)
+    with pytest.raises(ValueError, match="index values"):
+        dh.dash_hash4d_fwd(cfg_v, xyz, t, table, index=bad)
+    with pytest.raises(ValueError, match="dq"):
+        dh.dash_hash4d_bwd_input(cfg, xyz, t, table, dout, dq=torch.empty((n, 3), device="cuda"))
+    with pytest.raises(ValueError, match="slice"):
+        dh.dash_hash4d_slice_fwd(cfg, xyz, torch.zeros((enc.L, enc.T - 1, enc.F), device="cuda"))
+    with pytest.raises(ValueError, match="m holds"):
+        dh.dash_hash4d_adam_step(cfg, table, dtable, torch.zeros(5, device="cuda"), torch.zeros_like(table), 1)
+
+
+@pytest.mark.parametrize("group", [0, 1, 2, 4])
+def test_zero_grad_overwrites_garbage_for_every_group_size(group, set_debug):
+    """ZERO_GRAD zeroes each level group's slice (possibly only 4-byte aligned) right before scattering into it:
+    N spans many tiles with a ragged tail, L is not a multiple of G, T*F*4 is not always a multiple of 16."""
+    variant = 0
+    set_debug(dh.DEBUG_BWD_GROUP, group)
+    for (L, F, T, n) in [(7, 4, 1 << 13, 40_003), (5, 2, 1 << 12, 3_001), (3, 1, 1003, 777)]:
+        enc = EncoderParams(L, F, T, 8, 300, 4, 40)
+        rng = np.random.default_rng(L + n)
+        xyz, t = make_queries_uniform(L + n, n)
+        dout = rng.standard_normal((n, L * F)).astype(np.float32)
+        run_bwd_parity(enc, xyz, t, dout, flags=DC | dh.FLAG_ZERO_GRAD, what=f"zero-grad v{variant} G{group} L{L}")
+
+
+def test_zero_grad_through_the_raw_abi_without_workspace():
+    enc = EncoderParams(6, 4, 1 << 12, 8, 200, 4, 30)
+    ocfg, gcfg = both_configs(enc, DC | dh.FLAG_ZERO_GRAD)
+    n = 5000
+    xyz, t = make_queries_uniform(9, n)
+    dout = np.random.default_rng(9).standard_normal((n, 24)).astype(np.float32)
+    ref, mag = oracle.oracle_bwd(ocfg, n, xyz, t, dout, want_abs=True)
+    dt = torch.full((6, 1 << 12, 4), 7.0, device="cuda")
+    lib = dh.binding._load()
+    import ctypes as C
+    xd, td, dd = dev(xyz), dev(t), dev(dout)                                      # keep the device copies alive
+    rc = lib.dash_hash4d_bwd(C.byref(gcfg), n, C.c_void_p(xd.data_ptr()), 3, C.c_void_p(td.data_ptr()), 1,
+                             None, C.c_void_p(dd.data_ptr()), C.c_void_p(dt.data_ptr()), None, 0,
+                             C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    torch.cuda.synchronize()
+    assert rc == 0
+    check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 6, what="zero-grad, no workspace")
