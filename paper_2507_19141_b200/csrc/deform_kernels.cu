@@ -23,14 +23,13 @@
 // ~70 % of its wavefront rate); the tensor pipe (~4 % busy) and the epilogue run underneath them.  D = 3: 8-corner
 // gathers in a per-frame time slice of the tables (Q29).  FUSED = false: the producer warps read a
 // feature matrix from global memory instead (two-pass path for tables that do not fit L2 in one level group).
-// Build with -DDASH_DEFORM_PROFILE for clock64() phase timers printed by CTA 0 (development only).
+// Phase timers for development builds live in deform_profile.cuh (DASH_PROF_* macros; empty in the product build).
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
-#include <cstdio>
-
 #include "deform_kernels.h"
+#include "deform_profile.cuh"
 #include "hash4d_device.cuh"
 
 namespace dash {
@@ -187,6 +186,30 @@ __device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint3
     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
 
+// One lane of a converged warp.  The MMA issue runs as "whole warp enters, elected lane issues" with every operand
+// derived from warp-uniform values: behind a per-thread `if (lane == 0)` the compiler cannot prove the descriptors
+// uniform and wraps EVERY tcgen05.mma in an ELECT / R2UR.BROADCAST / BRA.U.ANY loop (~120 cycles per instruction,
+// 3.2K cycles of issue per tile in the round-1 kernel: clock64 phase timers, profiles/experiments_r02.md §3).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred P;\n"
+        "elect.sync _|P, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, P;\n"
+        "}"
+        : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ uint32_t uniform(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
+
+// max(x, 0) and round to bf16, two values per instruction (cvt.rn.relu.bf16x2.f32: NaN -> canonical NaN)
+__device__ __forceinline__ uint32_t pack_bf16_relu(float lo, float hi) {
+    uint32_t r;
+    asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));   // first source -> upper half
+    return r;
+}
+
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     const __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);  // .x = lo (low 16 bits)
     return *reinterpret_cast<const uint32_t*>(&h);
@@ -203,9 +226,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                     const float* __restrict__ feat, const float* __restrict__ params,
                     const float* __restrict__ base, float* __restrict__ out) {
     extern __shared__ __align__(128) unsigned char smem[];
-#ifdef DASH_DEFORM_PROFILE
-    const long long t_entry = clock64();
-#endif
+    DASH_PROF_ENTRY();
     uint32_t sbase = smem_u32(smem);
     asm volatile("" : "+r"(sbase));   // opaque: keep it in a register instead of re-deriving the shared window base
     const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31u;
@@ -234,6 +255,19 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                      : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = uniform(*tmem_slot);
+    DASH_PROF_BEGIN(tid);
+
+    // FUSED: the weights are staged by the CONSUMER warps only, while the producers already gather their first tile
+    // (the producers never read them): the 5-6K cycles of setup of the round-1 kernel leave the critical path.
+    // MLP-only mode has nothing to overlap them with: all threads stage, then one CTA barrier.
+    constexpr uint32_t kStageFirst = FUSED ? kProducerThreads : 0u;
+    constexpr uint32_t kStagers = kDeformThreads - kStageFirst;
+    if (!FUSED || warp >= kDeformEncWarps)
     for (uint32_t l = 0; l < M.n_layers; ++l) {
         // W_l as the B operand [npad][kpad], one 16-byte chunk (8 consecutive k of one output row j) per step;
         // consecutive threads take consecutive chunks of a row: coalesced (float4 when aligned) global reads; the
@@ -246,7 +280,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
         unsigned char* ws = smem + M.w_off[l];
         const uint32_t cpr = kp >> 3, w_lbo = operand_lbo(np);
         const bool vec = (K & 7u) == 0 && (reinterpret_cast<uintptr_t>(W) & 15u) == 0;  // float4 row chunks
-        for (uint32_t i = tid; i < np * cpr; i += kDeformThreads) {
+        for (uint32_t i = tid - kStageFirst; i < np * cpr; i += kStagers) {
             const uint32_t j = i / cpr, c = i - j * cpr, k0 = c * 8u;   // consecutive threads: consecutive chunks
             float w[8];
 #pragma unroll
@@ -275,27 +309,25 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                            pack_bf16(w[6], w[7]));
         }
     }
-    for (uint32_t i = tid; i < (2u * a0_bytes) / 16u; i += kDeformThreads) {
-        const uint32_t within = (i * 16u) % a0_bytes;                     // byte offset inside one A buffer
-        reinterpret_cast<uint4*>(smem + M.a0_off)[i] =
-            (within / a_lbo == (M.kbias[0] >> 3)) ? ones_chunk : make_uint4(0u, 0u, 0u, 0u);
+    if constexpr (!FUSED) {
+        fence_async_smem();
+        __syncthreads();
     }
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot;
-
-#ifdef DASH_DEFORM_PROFILE
-    __shared__ long long prof[3][64];
-    __shared__ long long prof_t0;
-    if (tid == 0) { prof_t0 = clock64(); prof[0][40] = prof[0][41] = prof[0][42] = 0; }
-    __syncthreads();
-    const long long t_setup = prof_t0;   // one time base for all roles (SM clock)
-#define PROF(role, idx) do { if (blockIdx.x == 0 && (idx) < 64) prof[role][idx] = clock64() - t_setup; } while (0)
-#else
-#define PROF(role, idx) do { } while (0)
-#endif
+    if (warp >= kDeformEncWarps) {
+        if constexpr (FUSED) {
+            fence_async_smem();   // the staged weights are read by the async proxy (tcgen05.mma)
+            asm volatile("bar.sync %0, %1;" ::"r"(3u), "r"(kDeformThreads - kProducerThreads) : "memory");
+        }
+    } else {
+        // the A buffers are the producers': zeros, and (1, 1) in the chunk that multiplies the bias columns; their
+        // tile writes follow behind a producers-only barrier, and every producer fences before it signals "full"
+        for (uint32_t i = tid; i < (2u * a0_bytes) / 16u; i += kProducerThreads) {
+            const uint32_t within = (i * 16u) % a0_bytes;                 // byte offset inside one A buffer
+            reinterpret_cast<uint4*>(smem + M.a0_off)[i] =
+                (within / a_lbo == (M.kbias[0] >> 3)) ? ones_chunk : make_uint4(0u, 0u, 0u, 0u);
+        }
+        asm volatile("bar.sync %0, %1;" ::"r"(4u), "r"(kProducerThreads) : "memory");
+    }
 
     // Each CTA owns a contiguous range of rows [r_begin, r_end) — an equal share of N, not a whole number of
     // tiles — and walks it in tiles of 128; in its last, partial tile the producers skip the missing rows, so the
@@ -312,7 +344,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
             const uint64_t row0 = r_begin + static_cast<uint64_t>(i) * kDeformTileM;
             const uint32_t rows_here = r_end - row0 < kDeformTileM ? static_cast<uint32_t>(r_end - row0) : kDeformTileM;
             mbar_wait(bar_empty + 8 * s, ((i >> 1) & 1u) ^ 1u);  // first use of each buffer passes at once
-            if (tid == 0) PROF(0, 2 * i);
+            if (tid == 0) DASH_PROF(0, 2 * i);
             const uint32_t a0 = sbase + M.a0_off + s * a0_bytes;   // shared-space address of this tile's A buffer
             if constexpr (FUSED) {
                 // One ROUND = 16 (query, level) items = one warp instruction's worth of lane pairs; a full tile has
@@ -352,9 +384,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                     if (w0 < rounds) load_coords<D>(P, item_row(rk < rounds ? rk : w0), xyz, t, index, cq[k]);
                 }
                 for (uint32_t ra = w0; ra < rounds; ra += kStep) {
-#ifdef DASH_DEFORM_PROFILE
-                    const long long q0 = clock64();
-#endif
+                    DASH_PROF_CLOCK(q0);
                     uint32_t rk[R];
                     uint32_t slot[R][NC];
                     float W[R][NC];
@@ -374,9 +404,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
 #pragma unroll
                         for (int j = 0; j < NC; ++j) load_slot<F, HALF>(level_base, slot[k][j], v[k][j]);
                     }
-#ifdef DASH_DEFORM_PROFILE
-                    const long long q1 = clock64();
-#endif
+                    DASH_PROF_CLOCK(q1);
                     if (ra + kStep < rounds) {   // next iteration's coordinates, under the gathers
 #pragma unroll
                         for (int k = 0; k < R; ++k) {
@@ -395,12 +423,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                             for (int f = 0; f < F; ++f) acc[f] = fmaf(W[k][j], v[k][j][f], acc[f]);
 #pragma unroll
                         for (int f = 0; f < F; ++f) acc[f] += __shfl_xor_sync(0xffffffffu, acc[f], 1);
-#ifdef DASH_DEFORM_PROFILE
-                        if (blockIdx.x == 0 && tid == 0) {
-                            const long long q2 = clock64();
-                            prof[0][40] += q1 - q0; prof[0][41] += q2 - q1; prof[0][42] += 1;
-                        }
-#endif
+                        DASH_PROF_ACCUM(tid == 0, q1 - q0, clock64() - q1);
                         if (xc == 0 && (k == 0 || rk[k] != ra)) {
                             // fp32 feature -> bf16 operand element (row q, column l*F + f)
                             const uint32_t it = rk[k] * 16u + pair;
@@ -438,7 +461,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
             }
             fence_async_smem();
             mbar_arrive(bar_full + 8 * s);
-            if (tid == 0) PROF(0, 2 * i + 1);
+            if (tid == 0) DASH_PROF(0, 2 * i + 1);
         }
     } else {
         // ================================================================================== CONSUMER PIPELINE p
@@ -447,9 +470,10 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
         // (tcgen05.st) and the next layer's MMA reads its A operand from there (TS form).  A consumer thread touches
         // shared memory only to wait on an mbarrier: everything that goes through the SM's LSU queue waits behind
         // the producers' gathers (measured: 6-14K cycles per layer with shared-memory activations, profiles/).
-        const uint32_t cw = warp - kDeformEncWarps;
+        const uint32_t cw = uniform(warp) - kDeformEncWarps;   // warp-uniform by construction (see elect_one)
         const uint32_t p = cw >> 2, e = cw & 3u;            // e == warp % 4: owns TMEM lanes 32e .. 32e+31
-        const bool issuer = e == 0 && lane == 0;            // this pipeline's MMA-issuing thread
+        const bool issue_warp = e == 0;                     // this pipeline's MMA-issuing warp (one elected lane)
+        const uint32_t sb = uniform(sbase);
         const uint32_t r = e * 32u + lane;                  // accumulator row = query within the tile
         const uint32_t tmem_d = tmem_base + p * M.tmem_pipe_cols;        // accumulator columns of this pipeline
         const uint32_t tmem_a = tmem_d + M.tmem_a_off;                   // bf16 A operand of layers 2..n
@@ -459,40 +483,47 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
         for (uint32_t i = p; i < my_tiles && p < M.npipes; i += M.npipes) {
             const uint32_t s = i & 1u;
             const uint64_t n = r_begin + static_cast<uint64_t>(i) * kDeformTileM + r;
-            for (uint32_t l = 0; l < M.n_layers; ++l, ++batch) {
-                if (issuer) {
-                    if (l == 0) mbar_wait(bar_full + 8 * s, (i >> 1) & 1u);
+#pragma unroll
+            for (uint32_t l = 0; l < kMlpMaxLayers; ++l, ++batch) {   // unrolled: M.*[l] become direct constant reads
+                if (l >= M.n_layers) break;
+                if (issue_warp) {
+                    if (l == 0) mbar_wait(sb + 8 * s, (i >> 1) & 1u);   // bar_full[s]
                     tc_fence_after();
-                    if (p == 0) PROF(1, 2 * batch);
-                    const uint32_t w_addr = sbase + M.w_off[l];
-                    const uint32_t np = M.npad[l], ksteps = M.kpad[l] >> 4;
-                    const uint32_t w_lbo = operand_lbo(np);
-                    const uint32_t idesc = umma_idesc(np);
-                    if (l == 0) {
-                        const uint32_t a_addr = sbase + M.a0_off + s * a0_bytes;
-                        for (uint32_t kk = 0; kk < ksteps; ++kk) {
-                            const uint64_t ad = umma_desc(a_addr + kk * 2u * a_lbo, a_lbo, 128u);
-                            const uint64_t bd = umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u);
-                            tc_mma_bf16(tmem_d, ad, bd, idesc, kk > 0 ? 1u : 0u);
+                    if (p == 0 && lane == 0) DASH_PROF(1, 2 * batch);
+                    if (elect_one()) {
+                        const uint32_t w_addr = sb + M.w_off[l];
+                        const uint32_t np = M.npad[l], ksteps = M.kpad[l] >> 4;
+                        const uint32_t w_lbo = operand_lbo(np);
+                        const uint32_t idesc = umma_idesc(np);
+                        if (l == 0) {
+                            const uint32_t a_addr = sb + M.a0_off + s * a0_bytes;
+                            for (uint32_t kk = 0; kk < ksteps; ++kk) {
+                                const uint64_t ad = umma_desc(a_addr + kk * 2u * a_lbo, a_lbo, 128u);
+                                const uint64_t bd = umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u);
+                                tc_mma_bf16(tmem_d, ad, bd, idesc, kk > 0 ? 1u : 0u);
+                            }
+                            tc_commit(sb + 16 + 8 * s);  // bar_empty[s]: A buffer free once these MMAs have read it
+                        } else {
+                            for (uint32_t kk = 0; kk < ksteps; ++kk) {   // K = 16 per instruction = 8 TMEM columns of A
+                                const uint64_t bd = umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u);
+                                tc_mma_bf16_ts(tmem_d, tmem_a + kk * 8u, bd, idesc, kk > 0 ? 1u : 0u);
+                            }
                         }
-                        tc_commit(bar_empty + 8 * s);  // A buffer free once these MMAs have read it
-                    } else {
-                        for (uint32_t kk = 0; kk < ksteps; ++kk) {   // K = 16 per instruction = 8 TMEM columns of A
-                            const uint64_t bd = umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u);
-                            tc_mma_bf16_ts(tmem_d, tmem_a + kk * 8u, bd, idesc, kk > 0 ? 1u : 0u);
-                        }
+                        tc_commit(sb + 32 + 8 * p);      // bar_mma[p]
                     }
-                    tc_commit(bar_mma);
-                    if (p == 0) PROF(1, 2 * batch + 1);
+                    __syncwarp();
+                    if (p == 0 && lane == 0) DASH_PROF(1, 2 * batch + 1);
                 }
                 mbar_wait(bar_mma, mma_phase);
                 mma_phase ^= 1u;
                 __syncwarp();
                 tc_fence_after();
-                if (cw == 0 && lane == 0) PROF(2, 2 * batch);
+                if (cw == 0 && lane == 0) DASH_PROF(2, 2 * batch);
                 const uint32_t np = M.npad[l];
                 if (l + 1 < M.n_layers) {
-                    // hidden layer: relu, -> bf16 pairs, -> tensor memory (the bias came out of the MMA)
+                    // hidden layer: relu, -> bf16 pairs, -> tensor memory (the bias came out of the MMA).  (A version
+                    // with 16-column steps and one load kept in flight under the conversion was measured slower:
+                    // 1.2K instead of 1.0K cycles per layer, profiles/experiments_r02.md §3.)
                     for (uint32_t c = 0; c < np; c += 32u) {   // np is a multiple of 16: the last round may be half
                         uint32_t rr[32];
                         tc_ld32_nowait(tmem_d + lane_off + c, rr);
@@ -500,8 +531,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                         uint32_t w[16];
 #pragma unroll
                         for (int j = 0; j < 16; ++j)
-                            w[j] = pack_bf16(fmaxf(__uint_as_float(rr[2 * j]), 0.0f),
-                                             fmaxf(__uint_as_float(rr[2 * j + 1]), 0.0f));
+                            w[j] = pack_bf16_relu(__uint_as_float(rr[2 * j]), __uint_as_float(rr[2 * j + 1]));
                         if (c + 16u < np) {
                             tc_st16(tmem_a + lane_off + (c >> 1), w);
                         } else {
@@ -512,6 +542,32 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                     const uint32_t tail[8] = {0x3f803f80u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
                     tc_st8(tmem_a + lane_off + (np >> 1), tail);
                     tc_st_wait();
+                } else if (M.out_stage_off != 0u) {
+                    // narrow last layer (n_out <= 16, the deformation heads): a thread owns a row, i.e. n_out floats
+                    // at a 4*n_out-byte stride from its neighbours' — stored directly, every store instruction touches
+                    // 32 sectors (measured: 1.5K of the 2.1K cycles of this epilogue, profiles/experiments_r02.md §3).
+                    // The warp's 32 rows are ONE contiguous block of `out`: transpose through 2 KB of shared memory
+                    // and store it with lane-contiguous (fully coalesced) instructions; `base` is read the same way.
+                    float v[16];
+                    tc_ld16(tmem_d + lane_off, v);
+                    const uint32_t stage = sb + M.out_stage_off + cw * 2048u;
+                    const uint32_t n_out = M.n_out;
+#pragma unroll
+                    for (int j = 0; j < 16; ++j)
+                        if (static_cast<uint32_t>(j) < n_out) sts32(stage + (lane * n_out + j) * 4u, __float_as_uint(v[j]));
+                    __syncwarp();
+                    const uint64_t n0 = n - lane;                                   // first row of this warp
+                    const uint32_t rows_valid = n0 < r_end ? (r_end - n0 < 32u ? static_cast<uint32_t>(r_end - n0) : 32u) : 0u;
+                    const uint32_t count = rows_valid * n_out;
+                    float* o = out + n0 * n_out;
+                    const float* bb = base ? base + n0 * n_out : nullptr;
+#pragma unroll 4
+                    for (uint32_t k = lane; k < count; k += 32u) {
+                        float val;
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(val) : "r"(stage + k * 4u) : "memory");
+                        __stcs(o + k, val + (bb ? __ldcs(bb + k) : 0.0f));
+                    }
+                    __syncwarp();   // the staging block is rewritten by this warp's next tile
                 } else {
                     for (uint32_t c = 0; c < np; c += 16u) {
                         float v[16];
@@ -528,7 +584,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
                 tc_fence_before();
                 // the 4 warps of this pipeline: activations written and TMEM drained before the next MMAs
                 asm volatile("bar.sync %0, %1;" ::"r"(1u + p), "r"(kEpilogueThreads) : "memory");
-                if (cw == 0 && lane == 0) PROF(2, 2 * batch + 1);
+                if (cw == 0 && lane == 0) DASH_PROF(2, 2 * batch + 1);
             }
         }
     }
@@ -536,15 +592,7 @@ deform_fused_kernel(const __grid_constant__ Plan P, const __grid_constant__ MlpP
     // ---- teardown: every TMEM read has completed (each consumer thread waited on its loads)
     tc_fence_before();
     __syncthreads();
-#ifdef DASH_DEFORM_PROFILE
-    if (blockIdx.x == 0 && tid == 0) {
-        printf("tiles=%u setup=%lld end=%lld\n", my_tiles, t_setup - t_entry, clock64() - t_setup);
-        printf("warp0 rounds=%lld issue_cycles=%lld wait_cycles=%lld\n", prof[0][42], prof[0][40], prof[0][41]);
-        for (int k = 0; k < 2 * (int)my_tiles && k < 64; ++k) printf("prod[%d]=%lld\n", k, prof[0][k]);
-        for (int k = 0; k < (int)(my_tiles + 1) / 2 * 2 * (int)M.n_layers && k < 64; ++k)
-            printf("mma0[%d]=%lld epi0[%d]=%lld\n", k, prof[1][k], k, prof[2][k]);
-    }
-#endif
+    DASH_PROF_REPORT(tid, my_tiles, M.n_layers);
     if (warp == kDeformEncWarps) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(M.tmem_cols)

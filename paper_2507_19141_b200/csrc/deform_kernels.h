@@ -34,6 +34,7 @@ struct MlpPlan {
     uint32_t p_off[kMlpMaxLayers];      // float offset of W_l in the packed parameter buffer (b_l follows W_l)
     uint32_t w_off[kMlpMaxLayers];      // byte offset of the bf16 operand copy of W_l in shared memory
     uint32_t a0_off;             // two A buffers of the first layer, 128 x kpad[0] bf16 each
+    uint32_t out_stage_off;      // 2 KB per consumer warp to transpose a narrow (<= 16 wide) output tile; 0 = unused
     uint32_t smem_bytes;
     uint32_t tmem_cols;          // allocated TMEM columns: power of two >= npipes * tmem_pipe_cols, >= 32
     uint32_t tmem_pipe_cols;     // per pipeline: accumulator (max npad) + bf16 A operand of layers 2..n (max kpad/2)

@@ -619,6 +619,13 @@ int fill_mlp_plan(const dash_mlp_config* m, uint64_t N, dash::MlpPlan* M) {
     const uint32_t a_lbo = dash::kDeformTileM * 16 + 16;
     M->a0_off = off;
     off += 2 * (M->kpad[0] / 8) * a_lbo;
+    // narrow last layer: the consumer warps transpose their 32 x n_out output block through shared memory
+    M->out_stage_off = 0;
+    if (M->npad[m->n_layers - 1] == 16 && off + 4 * dash::kDeformPipes * 2048u <= dash::kDeformSmemLimit) {
+        off = round_up(off, 16);
+        M->out_stage_off = off;
+        off += 4 * dash::kDeformPipes * 2048u;
+    }
     M->smem_bytes = off;
     // tensor memory per pipeline: fp32 accumulator (nmax columns) + the bf16 A operand of layers 2..n (two
     // elements per 32-bit column: kmax / 2 columns).  Two pipelines when both fit the SM's 512 columns.
