@@ -247,7 +247,11 @@ def run_ceilings(args):
         raise SystemExit("bench.py --ceilings: no CUDA device")
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
     from paper_2507_19141_b200 import ceilings
-    print(json.dumps({"ceilings": ceilings.full()}), flush=True)
+    res = ceilings.full()
+    if args.md:
+        with open(args.md, "w") as fh:
+            fh.write(ceilings.to_markdown(res, "python bench.py --ceilings --md " + args.md))
+    print(json.dumps({"ceilings": res}), flush=True)
     return 0
 
 
@@ -653,6 +657,7 @@ def main():
                          "(keys: fwd_group bwd_group smooth_group deform_path bwd_variant fwd_variant)")
     ap.add_argument("--ceilings", action="store_true",
                     help="run the microbenchmarks of include/dash_ceilings.h and print their JSON line instead")
+    ap.add_argument("--md", default=None, help="with --ceilings: also write the table as markdown to this path")
     ap.add_argument("--sweep-groups", action="store_true",
                     help="time fwd / bwd for every level-group size G (dash_hash4d_set_debug) and print a JSON line")
     args = ap.parse_args()

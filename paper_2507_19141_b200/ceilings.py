@@ -99,3 +99,34 @@ def full():
     res["tma_gather_16B_L2_2_ctas_per_sm"] = _rate(b.CEIL_TMA_GATHER, buf, sink, 16, b.CEIL_INDEPENDENT, L2_RESIDENT,
                                                    8, grid=2 * sms, block=256)
     return res
+
+
+def to_markdown(res: dict, command: str) -> str:
+    """The `full()` dict as the table `profiles/ceilings_rNN.md` holds (written by `bench.py --ceilings --md PATH`)."""
+    sms = res["sms"]
+    ghz = res.get("sm_clock_ghz", 1.965)
+    per = lambda g: g / (sms * ghz)          # lane accesses per SM per cycle at the max SM clock
+    out = [f"# Chip ceilings of the encoder's access patterns — {res['device']}, {sms} SMs", "",
+           "Command:", "", "```", command, "```", "", res["method"] + ".",
+           f"Per-SM-cycle figures assume {ghz} GHz (the max SM clock of this pool's B200s).", "",
+           f"Stream copy (1 GiB each way): **{res['copy']['GBps_read_plus_write']:.0f} GB/s** read + write.", "",
+           "| kernel / pattern | footprint | G lane accesses / s | per SM per cycle | payload GB/s | ms |",
+           "|---|---|---|---|---|---|"]
+
+    def row(name, where, v):
+        out.append(f"| {name} | {where} | {v['G_lane_ops_per_s']:.1f} | {per(v['G_lane_ops_per_s']):.2f} | "
+                   f"{v['payload_GBps']:.0f} | {v['ms']:.3f} |")
+    for sec, label in (("gather", "ld.global.nc"), ("red", "red.global.add.f32")):
+        for k, v in res[sec].items():
+            width, rest = k.split("_", 1)
+            pat, where = rest.rsplit("_", 1)
+            row(f"{label} {width} {pat}", where, v)
+    for k, v in res["red_contention_16B"].items():
+        row(f"red.v4.f32, all lanes into {k.replace('_', ' ')}", "contention", v)
+    for k, v in res["sm_count_sweep_L2"].items():
+        row(f"{k.replace('_', ' ')} (1 CTA x 1024 threads per SM)", "L2", v)
+    row("atomicAdd(float) on 32 KB of shared memory (ATOMS.CAST.SPIN loop)", "smem", res["smem_atomic_f32"])
+    row("atomicAdd(u64) on 32 KB of shared memory", "smem", res["smem_atomic_u64"])
+    row("cp.async.bulk 16 B global -> shared (TMA), 8 CTAs/SM", "L2", res["tma_gather_16B_L2"])
+    row("cp.async.bulk 16 B global -> shared (TMA), 2 CTAs/SM", "L2", res["tma_gather_16B_L2_2_ctas_per_sm"])
+    return "\n".join(out) + "\n"
