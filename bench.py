@@ -300,6 +300,59 @@ def run_group_sweep(args):
     return 0
 
 
+def run_sorted_experiment(args):
+    """VERDICT r1 item 4 / SURVEY §7 step 7, decided on kernels: the hand-written counting sort
+    (dash_hash4d_sort_queries) is timed by itself, then fwd and bwd(ZERO_GRAD) are timed on the queries in the given
+    order and in the sorted order (same kernels, `index` = the sorted order; t / dout permuted outside the timing)."""
+    import torch
+    import paper_2507_19141_b200 as dh
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --sorted-experiment: no CUDA device")
+    out_rows = {}
+    for name in args.config.split(","):
+        wl = make_workload(name)
+        enc, N = wl.spec.enc, wl.N
+        cfg = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE | dh.FLAG_ZERO_GRAD)
+        to_dev = lambda a: None if a is None else torch.from_numpy(a).cuda()
+        xyz, t, index, table, dout = (to_dev(a) for a in (wl.xyz, wl.t, wl.index, wl.table, wl.dout))
+        out = torch.empty((N, enc.L * enc.F), dtype=torch.float32, device="cuda")
+        dtable = torch.empty((enc.L, enc.T, enc.F), dtype=torch.float32, device="cuda")
+
+        def timed(fn, iters=20):
+            for _ in range(3):
+                fn()
+            a, z = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(iters):
+                fn()
+            z.record(); z.synchronize()
+            return a.elapsed_time(z) / iters
+
+        row = {"N": N,
+               "fwd_ms": timed(lambda: dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index)),
+               "bwd_ms": timed(lambda: dh.dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=index))}
+        for bits in (5, 6, 7):
+            order = torch.empty((N,), dtype=torch.int32, device="cuda")
+            ws = torch.empty(max(16, dh.binding._load().dash_hash4d_sort_workspace_bytes(N, bits)), dtype=torch.uint8,
+                             device="cuda")
+            sort_ms = timed(lambda: dh.dash_hash4d_sort_queries(xyz, index=index, bits=bits, N=N, order=order,
+                                                                workspace=ws))
+            o64 = order.long()
+            index_s = (index[o64] if index is not None else order).contiguous()
+            t_s, dout_s = t[o64].contiguous(), dout[o64].contiguous()
+            row[f"bits={bits}"] = {
+                "sort_ms": sort_ms,
+                "fwd_sorted_ms": timed(lambda: dh.dash_hash4d_fwd(cfg, xyz, t_s, table, out=out, index=index_s)),
+                "bwd_sorted_ms": timed(lambda: dh.dash_hash4d_bwd(cfg, xyz, t_s, dout_s, dtable, index=index_s)),
+            }
+            r = row[f"bits={bits}"]
+            r["step_delta_ms_if_sorted_each_step"] = (r["sort_ms"] + r["fwd_sorted_ms"] + r["bwd_sorted_ms"]
+                                                      - row["fwd_ms"] - row["bwd_ms"])
+        out_rows[name] = row
+    print(json.dumps({"sorted_experiment": out_rows}), flush=True)
+    return 0
+
+
 # ------------------------------------------------------------------------------------------ CUDA arm
 
 def run_cuda(args):
@@ -639,7 +692,10 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None, help="default 200 (cuda arm) / 10 (reference arm)")
     ap.add_argument("--warmup", type=int, default=None, help="default 20 (cuda arm) / 2 (reference arm)")
-    ap.add_argument("--config", default="C4", choices=sorted(CONFIGS))
+    ap.add_argument("--config", default="C4",
+                    help="C1..C5 (BASELINE.json configs); --sorted-experiment takes a comma-separated list")
+    ap.add_argument("--sorted-experiment", action="store_true",
+                    help="time dash_hash4d_sort_queries and fwd / bwd in the given vs the sorted order (JSON line)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference", "plumbing"],
                     help="cuda: the product; reference: the CPU oracle; plumbing: launcher/rank self-test on gloo "
                          "(no kernels, no measurement; tests/test_replicas_gloo.py)")
@@ -663,6 +719,8 @@ def main():
     args = ap.parse_args()
     if args.gpus < 1:
         ap.error("--gpus must be >= 1")
+    if not args.sorted_experiment and args.config not in CONFIGS:
+        ap.error(f"--config must be one of {sorted(CONFIGS)}")
     if args.impl in ("cuda", "plumbing") and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         return launch_replicas(args)
     if "WORLD_SIZE" in os.environ and int(os.environ["WORLD_SIZE"]) != args.gpus:
@@ -673,6 +731,8 @@ def main():
         return run_ceilings(args)
     if args.sweep_groups:
         return run_group_sweep(args)
+    if args.sorted_experiment:
+        return run_sorted_experiment(args)
     if args.steps is None:
         args.steps = 10 if args.impl == "reference" else 200
     if args.warmup is None:

@@ -232,6 +232,18 @@ DASH_API int dash_hash4d_adam_step(const dash_hash4d_config* cfg, const dash_ada
                                    float* theta, void* table16, float* dtable, float* m, float* v,
                                    void* cuda_stream);
 
+/* Optional helper: a spatial ordering of the queries (the counting sort SURVEY.md §7 step 7 asks to be decided on a
+ * kernel; measured in profiles/experiments_r02.md §5).  Key of query n = Morton code of floor(clamp(x_d) * 2^bits) over
+ * the three spatial axes of its row (row = index ? index[n] : n); `order` ([N] int32, written) receives the query
+ * numbers n sorted by non-decreasing key (ties in no particular order).  Nothing else changes: a caller that wants its
+ * queries processed in this order passes `order` (composed with its own index list) as `index` and permutes t / dout
+ * alike.  bits: 1..7.  workspace: dash_hash4d_sort_workspace_bytes(N, bits) bytes, 16-byte aligned.  Hand-written
+ * histogram + scan + scatter, five launches on `cuda_stream`; PAPER.md:111 (the dynamic subset is an index list). */
+DASH_API size_t dash_hash4d_sort_workspace_bytes(uint64_t N, uint32_t bits);
+DASH_API int dash_hash4d_sort_queries(uint64_t N, const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                      uint32_t bits, int32_t* order, void* workspace, size_t workspace_bytes,
+                                      void* cuda_stream);
+
 /* dtable <- 0 for the whole [L][T][F] fp32 gradient buffer (the accumulation's initial state), with the
  * library's own fill kernel on `cuda_stream`. */
 DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream);

@@ -26,7 +26,8 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4
            "dash_hash4d_launch_count", "dash_hash4d_set_debug", "dash_hash4d_build_id",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
            "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd",
-           "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch"]
+           "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch",
+           "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries"]
 
 
 class Hash4DError(RuntimeError):
@@ -141,6 +142,10 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_deform_slice_fwd.restype = C.c_int
     lib.dash_hash4d_launch_count.argtypes = [C.c_int]
     lib.dash_hash4d_launch_count.restype = u64
+    lib.dash_hash4d_sort_workspace_bytes.argtypes = [u64, u32]
+    lib.dash_hash4d_sort_workspace_bytes.restype = sz
+    lib.dash_hash4d_sort_queries.argtypes = [u64, vp, u32, vp, u32, vp, vp, sz, vp]
+    lib.dash_hash4d_sort_queries.restype = C.c_int
     lib.dash_ceiling_launch.argtypes = [C.POINTER(CeilingParams), vp, vp, C.POINTER(C.c_uint64), vp]
     lib.dash_ceiling_launch.restype = C.c_int
     lib.dash_hash4d_build_id.argtypes = []
@@ -392,6 +397,30 @@ def dash_hash4d_zero(cfg, dtable):
     _exactly(dtable, _table_elems(cfg), "dtable"); _one_device(dtable)
     _check(_load().dash_hash4d_zero(C.byref(cfg), _ptr(dtable), _stream()))
     return dtable
+
+
+def dash_hash4d_sort_queries(xyz, index=None, bits=6, N=None, order=None, workspace=None):
+    """-> order [N] int32: query numbers sorted by the Morton code of their coarse spatial cell (2^bits per axis)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index")
+    xs = int(xyz.shape[1])
+    if xyz.dim() != 2 or xs not in (3, 4):
+        raise ValueError("xyz must be [rows][3] or [rows][4]")
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    if index is not None:
+        _at_least(index, N, "index")
+    elif xyz.shape[0] < N:
+        raise ValueError(f"xyz has {xyz.shape[0]} rows, the call needs {N}")
+    if order is None:
+        order = torch.empty((N,), dtype=torch.int32, device=xyz.device)
+    _dev(order, torch.int32, "order"); _at_least(order, N, "order")
+    need = int(_load().dash_hash4d_sort_workspace_bytes(N, int(bits)))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=xyz.device)
+    _one_device(xyz, index, order, workspace)
+    _check(_load().dash_hash4d_sort_queries(N, _ptr(xyz), xs, _ptr(index), int(bits), _ptr(order), _ptr(workspace),
+                                            workspace.numel(), _stream()))
+    return order
 
 
 # ---- G_3D (PAPER.md:97-101, Eq. 3): the same encoder with d = 3; temporal config fields ignored -------

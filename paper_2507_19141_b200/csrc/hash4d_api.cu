@@ -552,6 +552,38 @@ DASH_API int dash_hash4d_adam_step(const dash_hash4d_config* cfg, const dash_ada
     return ok();
 }
 
+static size_t round16(size_t v) { return (v + 15u) & ~static_cast<size_t>(15u); }
+
+DASH_API size_t dash_hash4d_sort_workspace_bytes(uint64_t N, uint32_t bits) {
+    if (bits < 1 || bits > 7) return 0;
+    const size_t n_bins = static_cast<size_t>(1) << (3 * bits);
+    return round16(N * 4) + round16(n_bins * 4) + round16((n_bins + 1023) / 1024 * 4);
+}
+
+DASH_API int dash_hash4d_sort_queries(uint64_t N, const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                      uint32_t bits, int32_t* order, void* workspace, size_t workspace_bytes,
+                                      void* cuda_stream) {
+    if (bits < 1 || bits > 7) return fail(DASH_HASH4D_INVALID_ARG, "bits = %u outside 1..7", bits);
+    if (N == 0) return ok();
+    if (N > 0x7fffffffull) return fail(DASH_HASH4D_UNSUPPORTED, "N too large for an int32 order list");
+    if (!xyz || !order) return fail(DASH_HASH4D_INVALID_ARG, "xyz or order is NULL");
+    if (!(xyz_stride == 3 || xyz_stride == 4))
+        return fail(DASH_HASH4D_INVALID_ARG, "xyz_stride = %u (want 3 or 4)", xyz_stride);
+    const size_t need = dash_hash4d_sort_workspace_bytes(N, bits);
+    if (!workspace || workspace_bytes < need)
+        return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "sort needs %zu workspace bytes, got %zu", need, workspace_bytes);
+    if (!aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
+    const size_t n_bins = static_cast<size_t>(1) << (3 * bits);
+    char* w = static_cast<char*>(workspace);
+    uint32_t* keys = reinterpret_cast<uint32_t*>(w);
+    uint32_t* bins = reinterpret_cast<uint32_t*>(w + round16(N * 4));
+    uint32_t* totals = reinterpret_cast<uint32_t*>(w + round16(N * 4) + round16(n_bins * 4));
+    cudaError_t e = dash::launch_sort_queries(N, xyz, xyz_stride, index, bits, order, keys, bins, totals,
+                                              static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "sort launch");
+    return ok();
+}
+
 DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream) {
     if (int rc = check_config(cfg, 3)) return rc;  // only L, T, F matter here (serves G_3D tables too)
     if (!dtable) return fail(DASH_HASH4D_INVALID_ARG, "dtable is NULL");

@@ -599,6 +599,116 @@ slice_t_kernel(const __grid_constant__ Plan P, const float* __restrict__ t,
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Spatial counting sort of the queries (dash_hash4d_sort_queries): key = Morton code of the coarse cell.
+// keys + histogram -> 3-launch exclusive scan over the bins (1024 bins per CTA) -> scatter through per-bin cursors.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t spread3(uint32_t v) {   // 7 bits -> every third bit
+    v &= 0x7fu;
+    v = (v | (v << 8)) & 0x0000700fu;
+    v = (v | (v << 4)) & 0x000430c3u;
+    v = (v | (v << 2)) & 0x00049249u;
+    return v;
+}
+
+__global__ void __launch_bounds__(kBlockThreads)
+sort_keys_kernel(uint64_t N, const float* __restrict__ xyz, uint32_t xyz_stride,
+                 const int32_t* __restrict__ index, float scale, uint32_t cell_max,
+                 uint32_t* __restrict__ keys, uint32_t* __restrict__ hist) {
+    const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
+    for (uint64_t n = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x; n < N; n += stride) {
+        const uint64_t row = index ? static_cast<uint64_t>(__ldg(index + n)) : n;
+        const float* p = xyz + row * xyz_stride;
+        uint32_t key = 0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const uint32_t c = min(static_cast<uint32_t>(clamp_unit(__ldg(p + d)) * scale), cell_max);
+            key |= spread3(c) << d;
+        }
+        keys[n] = key;
+        atomicAdd(hist + key, 1u);
+    }
+}
+
+// exclusive scan, phase 1: each CTA scans 1024 bins in place and writes its total
+__global__ void __launch_bounds__(1024) sort_scan_local_kernel(uint32_t* __restrict__ bins, uint32_t n_bins,
+                                                               uint32_t* __restrict__ totals) {
+    __shared__ uint32_t warp_sum[32];
+    const uint32_t i = blockIdx.x * 1024u + threadIdx.x, lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    const uint32_t v = i < n_bins ? bins[i] : 0u;
+    uint32_t x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= static_cast<uint32_t>(o)) x += y;
+    }
+    if (lane == 31) warp_sum[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t s = warp_sum[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= static_cast<uint32_t>(o)) s += y;
+        }
+        warp_sum[lane] = s;   // inclusive over warps
+    }
+    __syncthreads();
+    const uint32_t before = w ? warp_sum[w - 1] : 0u;
+    if (i < n_bins) bins[i] = before + x - v;   // exclusive within the CTA
+    if (threadIdx.x == 1023) totals[blockIdx.x] = before + x;
+}
+
+// phase 2: one CTA turns the (<= 2048) CTA totals into exclusive offsets
+__global__ void __launch_bounds__(1024) sort_scan_totals_kernel(uint32_t* __restrict__ totals, uint32_t n) {
+    __shared__ uint32_t warp_sum[32];
+    __shared__ uint32_t carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (uint32_t base = 0; base < n; base += 1024u) {
+        const uint32_t i = base + threadIdx.x, lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+        const uint32_t v = i < n ? totals[i] : 0u;
+        uint32_t x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= static_cast<uint32_t>(o)) x += y;
+        }
+        if (lane == 31) warp_sum[w] = x;
+        __syncthreads();
+        if (w == 0) {
+            uint32_t s = warp_sum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
+                if (lane >= static_cast<uint32_t>(o)) s += y;
+            }
+            warp_sum[lane] = s;
+        }
+        __syncthreads();
+        const uint32_t before = carry + (w ? warp_sum[w - 1] : 0u);
+        if (i < n) totals[i] = before + x - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = before + x;
+        __syncthreads();
+    }
+}
+
+// phase 3: add the CTA offsets
+__global__ void __launch_bounds__(1024) sort_scan_add_kernel(uint32_t* __restrict__ bins, uint32_t n_bins,
+                                                             const uint32_t* __restrict__ totals) {
+    const uint32_t i = blockIdx.x * 1024u + threadIdx.x;
+    if (i < n_bins) bins[i] += totals[blockIdx.x];
+}
+
+__global__ void __launch_bounds__(kBlockThreads)
+sort_scatter_kernel(uint64_t N, const uint32_t* __restrict__ keys, uint32_t* __restrict__ cursor,
+                    int32_t* __restrict__ order) {
+    const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
+    for (uint64_t n = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x; n < N; n += stride)
+        order[atomicAdd(cursor + keys[n], 1u)] = static_cast<int32_t>(n);
+}
+
 // SM count / L2 bytes of the CURRENT device, cached per device ordinal (a process may drive several GPUs).
 struct DeviceInfo {
     int sms;
@@ -823,6 +933,28 @@ cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t co
     const size_t cap = static_cast<size_t>(sm_count()) * 16;
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
     fixed_finalize_kernel<<<blocks, kBlockThreads, 0, s>>>(acc, dtable, count, hdr, overwrite ? 1 : 0);
+    return after_launch();
+}
+
+cudaError_t launch_sort_queries(uint64_t N, const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                uint32_t bits, int32_t* order, uint32_t* keys, uint32_t* bins, uint32_t* totals,
+                                cudaStream_t s) {
+    const uint32_t n_bins = 1u << (3u * bits), scan_ctas = (n_bins + 1023u) / 1024u;
+    const size_t want = (N + kBlockThreads - 1) / kBlockThreads;
+    const size_t cap = static_cast<size_t>(sm_count()) * 16;
+    const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
+    cudaError_t e = launch_zero(bins, static_cast<size_t>(n_bins) * sizeof(uint32_t), s);
+    if (e != cudaSuccess) return e;
+    sort_keys_kernel<<<blocks, kBlockThreads, 0, s>>>(N, xyz, xyz_stride, index, static_cast<float>(1u << bits),
+                                                      (1u << bits) - 1u, keys, bins);
+    if ((e = after_launch()) != cudaSuccess) return e;
+    sort_scan_local_kernel<<<scan_ctas, 1024, 0, s>>>(bins, n_bins, totals);
+    if ((e = after_launch()) != cudaSuccess) return e;
+    sort_scan_totals_kernel<<<1, 1024, 0, s>>>(totals, scan_ctas);
+    if ((e = after_launch()) != cudaSuccess) return e;
+    sort_scan_add_kernel<<<scan_ctas, 1024, 0, s>>>(bins, n_bins, totals);
+    if ((e = after_launch()) != cudaSuccess) return e;
+    sort_scatter_kernel<<<blocks, kBlockThreads, 0, s>>>(N, keys, bins, order);
     return after_launch();
 }
 

@@ -39,6 +39,9 @@ cudaError_t launch_absmax(const float* v, size_t count, WorkspaceHeader* hdr, ui
                           cudaStream_t s);
 cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t count,
                                   const WorkspaceHeader* hdr, bool overwrite, cudaStream_t s);
+cudaError_t launch_sort_queries(uint64_t N, const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                uint32_t bits, int32_t* order, uint32_t* keys, uint32_t* bins, uint32_t* totals,
+                                cudaStream_t s);
 cudaError_t launch_slice_t(const Plan& P, const float* t, const void* table, bool table_half, float* slice,
                            cudaStream_t s);
 cudaError_t launch_adam(size_t count, double lr, double beta1, double beta2, double eps, uint32_t step,

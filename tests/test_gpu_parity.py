@@ -680,3 +680,36 @@ def test_zero_grad_through_the_raw_abi_without_workspace():
     torch.cuda.synchronize()
     assert rc == 0
     check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 6, what="zero-grad, no workspace")
+
+
+@pytest.mark.parametrize("bits", [1, 4, 6, 7])
+@pytest.mark.parametrize("with_index", [False, True])
+def test_sort_queries_is_a_permutation_in_key_order(bits, with_index):
+    """dash_hash4d_sort_queries: `order` is a permutation of 0..N-1 and the Morton keys of the coarse spatial cells
+    (rebuilt here with numpy: one exact power-of-two fp32 product, floor, bit interleave) are non-decreasing along it.
+    Ties may come in any order, so only what is unique is compared."""
+    rng = np.random.default_rng(bits)
+    rows = 5000
+    xyz = rng.random((rows, 3), dtype=np.float32)
+    xyz[:5] = [[0, 0, 0], [1, 1, 1], [np.nan, 0.5, -3], [np.float32(1) - np.float32(2.0 ** -24)] * 3, [0.5, 0.25, 0.75]]
+    index = rng.integers(0, rows, 7001).astype(np.int32) if with_index else None
+    order = dh.dash_hash4d_sort_queries(dev(xyz), index=dev(index), bits=bits).cpu().numpy()
+    n = len(index) if with_index else rows
+    assert order.shape == (n,) and np.array_equal(np.sort(order), np.arange(n))
+    pts = xyz[index] if with_index else xyz
+    c = np.clip(np.nan_to_num(pts, nan=0.0), 0, np.float32(1) - np.float32(2.0 ** -24)).astype(np.float32)
+    cell = np.minimum((c * np.float32(2 ** bits)).astype(np.uint32), 2 ** bits - 1)
+    key = np.zeros(n, np.uint64)
+    for b in range(bits):
+        for d in range(3):
+            key |= ((cell[:, d].astype(np.uint64) >> b) & 1) << (3 * b + d)
+    assert (np.diff(key[order].astype(np.int64)) >= 0).all()
+    # the sorted order is a valid index list: the forward in that order is the forward, permuted
+    enc = EncoderParams(4, 2, 1 << 10, 8, 64, 4, 16)
+    cfg = dh.config_from_params(enc)
+    t = rng.random(n, dtype=np.float32)
+    table = dev(rng.uniform(-1, 1, (4, 1 << 10, 2)).astype(np.float32))
+    base = dh.dash_hash4d_fwd(cfg, dev(xyz), dev(t), table, index=dev(index)).cpu().numpy()
+    idx_s = (index[order] if with_index else order.astype(np.int32))
+    got = dh.dash_hash4d_fwd(cfg, dev(xyz), dev(t[order]), table, index=dev(idx_s)).cpu().numpy()
+    np.testing.assert_array_equal(got, base[order])
