@@ -90,11 +90,16 @@ DASH_API int dash_hash4d_slice_fwd(const dash_hash4d_config* cfg, uint64_t N,
                                    const float* xyz, uint32_t xyz_stride, const int32_t* index,
                                    const float* slice, float* out, void* cuda_stream);
 
-/* dash_deform_fwd on a slice: out[n] = base[n] + MLP(G_4D(xyz_n, t)), the fused kernel with 8-corner gathers. */
+/* dash_deform_fwd on a slice: out[n] = base[n] + MLP(G_4D(xyz_n, t)).  The fused kernel with 8-corner gathers when
+ * the fp32 slice (L*T*F*4 bytes) stays L2-resident; otherwise, like dash_deform_fwd, two passes (level-grouped
+ * dash_hash4d_slice_fwd into the workspace, then the MLP kernel).  dash_deform_slice_workspace_bytes gives the bytes
+ * that second case needs (0 when the fused kernel applies); workspace 16-byte aligned, nullable when 0. */
+DASH_API size_t dash_deform_slice_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp,
+                                                  uint64_t N);
 DASH_API int dash_deform_slice_fwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
                                    const float* xyz, uint32_t xyz_stride, const int32_t* index,
                                    const float* slice, const float* params, const float* base,
-                                   float* out, void* cuda_stream);
+                                   float* out, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 #ifdef __cplusplus
 }

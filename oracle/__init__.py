@@ -279,6 +279,24 @@ def oracle_mlp(mcfg: OracleMlpConfig, feat, params, base=None, want_abs=False):
     return (out, mag) if want_abs else out
 
 
+def oracle_mlp_bwd(mcfg: OracleMlpConfig, feat, params, dout, want_dfeat=True, want_abs=False):
+    """Backward of oracle_mlp by the chain rule (forward recomputed): -> (dfeat [N][width_0] fp32 or None,
+    dparams [P] float64, packed like params[, dfeat_abs, dparams_abs, margin])."""
+    widths = list(mcfg.width)[:mcfg.n_layers + 1]
+    assert feat.dtype == np.float32 and feat.flags.c_contiguous and feat.ndim == 2 and feat.shape[1] == widths[0]
+    assert params.dtype == np.float32 and params.flags.c_contiguous and params.size == mlp_param_count(widths)
+    N = feat.shape[0]
+    assert dout.dtype == np.float32 and dout.flags.c_contiguous and dout.shape == (N, widths[-1])
+    dfeat = np.zeros((N, widths[0]), np.float32) if want_dfeat else None
+    dparams = np.zeros(params.size, np.float64)
+    fa = np.zeros((N, widths[0]), np.float64) if want_abs else None
+    pa = np.zeros(params.size, np.float64) if want_abs else None
+    mg = np.zeros(N, np.float64) if want_abs else None
+    _check(lib().dash_oracle_mlp_bwd(C.byref(mcfg), C.c_uint64(N), _p(feat), _p(params), _p(dout), _p(dfeat),
+                                     _p(dparams), _p(fa), _p(pa), _p(mg)), "mlp_bwd")
+    return (dfeat, dparams, fa, pa, mg) if want_abs else (dfeat, dparams)
+
+
 def oracle_deform(cfg, mcfg, N, xyz, t, table, params, base=None, index=None, t_stride=1, want_abs=False):
     """Eq. 9-10: out = base + MLP(G_4D(x)); the features are the fp32 outputs of oracle_fwd."""
     feat = oracle_fwd(cfg, N, xyz, t, table, index=index, t_stride=t_stride)

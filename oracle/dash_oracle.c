@@ -769,6 +769,127 @@ int dash_oracle_mlp(const dash_oracle_mlp_config *m, uint64_t N, const float *in
     return failed ? ORACLE_NOMEM : ORACLE_OK;
 }
 
+/* ---- beyond §8f (DESIGN.md §9 "missing CUDA work" item 1): backward through phi_d and the heads ----------------
+ * The chain of dash_oracle_mlp is differentiated by the chain rule (the paper trains phi_d and the heads by gradient
+ * descent on the losses of PAPER.md:146-156; it gives no formulas, the ones below are the textbook ones):
+ *     delta_n = dout;   for l = n .. 1:   dW_l += delta_l a_{l-1}^T,   db_l += delta_l,
+ *     g_{l-1} = W_l^T delta_l,   delta_{l-1} = g_{l-1} * [z_{l-1} > 0]   (relu'(0) = 0),   dfeat = g_0.
+ * The forward activations are recomputed here exactly as dash_oracle_mlp computes them (nothing is saved).
+ * Arithmetic: double.  flags bit0 (QUANT_BF16): the operands of every product — W, a_{l-1} and delta_l — are first
+ * rounded to bfloat16, which is what the CUDA path feeds its tensor cores with (Q30).
+ *   dfeat        [N][width_0] fp32 (nullable), rounded once.
+ *   dparams      [param_count] double, OVERWRITTEN with the sums over all N rows, packed like params.
+ *   dfeat_abs    (nullable, [N][width_0] double): |W_1|^T ( ... |W_n|^T |dout| ) with the same relu masks.
+ *   dparams_abs  (nullable, [param_count] double): sum over rows of Delta_l[j] |a_{l-1}[k]| (and of Delta_l[j]), Delta
+ *                the bound |W|^T ... |dout| of dfeat_abs one layer up: delta_l carries the rounding of everything
+ *                above it, so ITS conditioning, not |delta_l|, scales the error of dW_l.
+ *   margin       (nullable, [N] double): min over the hidden units of |z| / (|b| + sum |w x|): how far the row is from
+ *                a relu kink, relative to the rounding scale of z.  The mask is a DECISION taken from a floating-point
+ *                value; rows closer to a kink than the arithmetic's accuracy have no unique gradient. */
+int dash_oracle_mlp_bwd(const dash_oracle_mlp_config *m, uint64_t N, const float *in, const float *params,
+                        const float *dout, float *dfeat, double *dparams, double *dfeat_abs,
+                        double *dparams_abs, double *margin) {
+    if (!m || m->struct_size != sizeof(*m) || m->n_layers < 1 || m->n_layers > 4) return ORACLE_INVALID;
+    for (uint32_t l = 0; l <= m->n_layers; ++l)
+        if (m->width[l] < 1 || m->width[l] > 4096) return ORACLE_INVALID;
+    if (!dparams) return ORACLE_INVALID;
+    const uint32_t n_layers = m->n_layers;
+    size_t P = 0, p_off[5] = {0, 0, 0, 0, 0};
+    uint32_t wmax = 0;
+    for (uint32_t l = 1; l <= n_layers; ++l) {
+        p_off[l] = P;
+        P += (size_t)m->width[l] * m->width[l - 1] + m->width[l];
+    }
+    for (uint32_t l = 0; l <= n_layers; ++l)
+        if (m->width[l] > wmax) wmax = m->width[l];
+    for (size_t i = 0; i < P; ++i) {
+        dparams[i] = 0.0;
+        if (dparams_abs) dparams_abs[i] = 0.0;
+    }
+    if (N == 0) return ORACLE_OK;
+    if (!in || !params || !dout) return ORACLE_INVALID;
+    const int quant = (m->flags & 1u) != 0;
+    /* one row at a time, in order: obviously correct, deterministic sums */
+    double *a = (double *)malloc(sizeof(double) * wmax * (n_layers + 1) * 2 + sizeof(double) * wmax * 4);
+    if (!a) return ORACLE_NOMEM;
+    double *mask = a + (size_t)wmax * (n_layers + 1);        /* [l][k]: 1 if z_l[k] > 0 (hidden layers) */
+    double *delta = mask + (size_t)wmax * (n_layers + 1), *Delta = delta + wmax, *g = Delta + wmax, *G = g + wmax;
+    for (uint64_t n = 0; n < N; ++n) {
+        double worst = INFINITY;
+        for (uint32_t k = 0; k < m->width[0]; ++k) a[k] = (double)in[(size_t)n * m->width[0] + k];
+        for (uint32_t l = 1; l <= n_layers; ++l) { /* forward, as dash_oracle_mlp */
+            const uint32_t K = m->width[l - 1], J = m->width[l];
+            const float *W = params + p_off[l], *b = W + (size_t)J * K;
+            const double *x = a + (size_t)(l - 1) * wmax;
+            double *y = a + (size_t)l * wmax, *mk = mask + (size_t)l * wmax;
+            for (uint32_t j = 0; j < J; ++j) {
+                double s = (double)b[j], S = fabs((double)b[j]);
+                for (uint32_t k = 0; k < K; ++k) {
+                    double w = (double)W[(size_t)j * K + k], xv = x[k];
+                    if (quant) {
+                        w = to_bf16(w);
+                        xv = to_bf16(xv);
+                    }
+                    s += w * xv;
+                    S += fabs(w * xv);
+                }
+                if (l < n_layers) {
+                    mk[j] = s > 0.0 ? 1.0 : 0.0;
+                    y[j] = s > 0.0 ? s : 0.0;
+                    double rel = S > 0.0 ? fabs(s) / S : INFINITY;
+                    if (rel < worst) worst = rel;
+                } else {
+                    y[j] = s;
+                }
+            }
+        }
+        if (margin) margin[n] = worst;
+        const uint32_t n_out = m->width[n_layers];
+        for (uint32_t j = 0; j < n_out; ++j) {
+            delta[j] = (double)dout[(size_t)n * n_out + j];
+            Delta[j] = fabs(delta[j]);
+        }
+        for (uint32_t l = n_layers; l >= 1; --l) { /* backward */
+            const uint32_t K = m->width[l - 1], J = m->width[l];
+            const float *W = params + p_off[l];
+            double *dW = dparams + p_off[l], *db = dW + (size_t)J * K;
+            double *dWa = dparams_abs ? dparams_abs + p_off[l] : NULL, *dba = dWa ? dWa + (size_t)J * K : NULL;
+            const double *x = a + (size_t)(l - 1) * wmax;
+            for (uint32_t k = 0; k < K; ++k) g[k] = G[k] = 0.0;
+            for (uint32_t j = 0; j < J; ++j) {
+                const double d = quant ? to_bf16(delta[j]) : delta[j];
+                db[j] += d;
+                if (dba) dba[j] += Delta[j];
+                for (uint32_t k = 0; k < K; ++k) {
+                    double w = (double)W[(size_t)j * K + k], xv = x[k];
+                    if (quant) {
+                        w = to_bf16(w);
+                        xv = to_bf16(xv);
+                    }
+                    dW[(size_t)j * K + k] += d * xv;
+                    if (dWa) dWa[(size_t)j * K + k] += Delta[j] * fabs(xv);
+                    g[k] += w * d;
+                    G[k] += fabs(w) * Delta[j];
+                }
+            }
+            if (l > 1) {
+                const double *mk = mask + (size_t)(l - 1) * wmax;
+                for (uint32_t k = 0; k < K; ++k) {
+                    delta[k] = g[k] * mk[k];
+                    Delta[k] = G[k] * mk[k];
+                }
+            } else {
+                for (uint32_t k = 0; k < K; ++k) {
+                    if (dfeat) dfeat[(size_t)n * K + k] = (float)g[k];
+                    if (dfeat_abs) dfeat_abs[(size_t)n * K + k] = G[k];
+                }
+            }
+        }
+    }
+    free(a);
+    return ORACLE_OK;
+}
+
 /* ---- NEXT #4: sparse optimiser step over the touched table entries -------------------
  * The paper does not name its optimiser ("primarily based on the PyTorch framework"; 3DGS [14]
  * and Instant-NGP [25], which it follows, both train with Adam).  Reading (Q28): Adam (Kingma & Ba),

@@ -27,7 +27,7 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
            "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd",
            "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch",
-           "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries"]
+           "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_deform_slice_workspace_bytes"]
 
 
 class Hash4DError(RuntimeError):
@@ -138,7 +138,9 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_hash4d_slice_t.restype = C.c_int
     lib.dash_hash4d_slice_fwd.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp]
     lib.dash_hash4d_slice_fwd.restype = C.c_int
-    lib.dash_deform_slice_fwd.argtypes = [cfgp, mlpp, u64, vp, u32, vp, vp, vp, vp, vp, vp]
+    lib.dash_deform_slice_fwd.argtypes = [cfgp, mlpp, u64, vp, u32, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.dash_deform_slice_workspace_bytes.argtypes = [cfgp, mlpp, u64]
+    lib.dash_deform_slice_workspace_bytes.restype = sz
     lib.dash_deform_slice_fwd.restype = C.c_int
     lib.dash_hash4d_launch_count.argtypes = [C.c_int]
     lib.dash_hash4d_launch_count.restype = u64
@@ -601,7 +603,11 @@ def dash_hash4d_slice_fwd(cfg, xyz, slice_t, out=None, index=None, N=None):
     return out
 
 
-def dash_deform_slice_fwd(cfg, mlp, xyz, slice_t, params, base=None, out=None, index=None, N=None):
+def dash_deform_slice_workspace_bytes(cfg, mlp, N: int) -> int:
+    return int(_load().dash_deform_slice_workspace_bytes(C.byref(cfg), C.byref(mlp), N))
+
+
+def dash_deform_slice_fwd(cfg, mlp, xyz, slice_t, params, base=None, out=None, index=None, N=None, workspace=None):
     """out[n] = base[n] + MLP(G_4D(xyz_n, t)) from a slice, fused kernel with 8-corner gathers."""
     _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index"); _dev(slice_t, torch.float32, "slice")
     _dev(params, torch.float32, "params"); _dev(base, torch.float32, "base")
@@ -615,9 +621,13 @@ def dash_deform_slice_fwd(cfg, mlp, xyz, slice_t, params, base=None, out=None, i
     _check_queries(cfg, xyz, None, index, 0, N)
     _exactly(slice_t, _table_elems(cfg), "slice"); _exactly(params, dash_mlp_param_count(mlp), "params")
     _at_least(base, N * n_out, "base"); _at_least(out, N * n_out, "out")
-    _one_device(xyz, index, slice_t, params, base, out)
+    _one_device(xyz, index, slice_t, params, base, out, workspace)
+    need = dash_deform_slice_workspace_bytes(cfg, mlp, N)
+    if need and workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=xyz.device)
+    wbytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     _check(_load().dash_deform_slice_fwd(C.byref(cfg), C.byref(mlp), N, _ptr(xyz), xs, _ptr(index), _ptr(slice_t),
-                                         _ptr(params), _ptr(base), _ptr(out), _stream()))
+                                         _ptr(params), _ptr(base), _ptr(out), _ptr(workspace), wbytes, _stream()))
     return out
 
 

@@ -681,10 +681,10 @@ size_t mlp_params(const dash_mlp_config* m) {
     return p;
 }
 
-// the fused kernel walks all L levels per tile: the whole table must stay L2-resident
-bool deform_fused_applies(const dash_hash4d_config* enc) {
+// the fused kernel walks all L levels per tile: the whole table (or fp32 time slice) must stay L2-resident
+bool deform_fused_applies(const dash_hash4d_config* enc, bool slice = false) {
     if (const uint32_t forced = debug_u32(DASH_DEBUG_DEFORM_PATH)) return forced == 1;  // 1 fused, 2 two-pass
-    const size_t elem = enc->table_dtype == DASH_HASH4D_FP16 ? 2 : 4;
+    const size_t elem = (!slice && enc->table_dtype == DASH_HASH4D_FP16) ? 2 : 4;
     const size_t table_bytes = static_cast<size_t>(enc->L) * enc->T * enc->F * elem;
     return table_bytes <= l2_bytes() / 100 * 55;
 }
@@ -835,10 +835,18 @@ DASH_API int dash_hash4d_slice_fwd(const dash_hash4d_config* cfg, uint64_t N, co
     return ok();
 }
 
+DASH_API size_t dash_deform_slice_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp,
+                                                  uint64_t N) {
+    if (check_sliceable(enc) || check_mlp(mlp)) return 0;
+    g_error[0] = '\0';
+    if (deform_fused_applies(enc, true)) return 0;
+    return static_cast<size_t>(N) * enc->L * enc->F * sizeof(float);
+}
+
 DASH_API int dash_deform_slice_fwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
                                    const float* xyz, uint32_t xyz_stride, const int32_t* index,
                                    const float* slice, const float* params, const float* base, float* out,
-                                   void* cuda_stream) {
+                                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
     if (int rc = check_sliceable(enc)) return rc;
     if (int rc = check_mlp(mlp)) return rc;
     if (mlp->width[0] != enc->L * enc->F)
@@ -852,6 +860,19 @@ DASH_API int dash_deform_slice_fwd(const dash_hash4d_config* enc, const dash_mlp
     if ((reinterpret_cast<uintptr_t>(params) | reinterpret_cast<uintptr_t>(base) |
          reinterpret_cast<uintptr_t>(out)) & 3u)
         return fail(DASH_HASH4D_INVALID_ARG, "params / base / out not 4-byte aligned");
+    if (!deform_fused_applies(enc, true)) {   // slice beyond L2: level-grouped 8-corner lookups, then the MLP kernel
+        const size_t need = static_cast<size_t>(N) * enc->L * enc->F * sizeof(float);
+        if (!workspace || workspace_bytes < need)
+            return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL,
+                        "deform_slice_fwd (two-pass) needs %zu workspace bytes, got %zu", need, workspace_bytes);
+        if (!aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
+        float* feat = static_cast<float*>(workspace);
+        if (int rc = dash_hash4d_slice_fwd(enc, N, xyz, xyz_stride, index, slice, feat, cuda_stream)) return rc;
+        cudaError_t e2 = dash::launch_mlp(M, feat, params, base, out, dash::device_sm_count(),
+                                          static_cast<cudaStream_t>(cuda_stream));
+        if (e2 != cudaSuccess) return cuda_fail(e2, "mlp launch");
+        return ok();
+    }
     Plan P;
     if (int rc = fill_slice_plan(enc, N, xyz_stride, 1, &P)) return rc;
     cudaError_t e = dash::launch_deform_fused(P, M, xyz, nullptr, index, slice, false, params, base, out,

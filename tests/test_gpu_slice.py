@@ -70,8 +70,10 @@ def test_slice_full_size_c3_and_index_list():
     torch.testing.assert_close(out_i, out[torch.from_numpy(index).long().cuda()], rtol=0, atol=0)
 
 
+@pytest.mark.parametrize("path", [0, 2])       # 0: the library decides (fused here); 2: two-pass, as for a slice beyond L2
 @pytest.mark.parametrize("name,widths_tail", [("C2", [64, 64, 10]), ("C2", [128, 10])])
-def test_deform_slice_fwd_parity(name, widths_tail):
+def test_deform_slice_fwd_parity(name, widths_tail, path, set_debug):
+    set_debug(dh.DEBUG_DEFORM_PATH, path)
     wl = make_workload(name, n_override=30_000, with_dout=False)
     enc, N = wl.spec.enc, wl.N
     widths = [enc.L * enc.F] + widths_tail
@@ -82,6 +84,8 @@ def test_deform_slice_fwd_parity(name, widths_tail):
     t = np.array([0.6180339], np.float32)
     m = dh.make_mlp_config(widths)
     sl = dh.dash_hash4d_slice_t(gcfg, dev(t), dev(table))
+    need = dh.dash_deform_slice_workspace_bytes(gcfg, m, N)
+    assert (need == 0) == (path == 0) and (path == 0 or need == N * enc.L * enc.F * 4)
     out = dh.dash_deform_slice_fwd(gcfg, m, dev(wl.xyz), sl, dev(params), base=dev(base))
     torch.cuda.synchronize()
     feat = oracle.oracle_fwd(ocfg, N, wl.xyz, t, table, t_stride=0)
