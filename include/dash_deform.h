@@ -51,6 +51,22 @@ DASH_API int dash_mlp_fwd(const dash_mlp_config* mlp, uint64_t N,
                           const float* feat, const float* params, const float* base,
                           float* out, void* cuda_stream);
 
+/* Backward of dash_mlp_fwd by the chain rule (the paper trains phi_d and the heads by gradient descent on the losses
+ * of PAPER.md:146-156 and gives no formulas; Q30).  With delta_n = dout, for l = n .. 1:
+ *     dW_l += delta_l^T a_{l-1},   db_l += sum over rows of delta_l,
+ *     g_{l-1} = delta_l W_l,   delta_{l-1} = g_{l-1} * [a_{l-1} > 0]  (relu'(0) = 0),   dfeat = g_0.
+ * The forward activations are recomputed from `feat` (dash_mlp_fwd saves nothing).  Like the forward, the products run
+ * on the tensor cores with bf16 operands (W, a_{l-1}, delta_l rounded to nearest even) and fp32 accumulation.
+ *   feat     [N][width[0]] fp32.     params   packed fp32 parameters.     dout   [N][width[n_layers]] fp32 = dL/d out
+ *            (dL/d base is dout itself).
+ *   dfeat    nullable, [N][width[0]] fp32, 16-byte aligned, written: dL/d feat — the `dout` of dash_hash4d_bwd /
+ *            dash_hash4d_bwd_input when feat = G_4D(x).
+ *   dparams  [dash_mlp_param_count] fp32, packed like params, ACCUMULATED into (+=): the caller zeroes it.
+ * UNSUPPORTED when a width exceeds 240, or the tiles / accumulators of the chain exceed 227 KB of shared memory or
+ * the 512 tensor-memory columns of an SM (accumulator + one kpad-wide weight-gradient block per layer). */
+DASH_API int dash_mlp_bwd(const dash_mlp_config* mlp, uint64_t N, const float* feat, const float* params,
+                          const float* dout, float* dfeat, float* dparams, void* cuda_stream);
+
 /* Device workspace dash_deform_fwd needs: 0 when the fused kernel applies (the table fits L2 as one level
  * group), else N * L*F * 4 bytes for the feature matrix of the two-pass path. */
 DASH_API size_t dash_deform_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp,

@@ -25,7 +25,7 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count", "dash_hash4d_set_debug", "dash_hash4d_build_id",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
-           "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_deform_workspace_bytes", "dash_deform_fwd",
+           "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_mlp_bwd", "dash_deform_workspace_bytes", "dash_deform_fwd",
            "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch",
            "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_deform_slice_workspace_bytes"]
 
@@ -130,6 +130,8 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_mlp_param_count.restype = sz
     lib.dash_mlp_fwd.argtypes = [mlpp, u64, vp, vp, vp, vp, vp]
     lib.dash_mlp_fwd.restype = C.c_int
+    lib.dash_mlp_bwd.argtypes = [mlpp, u64, vp, vp, vp, vp, vp, vp]
+    lib.dash_mlp_bwd.restype = C.c_int
     lib.dash_deform_workspace_bytes.argtypes = [cfgp, mlpp, u64]
     lib.dash_deform_workspace_bytes.restype = sz
     lib.dash_deform_fwd.argtypes = [cfgp, mlpp, u64, vp, u32, vp, u32, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -538,6 +540,22 @@ def dash_mlp_fwd(mlp, feat, params, base=None, out=None):
     _at_least(base, N * n_out, "base"); _at_least(out, N * n_out, "out"); _one_device(feat, params, base, out)
     _check(_load().dash_mlp_fwd(C.byref(mlp), N, _ptr(feat), _ptr(params), _ptr(base), _ptr(out), _stream()))
     return out
+
+
+def dash_mlp_bwd(mlp, feat, params, dout, dparams, dfeat=None, want_dfeat=True):
+    """Backward of dash_mlp_fwd: dparams += dL/d params (packed like params); returns (dfeat or None, dparams)."""
+    for name, a in (("feat", feat), ("params", params), ("dout", dout), ("dparams", dparams), ("dfeat", dfeat)):
+        _dev(a, torch.float32, name)
+    N = int(feat.shape[0])
+    n_out = int(mlp.width[mlp.n_layers])
+    if want_dfeat and dfeat is None:
+        dfeat = torch.empty((N, int(mlp.width[0])), dtype=torch.float32, device=feat.device)
+    _exactly(feat, N * int(mlp.width[0]), "feat"); _exactly(params, dash_mlp_param_count(mlp), "params")
+    _exactly(dparams, dash_mlp_param_count(mlp), "dparams"); _at_least(dout, N * n_out, "dout")
+    _at_least(dfeat, N * int(mlp.width[0]), "dfeat"); _one_device(feat, params, dout, dparams, dfeat)
+    _check(_load().dash_mlp_bwd(C.byref(mlp), N, _ptr(feat), _ptr(params), _ptr(dout), _ptr(dfeat), _ptr(dparams),
+                                _stream()))
+    return dfeat, dparams
 
 
 def dash_deform_workspace_bytes(cfg, mlp, N: int) -> int:

@@ -43,6 +43,28 @@ struct MlpPlan {
     uint32_t n_out;              // width[n_layers]
 };
 
+// Backward through the chain (mlp_bwd_kernels.cu): shared-memory / tensor-memory map of one CTA.  The forward is
+// recomputed per 128-row tile; every operand tile is bf16 in the same no-swizzle core-matrix layout (chunk (row, c) at
+// c * (rows*16+16) + row*16), read K-major by the forward / dgrad MMAs and MN-major by the wgrad MMAs.
+constexpr uint32_t kMlpBwdThreads = 256;    // warps 0-3: MMA issue + epilogues (TMEM lane quarters); warps 4-7: loaders
+struct MlpBwdPlan {
+    MlpPlan fwd;                        // widths, paddings, p_off; w_off / a0_off / smem_bytes are re-laid-out below
+    uint32_t w_off[kMlpMaxLayers];      // bf16 weights of layer l, [npad][kpad] (as in the forward)
+    uint32_t a_off[kMlpMaxLayers];      // activation tile a_l, l = 0..n-1: 128 x kpad[l]; a_0 is double buffered
+    uint32_t a0_bytes;                  // bytes of one a_0 buffer
+    uint32_t d_off[2];                  // delta tiles (ping-pong), 128 x 128
+    uint32_t dn_off;                    // delta_n tile (from dout), 128 x npad[n-1]
+    uint32_t bar_off;                   // mbarriers + TMEM slot
+    uint32_t smem_bytes;
+    uint32_t acc_col;                   // working accumulator (forward z_l / dgrad g): columns [acc_col, acc_col + acc_cols)
+    uint32_t acc_cols;
+    uint32_t dw_col[kMlpMaxLayers];     // persistent wgrad accumulators: kpad[l] columns each, lane = output row j
+    uint32_t tmem_cols;                 // power of two >= total, <= 512
+};
+
+cudaError_t launch_mlp_bwd(const MlpBwdPlan& B, const float* feat, const float* params, const float* dout,
+                           float* dfeat, float* dparams, cudaStream_t s);
+
 cudaError_t launch_deform_fused(const Plan& P, const MlpPlan& M, const float* xyz, const float* t,
                                 const int32_t* index, const void* table, bool table_half,
                                 const float* params, const float* base, float* out, int sms,

@@ -715,6 +715,82 @@ DASH_API int dash_mlp_fwd(const dash_mlp_config* mlp, uint64_t N, const float* f
     return ok();
 }
 
+}  // extern "C"
+
+namespace {
+
+// Shared-memory / tensor-memory map of mlp_bwd_kernel (deform_kernels.h MlpBwdPlan).
+int fill_mlp_bwd_plan(const dash_mlp_config* m, uint64_t N, dash::MlpBwdPlan* B) {
+    std::memset(B, 0, sizeof(*B));
+    if (int rc = fill_mlp_plan(m, N, &B->fwd)) return rc;
+    const dash::MlpPlan& M = B->fwd;
+    const uint32_t nl = M.n_layers, tile_lbo = dash::kDeformTileM * 16 + 16;
+    uint32_t off = 0;
+    for (uint32_t l = 0; l < nl; ++l) {
+        if (M.kpad[l] > 256)
+            return fail(DASH_HASH4D_UNSUPPORTED, "mlp_bwd: width[%u] = %u exceeds 240 (one wgrad MMA covers N <= 256)",
+                        l, M.width[l]);
+        B->w_off[l] = off;
+        off += (M.kpad[l] / 8) * (M.npad[l] * 16 + 16);
+    }
+    off = round_up(off, 128);
+    B->a_off[0] = off;
+    B->a0_bytes = (M.kpad[0] / 8) * tile_lbo;
+    off += 2 * B->a0_bytes;
+    for (uint32_t l = 1; l < nl; ++l) {
+        B->a_off[l] = off;
+        off += (M.kpad[l] / 8) * tile_lbo;
+    }
+    B->dn_off = off;                       // delta_n first: the wgrad reads 16 chunks from it, the overrun lands in
+    off += (M.npad[nl - 1] / 8) * tile_lbo;   // the delta buffers behind it (garbage rows of the accumulator, never read)
+    B->d_off[0] = off;
+    B->d_off[1] = off + 16 * tile_lbo;
+    off += 32 * tile_lbo;
+    B->bar_off = round_up(off, 128);
+    B->smem_bytes = B->bar_off + 128;
+    if (B->smem_bytes > dash::kDeformSmemLimit)
+        return fail(DASH_HASH4D_UNSUPPORTED, "mlp_bwd: this layer chain needs %u bytes of shared memory per CTA (limit %u)",
+                    B->smem_bytes, dash::kDeformSmemLimit);
+    uint32_t acc = 32;
+    for (uint32_t l = 0; l + 1 < nl; ++l) acc = M.npad[l] > acc ? M.npad[l] : acc;
+    for (uint32_t l = 0; l < nl; ++l) acc = M.kbias[l] > acc ? M.kbias[l] : acc;
+    B->acc_col = 0;
+    B->acc_cols = round_up(acc, 32);
+    uint32_t col = B->acc_cols;
+    for (uint32_t l = 0; l < nl; ++l) {
+        B->dw_col[l] = col;
+        col += M.kpad[l];
+    }
+    if (col > 512)
+        return fail(DASH_HASH4D_UNSUPPORTED, "mlp_bwd: %u tensor-memory columns needed (accumulator %u + weight "
+                    "gradients), 512 available", col, B->acc_cols);
+    uint32_t cols = 32;
+    while (cols < col) cols *= 2;
+    B->tmem_cols = cols;
+    return DASH_HASH4D_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+DASH_API int dash_mlp_bwd(const dash_mlp_config* mlp, uint64_t N, const float* feat, const float* params,
+                          const float* dout, float* dfeat, float* dparams, void* cuda_stream) {
+    if (int rc = check_mlp(mlp)) return rc;
+    dash::MlpBwdPlan B;
+    if (int rc = fill_mlp_bwd_plan(mlp, N, &B)) return rc;
+    if (N == 0) return ok();
+    if (!feat || !params || !dout || !dparams)
+        return fail(DASH_HASH4D_INVALID_ARG, "feat, params, dout or dparams is NULL");
+    if ((reinterpret_cast<uintptr_t>(feat) | reinterpret_cast<uintptr_t>(params) | reinterpret_cast<uintptr_t>(dout) |
+         reinterpret_cast<uintptr_t>(dparams)) & 3u)
+        return fail(DASH_HASH4D_INVALID_ARG, "feat / params / dout / dparams not 4-byte aligned");
+    if (dfeat && !aligned16(dfeat)) return fail(DASH_HASH4D_INVALID_ARG, "dfeat not 16-byte aligned");
+    cudaError_t e = dash::launch_mlp_bwd(B, feat, params, dout, dfeat, dparams, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "mlp_bwd launch");
+    return ok();
+}
+
 DASH_API size_t dash_deform_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp,
                                             uint64_t N) {
     if (check_config(enc) || check_mlp(mlp)) return 0;

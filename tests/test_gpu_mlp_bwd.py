@@ -1,0 +1,139 @@
+"""GPU parity of dash_mlp_bwd / dash_deform_bwd (include/dash_deform.h; Q30) against the CPU oracle, through
+the C ABI.
+
+Tolerance (derived in DESIGN.md §3b): the kernel feeds its tensor cores bf16 operands; against the oracle run with the
+SAME operand rounding what is left is fp32 accumulation order and rare one-ulp flips of a bf16-rounded activation or
+delta (2^-8 of ONE term of the next sum): elementwise 4e-3 * A with A the oracle's propagated magnitude bound, normwise
+1e-3 (dfeat) / 4e-3 (dparams, which sums every row's flips).  The relu mask is a DECISION taken from a floating-point
+value: rows whose closest pre-activation is within 1e-3 of its rounding scale of a kink (oracle `margin`) have no unique
+gradient; for them only a validity bound is checked (|err| within twice the unmasked magnitude bound)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2507_19141_b200 as dh
+from dash_inputs import EncoderParams, make_mlp_params, make_queries_uniform
+
+pytestmark = pytest.mark.gpu
+
+
+def dev(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def unmasked_bound(widths, params, dout):
+    D, o, mats = np.abs(dout.astype(np.float64)), 0, []
+    for l in range(1, len(widths)):
+        J, K = widths[l], widths[l - 1]
+        mats.append(np.abs(params[o:o + J * K].astype(np.float64)).reshape(J, K)); o += J * K + J
+    for w in reversed(mats):
+        D = D @ w
+    return D
+
+
+def check_bwd(widths, feat, params, dout, dfeat, dparams, what):
+    fq, pq, fa, pa, mg = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout,
+                                               want_abs=True)
+    dfeat, dparams = np.asarray(dfeat, np.float64), np.asarray(dparams, np.float64)
+    assert np.isfinite(dfeat).all() and np.isfinite(dparams).all(), what
+    ok = mg > 1e-3
+    err = np.abs(dfeat - fq)
+    assert (err[ok] <= 4e-3 * fa[ok] + 1e-30).all(), f"{what}: dfeat worst err/A {(err[ok] / (fa[ok] + 1e-300)).max():.3e}"
+    if ok.any():
+        nrm = np.linalg.norm((dfeat - fq)[ok]) / max(np.linalg.norm(fq[ok]), 1e-300)
+        assert nrm <= 1e-3, f"{what}: dfeat normwise {nrm:.3e}"
+    loose = 2.0 * unmasked_bound(widths, params, dout)
+    assert (err[~ok] <= loose[~ok] + 1e-30).all(), f"{what}: dfeat of a near-kink row outside the validity bound"
+    errp = np.abs(dparams - pq)
+    assert (errp <= 4e-3 * pa + 1e-30).all(), f"{what}: dparams worst err/A {(errp / (pa + 1e-300)).max():.3e}"
+    nrmp = np.linalg.norm(dparams - pq) / max(np.linalg.norm(pq), 1e-300)
+    assert nrmp <= 4e-3, f"{what}: dparams normwise {nrmp:.3e}"
+    return float(ok.mean())
+
+
+SHAPES = [
+    ([32, 10], 128), ([32, 10], 1000), ([16, 16], 1), ([32, 64, 10], 300), ([64, 128, 10], 1000),
+    ([24, 40, 7], 300),                      # widths that need padding to 16
+    ([32, 64, 64, 10], 129), ([32, 128, 128, 10], 20_000), ([32, 64, 48, 32, 10], 777), ([64, 128, 10], 0),
+]
+
+
+@pytest.mark.parametrize("widths,N", SHAPES)
+def test_mlp_bwd_parity(widths, N):
+    rng = np.random.default_rng(sum(widths) + N)
+    feat = rng.standard_normal((N, widths[0])).astype(np.float32)
+    params = make_mlp_params(sum(widths), widths)
+    dout = rng.standard_normal((N, widths[-1])).astype(np.float32)
+    m = dh.make_mlp_config(widths)
+    start = rng.standard_normal(params.size).astype(np.float32)           # dparams is ACCUMULATED into
+    dp = dev(start)
+    fd = dev(feat) if N else torch.empty((0, widths[0]), device="cuda")
+    dd = dev(dout) if N else torch.empty((0, widths[-1]), device="cuda")
+    dfeat, dp = dh.dash_mlp_bwd(m, fd, dev(params), dd, dp)
+    torch.cuda.synchronize()
+    assert dfeat.shape == (N, widths[0])
+    if N == 0:
+        np.testing.assert_array_equal(dp.cpu().numpy(), start)
+        return
+    got_p = dp.cpu().numpy().astype(np.float64) - start
+    # the fp32 '+=' into a random start costs one rounding of the start's magnitude: fold it into the bound
+    frac = check_bwd_with_start(widths, feat, params, dout, dfeat.cpu().numpy(), got_p, start, f"mlp_bwd {widths} N={N}")
+    assert frac > 0.2
+
+
+def check_bwd_with_start(widths, feat, params, dout, dfeat, got_p, start, what):
+    fq, pq, fa, pa, mg = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout,
+                                               want_abs=True)
+    slack = 2.0 ** -22 * (np.abs(start) + np.abs(pq))
+    errp = np.abs(got_p - pq)
+    assert (errp <= 4e-3 * pa + slack + 1e-30).all(), f"{what}: dparams worst err/A {(errp / (pa + 1e-300)).max():.3e}"
+    return check_bwd(widths, feat, params, dout, dfeat, pq + np.clip(got_p - pq, -4e-3 * pa, 4e-3 * pa), what)
+
+
+def test_mlp_bwd_without_dfeat_and_twice_accumulates():
+    widths, N = [32, 64, 10], 500
+    rng = np.random.default_rng(1)
+    feat = rng.standard_normal((N, 32)).astype(np.float32)
+    params = make_mlp_params(2, widths)
+    dout = rng.standard_normal((N, 10)).astype(np.float32)
+    m = dh.make_mlp_config(widths)
+    dp = torch.zeros(params.size, device="cuda")
+    none, _ = dh.dash_mlp_bwd(m, dev(feat), dev(params), dev(dout), dp, want_dfeat=False)
+    assert none is None
+    once = dp.cpu().numpy().copy()
+    dh.dash_mlp_bwd(m, dev(feat), dev(params), dev(dout), dp, want_dfeat=False)
+    np.testing.assert_allclose(dp.cpu().numpy(), 2 * once, rtol=1e-6, atol=1e-6)
+    _, pq = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout)
+    assert np.linalg.norm(once - pq) / np.linalg.norm(pq) <= 4e-3
+
+
+def test_one_layer_is_exact_up_to_fp32_accumulation():
+    """No hidden layer: no activation rounding and no mask, so against the bf16-operand oracle only the fp32 summation
+    order is left: dfeat to 2e-6 of its magnitude bound, dparams to N * 2^-24."""
+    widths, N = [48, 12], 3000
+    rng = np.random.default_rng(5)
+    feat = rng.standard_normal((N, 48)).astype(np.float32)
+    params = make_mlp_params(5, widths)
+    dout = rng.standard_normal((N, 12)).astype(np.float32)
+    dp = torch.zeros(params.size, device="cuda")
+    dfeat, dp = dh.dash_mlp_bwd(dh.make_mlp_config(widths), dev(feat), dev(params), dev(dout), dp)
+    fq, pq, fa, pa, _ = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout,
+                                              want_abs=True)
+    assert (np.abs(dfeat.cpu().numpy() - fq) <= 2e-6 * fa + 1e-30).all()
+    assert (np.abs(dp.cpu().numpy() - pq) <= N * 2.0 ** -24 * pa + 1e-30).all()
+
+
+def test_mlp_bwd_errors():
+    big = dh.make_mlp_config([64, 128, 128, 128, 10])                       # tiles + weights beyond 227 KB
+    z = lambda *s: torch.zeros(s, device="cuda")
+    with pytest.raises(dh.Hash4DError) as e:
+        dh.dash_mlp_bwd(big, z(4, 64), z(dh.dash_mlp_param_count(big)), z(4, 10), z(dh.dash_mlp_param_count(big)))
+    assert e.value.status == 2
+    wide = dh.make_mlp_config([250, 10])
+    with pytest.raises(dh.Hash4DError) as e:
+        dh.dash_mlp_bwd(wide, z(4, 250), z(dh.dash_mlp_param_count(wide)), z(4, 10), z(dh.dash_mlp_param_count(wide)))
+    assert e.value.status == 2
+    m = dh.make_mlp_config([32, 10])
+    with pytest.raises(ValueError, match="dparams"):
+        dh.dash_mlp_bwd(m, z(4, 32), z(330), z(4, 10), z(329))
