@@ -67,6 +67,21 @@ DASH_API int dash_mlp_fwd(const dash_mlp_config* mlp, uint64_t N,
 DASH_API int dash_mlp_bwd(const dash_mlp_config* mlp, uint64_t N, const float* feat, const float* params,
                           const float* dout, float* dfeat, float* dparams, void* cuda_stream);
 
+/* Training backward of dash_deform_fwd (out = base + MLP(G_4D(x)), Eq. 9-10), composed of the calls above and of
+ * include/dash_hash4d.h on `cuda_stream`; given dout = dL/d out [N][width[n_layers]]:
+ *     feat   = G_4D(x)                         dash_hash4d_fwd, recomputed into the workspace
+ *     dfeat, dparams += backward of the chain  dash_mlp_bwd
+ *     dtable += J(x)^T dfeat                   dash_hash4d_bwd (enc->flags: DENSE_COARSE, ZERO_GRAD honoured)
+ *     dq = d<dfeat, G_4D(x)>/d(x,y,z,t)        dash_hash4d_bwd_input, when dq ([N][4] fp32, overwritten) is not NULL
+ * dL/d base is dout itself.  workspace: dash_deform_bwd_workspace_bytes = 2 * N * L*F * 4 bytes, 16-byte aligned.
+ * enc->flags other than DENSE_COARSE | ZERO_GRAD: INVALID_ARG.  Errors of the composed calls are passed through. */
+DASH_API size_t dash_deform_bwd_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N);
+DASH_API int dash_deform_bwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
+                             const float* xyz, uint32_t xyz_stride, const float* t, uint32_t t_stride,
+                             const int32_t* index, const void* table, const float* params, const float* dout,
+                             float* dtable, float* dparams, float* dq,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Device workspace dash_deform_fwd needs: 0 when the fused kernel applies (the table fits L2 as one level
  * group), else N * L*F * 4 bytes for the feature matrix of the two-pass path. */
 DASH_API size_t dash_deform_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp,

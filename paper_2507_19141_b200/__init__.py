@@ -12,7 +12,7 @@ from .binding import (  # noqa: F401
     dash_hash3d_resolutions, dash_hash3d_fwd, dash_hash3d_bwd, dash_hash3d_indices,
     dash_hash4d_slice_t, dash_hash4d_slice_fwd, dash_deform_slice_fwd, dash_deform_slice_workspace_bytes,
     AdamConfig, ADAM_ZERO_GRAD, dash_hash4d_adam_step,
-    MlpConfig, make_mlp_config, dash_mlp_param_count, dash_mlp_fwd, dash_mlp_bwd, dash_deform_workspace_bytes, dash_deform_fwd,
+    MlpConfig, make_mlp_config, dash_mlp_param_count, dash_mlp_fwd, dash_mlp_bwd, dash_deform_bwd, dash_deform_workspace_bytes, dash_deform_fwd,
     dash_hash4d_fwd_host, dash_hash4d_bwd_host, exported_symbols, with_flags, HostStep,
     dash_hash4d_sort_queries, dash_hash4d_set_debug, DEBUG_FWD_GROUP, DEBUG_BWD_GROUP, DEBUG_SMOOTH_GROUP, DEBUG_DEFORM_PATH,
     DEBUG_BWD_VARIANT, DEBUG_FWD_VARIANT,

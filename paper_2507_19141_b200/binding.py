@@ -25,7 +25,7 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count", "dash_hash4d_set_debug", "dash_hash4d_build_id",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
-           "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_mlp_bwd", "dash_deform_workspace_bytes", "dash_deform_fwd",
+           "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_mlp_bwd", "dash_deform_bwd", "dash_deform_bwd_workspace_bytes", "dash_deform_workspace_bytes", "dash_deform_fwd",
            "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch",
            "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_deform_slice_workspace_bytes"]
 
@@ -132,6 +132,10 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_mlp_fwd.restype = C.c_int
     lib.dash_mlp_bwd.argtypes = [mlpp, u64, vp, vp, vp, vp, vp, vp]
     lib.dash_mlp_bwd.restype = C.c_int
+    lib.dash_deform_bwd_workspace_bytes.argtypes = [cfgp, mlpp, u64]
+    lib.dash_deform_bwd_workspace_bytes.restype = sz
+    lib.dash_deform_bwd.argtypes = [cfgp, mlpp, u64, vp, u32, vp, u32, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.dash_deform_bwd.restype = C.c_int
     lib.dash_deform_workspace_bytes.argtypes = [cfgp, mlpp, u64]
     lib.dash_deform_workspace_bytes.restype = sz
     lib.dash_deform_fwd.argtypes = [cfgp, mlpp, u64, vp, u32, vp, u32, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -556,6 +560,32 @@ def dash_mlp_bwd(mlp, feat, params, dout, dparams, dfeat=None, want_dfeat=True):
     _check(_load().dash_mlp_bwd(C.byref(mlp), N, _ptr(feat), _ptr(params), _ptr(dout), _ptr(dfeat), _ptr(dparams),
                                 _stream()))
     return dfeat, dparams
+
+
+def dash_deform_bwd(cfg, mlp, xyz, t, table, params, dout, dtable, dparams, dq=None, index=None, t_stride=None, N=None,
+                    workspace=None):
+    """Backward of dash_deform_fwd: dtable (+)= table gradient, dparams += MLP parameter gradient, dq (optional,
+    [N][4]) = coordinate gradient.  Returns (dtable, dparams, dq)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(t, torch.float32, "t"); _dev(index, torch.int32, "index")
+    _dev(table, torch.float16 if cfg.table_dtype == 1 else torch.float32, "table")
+    for name, a in (("params", params), ("dout", dout), ("dtable", dtable), ("dparams", dparams), ("dq", dq)):
+        _dev(a, torch.float32, name)
+    xs, ts = _strides(xyz, t, t_stride)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    n_out = int(mlp.width[mlp.n_layers])
+    _check_queries(cfg, xyz, t, index, ts, N)
+    _exactly(table, _table_elems(cfg), "table"); _exactly(dtable, _table_elems(cfg), "dtable")
+    _exactly(params, dash_mlp_param_count(mlp), "params"); _exactly(dparams, dash_mlp_param_count(mlp), "dparams")
+    _at_least(dout, N * n_out, "dout"); _at_least(dq, 4 * N, "dq")
+    need = int(_load().dash_deform_bwd_workspace_bytes(C.byref(cfg), C.byref(mlp), N))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=xyz.device)
+    _one_device(xyz, t, index, table, params, dout, dtable, dparams, dq, workspace)
+    _check(_load().dash_deform_bwd(C.byref(cfg), C.byref(mlp), N, _ptr(xyz), xs, _ptr(t), ts, _ptr(index), _ptr(table),
+                                   _ptr(params), _ptr(dout), _ptr(dtable), _ptr(dparams), _ptr(dq), _ptr(workspace),
+                                   workspace.numel(), _stream()))
+    return dtable, dparams, dq
 
 
 def dash_deform_workspace_bytes(cfg, mlp, N: int) -> int:

@@ -137,3 +137,70 @@ def test_mlp_bwd_errors():
     m = dh.make_mlp_config([32, 10])
     with pytest.raises(ValueError, match="dparams"):
         dh.dash_mlp_bwd(m, z(4, 32), z(330), z(4, 10), z(329))
+
+
+@pytest.mark.parametrize("dtype,with_index,zero_grad", [("fp32", False, True), ("fp16", True, False)])
+def test_deform_bwd_is_the_composition_and_matches_the_oracle(dtype, with_index, zero_grad):
+    """dash_deform_bwd = hash4d_fwd -> mlp_bwd -> hash4d_bwd (-> bwd_input).  Checked three ways: against the same
+    four calls made one by one; dparams against the oracle chain (oracle_fwd -> oracle_mlp_bwd); dtable and dq against
+    the oracle's scatter / coordinate gradient fed the GPU's own dfeat (both are linear in it: no mask ambiguity left)."""
+    from parity_utils import RTOL_FP32, check_close
+    L, F, T = 8, 4, 1 << 12
+    enc = EncoderParams(L, F, T, 8, 200, 4, 30, dtype)
+    widths = [L * F, 64, 10]
+    rng = np.random.default_rng(11)
+    rows = 3000
+    xyz_rows, _ = make_queries_uniform(3, rows)
+    index = rng.integers(0, rows, 4001).astype(np.int32) if with_index else None
+    n = len(index) if with_index else rows
+    t = rng.random(n, dtype=np.float32)
+    table = rng.uniform(-1, 1, (L, T, F)).astype(np.float16 if dtype == "fp16" else np.float32)
+    params = make_mlp_params(4, widths)
+    dout = rng.standard_normal((n, 10)).astype(np.float32)
+    flags = dh.FLAG_DENSE_COARSE | (dh.FLAG_ZERO_GRAD if zero_grad else 0)
+    gcfg, ocfg = dh.config_from_params(enc, flags=flags), oracle.config_from_params(enc)
+    m = dh.make_mlp_config(widths)
+    start = 7.0 if zero_grad else 0.0                                       # ZERO_GRAD must overwrite garbage
+    dtable = torch.full((L, T, F), start, device="cuda")
+    dparams = torch.zeros(params.size, device="cuda")
+    dq = torch.empty((n, 4), device="cuda")
+    xd, td, idx, tabd, pd, dd = dev(xyz_rows), dev(t), dev(index), dev(table), dev(params), dev(dout)
+    dh.dash_deform_bwd(gcfg, m, xd, td, tabd, pd, dd, dtable, dparams, dq=dq, index=idx)
+    torch.cuda.synchronize()
+    # (1) the same calls, one by one
+    plain = dh.config_from_params(enc)
+    feat = dh.dash_hash4d_fwd(plain, xd, td, tabd, index=idx)
+    dp2 = torch.zeros_like(dparams)
+    dfeat, _ = dh.dash_mlp_bwd(m, feat, pd, dd, dp2)
+    dt2 = torch.zeros((L, T, F), device="cuda")
+    dh.dash_hash4d_bwd(plain, xd, td, dfeat, dt2, index=idx)
+    dq2 = dh.dash_hash4d_bwd_input(plain, xd, td, tabd, dfeat, index=idx)
+    torch.testing.assert_close(dparams, dp2, rtol=1e-5, atol=1e-5)          # fp32 reductions in a different order
+    torch.testing.assert_close(dtable, dt2, rtol=1e-4, atol=1e-5)
+    torch.testing.assert_close(dq, dq2, rtol=1e-4, atol=1e-4)
+    # (2) dparams against the oracle chain
+    feat_o = oracle.oracle_fwd(ocfg, n, xyz_rows, t, table, index=index)
+    fq, pq, fa, pa, mg = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat_o, params, dout,
+                                               want_abs=True)
+    assert (np.abs(dparams.cpu().numpy() - pq) <= 4e-3 * pa + 1e-30).all()
+    # (3) scatter and coordinate gradient of the GPU's dfeat, by the oracle
+    dfeat_h = dfeat.cpu().numpy()
+    ref_t, mag_t, hits = oracle.oracle_bwd(ocfg, n, xyz_rows, t, dfeat_h, index=index, want_abs=True, want_hits=True)
+    check_close(dtable.cpu().numpy(), ref_t, mag_t, RTOL_FP32, L, hits=hits, what="deform_bwd dtable")
+    ref_q, mag_q = oracle.oracle_bwd_input(ocfg, n, xyz_rows, t, table, dfeat_h, index=index, want_abs=True)
+    assert (np.abs(dq.cpu().numpy() - ref_q) <= (2e-3 if dtype == "fp16" else 1e-5) * mag_q + 1e-30).all()
+
+
+def test_deform_bwd_errors():
+    enc = EncoderParams(4, 2, 1 << 10, 8, 64, 4, 16)
+    z = lambda *s: torch.zeros(s, device="cuda")
+    m = dh.make_mlp_config([8, 10])
+    det = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE | dh.FLAG_DETERMINISTIC_BWD)
+    with pytest.raises(dh.Hash4DError) as e:
+        dh.dash_deform_bwd(det, m, z(5, 3), z(5), z(4, 1 << 10, 2), z(90), z(5, 10), z(4, 1 << 10, 2), z(90))
+    assert e.value.status == 1
+    cfg = dh.config_from_params(enc)
+    with pytest.raises(dh.Hash4DError) as e:                               # width[0] != L*F
+        dh.dash_deform_bwd(cfg, dh.make_mlp_config([16, 10]), z(5, 3), z(5), z(4, 1 << 10, 2), z(170), z(5, 10),
+                           z(4, 1 << 10, 2), z(170))
+    assert e.value.status == 1
