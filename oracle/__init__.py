@@ -233,6 +233,16 @@ def oracle3d_bwd(cfg, N, xyz, dout, index=None, dtable=None, want_abs=False, wan
     return res[0] if len(res) == 1 else tuple(res)
 
 
+def oracle3d_bwd_input(cfg, N, xyz, table, dout, index=None, want_abs=False):
+    """dq[n] = d<dout[n], G_3D(p_n)>/d(x,y,z): [N][3] fp32 (DESIGN.md §9 item 2)."""
+    xs = _point_args(xyz, index)
+    dq = np.zeros((N, 3), np.float32)
+    mag = np.zeros((N, 3), np.float64) if want_abs else None
+    _check(lib().dash_oracle3d_bwd_input(C.byref(cfg), C.c_uint64(N), _p(xyz), xs, _p(index), _p(table), _p(dout),
+                                         _p(dq), _p(mag)), "3d bwd_input")
+    return (dq, mag) if want_abs else dq
+
+
 # ---- phi_d + multi-head deformation decoder (PAPER.md:133-142, Eq. 9-10; SURVEY §8f NEXT #3; DESIGN.md Q27) ----
 
 MLP_QUANT_BF16 = 1

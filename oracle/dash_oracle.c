@@ -670,6 +670,52 @@ int dash_oracle3d_bwd(const dash_oracle_config *c, uint64_t N, const float *xyz,
     return failed ? ORACLE_NOMEM : ORACLE_OK;
 }
 
+/* Coordinate gradient of G_3D (DESIGN.md §9 item 2; the d = 3 form of dash_oracle_bwd_input, reading Q24):
+ *   dq[n][d] = sum_{l,f} dout[n][l*F+f] * N_l * sum_k s_d(k) * prod_{e != d} omega_e(k) * table[l][slot_k][f],  d = x,y,z
+ * on the open cell; a coordinate the Q12 clamp moved has derivative 0.  dq [N][3] fp32; dq_abs (nullable): sum |terms|. */
+int dash_oracle3d_bwd_input(const dash_oracle_config *c, uint64_t N, const float *xyz, uint32_t xyz_stride,
+                            const int32_t *index, const void *table, const float *dout, float *dq,
+                            double *dq_abs) {
+    uint32_t res[ORACLE_MAX_L], pi[4];
+    uint8_t dn[ORACLE_MAX_L];
+    if (dash_oracle3d_resolutions(c, res, dn)) return ORACLE_INVALID;
+    if (N == 0) return ORACLE_OK;
+    if (!xyz || !(xyz_stride == 3 || xyz_stride == 4) || !table || !dout || !dq) return ORACLE_INVALID;
+    get_primes(c, pi);
+    const uint32_t L = c->L, F = c->F;
+#pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < (int64_t)N; ++n) {
+        float p[3];
+        fetch_point((uint64_t)n, xyz, xyz_stride, index, p);
+        double acc[3] = {0, 0, 0}, mag[3] = {0, 0, 0};
+        for (uint32_t l = 0; l < L; ++l) {
+            uint32_t cell[3], slot[8];
+            float frac[3];
+            double W[8];
+            for (int d = 0; d < 3; ++d) locate(clamp_unit(p[d]), res[l], &cell[d], &frac[d]);
+            corners3(c, pi, res[l], dn[l], p, slot, W); /* the slots; the weights are differentiated below */
+            for (int k = 0; k < 8; ++k)
+                for (int d = 0; d < 3; ++d) {
+                    double wd = ((k >> d) & 1) ? 1.0 : -1.0;
+                    for (int e = 0; e < 3; ++e)
+                        if (e != d) wd *= ((k >> e) & 1) ? (double)frac[e] : 1.0 - (double)frac[e];
+                    for (uint32_t f = 0; f < F; ++f) {
+                        double term = (double)dout[(size_t)n * L * F + (size_t)l * F + f] * (double)res[l] * wd *
+                                      table_value(c, table, l, slot[k], f);
+                        acc[d] += term;
+                        mag[d] += fabs(term);
+                    }
+                }
+        }
+        for (int d = 0; d < 3; ++d) {
+            int moved = isnan(p[d]) || p[d] < 0.0f || p[d] > 0x1.fffffep-1f;
+            dq[(size_t)n * 3 + d] = moved ? 0.0f : (float)acc[d];
+            if (dq_abs) dq_abs[(size_t)n * 3 + d] = moved ? 0.0 : mag[d];
+        }
+    }
+    return ORACLE_OK;
+}
+
 /* ---- NEXT #3: the tiny MLP phi_d and the multi-head deformation decoder ---------------
  * "quadrilinear interpolation ..., followed by a tiny MLP phi_d", f_4D = phi_d(f_h) (Eq. 9);
  * "a multi-head deformation decoder D = {phi_x, phi_r, phi_s}": dx = phi_x(f_4D), dr = phi_r(f_4D),

@@ -148,3 +148,46 @@ def test_multi_affine_reproduction_weights_and_adjoint():
     index = rng.integers(0, n, 77).astype(np.int32)
     np.testing.assert_array_equal(oracle.oracle3d_fwd(cfg2, 77, xyz, theta, index=index),
                                   oracle.oracle3d_fwd(cfg2, 77, np.ascontiguousarray(xyz[index]), theta))
+
+
+def test_coordinate_gradient_equals_the_4d_oracle_and_exact_central_differences():
+    """oracle3d_bwd_input pinned (i) to the 4D coordinate gradient at Nt = 1, t = 0 with Eq. 8 on every level (g_t = 0
+    adds nothing to the XOR; the t-derivative is dropped), (ii) by central differences of the pinned 3D forward on
+    power-of-two grids (the interpolant is affine in x inside a cell, steps of 2^-14 stay inside), (iii) a clamped
+    coordinate has gradient 0 and the magnitude term is the value itself when every term has one sign."""
+    L, F, T = 4, 2, 1 << 11
+    rng = np.random.default_rng(21)
+    n = 300
+    cfg3 = oracle.make_config(L, F, T, 8, 64, 1, 1, dense_coarse=False)
+    cfg4 = oracle.make_config(L, F, T, 8, 64, 1, 1, dense_coarse=False)
+    xyz, _ = make_queries_uniform(21, n)
+    table = rng.uniform(-1, 1, (L, T, F)).astype(np.float32)
+    dout = rng.standard_normal((n, L * F)).astype(np.float32)
+    dq3, mag3 = oracle.oracle3d_bwd_input(cfg3, n, xyz, table, dout, want_abs=True)
+    dq4, mag4 = oracle.oracle_bwd_input(cfg4, n, xyz, np.zeros(1, np.float32), table, dout, t_stride=0, want_abs=True)
+    np.testing.assert_array_equal(dq3, dq4[:, :3])
+    np.testing.assert_allclose(mag3, mag4[:, :3], rtol=1e-14)
+    # (ii) exact central differences on a dense + hashed power-of-two schedule
+    cfgd = oracle.make_config(3, 1, 1 << 10, 4, 16, 1, 1)                       # levels 4, 8, 16: (8+1)^3 = 729 dense
+    tab = rng.uniform(-1, 1, (3, 1 << 10, 1)).astype(np.float32)
+    pts = (rng.integers(1, 60, (200, 3)) / 64.0 + 2.0 ** -9).astype(np.float32)  # strictly inside cells of every level
+    dy = rng.standard_normal((200, 3)).astype(np.float32)
+    dq = oracle.oracle3d_bwd_input(cfgd, 200, pts, tab, dy)
+    h = np.float32(2.0 ** -14)
+    for d in range(3):
+        pp, pm = pts.copy(), pts.copy()
+        pp[:, d] += h; pm[:, d] -= h
+        fd = ((oracle.oracle3d_fwd(cfgd, 200, pp, tab).astype(np.float64) - oracle.oracle3d_fwd(cfgd, 200, pm, tab)) * dy).sum(1) / (2.0 * float(h))
+        np.testing.assert_allclose(dq[:, d], fd, rtol=0, atol=2e-3)             # the forward's fp32 rounding / 2^-13
+    # (iii) clamp and sign structure
+    bad = np.array([[-0.5, 0.3, 0.4], [0.2, np.nan, 0.4], [0.2, 0.3, 1.5]], np.float32)
+    dqb = oracle.oracle3d_bwd_input(cfgd, 3, bad, tab, np.ones((3, 3), np.float32))
+    assert dqb[0, 0] == 0 and dqb[1, 1] == 0 and dqb[2, 2] == 0 and np.abs(dqb).sum() > 0
+    S = 5
+    gx = np.arange(1 << 10) % S
+    mono = np.zeros((1, 1 << 10, 1), np.float32); mono[0, :, 0] = 1.0 + gx       # v = 1 + g_x on the level-4 dense grid
+    c1 = oracle.make_config(1, 1, 1 << 10, 4, 4, 1, 1)
+    q, m = oracle.oracle3d_bwd_input(c1, 100, xyz[:100], mono, np.ones((100, 1), np.float32), want_abs=True)
+    np.testing.assert_allclose(q[:, 0], 4.0, rtol=1e-6)
+    cell = np.floor(xyz[:100, 0] * np.float32(4)).astype(np.float64)
+    np.testing.assert_allclose(m[:, 0], 4 * (2 * (1 + cell) + 1), rtol=1e-12)
