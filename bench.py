@@ -635,6 +635,21 @@ def run_cuda(args):
             row["frame_ms_slice_path"] = row["slice_t_ms"] + row["slice_fused_ms"]
             row["mlp_tflops"] = 2.0 * w2.N * sum(a * b for a, b in zip(widths[:-1], widths[1:])) / (
                 row["mlp_only_ms"] * 1e-3) / 1e12
+            # training direction (Q30): backward through the chain, and the whole deformation backward
+            dy2 = torch.randn((w2.N, 10), device="cuda", generator=gen)
+            dprm = torch.zeros_like(prm)
+            dft = torch.empty((w2.N, e2.L * e2.F), dtype=torch.float32, device="cuda")
+            row["mlp_bwd_ms"] = timed(lambda: dh.dash_mlp_bwd(mlp, f2, prm, dy2, dprm, dfeat=dft), 20)
+            # forward recompute (1x) + dgrad (1x) + wgrad (1x) of every layer
+            row["mlp_bwd_tflops"] = 3.0 * 2.0 * w2.N * sum(a * b for a, b in zip(widths[:-1], widths[1:])) / (
+                row["mlp_bwd_ms"] * 1e-3) / 1e12
+            dt2 = torch.empty((e2.L, e2.T, e2.F), dtype=torch.float32, device="cuda")
+            tq = to_dev(w2.t)
+            cfg2z = dh.config_from_params(e2, flags=dh.FLAG_DENSE_COARSE | dh.FLAG_ZERO_GRAD)
+            wsb = torch.empty(2 * w2.N * e2.L * e2.F * 4 + 64, dtype=torch.uint8, device="cuda")
+            row["deform_bwd_ms_per_query_t"] = timed(lambda: dh.dash_deform_bwd(cfg2z, mlp, x2, tq, tab2, prm, dy2, dt2,
+                                                                              dprm, workspace=wsb), 20)
+            del dy2, dprm, dft, dt2, wsb
             extras["deform"][name] = row
             del x2, tab2, o2, f2, ws2, sl2
 

@@ -202,6 +202,12 @@ DASH_API int dash_hash3d_bwd(const dash_hash4d_config* cfg, uint64_t N,
                              const float* dout,
                              float* dtable,
                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+/* Coordinate gradient of G_3D: dq[n][d] = d<dout[n], G_3D(p_n)>/dp_d, d = x,y,z; dq [N][3] fp32 (overwritten, 4-byte
+ * aligned).  The D = 3 form of dash_hash4d_bwd_input (reading Q24: one-sided at vertices, 0 for a clamped coordinate). */
+DASH_API int dash_hash3d_bwd_input(const dash_hash4d_config* cfg, uint64_t N,
+                                   const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                   const void* table, const float* dout, float* dq,
+                                   void* workspace, size_t workspace_bytes, void* cuda_stream);
 DASH_API int dash_hash3d_indices(const dash_hash4d_config* cfg, uint64_t N,
                                  const float* xyz, uint32_t xyz_stride,
                                  const int32_t* index,

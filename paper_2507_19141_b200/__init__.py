@@ -9,7 +9,7 @@ from .binding import (  # noqa: F401
     FLAG_ZERO_GRAD, OP_FWD, OP_BWD, OP_INDICES, OP_BWD_INPUT, OP_SMOOTH, make_config, config_from_params, library_path,
     dash_hash4d_resolutions, dash_hash4d_workspace_bytes, dash_hash4d_fwd, dash_hash4d_bwd, dash_hash4d_bwd_input, dash_hash4d_smooth,
     dash_hash4d_indices, dash_hash4d_zero, dash_hash4d_last_error, dash_hash4d_launch_count,
-    dash_hash3d_resolutions, dash_hash3d_fwd, dash_hash3d_bwd, dash_hash3d_indices,
+    dash_hash3d_resolutions, dash_hash3d_fwd, dash_hash3d_bwd, dash_hash3d_indices, dash_hash3d_bwd_input,
     dash_hash4d_slice_t, dash_hash4d_slice_fwd, dash_deform_slice_fwd, dash_deform_slice_workspace_bytes,
     AdamConfig, ADAM_ZERO_GRAD, dash_hash4d_adam_step,
     MlpConfig, make_mlp_config, dash_mlp_param_count, dash_mlp_fwd, dash_mlp_bwd, dash_deform_bwd, dash_deform_workspace_bytes, dash_deform_fwd,

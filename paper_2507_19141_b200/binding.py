@@ -24,7 +24,7 @@ _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUD
 EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4d_fwd",
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count", "dash_hash4d_set_debug", "dash_hash4d_build_id",
-           "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices",
+           "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices", "dash_hash3d_bwd_input",
            "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_mlp_bwd", "dash_deform_bwd", "dash_deform_bwd_workspace_bytes", "dash_deform_workspace_bytes", "dash_deform_fwd",
            "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch",
            "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_deform_slice_workspace_bytes"]
@@ -121,6 +121,8 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_hash3d_fwd.restype = C.c_int
     lib.dash_hash3d_bwd.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp, sz, vp]
     lib.dash_hash3d_bwd.restype = C.c_int
+    lib.dash_hash3d_bwd_input.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp, vp, sz, vp]
+    lib.dash_hash3d_bwd_input.restype = C.c_int
     lib.dash_hash3d_indices.argtypes = [cfgp, u64, vp, u32, vp, vp, vp, vp]
     lib.dash_hash3d_indices.restype = C.c_int
     lib.dash_hash4d_adam_step.argtypes = [cfgp, C.POINTER(AdamConfig), vp, vp, vp, vp, vp, vp]
@@ -480,6 +482,25 @@ def dash_hash3d_bwd(cfg, xyz, dout, dtable, index=None, N=None, workspace=None):
     _check(_load().dash_hash3d_bwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(dout), _ptr(dtable),
                                    _ptr(workspace), wbytes, _stream()))
     return dtable
+
+
+def dash_hash3d_bwd_input(cfg, xyz, table, dout, dq=None, index=None, N=None, workspace=None):
+    """dq[n] = d<dout[n], G_3D(p_n)>/d(x,y,z); returns `dq` ([N][3] fp32, CUDA, overwritten)."""
+    _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index"); _dev(dout, torch.float32, "dout")
+    _dev(table, torch.float16 if cfg.table_dtype == 1 else torch.float32, "table")
+    xs = _xyz_stride(xyz)
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    if dq is None:
+        dq = torch.empty((N, 3), dtype=torch.float32, device=xyz.device)
+    _dev(dq, torch.float32, "dq")
+    _check_queries(cfg, xyz, None, index, 0, N)
+    _exactly(table, _table_elems(cfg), "table"); _at_least(dout, N * cfg.L * cfg.F, "dout"); _at_least(dq, 3 * N, "dq")
+    _one_device(xyz, index, table, dout, dq, workspace)
+    workspace, wbytes = _workspace(cfg, N, OP_BWD_INPUT, workspace, xyz.device)
+    _check(_load().dash_hash3d_bwd_input(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(table), _ptr(dout),
+                                         _ptr(dq), _ptr(workspace), wbytes, _stream()))
+    return dq
 
 
 def dash_hash3d_indices(cfg, xyz, index=None, N=None, want_weights=True):

@@ -330,29 +330,45 @@ DASH_API int dash_hash3d_fwd(const dash_hash4d_config* cfg, uint64_t N, const fl
                     workspace_bytes, cuda_stream);
 }
 
+static int bwd_input_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                          uint32_t xyz_stride, const float* t, uint32_t t_stride, const int32_t* index,
+                          const void* table, const float* dout, float* dq, void* workspace,
+                          size_t workspace_bytes, void* cuda_stream) {
+    if (int rc = check_config(cfg, dims)) return rc;
+    if (N == 0) return ok();
+    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index, dims)) return rc;
+    if (!table || !dout || !dq) return fail(DASH_HASH4D_INVALID_ARG, "table, dout or dq is NULL");
+    if (!aligned16(table) || !aligned16(dout) || (dims == 4 ? !aligned16(dq) : (reinterpret_cast<uintptr_t>(dq) & 3u)))
+        return fail(DASH_HASH4D_INVALID_ARG, "table / dout / dq not aligned (16 bytes; dq of the 3D call 4 bytes)");
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const bool half = cfg->table_dtype == DASH_HASH4D_FP16;
+    const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * (half ? 2 : 4);
+    Plan P;
+    uint32_t group = pick_group(cfg, level_bytes, DASH_DEBUG_FWD_GROUP);
+    if (dims == 3 && group > 4 && 4 * cfg->F * sizeof(float) >= 32 && !debug_u32(DASH_DEBUG_FWD_GROUP)) group = 4;
+    if (int rc = fill_plan(cfg, N, xyz_stride, t_stride, group, &P, dims)) return rc;
+    if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
+    cudaError_t e = dash::launch_zero(dq, static_cast<size_t>(N) * dims * sizeof(float), s);
+    if (e == cudaSuccess) e = dash::launch_bwd_input(P, xyz, t, index, table, half, dout, dq, s);
+    if (e != cudaSuccess) return cuda_fail(e, "bwd_input launch");
+    return ok();
+}
+
 DASH_API int dash_hash4d_bwd_input(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
                                    uint32_t xyz_stride, const float* t, uint32_t t_stride,
                                    const int32_t* index, const void* table, const float* dout,
                                    float* dq, void* workspace, size_t workspace_bytes,
                                    void* cuda_stream) {
-    if (int rc = check_config(cfg)) return rc;
-    if (N == 0) return ok();
-    if (int rc = check_queries(xyz, xyz_stride, t, t_stride, index)) return rc;
-    if (!table || !dout || !dq) return fail(DASH_HASH4D_INVALID_ARG, "table, dout or dq is NULL");
-    if (!aligned16(table) || !aligned16(dout) || !aligned16(dq))
-        return fail(DASH_HASH4D_INVALID_ARG, "table / dout / dq not 16-byte aligned");
-    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-    const bool half = cfg->table_dtype == DASH_HASH4D_FP16;
-    const size_t level_bytes = static_cast<size_t>(cfg->T) * cfg->F * (half ? 2 : 4);
-    Plan P;
-    if (int rc = fill_plan(cfg, N, xyz_stride, t_stride,
-                           pick_group(cfg, level_bytes, DASH_DEBUG_FWD_GROUP), &P))
-        return rc;
-    if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
-    cudaError_t e = dash::launch_zero(dq, static_cast<size_t>(N) * 4 * sizeof(float), s);
-    if (e == cudaSuccess) e = dash::launch_bwd_input(P, xyz, t, index, table, half, dout, dq, s);
-    if (e != cudaSuccess) return cuda_fail(e, "bwd_input launch");
-    return ok();
+    return bwd_input_impl(4, cfg, N, xyz, xyz_stride, t, t_stride, index, table, dout, dq, workspace,
+                          workspace_bytes, cuda_stream);
+}
+
+DASH_API int dash_hash3d_bwd_input(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
+                                   uint32_t xyz_stride, const int32_t* index, const void* table,
+                                   const float* dout, float* dq, void* workspace, size_t workspace_bytes,
+                                   void* cuda_stream) {
+    return bwd_input_impl(3, cfg, N, xyz, xyz_stride, nullptr, 0, index, table, dout, dq, workspace,
+                          workspace_bytes, cuda_stream);
 }
 
 DASH_API int dash_hash4d_smooth(const dash_hash4d_config* cfg, uint64_t N, const float* xyz,

@@ -199,55 +199,60 @@ hash4d_bwd_fixed_kernel(const __grid_constant__ Plan P, const float* __restrict_
 // interpolated value and the difference along the folded axis, so each axis derivative costs one
 // extra subtraction per fold instead of a second pass over the 16 corners.
 // ------------------------------------------------------------------------------------------------
-template <int F, bool HALF>
+template <int F, bool HALF, int D>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_bwd_input_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                         const float* __restrict__ t, const int32_t* __restrict__ index,
                         const void* __restrict__ table, const float* __restrict__ dout,
                         float* __restrict__ dq) {
+    constexpr int NC = 1 << (D - 1);   // D = 3: G_3D, 4 (y,z) corners per lane, dq is [N][3]
     const Item it = this_item(P);
     const LevelParams lp = P.lv[it.l];
     float g[F];
     load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F,
                  it.xc, g);
-    const Query q = load_query(P, lp, it.n, xyz, t, index);
-    uint32_t slot[8];
-    float W[8];
-    half_cell(P, lp, q, it.xc, slot, W);  // W unused here; slots shared with fwd
+    const Query q = load_query<D>(P, lp, it.n, xyz, t, index);
+    uint32_t slot[NC];
+    float W[NC];
+    half_cell<D>(P, lp, q, it.xc, slot, W);  // W unused here; slots shared with fwd
     constexpr size_t kElem = HALF ? 2 : 4;
     const char* level_base =
         static_cast<const char*>(table) + static_cast<size_t>(it.l) * P.T * (F * kElem);
-    float v[8][F];
+    float v[NC][F];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);
-    float S[8];
+    for (int j = 0; j < NC; ++j) load_slot<F, HALF>(level_base, slot[j], v[j]);
+    float S[NC];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < NC; ++j) {
         S[j] = 0.0f;
 #pragma unroll
         for (int f = 0; f < F; ++f) S[j] = fmaf(g[f], v[j][f], S[j]);
     }
     const float wy = q.w[1], wz = q.w[2], wt = q.w[3];
-    // fold y (corner bit 0): value and d/dy for the 4 (z,t) combinations
-    float a[4], ay[4];
+    // fold y (corner bit 0): value and d/dy for the NC/2 (z[,t]) combinations
+    float a[NC / 2], ay[NC / 2];
 #pragma unroll
-    for (int m = 0; m < 4; ++m) {
+    for (int m = 0; m < NC / 2; ++m) {
         ay[m] = S[2 * m + 1] - S[2 * m];
         a[m] = fmaf(wy, ay[m], S[2 * m]);
     }
     // fold z (corner bit 1)
-    float b[2], by[2], bz[2];
+    float b[NC / 4], by[NC / 4], bz[NC / 4];
 #pragma unroll
-    for (int m = 0; m < 2; ++m) {
+    for (int m = 0; m < NC / 4; ++m) {
         bz[m] = a[2 * m + 1] - a[2 * m];
         b[m] = fmaf(wz, bz[m], a[2 * m]);
         by[m] = fmaf(wz, ay[2 * m + 1] - ay[2 * m], ay[2 * m]);
     }
-    // fold t (corner bit 2)
-    const float val = fmaf(wt, b[1] - b[0], b[0]);
-    const float dy = fmaf(wt, by[1] - by[0], by[0]);
-    const float dz = fmaf(wt, bz[1] - bz[0], bz[0]);
-    const float dt = b[1] - b[0];
+    float val, dy, dz, dt;
+    if constexpr (D == 4) {   // fold t (corner bit 2)
+        val = fmaf(wt, b[1] - b[0], b[0]);
+        dy = fmaf(wt, by[1] - by[0], by[0]);
+        dz = fmaf(wt, bz[1] - bz[0], bz[0]);
+        dt = b[1] - b[0];
+    } else {
+        val = b[0]; dy = by[0]; dz = bz[0]; dt = 0.0f;
+    }
     // this lane is x-corner xc: d/dx takes the sign, the other axes the x weight
     const float wx = it.xc ? q.w[0] : 1.0f - q.w[0];
     float d4[4] = {it.xc ? val : -val, wx * dy, wx * dz, wx * dt};
@@ -255,7 +260,7 @@ hash4d_bwd_input_kernel(const __grid_constant__ Plan P, const float* __restrict_
 #pragma unroll
     for (int d = 0; d < 4; ++d) {
         d4[d] *= scale[d];
-        if (!it.active || ((q.moved >> d) & 1u)) d4[d] = 0.0f;
+        if (!it.active || ((q.moved >> d) & 1u) || d >= D) d4[d] = 0.0f;
     }
     // sum the lane pair, then the G levels of this query that sit in this warp (2G adjacent lanes)
     const uint32_t span = 2u * P.group;
@@ -263,14 +268,20 @@ hash4d_bwd_input_kernel(const __grid_constant__ Plan P, const float* __restrict_
     for (uint32_t o = 1; o < 32; o <<= 1) {
         if (o < span) {
 #pragma unroll
-            for (int d = 0; d < 4; ++d) d4[d] += __shfl_xor_sync(0xffffffffu, d4[d], o);
+            for (int d = 0; d < D; ++d) d4[d] += __shfl_xor_sync(0xffffffffu, d4[d], o);
         }
     }
     if (it.active && (threadIdx.x & (span - 1u)) == 0) {
-        float* o = dq + it.n * 4;
-        asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(o), "f"(d4[0]),
-                     "f"(d4[1]), "f"(d4[2]), "f"(d4[3])
-                     : "memory");
+        if constexpr (D == 4) {
+            float* o = dq + it.n * 4;
+            asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(o), "f"(d4[0]),
+                         "f"(d4[1]), "f"(d4[2]), "f"(d4[3])
+                         : "memory");
+        } else {
+            float* o = dq + it.n * 3;   // rows of 12 bytes: scalar reductions
+#pragma unroll
+            for (int d = 0; d < 3; ++d) asm volatile("red.global.add.f32 [%0], %1;" ::"l"(o + d), "f"(d4[d]) : "memory");
+        }
     }
 }
 
@@ -789,8 +800,13 @@ cudaError_t launch_bwd_input(const Plan& P, const float* xyz, const float* t, co
                              const void* table, bool table_half, const float* dout, float* dq,
                              cudaStream_t s) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
-#define DASH_BWI(FV, HV) \
-    hash4d_bwd_input_kernel<FV, HV><<<grid, block, 0, s>>>(P, xyz, t, index, table, dout, dq)
+#define DASH_BWI(FV, HV)                                                                                \
+    do {                                                                                                \
+        if (P.dims == 3)                                                                                \
+            hash4d_bwd_input_kernel<FV, HV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, table, dout, dq); \
+        else                                                                                            \
+            hash4d_bwd_input_kernel<FV, HV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, table, dout, dq); \
+    } while (0)
     switch (P.F * 2 + (table_half ? 1 : 0)) {
         case 2: DASH_BWI(1, false); break;
         case 3: DASH_BWI(1, true); break;

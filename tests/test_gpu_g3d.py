@@ -152,3 +152,29 @@ def test_g3d_full_size_workload():
     ref_idx, _ = oracle.oracle3d_indices(ocfg, len(sel), np.ascontiguousarray(wl.xyz[sel]), want_weights=False)
     idx, _ = dh.dash_hash3d_indices(gcfg, dev(wl.xyz[sel]), want_weights=False)
     assert np.array_equal(idx.cpu().numpy().view(np.uint32), ref_idx)
+
+
+@pytest.mark.parametrize("L,F,T,rs,dtype,N", [v for v in VARIANTS if v[5] > 0])
+@pytest.mark.parametrize("group", [0, 1, 4])
+def test_g3d_coordinate_gradient_parity(L, F, T, rs, dtype, N, group, set_debug):
+    """dash_hash3d_bwd_input against oracle3d_bwd_input: |err| <= rtol * sum|terms| (rtol as the 4D call: 1e-5 fp32,
+    2e-3 fp16 tables), with edge points (vertices, clamped and NaN coordinates) and an index list."""
+    set_debug(dh.DEBUG_FWD_GROUP, group)
+    ocfg, gcfg = configs(L, F, T, rs, dtype)
+    rng = np.random.default_rng(L * 31 + F + N)
+    pts = make_points_clustered(L + F, N)
+    pts[:6] = [[0, 0, 0], [1, 1, 1], [0.5, 0.25, 0.75], [-1, 0.3, 2], [np.nan, 0.5, 0.5], [np.float32(1) - np.float32(2.0 ** -24)] * 3]
+    table = rng.uniform(-1, 1, (L, T, F)).astype(np.float16 if dtype == "fp16" else np.float32)
+    dout = rng.standard_normal((N, L * F)).astype(np.float32)
+    ref, mag = oracle.oracle3d_bwd_input(ocfg, N, pts, table, dout, want_abs=True)
+    dq = torch.full((N, 3), 7.0, device="cuda")                                # overwritten, not accumulated
+    dh.dash_hash3d_bwd_input(gcfg, dev(pts), dev(table), dev(dout), dq=dq)
+    torch.cuda.synchronize()
+    rtol = RTOL_FP16 if dtype == "fp16" else RTOL_FP32
+    err = np.abs(dq.cpu().numpy().astype(np.float64) - ref)
+    assert (err <= rtol * mag + 1e-30).all(), f"worst err/A {(err / (mag + 1e-300)).max():.3e}"
+    assert dq[3, 0] == 0 and dq[3, 2] == 0 and dq[4, 0] == 0                    # clamped / NaN coordinates
+    index = rng.integers(0, N, 500).astype(np.int32)
+    got = dh.dash_hash3d_bwd_input(gcfg, dev(pts), dev(table), dev(dout[:500].copy()), index=dev(index)).cpu().numpy()
+    ref_i, mag_i = oracle.oracle3d_bwd_input(ocfg, 500, pts, table, dout[:500].copy(), index=index, want_abs=True)
+    assert (np.abs(got - ref_i) <= rtol * mag_i + 1e-30).all()
