@@ -313,6 +313,22 @@ def oracle_deform(cfg, mcfg, N, xyz, t, table, params, base=None, index=None, t_
     return oracle_mlp(mcfg, feat, params, base=base, want_abs=want_abs)
 
 
+# ---- self-supervised decomposition (Eq. 5; Q31) ----
+
+def oracle_decompose(dp, k_percent, grad_scale=1.0, want_grad=True):
+    """dp [N][3] fp32 -> dict(mag [N] fp32, tau fp32, index (ascending int32 list of the dynamic Gaussians), loss (L_s,
+    float), ddp [N][3] fp32 or None)."""
+    assert dp.dtype == np.float32 and dp.flags.c_contiguous and dp.ndim == 2 and dp.shape[1] == 3
+    N = dp.shape[0]
+    mag = np.zeros(N, np.float32)
+    idx = np.zeros(max(N, 1), np.int32)
+    tau, nd, loss = C.c_float(0), C.c_uint64(0), C.c_double(0)
+    ddp = np.zeros((N, 3), np.float32) if want_grad else None
+    _check(lib().dash_oracle_decompose(C.c_uint64(N), _p(dp), C.c_double(k_percent), C.c_double(grad_scale), _p(mag),
+                                       C.byref(tau), _p(idx), C.byref(nd), C.byref(loss), _p(ddp)), "decompose")
+    return {"mag": mag, "tau": float(tau.value), "index": idx[:nd.value].copy(), "loss": float(loss.value), "ddp": ddp}
+
+
 # ---- sparse Adam over the touched table entries (SURVEY §8f NEXT #4; DESIGN.md Q28) ----
 
 def oracle_double_to_half(d: float) -> int:

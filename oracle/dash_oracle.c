@@ -936,6 +936,76 @@ int dash_oracle_mlp_bwd(const dash_oracle_mlp_config *m, uint64_t N, const float
     return ORACLE_OK;
 }
 
+/* ---- beyond §8f (Q31): self-supervised decomposition (Eq. 5) ----------------------
+ * "We compute motion magnitudes ||dp|| for all Gaussians and set a threshold tau at the top k% percentile of these
+ * values.  Gaussians with ||dp|| > tau are classified as dynamic, the rest as static.  Static Gaussians are constrained
+ * by L_s = (1/N_s) sum_{static} ||dp||."  Readings (Q31):
+ *   mag[n] = fl32 sqrt of fl32( fl32( fl32(x*x) + fl32(y*y) ) + fl32(z*z) ): binary32 throughout, no contraction (the
+ *            classification is a decision on this value, so both sides form it identically); a NaN magnitude counts as 0.
+ *   m      = ceil(N * k / 100 - 1e-9), clamped to [0, N]: the size of "the top k %".
+ *   tau    = the largest magnitude NOT among the m largest (the (m+1)-th largest); m = 0 -> +inf; m = N -> -1.
+ *   dynamic = { n : mag[n] > tau } in ascending n (what nonzero(mask) yields; at most m entries, fewer on ties at tau).
+ *   L_s    = sum over static n of mag[n] / N_s (double; 0 when N_s = 0).
+ *   ddp[n] = grad_scale * dp[n] / (mag[n] * N_s) for static n with mag[n] > 0, else 0  (d L_s / d dp; the
+ *            classification is held fixed, as any top-k selection is when differentiated). */
+static int cmp_desc_f32(const void *a, const void *b) {
+    float x = *(const float *)a, y = *(const float *)b;
+    return (x < y) - (x > y);
+}
+
+int dash_oracle_decompose(uint64_t N, const float *dp, double k_percent, double grad_scale, float *mag,
+                          float *tau_out, int32_t *dyn_index, uint64_t *n_dyn_out, double *loss_out,
+                          float *ddp) {
+    if (!mag || !tau_out || !dyn_index || !n_dyn_out || !loss_out) return ORACLE_INVALID;
+    if (!(k_percent >= 0.0 && k_percent <= 100.0)) return ORACLE_INVALID;
+    *n_dyn_out = 0;
+    *loss_out = 0.0;
+    *tau_out = INFINITY;
+    if (N == 0) return ORACLE_OK;
+    if (!dp) return ORACLE_INVALID;
+    for (uint64_t n = 0; n < N; ++n) {
+        volatile float xx = dp[n * 3 + 0] * dp[n * 3 + 0];
+        volatile float yy = dp[n * 3 + 1] * dp[n * 3 + 1];
+        volatile float zz = dp[n * 3 + 2] * dp[n * 3 + 2];
+        volatile float s = xx + yy;
+        s = s + zz;
+        float v = sqrtf(s);
+        mag[n] = isnan(v) ? 0.0f : v;
+    }
+    double md = ceil((double)N * k_percent / 100.0 - 1e-9);
+    uint64_t m = md <= 0.0 ? 0 : (md >= (double)N ? N : (uint64_t)md);
+    float tau;
+    if (m == 0) {
+        tau = INFINITY;
+    } else if (m >= N) {
+        tau = -1.0f;
+    } else {
+        float *sorted = (float *)malloc(sizeof(float) * N);
+        if (!sorted) return ORACLE_NOMEM;
+        memcpy(sorted, mag, sizeof(float) * N);
+        qsort(sorted, N, sizeof(float), cmp_desc_f32);
+        tau = sorted[m];
+        free(sorted);
+    }
+    *tau_out = tau;
+    uint64_t nd = 0;
+    double sum = 0.0;
+    for (uint64_t n = 0; n < N; ++n) {
+        if (mag[n] > tau) dyn_index[nd++] = (int32_t)n;
+        else sum += (double)mag[n];
+    }
+    const uint64_t ns = N - nd;
+    *n_dyn_out = nd;
+    *loss_out = ns ? sum / (double)ns : 0.0;
+    if (ddp)
+        for (uint64_t n = 0; n < N; ++n)
+            for (int d = 0; d < 3; ++d)
+                ddp[n * 3 + d] = (!(mag[n] > tau) && mag[n] > 0.0f)
+                                     ? (float)(grad_scale * (double)dp[n * 3 + d] / ((double)mag[n] * (double)ns))
+                                     : 0.0f;
+    return ORACLE_OK;
+}
+
 /* ---- NEXT #4: sparse optimiser step over the touched table entries -------------------
  * The paper does not name its optimiser ("primarily based on the PyTorch framework"; 3DGS [14]
  * and Instant-NGP [25], which it follows, both train with Adam).  Reading (Q28): Adam (Kingma & Ba),
