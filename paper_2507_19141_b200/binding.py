@@ -27,7 +27,8 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices", "dash_hash3d_bwd_input",
            "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_mlp_bwd", "dash_deform_bwd", "dash_deform_bwd_workspace_bytes", "dash_deform_workspace_bytes", "dash_deform_fwd",
            "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch",
-           "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_deform_slice_workspace_bytes"]
+           "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_deform_slice_workspace_bytes",
+           "dash_decompose_workspace_bytes", "dash_decompose"]
 
 
 class Hash4DError(RuntimeError):
@@ -64,6 +65,11 @@ class CeilingParams(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("kind", C.c_uint32), ("width", C.c_uint32), ("pattern", C.c_uint32),
                 ("footprint_bytes", C.c_uint64), ("grid", C.c_uint32), ("block", C.c_uint32),
                 ("dyn_smem", C.c_uint32), ("iters", C.c_uint32), ("seed", C.c_uint32), ("reserved", C.c_uint32)]
+
+
+class DecomposeResult(C.Structure):
+    """Mirror of `struct dash_decompose_result` (include/dash_decompose.h)."""
+    _fields_ = [("n_dynamic", C.c_uint32), ("n_static", C.c_uint32), ("tau", C.c_float), ("loss", C.c_float)]
 
 
 CEIL_COPY, CEIL_GATHER, CEIL_RED, CEIL_SMEM_ATOMIC, CEIL_TMA_GATHER, CEIL_SMEM_ATOMIC_U64 = range(6)
@@ -156,6 +162,10 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_hash4d_sort_workspace_bytes.restype = sz
     lib.dash_hash4d_sort_queries.argtypes = [u64, vp, u32, vp, u32, vp, vp, sz, vp]
     lib.dash_hash4d_sort_queries.restype = C.c_int
+    lib.dash_decompose_workspace_bytes.argtypes = [u64]
+    lib.dash_decompose_workspace_bytes.restype = sz
+    lib.dash_decompose.argtypes = [u64, vp, C.c_double, C.c_float, vp, vp, vp, vp, vp, sz, vp]
+    lib.dash_decompose.restype = C.c_int
     lib.dash_ceiling_launch.argtypes = [C.POINTER(CeilingParams), vp, vp, C.POINTER(C.c_uint64), vp]
     lib.dash_ceiling_launch.restype = C.c_int
     lib.dash_hash4d_build_id.argtypes = []
@@ -817,3 +827,34 @@ def dash_ceiling_launch(kind, buf, sink, width=8, pattern=CEIL_INDEPENDENT, foot
     if rc != 0:
         raise Hash4DError(rc, "dash_ceiling_launch: bad parameters or launch failure")
     return int(ops.value)
+
+
+# ---- self-supervised decomposition (include/dash_decompose.h; Eq. 5) -------------------------
+
+def dash_decompose(dp, k_percent, grad_scale=1.0, want_grad=True, workspace=None):
+    """dp [N][3] CUDA fp32 -> dict(mag [N], index (the whole [N] int32 buffer; the first n_dynamic entries are valid),
+    result (4 x 32-bit CUDA tensor viewed as uint8: n_dynamic, n_static, tau, loss), ddp [N][3] or None).  Nothing is
+    synchronised: read `result` with `dash_decompose_read(result)` when the counts are needed on the host."""
+    _dev(dp, torch.float32, "dp")
+    if dp.dim() != 2 or dp.shape[1] != 3:
+        raise ValueError("dp must be [N][3]")
+    N = int(dp.shape[0])
+    dev = dp.device
+    mag = torch.empty((N,), dtype=torch.float32, device=dev)
+    index = torch.empty((max(N, 1),), dtype=torch.int32, device=dev)
+    result = torch.zeros(C.sizeof(DecomposeResult), dtype=torch.uint8, device=dev)
+    ddp = torch.empty((N, 3), dtype=torch.float32, device=dev) if want_grad else None
+    need = int(_load().dash_decompose_workspace_bytes(N))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=dev)
+    _one_device(dp, workspace)
+    rc = _load().dash_decompose(N, _ptr(dp), float(k_percent), float(grad_scale), _ptr(mag), _ptr(index), _ptr(result),
+                                _ptr(ddp), _ptr(workspace), workspace.numel(), _stream())
+    if rc != 0:
+        raise Hash4DError(rc, "dash_decompose: bad arguments, workspace too small or launch failure")
+    return {"mag": mag, "index": index, "result": result, "ddp": ddp}
+
+
+def dash_decompose_read(result: torch.Tensor) -> DecomposeResult:
+    """Copy the 16-byte result to the host (synchronises)."""
+    return DecomposeResult.from_buffer_copy(bytes(result.cpu().numpy().tobytes()))
