@@ -462,6 +462,15 @@ static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
         if (e != cudaSuccess) return cuda_fail(e, "bwd launch");
         return ok();
     }
+    // ZERO_GRAD, small tables: when the WHOLE gradient buffer fits the L2 budget there is nothing to keep resident group
+    // by group — one zero launch and one scatter launch over all groups (C2: 2 launches instead of 4).
+    if (level_bytes * cfg->L <= l2_bytes() * 3 / 10) {
+        const bool hint = debug_u32(DASH_DEBUG_BWD_VARIANT) != 1;
+        e = dash::launch_zero(dtable, level_bytes * cfg->L, s, hint);
+        if (e == cudaSuccess) e = dash::launch_bwd(P, xyz, t, index, dout, dtable, s, hint);
+        if (e != cudaSuccess) return cuda_fail(e, "bwd launch");
+        return ok();
+    }
     // ZERO_GRAD: zero one level group, scatter into it while the zeros are still in L2, next group.
     // (A one-launch variant whose tail CTAs zero the next group's slice was built and measured in round 2: slower,
     // profiles/experiments_r02.md §1.)
