@@ -15,9 +15,10 @@
 //   wgrad           D[M = j (128 lanes, rows >= J_l unused)][N = kpad_l] accumulates in tensor memory
 //                   across ALL tiles of the CTA (lane j, column k <-> dW_l[j][k]; the "ones" column of a_{l-1} makes
 //                   column kbias_l the bias gradient); one flush of fp32 reductions per CTA at the end.
-//   roles           warps 0-3: one elected lane of warp 0 issues the MMAs; all four run the epilogues (TMEM lane
-//                   quarter = warp).  warps 4-7: load the next tile's features (-> a_0, double buffered) and dout
-//                   (-> delta_n) as bf16 while the current tile computes.
+//   roles           warps 0-3: the epilogues (TMEM lane quarter = warp).  warp 4: one elected lane issues every MMA, so
+//                   that no epilogue warp spends its time in the issue loop (the wgrad MMAs are issued while the
+//                   epilogue of the dgrad before them already runs).  warps 5-7: load the next tile's features
+//                   (-> a_0, double buffered) and dout (-> delta_n) as bf16 while the current tile computes.
 // The dgrad of a layer is issued before its wgrad and committed alone, so the epilogue that forms delta_{l-1} runs
 // while the wgrad MMAs of layer l execute (they read delta_l, the epilogue writes the other ping-pong buffer).
 #include <cuda_bf16.h>
@@ -30,7 +31,7 @@ namespace dash {
 
 namespace {
 
-constexpr uint32_t kBwdComputeThreads = 128, kBwdLoaderThreads = 128;
+constexpr uint32_t kBwdComputeThreads = 128, kBwdLoaderThreads = 96;   // warps 0-3 | warp 4 issues | warps 5-7 load
 constexpr uint32_t kTileLbo = kDeformTileM * 16u + 16u;   // operand_lbo(128)
 
 // kind::f16 instruction descriptor with selectable major-ness: bit 15 = A is MN-major, bit 16 = B is MN-major
@@ -156,9 +157,9 @@ mlp_bwd_kernel(const __grid_constant__ MlpBwdPlan B, const float* __restrict__ f
         r_begin < r_end ? static_cast<uint32_t>((r_end - r_begin + kDeformTileM - 1) / kDeformTileM) : 0u;
     const uint32_t n_out = M.n_out;
 
-    if (warp >= 4) {
+    if (warp >= 5) {
         // ============================================================================================ LOADERS
-        const uint32_t lt = tid - kBwdComputeThreads;
+        const uint32_t lt = tid - kBwdComputeThreads - 32u;
         const uint32_t K0 = M.width[0], chunks0 = M.kbias[0] >> 3, chunksn = M.npad[nl - 1] >> 3;
         for (uint32_t i = 0; i < my_tiles; ++i) {
             const uint32_t s = i & 1u;
@@ -195,32 +196,73 @@ mlp_bwd_kernel(const __grid_constant__ MlpBwdPlan B, const float* __restrict__ f
             fence_async_smem();
             mbar_arrive(bar_full_dn);
         }
+    } else if (warp == 4) {
+        // ============================================================================================ MMA ISSUE
+        // Mirrors the epilogue warps' step sequence; after issuing the MMAs of a step it waits (named barrier 1, 160
+        // threads) until their epilogue has consumed the accumulator and written its tile.
+        const uint32_t acc = tmem_base + B.acc_col;
+        for (uint32_t i = 0; i < my_tiles; ++i) {
+            const uint32_t s = i & 1u;
+            const uint32_t a0 = sb + B.a_off[0] + s * B.a0_bytes;
+            for (uint32_t l = 0; l + 1 < nl; ++l) {   // forward recompute
+                if (l == 0) mbar_wait(bar_full_a0 + 8 * s, (i >> 1) & 1u);
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t a_addr = l == 0 ? a0 : sb + B.a_off[l];
+                    const uint32_t w_addr = sb + B.w_off[l], np = M.npad[l], w_lbo = operand_lbo(np);
+                    const uint32_t idesc = umma_idesc(np);
+                    for (uint32_t kk = 0; kk < (M.kpad[l] >> 4); ++kk)
+                        tc_mma_bf16(acc, umma_desc(a_addr + kk * 2u * kTileLbo, kTileLbo, 128u),
+                                    umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u), idesc, kk > 0 ? 1u : 0u);
+                    tc_commit(bar_mma);
+                }
+                __syncwarp();
+                asm volatile("bar.sync 1, 160;" ::: "memory");
+            }
+            for (int l = static_cast<int>(nl) - 1; l >= 0; --l) {   // backward
+                const bool last = l == static_cast<int>(nl) - 1;
+                const uint32_t dsrc = last ? sb + B.dn_off : sb + B.d_off[(l + 1) & 1];   // delta of this layer's output
+                const bool need_dgrad = l > 0 || dfeat != nullptr;
+                if (last) mbar_wait(bar_full_dn, i & 1u);
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t w_lbo = operand_lbo(M.npad[l]);
+                    if (need_dgrad) {   // g = delta W_l: contraction over the layer's outputs j (K-major A, MN-major B)
+                        const uint32_t idesc = umma_idesc_mn(M.kbias[l], false, true);
+                        for (uint32_t kk = 0; kk < (M.npad[l] >> 4); ++kk)
+                            tc_mma_bf16(acc, umma_desc(dsrc + kk * 2u * kTileLbo, kTileLbo, 128u),
+                                        umma_desc_mn(sb + B.w_off[l] + kk * 256u, w_lbo), idesc, kk > 0 ? 1u : 0u);
+                    }
+                    tc_commit(bar_mma);   // the dgrad alone (and everything before it): its epilogue may start
+                    // dW_l (+)= delta^T a_l: contraction over the 128 rows (both operands MN-major); accumulates over
+                    // all tiles of this CTA
+                    const uint32_t a_l = l == 0 ? a0 : sb + B.a_off[l];
+                    const uint32_t idesc_w = umma_idesc_mn(M.kpad[l], true, true);
+                    for (uint32_t kk = 0; kk < kDeformTileM / 16u; ++kk)
+                        tc_mma_bf16(tmem_base + B.dw_col[l], umma_desc_mn(dsrc + kk * 256u, kTileLbo),
+                                    umma_desc_mn(a_l + kk * 256u, kTileLbo), idesc_w, (i > 0 || kk > 0) ? 1u : 0u);
+                    if (last) tc_commit(bar_empty_dn);            // delta_n consumed (dgrad + wgrad of layer n)
+                    if (l == 0) tc_commit(bar_empty_a0 + 8 * s);  // a_0 consumed (forward + wgrad of layer 1)
+                }
+                __syncwarp();
+                asm volatile("bar.sync 1, 160;" ::: "memory");
+            }
+        }
+        if (my_tiles > 0) {
+            tc_fence_after();
+            if (elect_one()) tc_commit(bar_mma);   // covers the last wgrad MMAs: the flush may read the accumulators
+            __syncwarp();
+        }
     } else {
-        // ============================================================================================ COMPUTE
+        // ============================================================================================ EPILOGUES
         const uint32_t r = warp * 32u + lane;              // row of the tile = TMEM lane this thread reads
         const uint32_t lane_off = (warp * 32u) << 16;
         const uint32_t acc = tmem_base + B.acc_col;
         uint32_t mma_phase = 0;
         for (uint32_t i = 0; i < my_tiles; ++i) {
-            const uint32_t s = i & 1u;
-            const uint32_t a0 = sb + B.a_off[0] + s * B.a0_bytes;
             const uint64_t n = r_begin + static_cast<uint64_t>(i) * kDeformTileM + r;
             // ---------------------------------------------------------------- forward recompute: a_1 .. a_{n-1}
             for (uint32_t l = 0; l + 1 < nl; ++l) {
-                if (warp == 0) {
-                    if (l == 0) mbar_wait(bar_full_a0 + 8 * s, (i >> 1) & 1u);
-                    tc_fence_after();
-                    if (elect_one()) {
-                        const uint32_t a_addr = l == 0 ? a0 : sb + B.a_off[l];
-                        const uint32_t w_addr = sb + B.w_off[l], np = M.npad[l], w_lbo = operand_lbo(np);
-                        const uint32_t idesc = umma_idesc(np);
-                        for (uint32_t kk = 0; kk < (M.kpad[l] >> 4); ++kk)
-                            tc_mma_bf16(acc, umma_desc(a_addr + kk * 2u * kTileLbo, kTileLbo, 128u),
-                                        umma_desc(w_addr + kk * 2u * w_lbo, w_lbo, 128u), idesc, kk > 0 ? 1u : 0u);
-                        tc_commit(bar_mma);
-                    }
-                    __syncwarp();
-                }
                 mbar_wait(bar_mma, mma_phase);
                 mma_phase ^= 1u;
                 __syncwarp();
@@ -241,37 +283,10 @@ mlp_bwd_kernel(const __grid_constant__ MlpBwdPlan B, const float* __restrict__ f
                 }
                 fence_async_smem();
                 tc_fence_before();
-                asm volatile("bar.sync 1, 128;" ::: "memory");
+                asm volatile("bar.sync 1, 160;" ::: "memory");
             }
             // ---------------------------------------------------------------- backward: layers n .. 1 (l = n-1 .. 0)
             for (int l = static_cast<int>(nl) - 1; l >= 0; --l) {
-                const bool last = l == static_cast<int>(nl) - 1;
-                const uint32_t dsrc = last ? sb + B.dn_off : sb + B.d_off[(l + 1) & 1];   // delta of this layer's output
-                const bool need_dgrad = l > 0 || dfeat != nullptr;
-                if (warp == 0) {
-                    if (last) mbar_wait(bar_full_dn, i & 1u);
-                    tc_fence_after();
-                    if (elect_one()) {
-                        const uint32_t w_lbo = operand_lbo(M.npad[l]);
-                        if (need_dgrad) {   // g = delta W_l: contraction over the layer's outputs j (K-major A, MN-major B)
-                            const uint32_t idesc = umma_idesc_mn(M.kbias[l], false, true);
-                            for (uint32_t kk = 0; kk < (M.npad[l] >> 4); ++kk)
-                                tc_mma_bf16(acc, umma_desc(dsrc + kk * 2u * kTileLbo, kTileLbo, 128u),
-                                            umma_desc_mn(sb + B.w_off[l] + kk * 256u, w_lbo), idesc, kk > 0 ? 1u : 0u);
-                        }
-                        tc_commit(bar_mma);   // the dgrad alone (and everything before it): the epilogue may start
-                        // dW_l (+)= delta^T a_l: contraction over the 128 rows (both operands MN-major); accumulates
-                        // over all tiles of this CTA
-                        const uint32_t a_l = l == 0 ? a0 : sb + B.a_off[l];
-                        const uint32_t idesc_w = umma_idesc_mn(M.kpad[l], true, true);
-                        for (uint32_t kk = 0; kk < kDeformTileM / 16u; ++kk)
-                            tc_mma_bf16(tmem_base + B.dw_col[l], umma_desc_mn(dsrc + kk * 256u, kTileLbo),
-                                        umma_desc_mn(a_l + kk * 256u, kTileLbo), idesc_w, (i > 0 || kk > 0) ? 1u : 0u);
-                        if (last) tc_commit(bar_empty_dn);            // delta_n consumed (dgrad + wgrad of layer n)
-                        if (l == 0) tc_commit(bar_empty_a0 + 8 * s);  // a_0 consumed (forward + wgrad of layer 1)
-                    }
-                    __syncwarp();
-                }
                 mbar_wait(bar_mma, mma_phase);
                 mma_phase ^= 1u;
                 __syncwarp();
@@ -319,16 +334,11 @@ mlp_bwd_kernel(const __grid_constant__ MlpBwdPlan B, const float* __restrict__ f
                     }
                 }
                 tc_fence_before();
-                asm volatile("bar.sync 1, 128;" ::: "memory");
+                asm volatile("bar.sync 1, 160;" ::: "memory");
             }
         }
         // ---------------------------------------------------------------- flush the wgrad accumulators
         if (my_tiles > 0) {
-            if (warp == 0) {
-                tc_fence_after();
-                if (elect_one()) tc_commit(bar_mma);   // covers the last wgrad MMAs
-                __syncwarp();
-            }
             mbar_wait(bar_mma, mma_phase);
             __syncwarp();
             tc_fence_after();
