@@ -204,3 +204,65 @@ def test_deform_bwd_errors():
         dh.dash_deform_bwd(cfg, dh.make_mlp_config([16, 10]), z(5, 3), z(5), z(4, 1 << 10, 2), z(170), z(5, 10),
                            z(4, 1 << 10, 2), z(170))
     assert e.value.status == 1
+
+
+def test_training_calls_are_cuda_graph_capturable():
+    """dash_deform_bwd (four composed launches), dash_mlp_bwd and the C ABI of dash_decompose only enqueue kernels on the
+    current stream: a captured training step replays and gives the directly launched results (the index list, counts
+    and dfeat bit for bit; the reductions to their rounding)."""
+    import ctypes as C
+    L, F, T, n = 8, 2, 1 << 12, 6000
+    enc = EncoderParams(L, F, T, 8, 200, 4, 30)
+    cfg = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE | dh.FLAG_ZERO_GRAD)
+    widths = [L * F, 64, 10]
+    m = dh.make_mlp_config(widths)
+    rng = np.random.default_rng(3)
+    xyz, t = make_queries_uniform(5, n)
+    xd, td = dev(xyz), dev(t)
+    table = dev(rng.uniform(-1, 1, (L, T, F)).astype(np.float32))
+    prm = dev(make_mlp_params(2, widths)); dout = dev(rng.standard_normal((n, 10)).astype(np.float32))
+    feat = dev(rng.standard_normal((n, L * F)).astype(np.float32))
+    dtable = torch.empty((L, T, F), device="cuda"); dparams = torch.zeros(prm.numel(), device="cuda")
+    dq = torch.empty((n, 4), device="cuda"); dfeat = torch.empty((n, L * F), device="cuda")
+    dp2 = torch.zeros_like(dparams)
+    ws = torch.empty(dh.binding._load().dash_deform_bwd_workspace_bytes(C.byref(cfg), C.byref(m), n) + 16,
+                     dtype=torch.uint8, device="cuda")
+    mot = dev(rng.standard_normal((n, 3)).astype(np.float32))
+    lib = dh.binding._load()
+    mag = torch.empty(n, device="cuda"); idx = torch.empty(n, dtype=torch.int32, device="cuda")
+    res = torch.zeros(16, dtype=torch.uint8, device="cuda"); ddp = torch.empty((n, 3), device="cuda")
+    wsd = torch.empty(lib.dash_decompose_workspace_bytes(n) + 16, dtype=torch.uint8, device="cuda")
+
+    def step():
+        dparams.zero_(); dp2.zero_()
+        dh.dash_deform_bwd(cfg, m, xd, td, table, prm, dout, dtable, dparams, dq=dq, workspace=ws)
+        dh.dash_mlp_bwd(m, feat, prm, dout, dp2, dfeat=dfeat)
+        rc = lib.dash_decompose(n, C.c_void_p(mot.data_ptr()), 30.0, 1.0, C.c_void_p(mag.data_ptr()),
+                                C.c_void_p(idx.data_ptr()), C.c_void_p(res.data_ptr()), C.c_void_p(ddp.data_ptr()),
+                                C.c_void_p(wsd.data_ptr()), wsd.numel(), C.c_void_p(torch.cuda.current_stream().cuda_stream))
+        assert rc == 0
+
+    step()
+    torch.cuda.synchronize()
+    want = [a.clone() for a in (dtable, dparams, dq, dfeat, dp2, idx, res, ddp)]
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()
+    torch.cuda.current_stream().wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        step()
+    for a in (dtable, dq, dfeat, ddp):
+        a.fill_(-1)
+    idx.fill_(-1); res.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    nd = dh.dash_decompose_read(res).n_dynamic
+    assert nd == dh.dash_decompose_read(want[6]).n_dynamic == 1800
+    assert torch.equal(idx[:nd], want[5][:nd]) and torch.equal(res, want[6]) and torch.equal(ddp, want[7])
+    assert torch.equal(dfeat, want[3])                       # no reductions on this path: bit for bit
+    torch.testing.assert_close(dp2, want[4], rtol=1e-5, atol=1e-5)
+    torch.testing.assert_close(dparams, want[1], rtol=1e-5, atol=1e-5)
+    torch.testing.assert_close(dtable, want[0], rtol=1e-4, atol=1e-5)
+    torch.testing.assert_close(dq, want[2], rtol=1e-4, atol=1e-4)
