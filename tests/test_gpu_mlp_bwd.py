@@ -103,7 +103,7 @@ def test_mlp_bwd_without_dfeat_and_twice_accumulates():
     assert none is None
     once = dp.cpu().numpy().copy()
     dh.dash_mlp_bwd(m, dev(feat), dev(params), dev(dout), dp, want_dfeat=False)
-    np.testing.assert_allclose(dp.cpu().numpy(), 2 * once, rtol=1e-6, atol=1e-6)
+    np.testing.assert_allclose(dp.cpu().numpy(), 2 * once, rtol=1e-4, atol=2e-4)
     _, pq = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout)
     assert np.linalg.norm(once - pq) / np.linalg.norm(pq) <= 4e-3
 
@@ -175,7 +175,7 @@ def test_deform_bwd_is_the_composition_and_matches_the_oracle(dtype, with_index,
     dt2 = torch.zeros((L, T, F), device="cuda")
     dh.dash_hash4d_bwd(plain, xd, td, dfeat, dt2, index=idx)
     dq2 = dh.dash_hash4d_bwd_input(plain, xd, td, tabd, dfeat, index=idx)
-    torch.testing.assert_close(dparams, dp2, rtol=1e-5, atol=1e-5)          # fp32 reductions in a different order
+    torch.testing.assert_close(dparams, dp2, rtol=1e-4, atol=2e-4)          # fp32 reductions in a different order
     torch.testing.assert_close(dtable, dt2, rtol=1e-4, atol=1e-5)
     torch.testing.assert_close(dq, dq2, rtol=1e-4, atol=1e-4)
     # (2) dparams against the oracle chain
@@ -262,7 +262,8 @@ def test_training_calls_are_cuda_graph_capturable():
     assert nd == dh.dash_decompose_read(want[6]).n_dynamic == 1800
     assert torch.equal(idx[:nd], want[5][:nd]) and torch.equal(res, want[6]) and torch.equal(ddp, want[7])
     assert torch.equal(dfeat, want[3])                       # no reductions on this path: bit for bit
-    torch.testing.assert_close(dp2, want[4], rtol=1e-5, atol=1e-5)
-    torch.testing.assert_close(dparams, want[1], rtol=1e-5, atol=1e-5)
+    # fp32 reductions across CTAs land in another order: entries are sums of 6,000 O(1) terms that partly cancel
+    torch.testing.assert_close(dp2, want[4], rtol=1e-4, atol=2e-4)
+    torch.testing.assert_close(dparams, want[1], rtol=1e-4, atol=2e-4)
     torch.testing.assert_close(dtable, want[0], rtol=1e-4, atol=1e-5)
     torch.testing.assert_close(dq, want[2], rtol=1e-4, atol=1e-4)
