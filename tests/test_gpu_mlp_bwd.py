@@ -267,3 +267,18 @@ def test_training_calls_are_cuda_graph_capturable():
     torch.testing.assert_close(dparams, want[1], rtol=1e-4, atol=2e-4)
     torch.testing.assert_close(dtable, want[0], rtol=1e-4, atol=1e-5)
     torch.testing.assert_close(dq, want[2], rtol=1e-4, atol=1e-4)
+
+
+def test_one_layer_without_dfeat_issues_no_dgrad_at_all():
+    """n_layers = 1 and dfeat = NULL: the kernel's only MMAs are the wgrad; its per-step commit then tracks nothing."""
+    widths, N = [32, 10], 2000
+    rng = np.random.default_rng(8)
+    feat = rng.standard_normal((N, 32)).astype(np.float32)
+    params = make_mlp_params(8, widths)
+    dout = rng.standard_normal((N, 10)).astype(np.float32)
+    dp = torch.zeros(params.size, device="cuda")
+    none, dp = dh.dash_mlp_bwd(dh.make_mlp_config(widths), dev(feat), dev(params), dev(dout), dp, want_dfeat=False)
+    torch.cuda.synchronize()
+    _, pq, _, pa, _ = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout,
+                                            want_abs=True)
+    assert none is None and (np.abs(dp.cpu().numpy() - pq) <= N * 2.0 ** -24 * pa + 1e-30).all()
