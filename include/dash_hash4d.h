@@ -274,7 +274,7 @@ enum dash_debug_key {
     DASH_DEBUG_SMOOTH_GROUP = 2, /* ... of smooth */
     DASH_DEBUG_DEFORM_PATH = 3,  /* dash_deform_fwd: 1 = fused kernel, 2 = two-pass (encoder -> workspace -> MLP) */
     DASH_DEBUG_BWD_VARIANT = 4,  /* bwd with ZERO_GRAD: 1 = no L2 eviction hints on the zero stores / reductions */
-    DASH_DEBUG_FWD_VARIANT = 5,  /* fwd gather variant (0 = default) */
+    DASH_DEBUG_FWD_VARIANT = 5,  /* reserved (0) */
     DASH_DEBUG_KEY_COUNT = 6
 };
 DASH_API int dash_hash4d_set_debug(int key, int64_t value);

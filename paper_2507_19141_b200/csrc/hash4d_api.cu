@@ -734,8 +734,7 @@ DASH_API int dash_mlp_fwd(const dash_mlp_config* mlp, uint64_t N, const float* f
     if ((reinterpret_cast<uintptr_t>(feat) | reinterpret_cast<uintptr_t>(params) |
          reinterpret_cast<uintptr_t>(base) | reinterpret_cast<uintptr_t>(out)) & 3u)
         return fail(DASH_HASH4D_INVALID_ARG, "feat / params / base / out not 4-byte aligned");
-    cudaError_t e = dash::launch_mlp(M, feat, params, base, out, dash::device_sm_count(),
-                                     static_cast<cudaStream_t>(cuda_stream));
+    cudaError_t e = dash::launch_mlp(M, feat, params, base, out, dash::device_sm_count(), static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return cuda_fail(e, "mlp launch");
     return ok();
 }
@@ -1008,8 +1007,7 @@ DASH_API int dash_deform_slice_fwd(const dash_hash4d_config* enc, const dash_mlp
         if (!aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
         float* feat = static_cast<float*>(workspace);
         if (int rc = dash_hash4d_slice_fwd(enc, N, xyz, xyz_stride, index, slice, feat, cuda_stream)) return rc;
-        cudaError_t e2 = dash::launch_mlp(M, feat, params, base, out, dash::device_sm_count(),
-                                          static_cast<cudaStream_t>(cuda_stream));
+        cudaError_t e2 = dash::launch_mlp(M, feat, params, base, out, dash::device_sm_count(), static_cast<cudaStream_t>(cuda_stream));
         if (e2 != cudaSuccess) return cuda_fail(e2, "mlp launch");
         return ok();
     }

@@ -96,41 +96,9 @@ mlp_bwd_kernel(const __grid_constant__ MlpBwdPlan B, const float* __restrict__ f
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     // weights -> bf16 operand copies, exactly as the forward stages them (bias as bf16 hi + lo in columns kb, kb+1)
-    for (uint32_t l = 0; l < nl; ++l) {
-        const uint32_t K = M.width[l], J = M.width[l + 1], kp = M.kpad[l], np = M.npad[l], kb = M.kbias[l];
-        const float* W = params + M.p_off[l];
-        const float* b = W + static_cast<size_t>(J) * K;
-        unsigned char* ws = smem + B.w_off[l];
-        const uint32_t cpr = kp >> 3, w_lbo = operand_lbo(np);
-        const bool vec = (K & 7u) == 0 && (reinterpret_cast<uintptr_t>(W) & 15u) == 0;  // float4 row chunks
-        for (uint32_t i = tid; i < np * cpr; i += kMlpBwdThreads) {
-            const uint32_t j = i / cpr, c = i - j * cpr, k0 = c * 8u;
-            float w[8];
-#pragma unroll
-            for (int e = 0; e < 8; ++e) w[e] = 0.0f;
-            if (j < J) {
-                if (k0 < kb) {
-                    const float* src = W + static_cast<size_t>(j) * K + k0;
-                    if (vec && k0 + 8u <= K) {
-                        const float4 lo = __ldg(reinterpret_cast<const float4*>(src));
-                        const float4 hi = __ldg(reinterpret_cast<const float4*>(src) + 1);
-                        w[0] = lo.x; w[1] = lo.y; w[2] = lo.z; w[3] = lo.w;
-                        w[4] = hi.x; w[5] = hi.y; w[6] = hi.z; w[7] = hi.w;
-                    } else {
-#pragma unroll
-                        for (int e = 0; e < 8; ++e)
-                            if (k0 + e < K) w[e] = __ldg(src + e);
-                    }
-                } else if (k0 == kb) {
-                    const float bj = __ldg(b + j);
-                    w[0] = __bfloat162float(__float2bfloat16_rn(bj));
-                    w[1] = bj - w[0];
-                }
-            }
-            *reinterpret_cast<uint4*>(ws + c * w_lbo + j * 16u) =
-                make_uint4(pack_bf16(w[0], w[1]), pack_bf16(w[2], w[3]), pack_bf16(w[4], w[5]), pack_bf16(w[6], w[7]));
-        }
-    }
+    for (uint32_t l = 0; l < nl; ++l)
+        stage_weights_bf16(params + M.p_off[l], M.width[l], M.width[l + 1], M.kpad[l], M.npad[l], M.kbias[l],
+                           smem + B.w_off[l], tid, kMlpBwdThreads);
     // activation tiles: zeros, (1, 1) in the chunk behind the data columns (bias column of the forward, bias
     // gradient of the wgrad); a_0 has two buffers.  delta tiles: zeros (columns an epilogue never writes stay 0).
     for (uint32_t l = 0; l < nl; ++l) {

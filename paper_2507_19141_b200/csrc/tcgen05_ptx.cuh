@@ -189,5 +189,61 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 }
 
 
+// W_l (fp32, row-major [J][K], bias behind it) -> the bf16 B operand [npad][kpad] of layer l in shared memory: one
+// 16-byte chunk (8 consecutive k of one output row j) per step at chunk * LBO + j * 16, LBO = npad*16 + 16; columns
+// kb, kb+1 carry the bias as bf16 hi + lo (the A operand has 1.0 there).  Each thread takes up to four chunks per batch
+// and issues ALL their global loads before converting any: one L2 round trip per batch instead of one per chunk (the
+// one-chunk-at-a-time loop cost 5-6K cycles per CTA, 10 % of dash_mlp_fwd at N = 300k).
+__device__ __forceinline__ void stage_weights_bf16(const float* __restrict__ W, uint32_t K, uint32_t J, uint32_t kp,
+                                                   uint32_t np, uint32_t kb, unsigned char* ws, uint32_t first,
+                                                   uint32_t nthreads) {
+    const float* b = W + static_cast<size_t>(J) * K;
+    const uint32_t cpr = kp >> 3, w_lbo = operand_lbo(np), total = np * cpr;
+    const bool vec = (K & 7u) == 0 && (reinterpret_cast<uintptr_t>(W) & 15u) == 0;  // float4 row chunks
+    for (uint32_t i0 = first; i0 < total; i0 += 4u * nthreads) {
+        float w[4][8];
+        uint32_t dst[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t i = i0 + u * nthreads;
+            const uint32_t ii = i < total ? i : i0;
+            const uint32_t j = ii / cpr, c = ii - j * cpr, k0 = c * 8u;
+            dst[u] = c * w_lbo + j * 16u;
+#pragma unroll
+            for (int e = 0; e < 8; ++e) w[u][e] = 0.0f;
+            if (j < J) {
+                const float* src = W + static_cast<size_t>(j) * K + k0;
+                if (k0 < kb) {
+                    if (vec && k0 + 8u <= K) {
+                        const float4 lo = __ldg(reinterpret_cast<const float4*>(src));
+                        const float4 hi = __ldg(reinterpret_cast<const float4*>(src) + 1);
+                        w[u][0] = lo.x; w[u][1] = lo.y; w[u][2] = lo.z; w[u][3] = lo.w;
+                        w[u][4] = hi.x; w[u][5] = hi.y; w[u][6] = hi.z; w[u][7] = hi.w;
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 8; ++e)
+                            if (k0 + e < K) w[u][e] = __ldg(src + e);
+                    }
+                } else if (k0 == kb) {
+                    w[u][0] = __ldg(b + j);   // split into hi + lo below
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t i = i0 + u * nthreads;
+            if (i >= total) continue;
+            const uint32_t j = i / cpr, c = i - j * cpr;
+            if (c * 8u == kb && j < J) {
+                const float bj = w[u][0];
+                w[u][0] = __bfloat162float(__float2bfloat16_rn(bj));
+                w[u][1] = bj - w[u][0];
+            }
+            *reinterpret_cast<uint4*>(ws + dst[u]) = make_uint4(pack_bf16(w[u][0], w[u][1]), pack_bf16(w[u][2], w[u][3]),
+                                                                pack_bf16(w[u][4], w[u][5]), pack_bf16(w[u][6], w[u][7]));
+        }
+    }
+}
+
 }  // namespace
 }  // namespace dash
