@@ -370,7 +370,8 @@ def run_cuda(args):
 
     debug_keys = {"fwd_group": dh.DEBUG_FWD_GROUP, "bwd_group": dh.DEBUG_BWD_GROUP,
                   "smooth_group": dh.DEBUG_SMOOTH_GROUP, "deform_path": dh.DEBUG_DEFORM_PATH,
-                  "bwd_variant": dh.DEBUG_BWD_VARIANT, "fwd_variant": dh.DEBUG_FWD_VARIANT}
+                  "bwd_variant": dh.DEBUG_BWD_VARIANT, "fwd_variant": dh.DEBUG_FWD_VARIANT,
+                  "bwd_coarse_levels": dh.DEBUG_BWD_COARSE_LEVELS, "bwd_run_chunk": dh.DEBUG_BWD_RUN_CHUNK}
     for item in args.set_debug:
         key, _, val = item.partition("=")
         dh.dash_hash4d_set_debug(debug_keys[key], int(val))
@@ -378,7 +379,11 @@ def run_cuda(args):
     wl = make_workload(args.config)
     enc, N = wl.spec.enc, wl.N
     flags = dh.FLAG_DENSE_COARSE | (dh.FLAG_ZERO_GRAD if args.zero_grad_fused else 0)
+    if args.sort_coarse:
+        flags |= dh.FLAG_SORT_COARSE
     cfg = dh.config_from_params(enc, flags=flags)
+    bwd_ws_bytes = dh.dash_hash4d_workspace_bytes(cfg, N, dh.OP_BWD)
+    bwd_ws = torch.empty(bwd_ws_bytes, dtype=torch.uint8, device="cuda") if bwd_ws_bytes else None
     to_dev = lambda a: None if a is None else torch.from_numpy(a).cuda()
     xyz, t, index = to_dev(wl.xyz), to_dev(wl.t), to_dev(wl.index)
     table, dout = to_dev(wl.table), to_dev(wl.dout)
@@ -405,7 +410,7 @@ def run_cuda(args):
         dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index)
         if marks is not None:
             marks[2].record()
-        dh.dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=index)
+        dh.dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=index, workspace=bwd_ws)
         if marks is not None:
             marks[3].record()
 
@@ -716,6 +721,8 @@ def main():
                          "(no kernels, no measurement; tests/test_replicas_gloo.py)")
     ap.add_argument("--zero-grad-fused", type=int, default=1,
                     help="1: bwd zeroes each level group itself (DASH_HASH4D_FLAG_ZERO_GRAD)")
+    ap.add_argument("--sort-coarse", type=int, default=0,
+                    help="1: bwd scatters the coarse levels by sort + run-merged reduction (DASH_HASH4D_FLAG_SORT_COARSE)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", type=int, default=1,
                     help="1: also time bwd_input / smooth / one-timestamp fwd (information only)")

@@ -58,9 +58,16 @@ enum dash_hash4d_flags {
                                                bitwise identical results run to run; needs workspace.       */
     DASH_HASH4D_FLAG_VALIDATE_INPUTS = 4u,  /* debug: scan coordinates for NaN / values outside [0,1) before
                                                the op; synchronises the stream; needs workspace.            */
-    DASH_HASH4D_FLAG_ZERO_GRAD = 8u         /* bwd OVERWRITES: the library zeroes each level group of dtable
+    DASH_HASH4D_FLAG_ZERO_GRAD = 8u,        /* bwd OVERWRITES: the library zeroes each level group of dtable
                                                immediately before scattering into it (keeps it L2-resident)
                                                instead of accumulating into the caller's contents.          */
+    DASH_HASH4D_FLAG_SORT_COARSE = 16u      /* dash_hash4d_bwd, the high-collision case (BASELINE.json config 5): the
+                                               coarse levels (cell count <= 2N) are scattered by a sort + segmented
+                                               reduction — queries counting-sorted by their 4D cell, runs of queries
+                                               in one cell summed in registers, one vector reduction per run and
+                                               corner; the other levels are unchanged.  Same sums in another order
+                                               (same tolerance).  Needs workspace; ignored by DETERMINISTIC_BWD, by
+                                               the other calls and by dash_hash3d_bwd.                       */
 };
 
 enum dash_hash4d_op { DASH_HASH4D_OP_FWD = 0, DASH_HASH4D_OP_BWD = 1, DASH_HASH4D_OP_INDICES = 2,
@@ -88,7 +95,8 @@ typedef struct dash_hash4d_config {
 DASH_API int dash_hash4d_resolutions(const dash_hash4d_config* cfg, uint32_t* res_s, uint32_t* res_t,
                                      uint8_t* is_dense);
 
-/* Bytes of device workspace `op` needs for N queries under cfg->flags (0 for the default paths).
+/* Bytes of device workspace `op` needs for N queries under cfg->flags (0 for the default paths; SORT_COARSE:
+ * 24 bytes per query + the sort's bins).
  * Returns 0 on a bad config as well.  Needs no GPU. */
 DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op);
 
@@ -119,7 +127,8 @@ DASH_API int dash_hash4d_fwd(const dash_hash4d_config* cfg, uint64_t N,
  *              DASH_HASH4D_FLAG_ZERO_GRAD is set, in which case it is overwritten.
  * Default path: fp32 vector reductions at L2 (`red.global.add.v2/.v4.f32`): summation order, hence the
  * last bits, vary run to run; subnormal partial sums flush to zero.  DETERMINISTIC_BWD: 64-bit
- * fixed-point accumulation in `workspace`, bitwise reproducible.  Other arguments as in fwd. */
+ * fixed-point accumulation in `workspace`, bitwise reproducible.  SORT_COARSE: see the flag; the sort (five launches)
+ * and the run-merged scatter run inside this call, on `cuda_stream`, in `workspace`.  Other arguments as in fwd. */
 DASH_API int dash_hash4d_bwd(const dash_hash4d_config* cfg, uint64_t N,
                              const float* xyz, uint32_t xyz_stride,
                              const float* t, uint32_t t_stride,
@@ -275,7 +284,9 @@ enum dash_debug_key {
     DASH_DEBUG_DEFORM_PATH = 3,  /* dash_deform_fwd: 1 = fused kernel, 2 = two-pass (encoder -> workspace -> MLP) */
     DASH_DEBUG_BWD_VARIANT = 4,  /* bwd with ZERO_GRAD: 1 = no L2 eviction hints on the zero stores / reductions */
     DASH_DEBUG_FWD_VARIANT = 5,  /* reserved (0) */
-    DASH_DEBUG_KEY_COUNT = 6
+    DASH_DEBUG_BWD_COARSE_LEVELS = 6, /* SORT_COARSE: number of leading levels the run-merged scatter takes */
+    DASH_DEBUG_BWD_RUN_CHUNK = 7,     /* SORT_COARSE: consecutive sorted queries per lane pair */
+    DASH_DEBUG_KEY_COUNT = 8
 };
 DASH_API int dash_hash4d_set_debug(int key, int64_t value);
 

@@ -17,6 +17,7 @@ FLAG_DENSE_COARSE = 1
 FLAG_DETERMINISTIC_BWD = 2
 FLAG_VALIDATE_INPUTS = 4
 FLAG_ZERO_GRAD = 8
+FLAG_SORT_COARSE = 16
 OP_FWD, OP_BWD, OP_INDICES, OP_BWD_INPUT, OP_SMOOTH = 0, 1, 2, 3, 4
 
 _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUDA_ERROR"}
@@ -286,7 +287,8 @@ def dash_hash4d_launch_count(reset: bool = False) -> int:
     return int(_load().dash_hash4d_launch_count(1 if reset else 0))
 
 
-DEBUG_FWD_GROUP, DEBUG_BWD_GROUP, DEBUG_SMOOTH_GROUP, DEBUG_DEFORM_PATH, DEBUG_BWD_VARIANT, DEBUG_FWD_VARIANT = range(6)
+(DEBUG_FWD_GROUP, DEBUG_BWD_GROUP, DEBUG_SMOOTH_GROUP, DEBUG_DEFORM_PATH, DEBUG_BWD_VARIANT, DEBUG_FWD_VARIANT,
+ DEBUG_BWD_COARSE_LEVELS, DEBUG_BWD_RUN_CHUNK) = range(8)
 
 
 def dash_hash4d_set_debug(key: int, value: int) -> None:

@@ -61,7 +61,7 @@ int check_config(const dash_hash4d_config* c, int dims = 4) {
                     c->res_t_min, c->res_t_max);
     if (c->table_dtype != DASH_HASH4D_FP32 && c->table_dtype != DASH_HASH4D_FP16)
         return fail(DASH_HASH4D_INVALID_ARG, "table_dtype = %u", c->table_dtype);
-    if (c->flags & ~15u) return fail(DASH_HASH4D_INVALID_ARG, "unknown flag bits 0x%x", c->flags);
+    if (c->flags & ~31u) return fail(DASH_HASH4D_INVALID_ARG, "unknown flag bits 0x%x", c->flags);
     return DASH_HASH4D_OK;
 }
 
@@ -272,20 +272,68 @@ DASH_API int dash_hash4d_resolutions(const dash_hash4d_config* cfg, uint32_t* re
     return ok();
 }
 
-static size_t workspace_need(const dash_hash4d_config* cfg, int op) {
+static size_t round16(size_t v) { return (v + 15u) & ~static_cast<size_t>(15u); }
+
+// DASH_HASH4D_FLAG_SORT_COARSE: which leading levels the run-merged scatter takes and how the queries are keyed.
+// Levels whose cell count Ns^3 Nt is at most 2N (on average >= 1/2 query per cell; clustered inputs fill far fewer
+// cells) — measured rule, profiles/experiments_r02.md §8.  The key is the Morton code of the cell on the finest of
+// them, coarsened until it has at most 22 bits.  DASH_DEBUG_BWD_COARSE_LEVELS / _RUN_CHUNK override for sweeps.
+static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSort* cs) {
+    std::memset(cs, 0, sizeof(*cs));
+    if (!(c->flags & DASH_HASH4D_FLAG_SORT_COARSE) || (c->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD) || N == 0)
+        return false;
+    Schedule s;
+    make_schedule(c, &s, 4);
+    uint32_t nl = 0;
+    const uint32_t forced = debug_u32(DASH_DEBUG_BWD_COARSE_LEVELS);
+    if (forced) {
+        nl = forced < c->L ? forced : c->L;
+    } else {
+        while (nl < c->L && nl < 8) {
+            const double cells = static_cast<double>(s.res_s[nl]) * s.res_s[nl] * s.res_s[nl] * s.res_t[nl];
+            if (cells > 2.0 * static_cast<double>(N)) break;
+            ++nl;
+        }
+    }
+    if (nl == 0) return false;
+    cs->levels = nl;
+    cs->key_level = nl - 1;
+    auto ceil_log2 = [](uint32_t v) { uint32_t b = 0; while ((1ull << b) < v) ++b; return b; };
+    uint32_t bs = ceil_log2(s.res_s[nl - 1]), bt = ceil_log2(s.res_t[nl - 1]);
+    while (3 * (bs - cs->shift_s) + (bt - cs->shift_t) > 22 || bs - cs->shift_s > 7 || bt - cs->shift_t > 7) {
+        if (bt - cs->shift_t > bs - cs->shift_s) ++cs->shift_t; else ++cs->shift_s;
+    }
+    cs->bits_s = bs - cs->shift_s;
+    cs->bits_t = bt - cs->shift_t;
+    cs->n_bins = 1u << (3 * cs->bits_s + cs->bits_t);
+    const uint32_t chunk = debug_u32(DASH_DEBUG_BWD_RUN_CHUNK);
+    cs->chunk = chunk ? chunk : 64u;
+    return true;
+}
+
+static size_t coarse_workspace(const dash::CoarseSort& cs, uint64_t N) {
+    return round16(N * 4) * 2 + round16(N * 16) + round16(static_cast<size_t>(cs.n_bins) * 4) +
+           round16((static_cast<size_t>(cs.n_bins) + 1023) / 1024 * 4);
+}
+
+static size_t workspace_need(const dash_hash4d_config* cfg, int op, uint64_t N, int dims = 4) {
     size_t bytes = 0;
     if ((cfg->flags & DASH_HASH4D_FLAG_VALIDATE_INPUTS) && op != DASH_HASH4D_OP_INDICES)
         bytes = kHeaderBytes;
     if (op == DASH_HASH4D_OP_BWD && (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD))
         bytes = kHeaderBytes + table_elems(cfg) * sizeof(long long);
+    dash::CoarseSort cs;
+    if (op == DASH_HASH4D_OP_BWD && dims == 4 && plan_coarse(cfg, N, &cs)) bytes = kHeaderBytes + coarse_workspace(cs, N);
     return bytes;
 }
 
 DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op) {
-    (void)N;
     if (check_config(cfg, 3)) return 0;  // the temporal range is not needed to size a workspace
     g_error[0] = '\0';
-    return workspace_need(cfg, op);
+    // the coarse sort keys on the temporal resolutions too: a config that is only valid for G_3D gets none
+    const int dims = check_config(cfg, 4) == DASH_HASH4D_OK ? 4 : 3;
+    g_error[0] = '\0';
+    return workspace_need(cfg, op, N, dims);
 }
 
 static int fwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
@@ -431,7 +479,7 @@ static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
     if (!aligned16(dout) || !aligned16(dtable))
         return fail(DASH_HASH4D_INVALID_ARG, "dout / dtable not 16-byte aligned");
     const bool fixed = (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD) != 0;
-    const size_t need = workspace_need(cfg, DASH_HASH4D_OP_BWD);
+    const size_t need = workspace_need(cfg, DASH_HASH4D_OP_BWD, N, dims);
     if (need && (!workspace || workspace_bytes < need))
         return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "bwd needs %zu workspace bytes, got %zu", need,
                     workspace_bytes);
@@ -457,40 +505,71 @@ static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
         if (e != cudaSuccess) return cuda_fail(e, "deterministic bwd launch");
         return ok();
     }
+    // SORT_COARSE: the leading `cs.levels` levels go through the sort + run-merged scatter (bwd_runs_kernels.cu),
+    // the others through the one-reduction-per-corner kernel in the caller's order.
+    dash::CoarseSort cs;
+    const bool coarse = dims == 4 && plan_coarse(cfg, N, &cs);
+    const uint32_t l_first = coarse ? cs.levels : 0u;
+    auto scatter_coarse = [&](bool hint) -> cudaError_t {
+        char* w = static_cast<char*>(workspace) + kHeaderBytes;
+        int32_t* order = reinterpret_cast<int32_t*>(w);
+        uint32_t* keys = reinterpret_cast<uint32_t*>(w + round16(N * 4));
+        float4* sorted_q = reinterpret_cast<float4*>(w + 2 * round16(N * 4));
+        uint32_t* bins = reinterpret_cast<uint32_t*>(w + 2 * round16(N * 4) + round16(N * 16));
+        uint32_t* totals = bins + round16(static_cast<size_t>(cs.n_bins) * 4) / 4;
+        return dash::launch_bwd_runs(P, cs, xyz, t, index, dout, dtable, order, sorted_q, keys, bins, totals, s, hint);
+    };
+    // the levels [l0, L) in groups of P.group (a ragged last group shrinks to the largest power of two that fits)
+    auto scatter_rest = [&](uint32_t l0, bool hint) -> cudaError_t {
+        if (l0 >= cfg->L) return cudaSuccess;
+        Plan Pr = P;
+        Pr.level_begin = l0;
+        Pr.num_groups = (cfg->L - l0 + P.group - 1) / P.group;
+        return dash::launch_bwd(Pr, xyz, t, index, dout, dtable, s, hint);
+    };
     if (!zero_first) {
-        e = dash::launch_bwd(P, xyz, t, index, dout, dtable, s);
+        if (coarse) e = scatter_coarse(false);
+        if (e == cudaSuccess) e = scatter_rest(l_first, false);
         if (e != cudaSuccess) return cuda_fail(e, "bwd launch");
         return ok();
     }
+    const bool hint = debug_u32(DASH_DEBUG_BWD_VARIANT) != 1;
     // ZERO_GRAD, small tables: when the WHOLE gradient buffer fits the L2 budget there is nothing to keep resident group
     // by group — one zero launch and one scatter launch over all groups (C2: 2 launches instead of 4).
     if (level_bytes * cfg->L <= l2_bytes() * 3 / 10) {
-        const bool hint = debug_u32(DASH_DEBUG_BWD_VARIANT) != 1;
         e = dash::launch_zero(dtable, level_bytes * cfg->L, s, hint);
-        if (e == cudaSuccess) e = dash::launch_bwd(P, xyz, t, index, dout, dtable, s, hint);
+        if (e == cudaSuccess && coarse) e = scatter_coarse(hint);
+        if (e == cudaSuccess) e = scatter_rest(l_first, hint);
         if (e != cudaSuccess) return cuda_fail(e, "bwd launch");
         return ok();
     }
     // ZERO_GRAD: zero one level group, scatter into it while the zeros are still in L2, next group.
     // (A one-launch variant whose tail CTAs zero the next group's slice was built and measured in round 2: slower,
-    // profiles/experiments_r02.md §1.)
-    const uint32_t groups = P.num_groups;
-    for (uint32_t g = 0; g < groups; ++g) {
-        const uint32_t l0 = g * P.group;
-        const uint32_t l1 = (l0 + P.group < cfg->L) ? l0 + P.group : cfg->L;
+    // profiles/experiments_r02.md §1.)  L2 evict_last hints on the zero stores and the reductions keep the group's
+    // slice resident against the streamed dout / coordinates: C4 bwd 1.190 -> 1.168 ms, DRAM bytes per call 2.76 ->
+    // 1.54 GB (ncu, profiles/experiments_r02.md §2).  DASH_DEBUG_BWD_VARIANT = 1 turns the hints off for A/B runs.
+    if (coarse) {   // the coarse levels' slices first: only their dense / touched part is ever fetched again
+        e = dash::launch_zero(dtable, static_cast<size_t>(l_first) * level_bytes, s, hint);
+        if (e == cudaSuccess) e = scatter_coarse(hint);
+        if (e != cudaSuccess) return cuda_fail(e, "coarse bwd launch");
+    }
+    for (uint32_t l0 = l_first; l0 < cfg->L;) {
+        uint32_t g = P.group;
+        while (g > cfg->L - l0) g /= 2;   // ragged tail: a smaller power of two instead of idle lanes
         char* base = reinterpret_cast<char*>(dtable) + static_cast<size_t>(l0) * level_bytes;
-        const size_t bytes = static_cast<size_t>(l1 - l0) * level_bytes;
-        // L2 evict_last hints on the zero stores and the reductions keep the group's slice resident against the
-        // streamed dout / coordinates: C4 bwd 1.190 -> 1.168 ms, DRAM bytes per call 2.76 -> 1.54 GB (ncu,
-        // profiles/experiments_r02.md §2).  DASH_DEBUG_BWD_VARIANT = 1 turns the hints off for A/B runs.
-        const bool hint = debug_u32(DASH_DEBUG_BWD_VARIANT) != 1;
-        e = dash::launch_zero(base, bytes, s, hint);  // handles slices that are only 4-byte aligned
+        e = dash::launch_zero(base, static_cast<size_t>(g) * level_bytes, s, hint);  // handles 4-byte aligned slices
         if (e != cudaSuccess) return cuda_fail(e, "zero launch");
         Plan Pg = P;
+        uint32_t lg = 0;
+        while ((1u << lg) < g) ++lg;
+        Pg.group = g;
+        Pg.group_log2 = lg;
+        Pg.q_per_block = dash::kItemsPerBlock >> lg;
         Pg.level_begin = l0;
         Pg.num_groups = 1;
         e = dash::launch_bwd(Pg, xyz, t, index, dout, dtable, s, hint);
         if (e != cudaSuccess) return cuda_fail(e, "bwd launch");
+        l0 += g;
     }
     return ok();
 }
@@ -576,8 +655,6 @@ DASH_API int dash_hash4d_adam_step(const dash_hash4d_config* cfg, const dash_ada
     if (e != cudaSuccess) return cuda_fail(e, "adam launch");
     return ok();
 }
-
-static size_t round16(size_t v) { return (v + 15u) & ~static_cast<size_t>(15u); }
 
 DASH_API size_t dash_hash4d_sort_workspace_bytes(uint64_t N, uint32_t bits) {
     if (bits < 1 || bits > 7) return 0;

@@ -83,9 +83,8 @@ __device__ __forceinline__ Query load_query(const Plan& P, const LevelParams& lp
 // (XOR of g_d*pi_d) mod T (Eq. 8, uint32 wraparound, Q8/Q9); dense level: slot = sum of g_d*stride_d (Q10).
 // D = 3 is G_3D of the decomposition stage (Eq. 3; Q26): 4 (y,z) corners.
 template <int D = 4>
-__device__ __forceinline__ void half_cell(const Plan& P, const LevelParams& lp, const Query& q,
-                                          uint32_t xc, uint32_t* __restrict__ slot,
-                                          float* __restrict__ W) {
+__device__ __forceinline__ void half_cell_slots(const Plan& P, const LevelParams& lp, const Query& q,
+                                                uint32_t xc, uint32_t* __restrict__ slot) {
     constexpr int NC = 1 << (D - 1);
     const uint32_t ax = (q.c[0] + xc) * lp.m[0];
     const uint32_t ay0 = q.c[1] * lp.m[1], ay1 = ay0 + lp.m[1];
@@ -118,7 +117,11 @@ __device__ __forceinline__ void half_cell(const Plan& P, const LevelParams& lp, 
             for (int j = 0; j < NC; ++j) slot[j] %= P.T;
         }
     }
-    // multilinear weights: W = prod_d (corner bit ? w_d : 1 - w_d), fp32
+}
+
+// multilinear weights: W = prod_d (corner bit ? w_d : 1 - w_d), fp32
+template <int D = 4>
+__device__ __forceinline__ void half_cell_weights(const Query& q, uint32_t xc, float* __restrict__ W) {
     const float wx = xc ? q.w[0] : 1.0f - q.w[0];
     const float py0 = wx * (1.0f - q.w[1]), py1 = wx * q.w[1];
     const float z0 = 1.0f - q.w[2], z1 = q.w[2];
@@ -130,6 +133,14 @@ __device__ __forceinline__ void half_cell(const Plan& P, const LevelParams& lp, 
     } else {
         W[0] = py0 * z0; W[1] = py1 * z0; W[2] = py0 * z1; W[3] = py1 * z1;
     }
+}
+
+template <int D = 4>
+__device__ __forceinline__ void half_cell(const Plan& P, const LevelParams& lp, const Query& q,
+                                          uint32_t xc, uint32_t* __restrict__ slot,
+                                          float* __restrict__ W) {
+    half_cell_slots<D>(P, lp, q, xc, slot);
+    half_cell_weights<D>(q, xc, W);
 }
 
 // ------------------------------------------------------------------------------------------------

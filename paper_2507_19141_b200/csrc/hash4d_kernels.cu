@@ -952,10 +952,22 @@ cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t co
     return after_launch();
 }
 
+// bins[i] <- sum of bins[0..i) in place (three launches); totals: scratch of ceil(n_bins / 1024) uint32
+cudaError_t launch_exclusive_scan_u32(uint32_t* bins, uint32_t n_bins, uint32_t* totals, cudaStream_t s) {
+    const uint32_t scan_ctas = (n_bins + 1023u) / 1024u;
+    cudaError_t e;
+    sort_scan_local_kernel<<<scan_ctas, 1024, 0, s>>>(bins, n_bins, totals);
+    if ((e = after_launch()) != cudaSuccess) return e;
+    sort_scan_totals_kernel<<<1, 1024, 0, s>>>(totals, scan_ctas);
+    if ((e = after_launch()) != cudaSuccess) return e;
+    sort_scan_add_kernel<<<scan_ctas, 1024, 0, s>>>(bins, n_bins, totals);
+    return after_launch();
+}
+
 cudaError_t launch_sort_queries(uint64_t N, const float* xyz, uint32_t xyz_stride, const int32_t* index,
                                 uint32_t bits, int32_t* order, uint32_t* keys, uint32_t* bins, uint32_t* totals,
                                 cudaStream_t s) {
-    const uint32_t n_bins = 1u << (3u * bits), scan_ctas = (n_bins + 1023u) / 1024u;
+    const uint32_t n_bins = 1u << (3u * bits);
     const size_t want = (N + kBlockThreads - 1) / kBlockThreads;
     const size_t cap = static_cast<size_t>(sm_count()) * 16;
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
@@ -964,12 +976,7 @@ cudaError_t launch_sort_queries(uint64_t N, const float* xyz, uint32_t xyz_strid
     sort_keys_kernel<<<blocks, kBlockThreads, 0, s>>>(N, xyz, xyz_stride, index, static_cast<float>(1u << bits),
                                                       (1u << bits) - 1u, keys, bins);
     if ((e = after_launch()) != cudaSuccess) return e;
-    sort_scan_local_kernel<<<scan_ctas, 1024, 0, s>>>(bins, n_bins, totals);
-    if ((e = after_launch()) != cudaSuccess) return e;
-    sort_scan_totals_kernel<<<1, 1024, 0, s>>>(totals, scan_ctas);
-    if ((e = after_launch()) != cudaSuccess) return e;
-    sort_scan_add_kernel<<<scan_ctas, 1024, 0, s>>>(bins, n_bins, totals);
-    if ((e = after_launch()) != cudaSuccess) return e;
+    if ((e = launch_exclusive_scan_u32(bins, n_bins, totals, s)) != cudaSuccess) return e;
     sort_scatter_kernel<<<blocks, kBlockThreads, 0, s>>>(N, keys, bins, order);
     return after_launch();
 }

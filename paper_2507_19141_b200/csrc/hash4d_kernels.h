@@ -42,6 +42,19 @@ cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t co
 cudaError_t launch_sort_queries(uint64_t N, const float* xyz, uint32_t xyz_stride, const int32_t* index,
                                 uint32_t bits, int32_t* order, uint32_t* keys, uint32_t* bins, uint32_t* totals,
                                 cudaStream_t s);
+cudaError_t launch_exclusive_scan_u32(uint32_t* bins, uint32_t n_bins, uint32_t* totals, cudaStream_t s);
+// Run-merged scatter of the coarse levels (bwd_runs_kernels.cu; DASH_HASH4D_FLAG_SORT_COARSE): sort the queries by the
+// 4D cell of level `key_level`, then reduce runs of queries that share a cell in registers before they reach L2.
+struct CoarseSort {
+    uint32_t levels;      // leading levels [0, levels) taken by the run-merged scatter (0: path not used)
+    uint32_t key_level;   // the cell of this level is the sort key (the finest of them)
+    uint32_t bits_s, bits_t, shift_s, shift_t;  // Morton key: (cell >> shift) per axis, bits per spatial axis / for t
+    uint32_t chunk;       // consecutive sorted queries walked by one lane pair
+    uint32_t n_bins;      // 1 << (3 bits_s + bits_t)
+};
+cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* xyz, const float* t, const int32_t* index,
+                            const float* dout, float* dtable, int32_t* order, float4* sorted_q, uint32_t* keys,
+                            uint32_t* bins, uint32_t* totals, cudaStream_t s, bool l2_hint);
 cudaError_t launch_slice_t(const Plan& P, const float* t, const void* table, bool table_half, float* slice,
                            cudaStream_t s);
 cudaError_t launch_adam(size_t count, double lr, double beta1, double beta2, double eps, uint32_t step,

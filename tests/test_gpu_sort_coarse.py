@@ -1,0 +1,162 @@
+"""GPU parity of the collision-aware scatter (DASH_HASH4D_FLAG_SORT_COARSE): counting sort of the queries by the 4D cell
+of the finest coarse level + run-merged reductions on the coarse levels, the other levels unchanged.  The result is the
+same table gradient as the plain backward (same sums, another order), so every check is the plain backward's check
+against the oracle (tests/parity_utils.py): element by element with the hits-aware tolerance, normwise per level, and the
+whole-buffer checksum.  BASELINE.json config 5 is the workload the flag exists for.
+"""
+import ctypes as C
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2507_19141_b200 as dh
+from dash_inputs import EncoderParams, make_queries_uniform, make_workload
+from parity_utils import RTOL_FP32, check_close
+from test_gpu_parity import DC, both_configs, dev, run_bwd_parity
+
+pytestmark = pytest.mark.gpu
+
+SC = dh.FLAG_SORT_COARSE
+ZG = dh.FLAG_ZERO_GRAD
+
+
+@pytest.mark.parametrize("name", ["C3", "C4", "C5"])
+def test_full_size_configs(name):
+    """The bench's launch configuration (ZERO_GRAD + SORT_COARSE, the library's own choice of coarse levels)."""
+    wl = make_workload(name, with_table=False)
+    cfg = dh.config_from_params(wl.spec.enc, flags=DC | ZG | SC)
+    assert dh.dash_hash4d_workspace_bytes(cfg, wl.N, dh.OP_BWD) >= 24 * wl.N
+    run_bwd_parity(wl.spec.enc, wl.xyz, wl.t, wl.dout, index=wl.index, flags=DC | ZG | SC, what=name + " sort_coarse")
+
+
+@pytest.mark.parametrize("levels", [1, 2, 3, 5, 16])
+@pytest.mark.parametrize("chunk", [1, 7, 64])
+def test_forced_coarse_levels_and_chunks(levels, chunk, set_debug):
+    """Any number of leading levels (hashed ones included, up to all of them) and any chunk length give the plain result;
+    N is ragged against the chunk and against the 128-pair blocks."""
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, levels)
+    set_debug(dh.DEBUG_BWD_RUN_CHUNK, chunk)
+    for (L, F, T, n, flags) in [(5, 2, 1 << 12, 3001, DC | SC), (16, 4, 1 << 14, 2500, DC | ZG | SC),
+                                (7, 1, 100003, 1237, SC), (3, 8, 1 << 13, 777, DC | ZG | SC)]:
+        enc = EncoderParams(L, F, T, 4, 300, 2, 40)
+        rng = np.random.default_rng(L * 100 + levels + chunk)
+        xyz, t = make_queries_uniform(L + levels, n)
+        dout = rng.standard_normal((n, L * F)).astype(np.float32)
+        run_bwd_parity(enc, xyz, t, dout, flags=flags, what=f"sort_coarse L{L} F{F} levels{levels} chunk{chunk}")
+
+
+def test_long_runs_index_list_broadcast_t_and_existing_gradient(set_debug):
+    """Clustered queries (long runs on every coarse level), an index list with repeats, one timestamp for the whole call,
+    and accumulation into a gradient buffer that already holds values."""
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 4)
+    enc = EncoderParams(8, 2, 1 << 13, 8, 512, 4, 64)
+    rng = np.random.default_rng(5)
+    rows = 4000
+    xyz = np.clip(0.4 + 0.01 * rng.standard_normal((rows, 3)), 0, 0.999).astype(np.float32)
+    index = np.repeat(np.sort(rng.choice(rows, 1500, replace=False)).astype(np.int32), 4)
+    n = len(index)
+    t = rng.random(n, dtype=np.float32)
+    dout = rng.standard_normal((n, 16)).astype(np.float32)
+    run_bwd_parity(enc, xyz, t, dout, index=index, flags=DC | ZG | SC, what="clustered, indexed")
+    init = rng.standard_normal((8, 1 << 13, 2)).astype(np.float32)
+    run_bwd_parity(enc, xyz, t, dout, index=index, flags=DC | SC, init=init, what="clustered, accumulate")
+    t1 = np.array([0.37], np.float32)
+    run_bwd_parity(enc, xyz, t1, dout[:rows], t_stride=0, flags=DC | ZG | SC, what="one timestamp")
+
+
+def test_tiny_and_edge_inputs(set_debug):
+    """N = 1, N below one chunk, every query in one cell, clamped / NaN coordinates."""
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 2)
+    enc = EncoderParams(4, 2, 1 << 10, 8, 64, 4, 16)
+    rng = np.random.default_rng(11)
+    for n in (1, 2, 63):
+        xyz, t = make_queries_uniform(n, n)
+        dout = rng.standard_normal((n, 8)).astype(np.float32)
+        run_bwd_parity(enc, xyz, t, dout, flags=DC | ZG | SC, what=f"N={n}")
+    n = 300
+    xyz = np.full((n, 3), 0.51, np.float32)
+    t = np.full(n, 0.26, np.float32)
+    dout = rng.standard_normal((n, 8)).astype(np.float32)
+    run_bwd_parity(enc, xyz, t, dout, flags=DC | ZG | SC, what="one cell")
+    xyz, t = make_queries_uniform(3, n)
+    xyz[:6] = [[0, 0, 0], [1, 1, 1], [np.nan, 0.5, -3], [2, 0.1, 0.2], [-1, -1, -1], [0.5, np.inf, 0.5]]
+    t[:4] = [1.0, np.nan, -0.5, 7.0]
+    run_bwd_parity(enc, xyz, t, dout, flags=DC | ZG | SC, what="edge coordinates")
+
+
+def test_workspace_is_required_and_sized_by_the_library(set_debug):
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 2)
+    enc = EncoderParams(4, 2, 1 << 10, 8, 64, 4, 16)
+    cfg = dh.config_from_params(enc, flags=DC | SC)
+    n = 1000
+    need = dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD)
+    assert need >= 24 * n
+    assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_FWD) == 0          # only the backward sorts
+    assert dh.dash_hash4d_workspace_bytes(dh.with_flags(cfg, DC | SC | dh.FLAG_DETERMINISTIC_BWD), n, dh.OP_BWD) == \
+        dh.dash_hash4d_workspace_bytes(dh.with_flags(cfg, DC | dh.FLAG_DETERMINISTIC_BWD), n, dh.OP_BWD)
+    xyz, t = make_queries_uniform(1, n)
+    dout = np.zeros((n, 8), np.float32)
+    xd, td, dd = dev(xyz), dev(t), dev(dout)
+    dt = torch.zeros((4, 1 << 10, 2), device="cuda")
+    small = torch.empty(need - 16, dtype=torch.uint8, device="cuda")
+    lib = dh.binding._load()
+    rc = lib.dash_hash4d_bwd(C.byref(cfg), n, C.c_void_p(xd.data_ptr()), 3, C.c_void_p(td.data_ptr()), 1, None,
+                             C.c_void_p(dd.data_ptr()), C.c_void_p(dt.data_ptr()), C.c_void_p(small.data_ptr()),
+                             small.numel(), C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    assert rc == 3 and "workspace" in dh.dash_hash4d_last_error()          # DASH_HASH4D_WORKSPACE_TOO_SMALL
+    rc = lib.dash_hash4d_bwd(C.byref(cfg), n, C.c_void_p(xd.data_ptr()), 3, C.c_void_p(td.data_ptr()), 1, None,
+                             C.c_void_p(dd.data_ptr()), C.c_void_p(dt.data_ptr()), None, 0,
+                             C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    assert rc == 3
+
+
+def test_flag_is_ignored_by_g3d_and_by_the_deterministic_mode(set_debug):
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 2)
+    enc = EncoderParams(4, 2, 1 << 10, 8, 64, 4, 16)
+    n = 2000
+    rng = np.random.default_rng(2)
+    xyz, t = make_queries_uniform(2, n)
+    dout = rng.standard_normal((n, 8)).astype(np.float32)
+    # deterministic: bitwise equal with and without the flag
+    got = []
+    for flags in (DC | ZG | dh.FLAG_DETERMINISTIC_BWD, DC | ZG | dh.FLAG_DETERMINISTIC_BWD | SC):
+        cfg = dh.config_from_params(enc, flags=flags)
+        dt = torch.empty((4, 1 << 10, 2), device="cuda")
+        dh.dash_hash4d_bwd(cfg, dev(xyz), dev(t), dev(dout), dt)
+        got.append(dt.cpu().numpy())
+    assert np.array_equal(got[0], got[1])
+    # G_3D backward: the flag changes nothing (and needs no workspace)
+    o3 = oracle.make_config(4, 2, 1 << 10, 8, 64, 1, 1)
+    g3 = dh.make_config(4, 2, 1 << 10, 8, 64, 1, 1, flags=DC | ZG | SC)
+    ref, mag = oracle.oracle3d_bwd(o3, n, xyz, dout, want_abs=True)
+    dt = torch.empty((4, 1 << 10, 2), device="cuda")
+    dh.dash_hash3d_bwd(g3, dev(xyz), dev(dout), dt)
+    check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 4, what="g3d with the flag set")
+
+
+def test_sorted_path_is_cuda_graph_capturable(set_debug):
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 3)
+    enc = EncoderParams(6, 2, 1 << 12, 8, 256, 4, 32)
+    n = 5000
+    rng = np.random.default_rng(4)
+    xyz, t = make_queries_uniform(4, n)
+    dout = rng.standard_normal((n, 12)).astype(np.float32)
+    ocfg, gcfg = both_configs(enc, DC | ZG | SC)
+    ref, mag, hits = oracle.oracle_bwd(ocfg, n, xyz, t, dout, want_abs=True, want_hits=True)
+    xd, td, dd = dev(xyz), dev(t), dev(dout)
+    dt = torch.full((6, 1 << 12, 2), 7.0, device="cuda")
+    ws = torch.empty(dh.dash_hash4d_workspace_bytes(gcfg, n, dh.OP_BWD), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        dh.dash_hash4d_bwd(gcfg, xd, td, dd, dt, workspace=ws)                 # warm-up outside the capture
+        stream.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            dh.dash_hash4d_bwd(gcfg, xd, td, dd, dt, workspace=ws)
+    for _ in range(2):
+        dt.fill_(3.0)
+        graph.replay()
+        torch.cuda.synchronize()
+        check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 6, hits=hits, what="graph replay")
