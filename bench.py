@@ -382,6 +382,8 @@ def run_cuda(args):
     if args.sort_coarse:
         flags |= dh.FLAG_SORT_COARSE
     cfg = dh.config_from_params(enc, flags=flags)
+    # SORT_COARSE: the forward sorts the queries by coarse cell, the backward of the same step reuses that order
+    cfg_bwd = dh.with_flags(cfg, flags | dh.FLAG_ORDER_READY) if args.sort_coarse else cfg
     bwd_ws_bytes = dh.dash_hash4d_workspace_bytes(cfg, N, dh.OP_BWD)
     bwd_ws = torch.empty(bwd_ws_bytes, dtype=torch.uint8, device="cuda") if bwd_ws_bytes else None
     to_dev = lambda a: None if a is None else torch.from_numpy(a).cuda()
@@ -407,10 +409,10 @@ def run_cuda(args):
             dh.dash_hash4d_zero(cfg, dtable)
         if marks is not None:
             marks[1].record()
-        dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index)
+        dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index, workspace=bwd_ws)
         if marks is not None:
             marks[2].record()
-        dh.dash_hash4d_bwd(cfg, xyz, t, dout, dtable, index=index, workspace=bwd_ws)
+        dh.dash_hash4d_bwd(cfg_bwd, xyz, t, dout, dtable, index=index, workspace=bwd_ws)
         if marks is not None:
             marks[3].record()
 
@@ -551,7 +553,8 @@ def run_cuda(args):
         loss = torch.empty((N,), dtype=torch.float32, device="cuda")
         cfg_acc = dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE)
         gen = torch.Generator(device="cuda"); gen.manual_seed(1234)
-        extras = {"bwd_input_ms": timed(lambda: dh.dash_hash4d_bwd_input(cfg, xyz, t, table, dout, dq=dq,
+        cfg_x = dh.with_flags(cfg, flags & ~dh.FLAG_SORT_COARSE)   # the extras time the calls without the coarse sort
+        extras = {"bwd_input_ms": timed(lambda: dh.dash_hash4d_bwd_input(cfg_x, xyz, t, table, dout, dq=dq,
                                                                            index=index))}
         for delta in (1e-4, 1e-3, 1e-2):
             eps = (torch.rand((N, 4), device="cuda", generator=gen) * 2 - 1) * delta
@@ -560,7 +563,7 @@ def run_cuda(args):
                                               dtable=dtable, index=index))
         extras["smooth_unfused_equivalent_ms"] = 2 * (ms_fwd + ms_bwd)
         one_t = t[:1].contiguous()
-        extras["fwd_one_timestamp_ms"] = timed(lambda: dh.dash_hash4d_fwd(cfg, xyz, one_t, table, out=out,
+        extras["fwd_one_timestamp_ms"] = timed(lambda: dh.dash_hash4d_fwd(cfg_x, xyz, one_t, table, out=out,
                                                                            index=index, t_stride=0))
         # G_3D of the decomposition stage on its own workload (dash_inputs.G3D_SPEC)
         from dash_inputs import make_g3d_workload

@@ -61,13 +61,20 @@ enum dash_hash4d_flags {
     DASH_HASH4D_FLAG_ZERO_GRAD = 8u,        /* bwd OVERWRITES: the library zeroes each level group of dtable
                                                immediately before scattering into it (keeps it L2-resident)
                                                instead of accumulating into the caller's contents.          */
-    DASH_HASH4D_FLAG_SORT_COARSE = 16u      /* dash_hash4d_bwd, the high-collision case (BASELINE.json config 5): the
-                                               coarse levels (cell count <= 2N) are scattered by a sort + segmented
-                                               reduction — queries counting-sorted by their 4D cell, runs of queries
-                                               in one cell summed in registers, one vector reduction per run and
-                                               corner; the other levels are unchanged.  Same sums in another order
-                                               (same tolerance).  Needs workspace; ignored by DETERMINISTIC_BWD, by
-                                               the other calls and by dash_hash3d_bwd.                       */
+    DASH_HASH4D_FLAG_SORT_COARSE = 16u,     /* dash_hash4d_fwd / _bwd, the high-collision case (BASELINE.json config 5):
+                                               the queries are counting-sorted by their 4D cell on the coarse levels
+                                               (cell count <= 2N; only for N >= 2^19, else the flag does nothing) and
+                                               those levels are processed in that order — bwd: a segmented reduction,
+                                               runs of queries in one cell summed in registers, one vector reduction
+                                               per run and corner; fwd: neighbouring lanes gather from the same cells.
+                                               The other levels are unchanged.  Same values (fwd) / same sums in
+                                               another order (bwd: same tolerance).  Needs workspace; ignored by
+                                               DETERMINISTIC_BWD, by the other calls and by dash_hash3d_*.       */
+    DASH_HASH4D_FLAG_ORDER_READY = 32u      /* with SORT_COARSE: `workspace` still holds the order that an earlier
+                                               dash_hash4d_fwd / _bwd call with SORT_COARSE wrote for the SAME
+                                               queries (N, xyz, t, index unchanged, e.g. the forward of this training
+                                               step): the sort (five launches) is skipped.  A false claim gives
+                                               wrong values but no out-of-bounds access.                        */
 };
 
 enum dash_hash4d_op { DASH_HASH4D_OP_FWD = 0, DASH_HASH4D_OP_BWD = 1, DASH_HASH4D_OP_INDICES = 2,
@@ -96,7 +103,7 @@ DASH_API int dash_hash4d_resolutions(const dash_hash4d_config* cfg, uint32_t* re
                                      uint8_t* is_dense);
 
 /* Bytes of device workspace `op` needs for N queries under cfg->flags (0 for the default paths; SORT_COARSE:
- * 24 bytes per query + the sort's bins).
+ * 24 bytes per query + the sort's bins, the same for OP_FWD and OP_BWD so that one buffer serves a step).
  * Returns 0 on a bad config as well.  Needs no GPU. */
 DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op);
 

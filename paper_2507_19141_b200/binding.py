@@ -18,6 +18,7 @@ FLAG_DETERMINISTIC_BWD = 2
 FLAG_VALIDATE_INPUTS = 4
 FLAG_ZERO_GRAD = 8
 FLAG_SORT_COARSE = 16
+FLAG_ORDER_READY = 32
 OP_FWD, OP_BWD, OP_INDICES, OP_BWD_INPUT, OP_SMOOTH = 0, 1, 2, 3, 4
 
 _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUDA_ERROR"}

@@ -77,12 +77,14 @@ sort4d_keys_kernel(const __grid_constant__ Plan P, const CoarseSort cs, const fl
 __global__ void __launch_bounds__(kBlockThreads)
 sort4d_scatter_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz, const float* __restrict__ t,
                       const int32_t* __restrict__ index, const uint32_t* __restrict__ keys,
-                      uint32_t* __restrict__ cursor, int32_t* __restrict__ order, float4* __restrict__ sorted_q) {
+                      uint32_t* __restrict__ cursor, const uint32_t* __restrict__ tile_offset,
+                      int32_t* __restrict__ order, float4* __restrict__ sorted_q) {
     const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
     for (uint64_t n = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x; n < P.N; n += stride) {
         float c[4];
         load_coords<4>(P, n, xyz, t, index, c);
-        const uint32_t pos = atomicAdd(cursor + keys[n], 1u);
+        const uint32_t key = keys[n];   // the scan is per tile of kScanTile bins: add the tile's offset here
+        const uint32_t pos = atomicAdd(cursor + key, 1u) + __ldg(tile_offset + key / kScanTile);
         order[pos] = static_cast<int32_t>(n);
         sorted_q[pos] = make_float4(c[0], c[1], c[2], c[3]);
     }
@@ -107,7 +109,7 @@ __device__ __forceinline__ void load_row(const float* __restrict__ d, float g[F]
 // One lane pair = (chunk of `chunk` consecutive sorted queries, one coarse level); adjacent pairs take the coarse
 // levels of the SAME chunk, so their coordinate loads coincide and their dY loads are neighbours in one row.
 template <int F, bool HINT>
-__global__ void __launch_bounds__(kBlockThreads)
+__global__ void __launch_bounds__(kBlockThreads, F == 4 ? 3 : 1)   // F = 4: 85 registers, three CTAs per SM
 hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, const uint32_t chunk,
                        const float4* __restrict__ sorted_q, const int32_t* __restrict__ order,
                        const float* __restrict__ dout, float* __restrict__ dtable) {
@@ -138,8 +140,9 @@ hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, co
     // while query s is accumulated
     float4 q_next = __ldg(sorted_q + begin);
     float g_next[F];
-    load_row<F>(dcol + static_cast<size_t>(__ldg(order + begin)) * row, g_next);
-    int32_t n_ahead = (begin + 1 < end) ? __ldg(order + begin + 1) : 0;
+    const uint32_t n_max = static_cast<uint32_t>(P.N - 1);   // clamped: memory-safe even if ORDER_READY was a false claim
+    load_row<F>(dcol + static_cast<size_t>(min(static_cast<uint32_t>(__ldg(order + begin)), n_max)) * row, g_next);
+    uint32_t n_ahead = (begin + 1 < end) ? min(static_cast<uint32_t>(__ldg(order + begin + 1)), n_max) : 0u;
     for (uint64_t s = begin; s < end; ++s) {
         const float4 qc = q_next;
         float g[F];
@@ -148,7 +151,7 @@ hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, co
         if (s + 1 < end) {
             q_next = __ldg(sorted_q + s + 1);
             load_row<F>(dcol + static_cast<size_t>(n_ahead) * row, g_next);
-            if (s + 2 < end) n_ahead = __ldg(order + s + 2);
+            if (s + 2 < end) n_ahead = min(static_cast<uint32_t>(__ldg(order + s + 2)), n_max);
         }
         const Query q = make_query<4>(lp, qc.x, qc.y, qc.z, qc.w);
         if ((q.c[0] != pc[0]) | (q.c[1] != pc[1]) | (q.c[2] != pc[2]) | (q.c[3] != pc[3])) {
@@ -188,9 +191,9 @@ inline cudaError_t launched() {
 
 }  // namespace
 
-cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* xyz, const float* t, const int32_t* index,
-                            const float* dout, float* dtable, int32_t* order, float4* sorted_q, uint32_t* keys,
-                            uint32_t* bins, uint32_t* totals, cudaStream_t s, bool l2_hint) {
+cudaError_t launch_coarse_sort(const Plan& P, const CoarseSort& cs, const float* xyz, const float* t,
+                               const int32_t* index, int32_t* order, float4* sorted_q, uint32_t* keys, uint32_t* bins,
+                               uint32_t* totals, cudaStream_t s) {
     const size_t want = (P.N + kBlockThreads - 1) / kBlockThreads;
     const size_t cap = static_cast<size_t>(device_sm_count()) * 16;
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
@@ -198,10 +201,13 @@ cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* xy
     if (e != cudaSuccess) return e;
     sort4d_keys_kernel<<<blocks, kBlockThreads, 0, s>>>(P, cs, xyz, t, index, keys, bins);
     if ((e = launched()) != cudaSuccess) return e;
-    if ((e = launch_exclusive_scan_u32(bins, cs.n_bins, totals, s)) != cudaSuccess) return e;
-    sort4d_scatter_kernel<<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, order, sorted_q);
-    if ((e = launched()) != cudaSuccess) return e;
+    if ((e = launch_exclusive_scan_u32(bins, cs.n_bins, totals, s, false)) != cudaSuccess) return e;
+    sort4d_scatter_kernel<<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, totals, order, sorted_q);
+    return launched();
+}
 
+cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* dout, float* dtable, const int32_t* order,
+                            const float4* sorted_q, cudaStream_t s, bool l2_hint) {
     const uint64_t chunks = (P.N + cs.chunk - 1) / cs.chunk;
     const uint64_t threads = chunks * cs.levels * 2;
     const uint64_t grid = (threads + kBlockThreads - 1) / kBlockThreads;

@@ -61,7 +61,7 @@ int check_config(const dash_hash4d_config* c, int dims = 4) {
                     c->res_t_min, c->res_t_max);
     if (c->table_dtype != DASH_HASH4D_FP32 && c->table_dtype != DASH_HASH4D_FP16)
         return fail(DASH_HASH4D_INVALID_ARG, "table_dtype = %u", c->table_dtype);
-    if (c->flags & ~31u) return fail(DASH_HASH4D_INVALID_ARG, "unknown flag bits 0x%x", c->flags);
+    if (c->flags & ~63u) return fail(DASH_HASH4D_INVALID_ARG, "unknown flag bits 0x%x", c->flags);
     return DASH_HASH4D_OK;
 }
 
@@ -164,6 +164,7 @@ int fill_plan(const dash_hash4d_config* c, uint64_t N, uint32_t xyz_stride, uint
     while ((1u << lg) < group) ++lg;
     P->group_log2 = lg;
     P->level_begin = 0;
+    P->level_end = c->L;
     P->num_groups = (c->L + group - 1) / group;
     P->q_per_block = dash::kItemsPerBlock >> lg;
     const bool defaults = !(c->primes[0] | c->primes[1] | c->primes[2] | c->primes[3]);
@@ -288,7 +289,7 @@ static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSor
     const uint32_t forced = debug_u32(DASH_DEBUG_BWD_COARSE_LEVELS);
     if (forced) {
         nl = forced < c->L ? forced : c->L;
-    } else {
+    } else if (N >= (1ull << 19)) {   // below that the sort costs more than the merged reductions save (C3: +0.04 ms)
         while (nl < c->L && nl < 8) {
             const double cells = static_cast<double>(s.res_s[nl]) * s.res_s[nl] * s.res_s[nl] * s.res_t[nl];
             if (cells > 2.0 * static_cast<double>(N)) break;
@@ -307,13 +308,32 @@ static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSor
     cs->bits_t = bt - cs->shift_t;
     cs->n_bins = 1u << (3 * cs->bits_s + cs->bits_t);
     const uint32_t chunk = debug_u32(DASH_DEBUG_BWD_RUN_CHUNK);
-    cs->chunk = chunk ? chunk : 64u;
+    cs->chunk = chunk ? chunk : 32u;   // 24-48 measure alike (C4, C5); 8 and 128 lose 1-3 %
     return true;
 }
 
 static size_t coarse_workspace(const dash::CoarseSort& cs, uint64_t N) {
     return round16(N * 4) * 2 + round16(N * 16) + round16(static_cast<size_t>(cs.n_bins) * 4) +
            round16((static_cast<size_t>(cs.n_bins) + 1023) / 1024 * 4);
+}
+
+struct CoarseBuffers {
+    int32_t* order;
+    uint32_t* keys;
+    float4* sorted_q;
+    uint32_t* bins;
+    uint32_t* totals;
+};
+
+static CoarseBuffers carve_coarse(void* workspace, const dash::CoarseSort& cs, uint64_t N) {
+    char* w = static_cast<char*>(workspace) + kHeaderBytes;
+    CoarseBuffers b;
+    b.order = reinterpret_cast<int32_t*>(w);
+    b.keys = reinterpret_cast<uint32_t*>(w + round16(N * 4));
+    b.sorted_q = reinterpret_cast<float4*>(w + 2 * round16(N * 4));
+    b.bins = reinterpret_cast<uint32_t*>(w + 2 * round16(N * 4) + round16(N * 16));
+    b.totals = b.bins + round16(static_cast<size_t>(cs.n_bins) * 4) / 4;
+    return b;
 }
 
 static size_t workspace_need(const dash_hash4d_config* cfg, int op, uint64_t N, int dims = 4) {
@@ -323,7 +343,8 @@ static size_t workspace_need(const dash_hash4d_config* cfg, int op, uint64_t N, 
     if (op == DASH_HASH4D_OP_BWD && (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD))
         bytes = kHeaderBytes + table_elems(cfg) * sizeof(long long);
     dash::CoarseSort cs;
-    if (op == DASH_HASH4D_OP_BWD && dims == 4 && plan_coarse(cfg, N, &cs)) bytes = kHeaderBytes + coarse_workspace(cs, N);
+    if ((op == DASH_HASH4D_OP_BWD || op == DASH_HASH4D_OP_FWD) && dims == 4 && plan_coarse(cfg, N, &cs))
+        bytes = kHeaderBytes + coarse_workspace(cs, N);
     return bytes;
 }
 
@@ -356,8 +377,52 @@ static int fwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
     if (dims == 3 && group > 4 && 4 * cfg->F * sizeof(float) >= 32 && !debug_u32(DASH_DEBUG_FWD_GROUP))
         group = 4;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride, group, &P, dims)) return rc;
+    dash::CoarseSort cs;
+    const bool coarse = dims == 4 && plan_coarse(cfg, N, &cs);
+    const size_t need = workspace_need(cfg, DASH_HASH4D_OP_FWD, N, dims);
+    if (coarse && (!workspace || workspace_bytes < need))
+        return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "fwd needs %zu workspace bytes, got %zu", need, workspace_bytes);
+    if (coarse && !aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
-    cudaError_t e = dash::launch_fwd(P, xyz, t, index, table, half, out, s);
+    cudaError_t e = cudaSuccess;
+    if (coarse) {
+        // SORT_COARSE: the coarse levels in cell-sorted order (a warp's lanes then share cells and lines: C4 levels 0-3
+        // 120 -> 72 us, profiles/experiments_r02.md §8), the others in the caller's order
+        const CoarseBuffers b = carve_coarse(workspace, cs, N);
+        if (!(cfg->flags & DASH_HASH4D_FLAG_ORDER_READY))
+            e = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s);
+        if (e != cudaSuccess) return cuda_fail(e, "coarse sort launch");
+        Plan Pc = P;
+        uint32_t g = P.group;
+        while (g > cs.levels) g /= 2;
+        uint32_t lg = 0;
+        while ((1u << lg) < g) ++lg;
+        Pc.group = g;
+        Pc.group_log2 = lg;
+        Pc.q_per_block = dash::kItemsPerBlock >> lg;
+        Pc.level_end = cs.levels;
+        Pc.num_groups = (cs.levels + g - 1) / g;
+        e = dash::launch_fwd(Pc, xyz, t, index, table, half, out, s, b.order, b.sorted_q);
+        if (e != cudaSuccess) return cuda_fail(e, "coarse fwd launch");
+        // the other levels: whole groups of P.group in one launch, a ragged rest as smaller power-of-two groups
+        for (uint32_t l0 = cs.levels; l0 < cfg->L;) {
+            uint32_t gr = P.group;
+            while (gr > cfg->L - l0) gr /= 2;
+            Plan Pr = P;
+            lg = 0;
+            while ((1u << lg) < gr) ++lg;
+            Pr.group = gr;
+            Pr.group_log2 = lg;
+            Pr.q_per_block = dash::kItemsPerBlock >> lg;
+            Pr.level_begin = l0;
+            Pr.num_groups = (cfg->L - l0) / gr;
+            e = dash::launch_fwd(Pr, xyz, t, index, table, half, out, s);
+            if (e != cudaSuccess) return cuda_fail(e, "fwd launch");
+            l0 += Pr.num_groups * gr;
+        }
+        return ok();
+    }
+    e = dash::launch_fwd(P, xyz, t, index, table, half, out, s);
     if (e != cudaSuccess) return cuda_fail(e, "fwd launch");
     return ok();
 }
@@ -511,13 +576,12 @@ static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
     const bool coarse = dims == 4 && plan_coarse(cfg, N, &cs);
     const uint32_t l_first = coarse ? cs.levels : 0u;
     auto scatter_coarse = [&](bool hint) -> cudaError_t {
-        char* w = static_cast<char*>(workspace) + kHeaderBytes;
-        int32_t* order = reinterpret_cast<int32_t*>(w);
-        uint32_t* keys = reinterpret_cast<uint32_t*>(w + round16(N * 4));
-        float4* sorted_q = reinterpret_cast<float4*>(w + 2 * round16(N * 4));
-        uint32_t* bins = reinterpret_cast<uint32_t*>(w + 2 * round16(N * 4) + round16(N * 16));
-        uint32_t* totals = bins + round16(static_cast<size_t>(cs.n_bins) * 4) / 4;
-        return dash::launch_bwd_runs(P, cs, xyz, t, index, dout, dtable, order, sorted_q, keys, bins, totals, s, hint);
+        const CoarseBuffers b = carve_coarse(workspace, cs, N);
+        cudaError_t ce = cudaSuccess;
+        if (!(cfg->flags & DASH_HASH4D_FLAG_ORDER_READY))
+            ce = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s);
+        if (ce == cudaSuccess) ce = dash::launch_bwd_runs(P, cs, dout, dtable, b.order, b.sorted_q, s, hint);
+        return ce;
     };
     // the levels [l0, L) in groups of P.group (a ragged last group shrinks to the largest power of two that fits)
     auto scatter_rest = [&](uint32_t l0, bool hint) -> cudaError_t {

@@ -41,9 +41,9 @@ __device__ __forceinline__ Item this_item(const Plan& P, uint32_t tile, uint32_t
     it.xc = threadIdx.x & 1u;
     it.n = static_cast<uint64_t>(tile) * P.q_per_block + (pair >> P.group_log2);
     it.l = P.level_begin + grp * P.group + (pair & (P.group - 1u));
-    it.active = (it.n < P.N) && (it.l < P.L);
+    it.active = (it.n < P.N) && (it.l < P.level_end);
     if (it.n >= P.N) it.n = P.N - 1;
-    if (it.l >= P.L) it.l = P.L - 1;
+    if (it.l >= P.level_end) it.l = P.level_end - 1;
     return it;
 }
 
@@ -56,11 +56,21 @@ template <int F, bool HALF, int D>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_fwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                   const float* __restrict__ t, const int32_t* __restrict__ index,
-                  const void* __restrict__ table, float* __restrict__ out) {
+                  const void* __restrict__ table, float* __restrict__ out,
+                  const int32_t* __restrict__ order, const float4* __restrict__ sorted_q) {
     constexpr int NC = 1 << (D - 1);
-    const Item it = this_item(P);
+    Item it = this_item(P);
     const LevelParams lp = P.lv[it.l];
-    const Query q = load_query<D>(P, lp, it.n, xyz, t, index);
+    Query q;
+    if (order) {   // SORT_COARSE: position it.n of the cell-sorted order (bwd_runs_kernels.cu) — neighbouring lanes
+                   // then gather from the same cells; the row of `out` is the query's own
+        const float4 c = __ldg(sorted_q + it.n);
+        q = make_query<D>(lp, c.x, c.y, c.z, c.w);
+        const uint64_t n = static_cast<uint64_t>(static_cast<uint32_t>(__ldg(order + it.n)));
+        it.n = n < P.N ? n : P.N - 1;   // memory-safe even if the caller's ORDER_READY claim is false
+    } else {
+        q = load_query<D>(P, lp, it.n, xyz, t, index);
+    }
     uint32_t slot[NC];
     float W[NC];
     half_cell<D>(P, lp, q, it.xc, slot, W);
@@ -641,13 +651,29 @@ sort_keys_kernel(uint64_t N, const float* __restrict__ xyz, uint32_t xyz_stride,
     }
 }
 
-// exclusive scan, phase 1: each CTA scans 1024 bins in place and writes its total
-__global__ void __launch_bounds__(1024) sort_scan_local_kernel(uint32_t* __restrict__ bins, uint32_t n_bins,
-                                                               uint32_t* __restrict__ totals) {
-    __shared__ uint32_t warp_sum[32];
-    const uint32_t i = blockIdx.x * 1024u + threadIdx.x, lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
-    const uint32_t v = i < n_bins ? bins[i] : 0u;
-    uint32_t x = v;
+// exclusive scan, phase 1: each CTA of 256 threads scans kScanTile = 4096 bins in place (16 per thread, four 16-byte
+// loads) and writes its total.  The bins array is allocated in multiples of 16 bytes; elements >= n_bins count as 0.
+__global__ void __launch_bounds__(kBlockThreads) sort_scan_local_kernel(uint32_t* __restrict__ bins, uint32_t n_bins,
+                                                                        uint32_t* __restrict__ totals) {
+    __shared__ uint32_t warp_sum[kBlockThreads / 32];
+    const uint32_t lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    const uint32_t first = blockIdx.x * kScanTile + threadIdx.x * 16u;
+    uint4* p = reinterpret_cast<uint4*>(bins + first);
+    uint32_t v[16];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        uint4 a = make_uint4(0u, 0u, 0u, 0u);
+        if (first + 4u * k < n_bins) a = p[k];
+        v[4 * k] = a.x; v[4 * k + 1] = a.y; v[4 * k + 2] = a.z; v[4 * k + 3] = a.w;
+    }
+    uint32_t sum = 0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const uint32_t x = (first + k < n_bins) ? v[k] : 0u;
+        v[k] = sum;            // exclusive within the thread
+        sum += x;
+    }
+    uint32_t x = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
@@ -655,22 +681,18 @@ __global__ void __launch_bounds__(1024) sort_scan_local_kernel(uint32_t* __restr
     }
     if (lane == 31) warp_sum[w] = x;
     __syncthreads();
-    if (w == 0) {
-        uint32_t s = warp_sum[lane];
+    uint32_t before = x - sum;   // exclusive within the warp
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t y = __shfl_up_sync(0xffffffffu, s, o);
-            if (lane >= static_cast<uint32_t>(o)) s += y;
-        }
-        warp_sum[lane] = s;   // inclusive over warps
-    }
-    __syncthreads();
-    const uint32_t before = w ? warp_sum[w - 1] : 0u;
-    if (i < n_bins) bins[i] = before + x - v;   // exclusive within the CTA
-    if (threadIdx.x == 1023) totals[blockIdx.x] = before + x;
+    for (uint32_t k = 0; k < kBlockThreads / 32; ++k)
+        if (k < w) before += warp_sum[k];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (first + 4u * k < n_bins)
+            p[k] = make_uint4(before + v[4 * k], before + v[4 * k + 1], before + v[4 * k + 2], before + v[4 * k + 3]);
+    if (threadIdx.x == kBlockThreads - 1) totals[blockIdx.x] = before + sum;
 }
 
-// phase 2: one CTA turns the (<= 2048) CTA totals into exclusive offsets
+// phase 2: one CTA turns the CTA totals into exclusive offsets
 __global__ void __launch_bounds__(1024) sort_scan_totals_kernel(uint32_t* __restrict__ totals, uint32_t n) {
     __shared__ uint32_t warp_sum[32];
     __shared__ uint32_t carry;
@@ -705,11 +727,19 @@ __global__ void __launch_bounds__(1024) sort_scan_totals_kernel(uint32_t* __rest
     }
 }
 
-// phase 3: add the CTA offsets
-__global__ void __launch_bounds__(1024) sort_scan_add_kernel(uint32_t* __restrict__ bins, uint32_t n_bins,
-                                                             const uint32_t* __restrict__ totals) {
-    const uint32_t i = blockIdx.x * 1024u + threadIdx.x;
-    if (i < n_bins) bins[i] += totals[blockIdx.x];
+// phase 3: add the CTA offsets (callers that index bins through their own kernel add totals[i / kScanTile] there)
+__global__ void __launch_bounds__(kBlockThreads) sort_scan_add_kernel(uint32_t* __restrict__ bins, uint32_t n_bins,
+                                                                      const uint32_t* __restrict__ totals) {
+    const uint32_t first = blockIdx.x * kScanTile + threadIdx.x * 16u;
+    const uint32_t off = totals[blockIdx.x];
+    uint4* p = reinterpret_cast<uint4*>(bins + first);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (first + 4u * k < n_bins) {
+            uint4 a = p[k];
+            a.x += off; a.y += off; a.z += off; a.w += off;
+            p[k] = a;
+        }
 }
 
 __global__ void __launch_bounds__(kBlockThreads)
@@ -772,14 +802,16 @@ uint64_t launch_counter(bool reset) {
 }
 
 cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
-                       const void* table, bool table_half, float* out, cudaStream_t s) {
+                       const void* table, bool table_half, float* out, cudaStream_t s, const int32_t* order,
+                       const float4* sorted_q) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
-#define DASH_FWD(FV, HV)                                                                       \
-    do {                                                                                       \
-        if (P.dims == 3)                                                                       \
-            hash4d_fwd_kernel<FV, HV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, table, out); \
-        else                                                                                   \
-            hash4d_fwd_kernel<FV, HV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, table, out); \
+    if (P.dims == 3 && order) return cudaErrorInvalidValue;
+#define DASH_FWD(FV, HV)                                                                                        \
+    do {                                                                                                        \
+        if (P.dims == 3)                                                                                        \
+            hash4d_fwd_kernel<FV, HV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, nullptr, nullptr); \
+        else                                                                                                    \
+            hash4d_fwd_kernel<FV, HV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, order, sorted_q); \
     } while (0)
     switch (P.F * 2 + (table_half ? 1 : 0)) {
         case 2: DASH_FWD(1, false); break;
@@ -952,15 +984,17 @@ cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t co
     return after_launch();
 }
 
-// bins[i] <- sum of bins[0..i) in place (three launches); totals: scratch of ceil(n_bins / 1024) uint32
-cudaError_t launch_exclusive_scan_u32(uint32_t* bins, uint32_t n_bins, uint32_t* totals, cudaStream_t s) {
-    const uint32_t scan_ctas = (n_bins + 1023u) / 1024u;
+// bins[i] <- sum of bins[0..i) in place; totals: scratch of ceil(n_bins / kScanTile) uint32.  add_offsets = false
+// leaves the scan per tile of kScanTile bins: the full value is bins[i] + totals[i / kScanTile] (one launch less).
+cudaError_t launch_exclusive_scan_u32(uint32_t* bins, uint32_t n_bins, uint32_t* totals, cudaStream_t s,
+                                      bool add_offsets) {
+    const uint32_t scan_ctas = (n_bins + kScanTile - 1u) / kScanTile;
     cudaError_t e;
-    sort_scan_local_kernel<<<scan_ctas, 1024, 0, s>>>(bins, n_bins, totals);
+    sort_scan_local_kernel<<<scan_ctas, kBlockThreads, 0, s>>>(bins, n_bins, totals);
     if ((e = after_launch()) != cudaSuccess) return e;
     sort_scan_totals_kernel<<<1, 1024, 0, s>>>(totals, scan_ctas);
-    if ((e = after_launch()) != cudaSuccess) return e;
-    sort_scan_add_kernel<<<scan_ctas, 1024, 0, s>>>(bins, n_bins, totals);
+    if ((e = after_launch()) != cudaSuccess || !add_offsets) return e;
+    sort_scan_add_kernel<<<scan_ctas, kBlockThreads, 0, s>>>(bins, n_bins, totals);
     return after_launch();
 }
 

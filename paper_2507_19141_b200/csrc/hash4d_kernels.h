@@ -19,8 +19,10 @@ struct WorkspaceHeader {
 };
 static_assert(sizeof(WorkspaceHeader) == 128, "workspace header is 128 bytes");
 
+// order / sorted_q (both or neither; G_4D only): walk the queries in the cell-sorted order of launch_coarse_sort
 cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
-                       const void* table, bool table_half, float* out, cudaStream_t s);
+                       const void* table, bool table_half, float* out, cudaStream_t s,
+                       const int32_t* order = nullptr, const float4* sorted_q = nullptr);
 cudaError_t launch_bwd_input(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                              const void* table, bool table_half, const float* dout, float* dq,
                              cudaStream_t s);
@@ -42,7 +44,9 @@ cudaError_t launch_fixed_finalize(const long long* acc, float* dtable, size_t co
 cudaError_t launch_sort_queries(uint64_t N, const float* xyz, uint32_t xyz_stride, const int32_t* index,
                                 uint32_t bits, int32_t* order, uint32_t* keys, uint32_t* bins, uint32_t* totals,
                                 cudaStream_t s);
-cudaError_t launch_exclusive_scan_u32(uint32_t* bins, uint32_t n_bins, uint32_t* totals, cudaStream_t s);
+constexpr uint32_t kScanTile = 4096;   // bins one CTA of the exclusive scan covers
+cudaError_t launch_exclusive_scan_u32(uint32_t* bins, uint32_t n_bins, uint32_t* totals, cudaStream_t s,
+                                      bool add_offsets = true);
 // Run-merged scatter of the coarse levels (bwd_runs_kernels.cu; DASH_HASH4D_FLAG_SORT_COARSE): sort the queries by the
 // 4D cell of level `key_level`, then reduce runs of queries that share a cell in registers before they reach L2.
 struct CoarseSort {
@@ -52,9 +56,12 @@ struct CoarseSort {
     uint32_t chunk;       // consecutive sorted queries walked by one lane pair
     uint32_t n_bins;      // 1 << (3 bits_s + bits_t)
 };
-cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* xyz, const float* t, const int32_t* index,
-                            const float* dout, float* dtable, int32_t* order, float4* sorted_q, uint32_t* keys,
-                            uint32_t* bins, uint32_t* totals, cudaStream_t s, bool l2_hint);
+// order[i] = number of the i-th query in key order, sorted_q[i] = its (x, y, z, t); keys / bins / totals: scratch
+cudaError_t launch_coarse_sort(const Plan& P, const CoarseSort& cs, const float* xyz, const float* t,
+                               const int32_t* index, int32_t* order, float4* sorted_q, uint32_t* keys, uint32_t* bins,
+                               uint32_t* totals, cudaStream_t s);
+cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* dout, float* dtable, const int32_t* order,
+                            const float4* sorted_q, cudaStream_t s, bool l2_hint);
 cudaError_t launch_slice_t(const Plan& P, const float* t, const void* table, bool table_half, float* slice,
                            cudaStream_t s);
 cudaError_t launch_adam(size_t count, double lr, double beta1, double beta2, double eps, uint32_t step,

@@ -28,6 +28,7 @@ struct Plan {
     uint32_t group;       // levels per level group G (power of two <= 16)
     uint32_t group_log2;
     uint32_t level_begin; // first level this launch covers (per-group launches), else 0
+    uint32_t level_end;   // one past the last level this launch covers (L unless a launch takes a leading part)
     uint32_t num_groups;  // level groups this launch covers (gridDim.y)
     uint32_t q_per_block; // kItemsPerBlock >> group_log2
     uint32_t dims;        // 4: G_4D (x,y,z,t); 3: G_3D of the decomposition stage (x,y,z), t unused

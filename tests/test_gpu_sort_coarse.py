@@ -1,8 +1,9 @@
-"""GPU parity of the collision-aware scatter (DASH_HASH4D_FLAG_SORT_COARSE): counting sort of the queries by the 4D cell
-of the finest coarse level + run-merged reductions on the coarse levels, the other levels unchanged.  The result is the
-same table gradient as the plain backward (same sums, another order), so every check is the plain backward's check
-against the oracle (tests/parity_utils.py): element by element with the hits-aware tolerance, normwise per level, and the
-whole-buffer checksum.  BASELINE.json config 5 is the workload the flag exists for.
+"""GPU parity of the collision-aware path (DASH_HASH4D_FLAG_SORT_COARSE): counting sort of the queries by the 4D cell
+of the finest coarse level; backward: run-merged reductions on the coarse levels; forward: the coarse levels walked in
+that order; the other levels unchanged.  The results are those of the plain calls (forward: same values; backward: same
+sums in another order), so every check is the plain call's check against the oracle (tests/parity_utils.py): element by
+element with the hits-aware tolerance, normwise per level, and the whole-buffer checksum.  BASELINE.json config 5 is the
+workload the flag exists for.
 """
 import ctypes as C
 
@@ -14,21 +15,40 @@ import oracle
 import paper_2507_19141_b200 as dh
 from dash_inputs import EncoderParams, make_queries_uniform, make_workload
 from parity_utils import RTOL_FP32, check_close
-from test_gpu_parity import DC, both_configs, dev, run_bwd_parity
+from test_gpu_parity import DC, both_configs, dev, run_bwd_parity, run_fwd_parity
 
 pytestmark = pytest.mark.gpu
 
 SC = dh.FLAG_SORT_COARSE
 ZG = dh.FLAG_ZERO_GRAD
+READY = dh.FLAG_ORDER_READY
 
 
 @pytest.mark.parametrize("name", ["C3", "C4", "C5"])
 def test_full_size_configs(name):
-    """The bench's launch configuration (ZERO_GRAD + SORT_COARSE, the library's own choice of coarse levels)."""
-    wl = make_workload(name, with_table=False)
-    cfg = dh.config_from_params(wl.spec.enc, flags=DC | ZG | SC)
-    assert dh.dash_hash4d_workspace_bytes(cfg, wl.N, dh.OP_BWD) >= 24 * wl.N
-    run_bwd_parity(wl.spec.enc, wl.xyz, wl.t, wl.dout, index=wl.index, flags=DC | ZG | SC, what=name + " sort_coarse")
+    """The bench's launch configuration (ZERO_GRAD + SORT_COARSE, the library's own choice of coarse levels; the forward
+    sorts, the backward of the same step reuses the order).  C3 (N < 2^19) takes the plain path and needs no workspace."""
+    wl = make_workload(name)
+    enc, N = wl.spec.enc, wl.N
+    cfg = dh.config_from_params(enc, flags=DC | ZG | SC)
+    need = dh.dash_hash4d_workspace_bytes(cfg, N, dh.OP_BWD)
+    assert need == dh.dash_hash4d_workspace_bytes(cfg, N, dh.OP_FWD)
+    assert (need >= 24 * N) if N >= (1 << 19) else (need == 0)
+    run_fwd_parity(enc, wl.xyz, wl.t, wl.table, index=wl.index, flags=DC | SC, what=name + " sort_coarse")
+    run_bwd_parity(enc, wl.xyz, wl.t, wl.dout, index=wl.index, flags=DC | ZG | SC, what=name + " sort_coarse")
+    if need:
+        # one step as bench.py runs it: fwd sorts into the workspace, bwd (ORDER_READY) reuses it
+        ocfg, _ = both_configs(enc, DC)
+        ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+        xd, td, idd = dev(wl.xyz), dev(wl.t), dev(wl.index)
+        out = dh.dash_hash4d_fwd(cfg, xd, td, dev(wl.table), index=idd, workspace=ws)
+        dt = torch.full((enc.L, enc.T, enc.F), 7.0, device="cuda")
+        dh.dash_hash4d_bwd(dh.with_flags(cfg, DC | ZG | SC | READY), xd, td, dev(wl.dout), dt, index=idd, workspace=ws)
+        torch.cuda.synchronize()
+        ref, mag, hits = oracle.oracle_bwd(ocfg, N, wl.xyz, wl.t, wl.dout, index=wl.index, want_abs=True, want_hits=True)
+        check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, enc.L, hits=hits, what=name + " bwd on the forward's order")
+        plain = dh.dash_hash4d_fwd(dh.config_from_params(enc, flags=DC), xd, td, dev(wl.table), index=idd)
+        assert torch.equal(out, plain), "the sorted forward computes the same fp32 values, in another thread order"
 
 
 @pytest.mark.parametrize("levels", [1, 2, 3, 5, 16])
@@ -45,6 +65,9 @@ def test_forced_coarse_levels_and_chunks(levels, chunk, set_debug):
         xyz, t = make_queries_uniform(L + levels, n)
         dout = rng.standard_normal((n, L * F)).astype(np.float32)
         run_bwd_parity(enc, xyz, t, dout, flags=flags, what=f"sort_coarse L{L} F{F} levels{levels} chunk{chunk}")
+        if chunk == 7:   # the forward does not depend on the chunk length
+            table = rng.uniform(-1, 1, (L, T, F)).astype(np.float32)
+            run_fwd_parity(enc, xyz, t, table, flags=flags & ~ZG, what=f"sort_coarse fwd L{L} F{F} levels{levels}")
 
 
 def test_long_runs_index_list_broadcast_t_and_existing_gradient(set_debug):
@@ -64,6 +87,10 @@ def test_long_runs_index_list_broadcast_t_and_existing_gradient(set_debug):
     run_bwd_parity(enc, xyz, t, dout, index=index, flags=DC | SC, init=init, what="clustered, accumulate")
     t1 = np.array([0.37], np.float32)
     run_bwd_parity(enc, xyz, t1, dout[:rows], t_stride=0, flags=DC | ZG | SC, what="one timestamp")
+    table = rng.uniform(-1, 1, (8, 1 << 13, 2)).astype(np.float16)
+    enc16 = EncoderParams(8, 2, 1 << 13, 8, 512, 4, 64, "fp16")
+    run_fwd_parity(enc16, xyz, t, table, index=index, flags=DC | SC, rtol=RTOL_FP32, what="clustered, indexed, fp16")
+    run_fwd_parity(enc16, xyz, t1, table, t_stride=0, flags=DC | SC, rtol=RTOL_FP32, what="one timestamp, fp16")
 
 
 def test_tiny_and_edge_inputs(set_debug):
@@ -93,7 +120,8 @@ def test_workspace_is_required_and_sized_by_the_library(set_debug):
     n = 1000
     need = dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD)
     assert need >= 24 * n
-    assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_FWD) == 0          # only the backward sorts
+    assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_FWD) == need       # one buffer serves fwd and bwd of a step
+    assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD_INPUT) == 0    # the other calls ignore the flag
     assert dh.dash_hash4d_workspace_bytes(dh.with_flags(cfg, DC | SC | dh.FLAG_DETERMINISTIC_BWD), n, dh.OP_BWD) == \
         dh.dash_hash4d_workspace_bytes(dh.with_flags(cfg, DC | dh.FLAG_DETERMINISTIC_BWD), n, dh.OP_BWD)
     xyz, t = make_queries_uniform(1, n)
