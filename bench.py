@@ -371,7 +371,8 @@ def run_cuda(args):
     debug_keys = {"fwd_group": dh.DEBUG_FWD_GROUP, "bwd_group": dh.DEBUG_BWD_GROUP,
                   "smooth_group": dh.DEBUG_SMOOTH_GROUP, "deform_path": dh.DEBUG_DEFORM_PATH,
                   "bwd_variant": dh.DEBUG_BWD_VARIANT, "fwd_variant": dh.DEBUG_FWD_VARIANT,
-                  "bwd_coarse_levels": dh.DEBUG_BWD_COARSE_LEVELS, "bwd_run_chunk": dh.DEBUG_BWD_RUN_CHUNK}
+                  "bwd_coarse_levels": dh.DEBUG_BWD_COARSE_LEVELS, "bwd_run_chunk": dh.DEBUG_BWD_RUN_CHUNK,
+                  "fwd_ordered_levels": dh.DEBUG_FWD_ORDERED_LEVELS}
     for item in args.set_debug:
         key, _, val = item.partition("=")
         dh.dash_hash4d_set_debug(debug_keys[key], int(val))

@@ -307,6 +307,11 @@ static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSor
     cs->bits_s = bs - cs->shift_s;
     cs->bits_t = bt - cs->shift_t;
     cs->n_bins = 1u << (3 * cs->bits_s + cs->bits_t);
+    // The forward walks EVERY level in the sorted order: neighbouring lanes share cells and lines well past the levels
+    // whose reductions merge (C4, key 48 per axis: levels of 16-48 per axis -40 %, 70-101 -38 %, 147-212 -21 %, finer
+    // ones -3 %), and one launch over all levels beats any split (profiles/experiments_r02.md §8).
+    const uint32_t forced_fwd = debug_u32(DASH_DEBUG_FWD_ORDERED_LEVELS);
+    cs->levels_fwd = forced_fwd ? (forced_fwd < c->L ? forced_fwd : c->L) : c->L;
     const uint32_t chunk = debug_u32(DASH_DEBUG_BWD_RUN_CHUNK);
     cs->chunk = chunk ? chunk : 32u;   // 24-48 measure alike (C4, C5); 8 and 128 lose 1-3 %
     return true;
@@ -393,19 +398,20 @@ static int fwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
             e = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s);
         if (e != cudaSuccess) return cuda_fail(e, "coarse sort launch");
         Plan Pc = P;
+        const uint32_t lf = cs.levels_fwd;
         uint32_t g = P.group;
-        while (g > cs.levels) g /= 2;
+        while (g > lf) g /= 2;
         uint32_t lg = 0;
         while ((1u << lg) < g) ++lg;
         Pc.group = g;
         Pc.group_log2 = lg;
         Pc.q_per_block = dash::kItemsPerBlock >> lg;
-        Pc.level_end = cs.levels;
-        Pc.num_groups = (cs.levels + g - 1) / g;
+        Pc.level_end = lf;
+        Pc.num_groups = (lf + g - 1) / g;
         e = dash::launch_fwd(Pc, xyz, t, index, table, half, out, s, b.order, b.sorted_q);
         if (e != cudaSuccess) return cuda_fail(e, "coarse fwd launch");
         // the other levels: whole groups of P.group in one launch, a ragged rest as smaller power-of-two groups
-        for (uint32_t l0 = cs.levels; l0 < cfg->L;) {
+        for (uint32_t l0 = lf; l0 < cfg->L;) {
             uint32_t gr = P.group;
             while (gr > cfg->L - l0) gr /= 2;
             Plan Pr = P;

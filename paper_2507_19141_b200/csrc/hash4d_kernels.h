@@ -51,6 +51,7 @@ cudaError_t launch_exclusive_scan_u32(uint32_t* bins, uint32_t n_bins, uint32_t*
 // 4D cell of level `key_level`, then reduce runs of queries that share a cell in registers before they reach L2.
 struct CoarseSort {
     uint32_t levels;      // leading levels [0, levels) taken by the run-merged scatter (0: path not used)
+    uint32_t levels_fwd;  // leading levels the FORWARD walks in the sorted order (>= levels)
     uint32_t key_level;   // the cell of this level is the sort key (the finest of them)
     uint32_t bits_s, bits_t, shift_s, shift_t;  // Morton key: (cell >> shift) per axis, bits per spatial axis / for t
     uint32_t chunk;       // consecutive sorted queries walked by one lane pair
