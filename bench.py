@@ -454,8 +454,12 @@ def run_cuda(args):
         dom_bytes += b_zero
     dom_ms = ms_bwd if dominant == "bwd" else ms_fwd
     kernel_name = f"hash4d_{dominant}_kernel"
+    sorted_path = bool(args.sort_coarse) and bwd_ws is not None
     if dominant == "bwd" and args.zero_grad_fused:
         kernel_name = "hash4d_bwd_kernel+zero_kernel (one dash_hash4d_bwd call, ZERO_GRAD)"
+        if sorted_path:
+            kernel_name = ("hash4d_bwd_kernel+hash4d_bwd_runs_kernel+zero_kernel (one dash_hash4d_bwd call, ZERO_GRAD, "
+                           "SORT_COARSE with the forward's order)")
     achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
     step_bytes = (b_fwd + b_bwd) * N + b_zero
     roofline = {
@@ -489,7 +493,9 @@ def run_cuda(args):
         "fwd_frac_of_gather_ceiling": lane_ops / (ms_fwd * 1e-3) / 1e9 / ceil["gather8_pair_xcorner_L2"]["G_lane_ops_per_s"],
         "bwd_frac_of_red_ceiling": lane_ops / (ms_bwd * 1e-3) / 1e9 / ceil[red_key]["G_lane_ops_per_s"],
         "note": "microbenchmarks of include/dash_ceilings.h run in this process (L2-resident 32 MiB footprint, "
-                "x-corner lane pairs, 8 accesses in flight per lane); bwd time includes the fused zero passes",
+                "x-corner lane pairs, 8 accesses in flight per lane, RANDOM addresses); bwd time includes the fused zero "
+                "passes, fwd time the coarse sort; with sort_coarse the path shares lines between neighbouring lanes and "
+                "merges reductions, so a fraction above 1 means fewer accesses reach L1 / L2 than the method names",
     }
 
     # ---- deterministic mode (DETERMINISTIC_BWD, 64-bit fixed point): what it costs on this workload
@@ -695,6 +701,7 @@ def run_cuda(args):
                    "queries_per_step_per_gpu": N, "parallelism": f"replicas x{world}",
                    "l2": l2_note,
                    "zero_grad_fused": bool(args.zero_grad_fused),
+                   "sort_coarse": sorted_path,
                    **({"debug_overrides": args.set_debug} if args.set_debug else {})},
         "roofline": roofline,
         "e2e": {"value": N * world / (e2e_ms * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -725,8 +732,10 @@ def main():
                          "(no kernels, no measurement; tests/test_replicas_gloo.py)")
     ap.add_argument("--zero-grad-fused", type=int, default=1,
                     help="1: bwd zeroes each level group itself (DASH_HASH4D_FLAG_ZERO_GRAD)")
-    ap.add_argument("--sort-coarse", type=int, default=0,
-                    help="1: bwd scatters the coarse levels by sort + run-merged reduction (DASH_HASH4D_FLAG_SORT_COARSE)")
+    ap.add_argument("--sort-coarse", type=int, default=1,
+                    help="1: DASH_HASH4D_FLAG_SORT_COARSE — fwd sorts the queries by coarse 4D cell and walks them in that "
+                         "order, bwd reuses the order (ORDER_READY) and merges runs on the coarse levels; the library "
+                         "ignores the flag below 2^19 queries.  0: the plain path (A/B)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", type=int, default=1,
                     help="1: also time bwd_input / smooth / one-timestamp fwd (information only)")

@@ -8,8 +8,9 @@
 Accepts both CSV shapes ncu writes: the wide `--page raw --csv` export (header row, units row, one row per launch)
 and the long `--csv --log-file` list of a `--metrics` run (one row per launch and metric).  Units are normalised
 (bytes, microseconds).  The traffic file gets, per config: DRAM bytes (read + write) of every launch class and of
-the C-ABI calls of ONE step — "fwd_call" (hash4d_fwd_kernel launches), "bwd_call" (zero_kernel + hash4d_bwd_kernel
-launches), "step" (both) — taken from the LAST complete step in the capture.  No number is typed by hand.
+the C-ABI calls of ONE step — "fwd_call" (hash4d_fwd_kernel launches and, under SORT_COARSE, the sort before them),
+"bwd_call" (zero_kernel + hash4d_bwd_kernel + hash4d_bwd_runs_kernel launches), "step" (both) — taken from the LAST
+complete step in the capture.  No number is typed by hand.
 """
 from __future__ import annotations
 
@@ -93,18 +94,50 @@ def read_launches(path: str):
     return [launches[k] for k in sorted(launches)]
 
 
+_BWD_CALL = ("hash4d_bwd_kernel", "hash4d_bwd_runs_kernel", "zero_kernel")   # launches of one dash_hash4d_bwd call
+_SORT = ("sort4d_", "sort_scan_")   # the coarse sort: in the forward call under SORT_COARSE (bench.py), else in bwd
+
+
+def _is(kernel: str, names) -> bool:
+    return any(n in kernel for n in names)
+
+
 def last_step(launches):
-    """The launches of the last complete step: from the last hash4d_fwd_kernel launch that is followed by at least
-    one hash4d_bwd_kernel launch up to (excluding) the next fwd launch / anything that is not zero or bwd."""
-    is_fwd = [("hash4d_fwd_kernel" in l["kernel"]) for l in launches]
-    starts = [i for i, f in enumerate(is_fwd) if f]
-    for s in reversed(starts):
-        e = s + 1
-        while e < len(launches) and ("hash4d_bwd_kernel" in launches[e]["kernel"] or "zero_kernel" in launches[e]["kernel"]):
+    """The launches of the last complete step.  A step is one forward call — the hash4d_fwd_kernel launch(es), preceded
+    under SORT_COARSE by the coarse sort (zero_kernel of its histogram + sort launches) — followed by the launches of
+    one backward call (zero / bwd / bwd_runs, and the sort when the backward does its own); it ends where the next
+    forward call starts or at anything else.  The last step that holds at least one hash4d_bwd_kernel wins."""
+    n = len(launches)
+    k = [l["kernel"] for l in launches]
+    starts = []                                        # (first launch of the forward call, its first fwd launch)
+    for f in range(n):
+        if "hash4d_fwd_kernel" in k[f] and (f == 0 or "hash4d_fwd_kernel" not in k[f - 1]):
+            s = f
+            while s > 0 and _is(k[s - 1], _SORT):
+                s -= 1
+            if s < f and s > 0 and "zero_kernel" in k[s - 1]:
+                s -= 1
+            starts.append((s, f))
+    for j in range(len(starts) - 1, -1, -1):
+        s, f = starts[j]
+        limit = starts[j + 1][0] if j + 1 < len(starts) else n
+        e = f
+        while e < limit and "hash4d_fwd_kernel" in k[e]:
             e += 1
-        if any("hash4d_bwd_kernel" in l["kernel"] for l in launches[s + 1:e]):
+        b = e
+        while e < limit and _is(k[e], _BWD_CALL + _SORT):
+            e += 1
+        if any("hash4d_bwd_kernel" in x for x in k[b:e]):
             return launches[s:e]
     return []
+
+
+def is_fwd_call(step, i) -> bool:
+    """Launch i of `step` belongs to the forward call: the hash4d_fwd_kernel launches and the sort before them."""
+    first_bwd = next((j for j, l in enumerate(step) if _is(l["kernel"], ("hash4d_bwd_kernel", "hash4d_bwd_runs_kernel"))),
+                     len(step))
+    last_fwd = max((j for j, l in enumerate(step) if "hash4d_fwd_kernel" in l["kernel"]), default=-1)
+    return i <= last_fwd and i < first_bwd
 
 
 def dram(l):
@@ -132,8 +165,8 @@ def markdown(launches, step, title, command):
                 cells.append(f"{v:.0f}")
         out.append(f"| {l['id']} | `{_short(l['kernel'])}` | {l['grid']} | " + " | ".join(cells) + " |")
     tot_t = sum(l.get("gpu__time_duration.sum") or 0 for l in step)
-    fwd = [l for l in step if "hash4d_fwd_kernel" in l["kernel"]]
-    bwd = [l for l in step if "hash4d_fwd_kernel" not in l["kernel"]]
+    fwd = [l for i, l in enumerate(step) if is_fwd_call(step, i)]
+    bwd = [l for i, l in enumerate(step) if not is_fwd_call(step, i)]
     out += ["", f"Step totals: {tot_t:.1f} us under ncu (serialised, cold cache — shares, not absolutes); DRAM read+write "
                 f"fwd call {sum(map(dram, fwd)) / 1e9:.3f} GB, bwd call {sum(map(dram, bwd)) / 1e9:.3f} GB, step "
                 f"{sum(map(dram, step)) / 1e9:.3f} GB.",
@@ -159,8 +192,8 @@ def main(argv=None):
         with open(args.md, "w") as fh:
             fh.write(markdown(launches, step, args.title or f"ncu per-launch table, one step of {args.config}",
                               args.command))
-    fwd = [l for l in step if "hash4d_fwd_kernel" in l["kernel"]]
-    bwd = [l for l in step if "hash4d_fwd_kernel" not in l["kernel"]]
+    fwd = [l for i, l in enumerate(step) if is_fwd_call(step, i)]
+    bwd = [l for i, l in enumerate(step) if not is_fwd_call(step, i)]
     summary = {"fwd_call": sum(map(dram, fwd)), "bwd_call": sum(map(dram, bwd)), "step": sum(map(dram, step)),
                "launches_in_step": len(step), "source_csv": os.path.basename(args.csv), "command": args.command}
     if args.traffic:
