@@ -648,6 +648,23 @@ def run_cuda(args):
             row["slice_encoder_only_ms"] = timed(lambda: dh.dash_hash4d_slice_fwd(cfg2, x2, sl2, out=f2), 20)
             row["slice_fused_ms"] = timed(lambda: dh.dash_deform_slice_fwd(cfg2, mlp, x2, sl2, prm, out=o2), 20)
             row["frame_ms_slice_path"] = row["slice_t_ms"] + row["slice_fused_ms"]
+            # The Gaussians of a scene do not move between rendered frames: a spatial (Morton) order computed ONCE
+            # (dash_hash4d_sort_queries) serves every frame, either as the call's index list or as the order the scene
+            # is stored in.  With one timestamp per frame neighbouring lanes then share cells on every coarse level.
+            order2 = dh.dash_hash4d_sort_queries(x2, bits=7)
+            xs2 = x2[order2.long()].contiguous()
+            row["sorted_once"] = {
+                "sort_ms_once_per_scene": timed(lambda: dh.dash_hash4d_sort_queries(x2, bits=7, order=order2), 10),
+                "fused_ms_index_list": timed(lambda: dh.dash_deform_fwd(cfg2, mlp, x2, one, tab2, prm, out=o2, t_stride=0,
+                                                                        index=order2), 20),
+                "fused_ms_stored_in_order": timed(lambda: dh.dash_deform_fwd(cfg2, mlp, xs2, one, tab2, prm, out=o2,
+                                                                             t_stride=0), 20),
+                "encoder_only_ms_stored_in_order": timed(lambda: dh.dash_hash4d_fwd(cfg2, xs2, one, tab2, out=f2,
+                                                                                    t_stride=0), 20),
+                "slice_fused_ms_stored_in_order": timed(lambda: dh.dash_deform_slice_fwd(cfg2, mlp, xs2, sl2, prm,
+                                                                                         out=o2), 20),
+            }
+            del order2, xs2
             row["mlp_tflops"] = 2.0 * w2.N * sum(a * b for a, b in zip(widths[:-1], widths[1:])) / (
                 row["mlp_only_ms"] * 1e-3) / 1e12
             # training direction (Q30): backward through the chain, and the whole deformation backward
