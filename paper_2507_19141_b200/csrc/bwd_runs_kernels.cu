@@ -106,10 +106,22 @@ __device__ __forceinline__ void load_row(const float* __restrict__ d, float g[F]
     }
 }
 
+// One run of equal cells is closed: one vector reduction per corner slot.
+template <int F, bool HINT>
+__device__ __forceinline__ void flush_run(const uint32_t slot[8], float* __restrict__ level_base, const float acc[8][F],
+                                          uint64_t pol) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        if constexpr (HINT) red_add_hint<F>(level_base + static_cast<size_t>(slot[j]) * F, acc[j], pol);
+        else red_add<F>(level_base + static_cast<size_t>(slot[j]) * F, acc[j]);
+    }
+}
+
 // One lane pair = (chunk of `chunk` consecutive sorted queries, one coarse level); adjacent pairs take the coarse
 // levels of the SAME chunk, so their coordinate loads coincide and their dY loads are neighbours in one row.
+// N < 2^31 here (the order is an int32 list): positions are 32-bit.
 template <int F, bool HINT>
-__global__ void __launch_bounds__(kBlockThreads, F == 4 ? 3 : 1)   // F = 4: 85 registers, three CTAs per SM
+__global__ void __launch_bounds__(kBlockThreads, F >= 8 ? 1 : (F == 4 ? 3 : 4))   // F = 4: 80 registers, three CTAs per SM; F <= 2: 64, four
 hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, const uint32_t chunk,
                        const float4* __restrict__ sorted_q, const int32_t* __restrict__ order,
                        const float* __restrict__ dout, float* __restrict__ dtable) {
@@ -117,33 +129,33 @@ hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, co
     const uint64_t pair = (static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x) >> 1;
     const uint64_t ch = pair / levels;
     const uint32_t l = static_cast<uint32_t>(pair - ch * levels);
-    const uint64_t begin = ch * chunk;
-    if (begin >= P.N) return;
-    const uint64_t end = (begin + chunk < P.N) ? begin + chunk : P.N;
+    const uint32_t n_total = static_cast<uint32_t>(P.N);
+    if (ch * chunk >= n_total) return;
+    const uint32_t begin = static_cast<uint32_t>(ch * chunk);
+    const uint32_t end = (n_total - begin > chunk) ? begin + chunk : n_total;
     const LevelParams lp = P.lv[l];
-    const size_t row = static_cast<size_t>(P.L) * F;
+    const uint32_t row = P.L * F;
     const float* dcol = dout + static_cast<size_t>(l) * F;
     float* level_base = dtable + static_cast<size_t>(l) * P.T * F;
     uint64_t pol = 0;
     if constexpr (HINT) pol = l2_policy_evict_last();
 
     float acc[8][F];
-    uint32_t slot[8];
+    uint32_t slot[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
     uint32_t pc[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};  // no cell: the first query opens a run
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        slot[j] = 0;
+    for (int j = 0; j < 8; ++j)
 #pragma unroll
         for (int f = 0; f < F; ++f) acc[j][f] = 0.0f;
-    }
     // two-deep software pipeline: coordinates and dY of query s+1 and the query number of s+2 are in flight
     // while query s is accumulated
+    const uint32_t n_max = n_total - 1u;   // clamped: memory-safe even if ORDER_READY was a false claim
     float4 q_next = __ldg(sorted_q + begin);
     float g_next[F];
-    const uint32_t n_max = static_cast<uint32_t>(P.N - 1);   // clamped: memory-safe even if ORDER_READY was a false claim
     load_row<F>(dcol + static_cast<size_t>(min(static_cast<uint32_t>(__ldg(order + begin)), n_max)) * row, g_next);
     uint32_t n_ahead = (begin + 1 < end) ? min(static_cast<uint32_t>(__ldg(order + begin + 1)), n_max) : 0u;
-    for (uint64_t s = begin; s < end; ++s) {
+#pragma unroll 1
+    for (uint32_t s = begin; s < end; ++s) {
         const float4 qc = q_next;
         float g[F];
 #pragma unroll
@@ -155,13 +167,7 @@ hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, co
         }
         const Query q = make_query<4>(lp, qc.x, qc.y, qc.z, qc.w);
         if ((q.c[0] != pc[0]) | (q.c[1] != pc[1]) | (q.c[2] != pc[2]) | (q.c[3] != pc[3])) {
-            if (pc[0] != 0xffffffffu) {   // close the run: one vector reduction per corner
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    if constexpr (HINT) red_add_hint<F>(level_base + static_cast<size_t>(slot[j]) * F, acc[j], pol);
-                    else red_add<F>(level_base + static_cast<size_t>(slot[j]) * F, acc[j]);
-                }
-            }
+            if (pc[0] != 0xffffffffu) flush_run<F, HINT>(slot, level_base, acc, pol);
             half_cell_slots<4>(P, lp, q, xc, slot);
 #pragma unroll
             for (int d = 0; d < 4; ++d) pc[d] = q.c[d];
@@ -177,11 +183,7 @@ hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, co
 #pragma unroll
             for (int f = 0; f < F; ++f) acc[j][f] = fmaf(W[j], g[f], acc[j][f]);
     }
-#pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        if constexpr (HINT) red_add_hint<F>(level_base + static_cast<size_t>(slot[j]) * F, acc[j], pol);
-        else red_add<F>(level_base + static_cast<size_t>(slot[j]) * F, acc[j]);
-    }
+    flush_run<F, HINT>(slot, level_base, acc, pol);
 }
 
 inline cudaError_t launched() {

@@ -281,7 +281,8 @@ static size_t round16(size_t v) { return (v + 15u) & ~static_cast<size_t>(15u); 
 // them, coarsened until it has at most 22 bits.  DASH_DEBUG_BWD_COARSE_LEVELS / _RUN_CHUNK override for sweeps.
 static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSort* cs) {
     std::memset(cs, 0, sizeof(*cs));
-    if (!(c->flags & DASH_HASH4D_FLAG_SORT_COARSE) || (c->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD) || N == 0)
+    if (!(c->flags & DASH_HASH4D_FLAG_SORT_COARSE) || (c->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD) || N == 0 ||
+        N > 0x7fffffffull)   // the order is an int32 list
         return false;
     Schedule s;
     make_schedule(c, &s, 4);

@@ -91,6 +91,33 @@ def test_workspace_sizes():
     assert dh.dash_hash4d_workspace_bytes(val, 1000, dh.OP_FWD) == 128
 
 
+def test_sort_coarse_workspace_and_flag_rules():
+    """DASH_HASH4D_FLAG_SORT_COARSE (include/dash_hash4d.h): needs a workspace only where the library takes the sorted
+    path (N >= 2^19, at least one level with Ns^3 Nt <= 2N), the same size for fwd and bwd, none for the other calls,
+    none under DETERMINISTIC_BWD; ORDER_READY changes no size; bit 64 is still an unknown flag."""
+    sc = dh.FLAG_DENSE_COARSE | dh.FLAG_SORT_COARSE
+    for name, n in (("C4", 1_000_000), ("C5", 1_800_000)):
+        cfg = dh.config_from_params(CONFIGS[name].enc, flags=sc)
+        need = dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD)
+        bins = 1 << 22                                        # level 3: 48^3 x 16 cells -> 6 + 6 + 6 + 4 key bits
+        assert need == 128 + 2 * 4 * n + 16 * n + 4 * bins + 4 * (bins // 1024)
+        assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_FWD) == need
+        assert dh.dash_hash4d_workspace_bytes(dh.with_flags(cfg, sc | dh.FLAG_ORDER_READY), n, dh.OP_BWD) == need
+        for op in (dh.OP_INDICES, dh.OP_BWD_INPUT, dh.OP_SMOOTH):
+            assert dh.dash_hash4d_workspace_bytes(cfg, n, op) == 0
+        assert dh.dash_hash4d_workspace_bytes(cfg, (1 << 19) - 1, dh.OP_BWD) == 0     # below the threshold: plain path
+        det = dh.with_flags(cfg, sc | dh.FLAG_DETERMINISTIC_BWD)
+        assert dh.dash_hash4d_workspace_bytes(det, n, dh.OP_FWD) == 0
+    c3 = dh.config_from_params(CONFIGS["C3"].enc, flags=sc)
+    assert dh.dash_hash4d_workspace_bytes(c3, CONFIGS["C3"].N, dh.OP_BWD) == 0
+    # a very fine coarsest level: no level qualifies, no workspace, the flag does nothing
+    fine = dh.make_config(4, 2, 1 << 19, 1024, 4096, 64, 300, flags=sc)
+    assert dh.dash_hash4d_workspace_bytes(fine, 1 << 20, dh.OP_BWD) == 0
+    bad = dh.config_from_params(CONFIGS["C4"].enc, flags=64)
+    res = (C.c_uint32 * 16)()
+    assert dh.binding._load().dash_hash4d_resolutions(C.byref(bad), res, res, None) == 1
+
+
 def test_null_and_stride_validation_happens_before_any_cuda_call():
     lib = C.CDLL(dh.library_path())
     lib.dash_hash4d_fwd.restype = C.c_int
