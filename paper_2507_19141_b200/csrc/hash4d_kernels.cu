@@ -439,24 +439,24 @@ hash4d_indices_kernel(const __grid_constant__ Plan P, const float* __restrict__ 
 // ------------------------------------------------------------------------------------------------
 template <bool HINT>
 __global__ void __launch_bounds__(kBlockThreads)
-zero_kernel(unsigned char* __restrict__ base, size_t head, size_t n16, size_t tail) {
-    // [base, base+head) bytes up to 16-byte alignment, then n16 aligned 16-byte stores, then tail bytes
-    uint4* body = reinterpret_cast<uint4*>(base + head);
+zero_kernel(unsigned char* __restrict__ base, size_t head, size_t n32, size_t tail) {
+    // [base, base+head) bytes up to 32-byte alignment, then n32 aligned 32-byte stores (STG.256), then tail bytes
+    unsigned char* body = base + head;
     const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
     uint64_t pol = 0;
     if constexpr (HINT) pol = l2_policy_evict_last();
-    for (size_t i = static_cast<size_t>(blockIdx.x) * kBlockThreads + threadIdx.x; i < n16;
-         i += stride) {
+    for (size_t i = static_cast<size_t>(blockIdx.x) * kBlockThreads + threadIdx.x; i < n32; i += stride) {
         if constexpr (HINT)
-            asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1, %1, %1, %1}, %2;" ::"l"(body + i), "r"(0u),
-                         "l"(pol)
+            asm volatile("st.global.L2::cache_hint.v8.b32 [%0], {%1, %1, %1, %1, %1, %1, %1, %1}, %2;" ::"l"(body + i * 32),
+                         "r"(0u), "l"(pol)
                          : "memory");
         else
-            body[i] = make_uint4(0u, 0u, 0u, 0u);
+            asm volatile("st.global.v8.b32 [%0], {%1, %1, %1, %1, %1, %1, %1, %1};" ::"l"(body + i * 32), "r"(0u)
+                         : "memory");
     }
     if (blockIdx.x == 0) {
         if (threadIdx.x < head) base[threadIdx.x] = 0;
-        if (threadIdx.x < tail) base[head + n16 * 16 + threadIdx.x] = 0;
+        if (threadIdx.x < tail) base[head + n32 * 32 + threadIdx.x] = 0;
     }
 }
 
@@ -950,16 +950,16 @@ cudaError_t launch_indices(const Plan& P, const float* xyz, const float* t, cons
 
 cudaError_t launch_zero(void* ptr, size_t bytes, cudaStream_t s, bool l2_hint) {
     if (bytes == 0) return cudaSuccess;
-    size_t head = (16 - (reinterpret_cast<uintptr_t>(ptr) & 15u)) & 15u;
+    size_t head = (32 - (reinterpret_cast<uintptr_t>(ptr) & 31u)) & 31u;
     if (head > bytes) head = bytes;
-    const size_t n16 = (bytes - head) / 16, tail = (bytes - head) % 16;
-    const size_t want = (n16 + kBlockThreads - 1) / kBlockThreads;
+    const size_t n32 = (bytes - head) / 32, tail = (bytes - head) % 32;
+    const size_t want = (n32 + kBlockThreads - 1) / kBlockThreads;
     const size_t cap = static_cast<size_t>(sm_count()) * 16;
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
     if (l2_hint)
-        zero_kernel<true><<<blocks, kBlockThreads, 0, s>>>(static_cast<unsigned char*>(ptr), head, n16, tail);
+        zero_kernel<true><<<blocks, kBlockThreads, 0, s>>>(static_cast<unsigned char*>(ptr), head, n32, tail);
     else
-        zero_kernel<false><<<blocks, kBlockThreads, 0, s>>>(static_cast<unsigned char*>(ptr), head, n16, tail);
+        zero_kernel<false><<<blocks, kBlockThreads, 0, s>>>(static_cast<unsigned char*>(ptr), head, n32, tail);
     return after_launch();
 }
 

@@ -188,3 +188,39 @@ def test_sorted_path_is_cuda_graph_capturable(set_debug):
         graph.replay()
         torch.cuda.synchronize()
         check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 6, hits=hits, what="graph replay")
+
+
+def test_packed_rows_custom_primes_non_power_of_two_table_and_validate_flag(set_debug):
+    """The sorted path under the other options of the ABI: packed [N][4] rows (xyz stride 4, t = base + 3, stride 4),
+    custom primes with Eq. 8 on every level (no dense levels), a table size that is not a power of two, a single level,
+    and VALIDATE_INPUTS sharing the workspace header with the sort."""
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 3)
+    rng = np.random.default_rng(21)
+    n = 2500
+    packed = np.ascontiguousarray(rng.random((n, 4), dtype=np.float32))
+    xyz, t = np.ascontiguousarray(packed[:, :3]), np.ascontiguousarray(packed[:, 3])
+    primes = (1, 2246822519, 3266489917, 668265263)
+    enc = EncoderParams(6, 2, 50021, 8, 256, 4, 32)
+    table = rng.uniform(-1, 1, (6, 50021, 2)).astype(np.float32)
+    dout = rng.standard_normal((n, 12)).astype(np.float32)
+    run_fwd_parity(enc, xyz, t, table, flags=SC, primes=primes, what="hashed everywhere, custom primes, T = 50021")
+    run_bwd_parity(enc, xyz, t, dout, flags=SC | ZG, primes=primes, what="hashed everywhere, custom primes, T = 50021")
+    ocfg, gcfg = both_configs(enc, DC | SC | ZG)
+    pd = dev(packed)
+    out = dh.dash_hash4d_fwd(gcfg, pd, pd.view(-1)[3:], dev(table), t_stride=4, N=n)
+    assert torch.equal(out, dh.dash_hash4d_fwd(dh.with_flags(gcfg, DC), dev(xyz), dev(t), dev(table)))
+    dt = torch.full((6, 50021, 2), 7.0, device="cuda")
+    dh.dash_hash4d_bwd(gcfg, pd, pd.view(-1)[3:], dev(dout), dt, t_stride=4, N=n)
+    ref, mag, hits = oracle.oracle_bwd(ocfg, n, xyz, t, dout, want_abs=True, want_hits=True)
+    check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 6, hits=hits, what="packed rows")
+    # one level only
+    enc1 = EncoderParams(1, 4, 1 << 12, 16, 16, 8, 8)
+    run_bwd_parity(enc1, xyz, t, rng.standard_normal((n, 4)).astype(np.float32), flags=DC | SC | ZG, what="L = 1")
+    run_fwd_parity(enc1, xyz, t, rng.uniform(-1, 1, (1, 1 << 12, 4)).astype(np.float32), flags=DC | SC, what="L = 1")
+    # VALIDATE_INPUTS: the scan uses the workspace header, the sort the bytes behind it
+    vcfg = dh.config_from_params(enc, flags=DC | SC | ZG | dh.FLAG_VALIDATE_INPUTS)
+    dh.dash_hash4d_bwd(vcfg, dev(xyz), dev(t), dev(dout), dt)
+    check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 6, hits=hits, what="validate + sort")
+    bad = xyz.copy(); bad[5, 0] = np.nan
+    with pytest.raises(dh.Hash4DError):
+        dh.dash_hash4d_bwd(vcfg, dev(bad), dev(t), dev(dout), dt)
