@@ -591,6 +591,16 @@ def run_cuda(args):
             "bwd_ms_via_4d_kernels_nt1_t0": timed(lambda: dh.dash_hash4d_bwd(cfg3, p3, t_zero, dy3, dt3,
                                                                                t_stride=0)),
         }
+        # the same with SORT_COARSE: the forward sorts the points by 3D cell, the backward reuses the order
+        cfg3s = dh.with_flags(cfg3, cfg3.flags | dh.FLAG_SORT_COARSE)
+        cfg3r = dh.with_flags(cfg3, cfg3.flags | dh.FLAG_SORT_COARSE | dh.FLAG_ORDER_READY)
+        ws3 = torch.empty(max(16, dh.dash_hash3d_workspace_bytes(cfg3s, g3.N, dh.OP_FWD)), dtype=torch.uint8, device="cuda")
+        extras["g3d"]["sort_coarse"] = {
+            "fwd_ms_with_sort": timed(lambda: dh.dash_hash3d_fwd(cfg3s, p3, tab3, out=out3, workspace=ws3)),
+            "fwd_ms_order_ready": timed(lambda: dh.dash_hash3d_fwd(cfg3r, p3, tab3, out=out3, workspace=ws3)),
+            "bwd_ms_order_ready": timed(lambda: dh.dash_hash3d_bwd(cfg3r, p3, dy3, dt3, workspace=ws3)),
+        }
+        del ws3
         del p3, tab3, dy3, out3, dt3
         # sparse Adam over the touched entries of the step's own gradient (dtable as the timed bwd left it)
         th32 = table.float().contiguous()

@@ -68,8 +68,9 @@ enum dash_hash4d_flags {
                                                runs of queries in one cell summed in registers, one vector reduction
                                                per run and corner; fwd: neighbouring lanes gather from the same cells.
                                                The other levels are unchanged.  Same values (fwd) / same sums in
-                                               another order (bwd: same tolerance).  Needs workspace; ignored by
-                                               DETERMINISTIC_BWD, by the other calls and by dash_hash3d_*.       */
+                                               another order (bwd: same tolerance).  Needs workspace.  Honoured by
+                                               dash_hash4d_fwd / _bwd and dash_hash3d_fwd / _bwd (3D cells, no t in
+                                               the key); ignored under DETERMINISTIC_BWD and by the other calls.  */
     DASH_HASH4D_FLAG_ORDER_READY = 32u      /* with SORT_COARSE: `workspace` still holds the order that an earlier
                                                dash_hash4d_fwd / _bwd call with SORT_COARSE wrote for the SAME
                                                queries (N, xyz, t, index unchanged, e.g. the forward of this training
@@ -106,6 +107,9 @@ DASH_API int dash_hash4d_resolutions(const dash_hash4d_config* cfg, uint32_t* re
  * 24 bytes per query + the sort's bins, the same for OP_FWD and OP_BWD so that one buffer serves a step).
  * Returns 0 on a bad config as well.  Needs no GPU. */
 DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op);
+/* The same for the dash_hash3d_* calls (op: DASH_HASH4D_OP_FWD / _BWD / _BWD_INPUT / _INDICES); the temporal fields of cfg
+ * are ignored, as in those calls. */
+DASH_API size_t dash_hash3d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op);
 
 /* Forward, Eq. 9:  out[n][l*F + f] = sum_{k<16} W_k * table[l][slot_k][f].
  *   N          number of queries.

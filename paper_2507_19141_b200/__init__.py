@@ -7,7 +7,7 @@ There is no CPU fallback: without the built library or without a CUDA device the
 from .binding import (  # noqa: F401
     Hash4DConfig, Hash4DError, FLAG_DENSE_COARSE, FLAG_DETERMINISTIC_BWD, FLAG_VALIDATE_INPUTS,
     FLAG_ZERO_GRAD, FLAG_SORT_COARSE, FLAG_ORDER_READY, OP_FWD, OP_BWD, OP_INDICES, OP_BWD_INPUT, OP_SMOOTH, make_config, config_from_params, library_path,
-    dash_hash4d_resolutions, dash_hash4d_workspace_bytes, dash_hash4d_fwd, dash_hash4d_bwd, dash_hash4d_bwd_input, dash_hash4d_smooth,
+    dash_hash4d_resolutions, dash_hash4d_workspace_bytes, dash_hash3d_workspace_bytes, dash_hash4d_fwd, dash_hash4d_bwd, dash_hash4d_bwd_input, dash_hash4d_smooth,
     dash_hash4d_indices, dash_hash4d_zero, dash_hash4d_last_error, dash_hash4d_launch_count,
     dash_hash3d_resolutions, dash_hash3d_fwd, dash_hash3d_bwd, dash_hash3d_indices, dash_hash3d_bwd_input,
     dash_hash4d_slice_t, dash_hash4d_slice_fwd, dash_deform_slice_fwd, dash_deform_slice_workspace_bytes,

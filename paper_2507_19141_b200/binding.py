@@ -23,7 +23,7 @@ OP_FWD, OP_BWD, OP_INDICES, OP_BWD_INPUT, OP_SMOOTH = 0, 1, 2, 3, 4
 
 _STATUS = {1: "INVALID_ARG", 2: "UNSUPPORTED", 3: "WORKSPACE_TOO_SMALL", 4: "CUDA_ERROR"}
 
-EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash4d_fwd",
+EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash3d_workspace_bytes", "dash_hash4d_fwd",
            "dash_hash4d_bwd", "dash_hash4d_bwd_input", "dash_hash4d_smooth", "dash_hash4d_indices", "dash_hash4d_zero", "dash_hash4d_last_error",
            "dash_hash4d_launch_count", "dash_hash4d_set_debug", "dash_hash4d_build_id",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices", "dash_hash3d_bwd_input",
@@ -109,6 +109,8 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_hash4d_resolutions.restype = C.c_int
     lib.dash_hash4d_workspace_bytes.argtypes = [cfgp, u64, C.c_int]
     lib.dash_hash4d_workspace_bytes.restype = sz
+    lib.dash_hash3d_workspace_bytes.argtypes = [cfgp, u64, C.c_int]
+    lib.dash_hash3d_workspace_bytes.restype = sz
     lib.dash_hash4d_fwd.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp, sz, vp]
     lib.dash_hash4d_fwd.restype = C.c_int
     lib.dash_hash4d_bwd.argtypes = [cfgp, u64, vp, u32, vp, u32, vp, vp, vp, vp, sz, vp]
@@ -309,8 +311,12 @@ def dash_hash4d_workspace_bytes(cfg: Hash4DConfig, N: int, op: int) -> int:
     return int(_load().dash_hash4d_workspace_bytes(C.byref(cfg), N, op))
 
 
-def _workspace(cfg, N, op, workspace, device):
-    need = dash_hash4d_workspace_bytes(cfg, N, op)
+def dash_hash3d_workspace_bytes(cfg: Hash4DConfig, N: int, op: int) -> int:
+    return int(_load().dash_hash3d_workspace_bytes(C.byref(cfg), N, op))
+
+
+def _workspace(cfg, N, op, workspace, device, dims=4):
+    need = dash_hash4d_workspace_bytes(cfg, N, op) if dims == 4 else dash_hash3d_workspace_bytes(cfg, N, op)
     if need and workspace is None:
         workspace = torch.empty(need, dtype=torch.uint8, device=device)
     if workspace is not None and not workspace.is_cuda:
@@ -475,7 +481,7 @@ def dash_hash3d_fwd(cfg, xyz, table, out=None, index=None, N=None, workspace=Non
     _check_queries(cfg, xyz, None, index, 0, N)
     _exactly(table, _table_elems(cfg), "table"); _at_least(out, N * cfg.L * cfg.F, "out")
     _one_device(xyz, index, table, out, workspace)
-    workspace, wbytes = _workspace(cfg, N, OP_FWD, workspace, xyz.device)
+    workspace, wbytes = _workspace(cfg, N, OP_FWD, workspace, xyz.device, dims=3)
     _check(_load().dash_hash3d_fwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(table), _ptr(out),
                                    _ptr(workspace), wbytes, _stream()))
     return out
@@ -491,7 +497,7 @@ def dash_hash3d_bwd(cfg, xyz, dout, dtable, index=None, N=None, workspace=None):
     _check_queries(cfg, xyz, None, index, 0, N)
     _at_least(dout, N * cfg.L * cfg.F, "dout"); _exactly(dtable, _table_elems(cfg), "dtable")
     _one_device(xyz, index, dout, dtable, workspace)
-    workspace, wbytes = _workspace(cfg, N, OP_BWD, workspace, xyz.device)
+    workspace, wbytes = _workspace(cfg, N, OP_BWD, workspace, xyz.device, dims=3)
     _check(_load().dash_hash3d_bwd(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(dout), _ptr(dtable),
                                    _ptr(workspace), wbytes, _stream()))
     return dtable
@@ -510,7 +516,7 @@ def dash_hash3d_bwd_input(cfg, xyz, table, dout, dq=None, index=None, N=None, wo
     _check_queries(cfg, xyz, None, index, 0, N)
     _exactly(table, _table_elems(cfg), "table"); _at_least(dout, N * cfg.L * cfg.F, "dout"); _at_least(dq, 3 * N, "dq")
     _one_device(xyz, index, table, dout, dq, workspace)
-    workspace, wbytes = _workspace(cfg, N, OP_BWD_INPUT, workspace, xyz.device)
+    workspace, wbytes = _workspace(cfg, N, OP_BWD_INPUT, workspace, xyz.device, dims=3)
     _check(_load().dash_hash3d_bwd_input(C.byref(cfg), N, _ptr(xyz), xs, _ptr(index), _ptr(table), _ptr(dout),
                                          _ptr(dq), _ptr(workspace), wbytes, _stream()))
     return dq

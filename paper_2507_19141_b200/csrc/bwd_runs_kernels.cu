@@ -43,11 +43,12 @@ __device__ __forceinline__ uint32_t morton4(const uint32_t c[4], uint32_t bits_s
     return key;
 }
 
+template <int D>
 __device__ __forceinline__ uint32_t coarse_key(const Plan& P, const CoarseSort& cs, uint64_t n,
                                                const float* __restrict__ xyz, const float* __restrict__ t,
                                                const int32_t* __restrict__ index, float4& coords) {
     float c[4];
-    load_coords<4>(P, n, xyz, t, index, c);
+    load_coords<D>(P, n, xyz, t, index, c);   // D = 3 (G_3D): no timestamp, c[3] = 0, bits_t = 0
     coords = make_float4(c[0], c[1], c[2], c[3]);
     const LevelParams& lp = P.lv[cs.key_level];
     uint32_t cell[4];
@@ -60,6 +61,7 @@ __device__ __forceinline__ uint32_t coarse_key(const Plan& P, const CoarseSort& 
     return morton4(cell, cs.bits_s, cs.bits_t);
 }
 
+template <int D>
 __global__ void __launch_bounds__(kBlockThreads)
 sort4d_keys_kernel(const __grid_constant__ Plan P, const CoarseSort cs, const float* __restrict__ xyz,
                    const float* __restrict__ t, const int32_t* __restrict__ index, uint32_t* __restrict__ keys,
@@ -67,13 +69,14 @@ sort4d_keys_kernel(const __grid_constant__ Plan P, const CoarseSort cs, const fl
     const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
     for (uint64_t n = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x; n < P.N; n += stride) {
         float4 q;
-        const uint32_t key = coarse_key(P, cs, n, xyz, t, index, q);
+        const uint32_t key = coarse_key<D>(P, cs, n, xyz, t, index, q);
         keys[n] = key;
         atomicAdd(hist + key, 1u);
     }
 }
 
 // order[pos] = n and sorted_q[pos] = (x, y, z, t) of query n: the run kernel streams both
+template <int D>
 __global__ void __launch_bounds__(kBlockThreads)
 sort4d_scatter_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz, const float* __restrict__ t,
                       const int32_t* __restrict__ index, const uint32_t* __restrict__ keys,
@@ -82,7 +85,7 @@ sort4d_scatter_kernel(const __grid_constant__ Plan P, const float* __restrict__ 
     const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
     for (uint64_t n = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x; n < P.N; n += stride) {
         float c[4];
-        load_coords<4>(P, n, xyz, t, index, c);
+        load_coords<D>(P, n, xyz, t, index, c);
         const uint32_t key = keys[n];   // the scan is per tile of kScanTile bins: add the tile's offset here
         const uint32_t pos = atomicAdd(cursor + key, 1u) + __ldg(tile_offset + key / kScanTile);
         order[pos] = static_cast<int32_t>(n);
@@ -107,11 +110,11 @@ __device__ __forceinline__ void load_row(const float* __restrict__ d, float g[F]
 }
 
 // One run of equal cells is closed: one vector reduction per corner slot.
-template <int F, bool HINT>
-__device__ __forceinline__ void flush_run(const uint32_t slot[8], float* __restrict__ level_base, const float acc[8][F],
-                                          uint64_t pol) {
+template <int F, bool HINT, int NC>
+__device__ __forceinline__ void flush_run(const uint32_t slot[NC], float* __restrict__ level_base,
+                                          const float acc[NC][F], uint64_t pol) {
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < NC; ++j) {
         if constexpr (HINT) red_add_hint<F>(level_base + static_cast<size_t>(slot[j]) * F, acc[j], pol);
         else red_add<F>(level_base + static_cast<size_t>(slot[j]) * F, acc[j]);
     }
@@ -120,7 +123,8 @@ __device__ __forceinline__ void flush_run(const uint32_t slot[8], float* __restr
 // One lane pair = (chunk of `chunk` consecutive sorted queries, one coarse level); adjacent pairs take the coarse
 // levels of the SAME chunk, so their coordinate loads coincide and their dY loads are neighbours in one row.
 // N < 2^31 here (the order is an int32 list): positions are 32-bit.
-template <int F, bool HINT>
+// D = 3: G_3D (dash_hash3d_bwd), 4 (y,z) corners per lane.
+template <int F, bool HINT, int D>
 __global__ void __launch_bounds__(kBlockThreads, F >= 8 ? 1 : (F == 4 ? 3 : 4))   // F = 4: 80 registers, three CTAs per SM; F <= 2: 64, four
 hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, const uint32_t chunk,
                        const float4* __restrict__ sorted_q, const int32_t* __restrict__ order,
@@ -140,11 +144,14 @@ hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, co
     uint64_t pol = 0;
     if constexpr (HINT) pol = l2_policy_evict_last();
 
-    float acc[8][F];
-    uint32_t slot[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+    constexpr int NC = 1 << (D - 1);
+    float acc[NC][F];
+    uint32_t slot[NC];
+#pragma unroll
+    for (int j = 0; j < NC; ++j) slot[j] = 0u;
     uint32_t pc[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};  // no cell: the first query opens a run
 #pragma unroll
-    for (int j = 0; j < 8; ++j)
+    for (int j = 0; j < NC; ++j)
 #pragma unroll
         for (int f = 0; f < F; ++f) acc[j][f] = 0.0f;
     // two-deep software pipeline: coordinates and dY of query s+1 and the query number of s+2 are in flight
@@ -165,25 +172,25 @@ hash4d_bwd_runs_kernel(const __grid_constant__ Plan P, const uint32_t levels, co
             load_row<F>(dcol + static_cast<size_t>(n_ahead) * row, g_next);
             if (s + 2 < end) n_ahead = min(static_cast<uint32_t>(__ldg(order + s + 2)), n_max);
         }
-        const Query q = make_query<4>(lp, qc.x, qc.y, qc.z, qc.w);
+        const Query q = make_query<D>(lp, qc.x, qc.y, qc.z, qc.w);
         if ((q.c[0] != pc[0]) | (q.c[1] != pc[1]) | (q.c[2] != pc[2]) | (q.c[3] != pc[3])) {
-            if (pc[0] != 0xffffffffu) flush_run<F, HINT>(slot, level_base, acc, pol);
-            half_cell_slots<4>(P, lp, q, xc, slot);
+            if (pc[0] != 0xffffffffu) flush_run<F, HINT, NC>(slot, level_base, acc, pol);
+            half_cell_slots<D>(P, lp, q, xc, slot);
 #pragma unroll
             for (int d = 0; d < 4; ++d) pc[d] = q.c[d];
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
+            for (int j = 0; j < NC; ++j)
 #pragma unroll
                 for (int f = 0; f < F; ++f) acc[j][f] = 0.0f;
         }
-        float W[8];
-        half_cell_weights<4>(q, xc, W);
+        float W[NC];
+        half_cell_weights<D>(q, xc, W);
 #pragma unroll
-        for (int j = 0; j < 8; ++j)
+        for (int j = 0; j < NC; ++j)
 #pragma unroll
             for (int f = 0; f < F; ++f) acc[j][f] = fmaf(W[j], g[f], acc[j][f]);
     }
-    flush_run<F, HINT>(slot, level_base, acc, pol);
+    flush_run<F, HINT, NC>(slot, level_base, acc, pol);
 }
 
 inline cudaError_t launched() {
@@ -201,10 +208,14 @@ cudaError_t launch_coarse_sort(const Plan& P, const CoarseSort& cs, const float*
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
     cudaError_t e = launch_zero(bins, static_cast<size_t>(cs.n_bins) * sizeof(uint32_t), s);
     if (e != cudaSuccess) return e;
-    sort4d_keys_kernel<<<blocks, kBlockThreads, 0, s>>>(P, cs, xyz, t, index, keys, bins);
+    if (P.dims == 3) sort4d_keys_kernel<3><<<blocks, kBlockThreads, 0, s>>>(P, cs, xyz, t, index, keys, bins);
+    else sort4d_keys_kernel<4><<<blocks, kBlockThreads, 0, s>>>(P, cs, xyz, t, index, keys, bins);
     if ((e = launched()) != cudaSuccess) return e;
     if ((e = launch_exclusive_scan_u32(bins, cs.n_bins, totals, s, false)) != cudaSuccess) return e;
-    sort4d_scatter_kernel<<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, totals, order, sorted_q);
+    if (P.dims == 3)
+        sort4d_scatter_kernel<3><<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, totals, order, sorted_q);
+    else
+        sort4d_scatter_kernel<4><<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, totals, order, sorted_q);
     return launched();
 }
 
@@ -214,14 +225,18 @@ cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* do
     const uint64_t threads = chunks * cs.levels * 2;
     const uint64_t grid = (threads + kBlockThreads - 1) / kBlockThreads;
     if (grid > 0x7fffffffull) return cudaErrorInvalidValue;
-#define DASH_RUNS(FV)                                                                                             \
-    do {                                                                                                          \
-        if (l2_hint)                                                                                              \
-            hash4d_bwd_runs_kernel<FV, true><<<static_cast<unsigned>(grid), kBlockThreads, 0, s>>>(               \
-                P, cs.levels, cs.chunk, sorted_q, order, dout, dtable);                                           \
-        else                                                                                                      \
-            hash4d_bwd_runs_kernel<FV, false><<<static_cast<unsigned>(grid), kBlockThreads, 0, s>>>(              \
-                P, cs.levels, cs.chunk, sorted_q, order, dout, dtable);                                           \
+#define DASH_RUNS_D(FV, HV, DV)                                                                         \
+    hash4d_bwd_runs_kernel<FV, HV, DV><<<static_cast<unsigned>(grid), kBlockThreads, 0, s>>>(           \
+        P, cs.levels, cs.chunk, sorted_q, order, dout, dtable)
+#define DASH_RUNS(FV)                                        \
+    do {                                                     \
+        if (P.dims == 3) {                                   \
+            if (l2_hint) DASH_RUNS_D(FV, true, 3);           \
+            else DASH_RUNS_D(FV, false, 3);                  \
+        } else {                                             \
+            if (l2_hint) DASH_RUNS_D(FV, true, 4);           \
+            else DASH_RUNS_D(FV, false, 4);                  \
+        }                                                    \
     } while (0)
     switch (P.F) {
         case 1: DASH_RUNS(1); break;
@@ -231,6 +246,7 @@ cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* do
         default: return cudaErrorInvalidValue;
     }
 #undef DASH_RUNS
+#undef DASH_RUNS_D
     return launched();
 }
 

@@ -279,13 +279,13 @@ static size_t round16(size_t v) { return (v + 15u) & ~static_cast<size_t>(15u); 
 // Levels whose cell count Ns^3 Nt is at most 2N (on average >= 1/2 query per cell; clustered inputs fill far fewer
 // cells) — measured rule, profiles/experiments_r02.md §8.  The key is the Morton code of the cell on the finest of
 // them, coarsened until it has at most 22 bits.  DASH_DEBUG_BWD_COARSE_LEVELS / _RUN_CHUNK override for sweeps.
-static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSort* cs) {
+static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSort* cs, int dims = 4) {
     std::memset(cs, 0, sizeof(*cs));
     if (!(c->flags & DASH_HASH4D_FLAG_SORT_COARSE) || (c->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD) || N == 0 ||
         N > 0x7fffffffull)   // the order is an int32 list
         return false;
     Schedule s;
-    make_schedule(c, &s, 4);
+    make_schedule(c, &s, dims);   // dims = 3 (G_3D): res_t = 1 on every level, the key has no t bits
     uint32_t nl = 0;
     const uint32_t forced = debug_u32(DASH_DEBUG_BWD_COARSE_LEVELS);
     if (forced) {
@@ -349,18 +349,21 @@ static size_t workspace_need(const dash_hash4d_config* cfg, int op, uint64_t N, 
     if (op == DASH_HASH4D_OP_BWD && (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD))
         bytes = kHeaderBytes + table_elems(cfg) * sizeof(long long);
     dash::CoarseSort cs;
-    if ((op == DASH_HASH4D_OP_BWD || op == DASH_HASH4D_OP_FWD) && dims == 4 && plan_coarse(cfg, N, &cs))
+    if ((op == DASH_HASH4D_OP_BWD || op == DASH_HASH4D_OP_FWD) && plan_coarse(cfg, N, &cs, dims))
         bytes = kHeaderBytes + coarse_workspace(cs, N);
     return bytes;
 }
 
 DASH_API size_t dash_hash4d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op) {
-    if (check_config(cfg, 3)) return 0;  // the temporal range is not needed to size a workspace
+    if (check_config(cfg, 4)) return 0;
     g_error[0] = '\0';
-    // the coarse sort keys on the temporal resolutions too: a config that is only valid for G_3D gets none
-    const int dims = check_config(cfg, 4) == DASH_HASH4D_OK ? 4 : 3;
+    return workspace_need(cfg, op, N, 4);
+}
+
+DASH_API size_t dash_hash3d_workspace_bytes(const dash_hash4d_config* cfg, uint64_t N, int op) {
+    if (check_config(cfg, 3)) return 0;  // the temporal fields are ignored
     g_error[0] = '\0';
-    return workspace_need(cfg, op, N, dims);
+    return workspace_need(cfg, op, N, 3);
 }
 
 static int fwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const float* xyz,
@@ -384,7 +387,7 @@ static int fwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
         group = 4;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride, group, &P, dims)) return rc;
     dash::CoarseSort cs;
-    const bool coarse = dims == 4 && plan_coarse(cfg, N, &cs);
+    const bool coarse = plan_coarse(cfg, N, &cs, dims);
     const size_t need = workspace_need(cfg, DASH_HASH4D_OP_FWD, N, dims);
     if (coarse && (!workspace || workspace_bytes < need))
         return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "fwd needs %zu workspace bytes, got %zu", need, workspace_bytes);
@@ -580,7 +583,7 @@ static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
     // SORT_COARSE: the leading `cs.levels` levels go through the sort + run-merged scatter (bwd_runs_kernels.cu),
     // the others through the one-reduction-per-corner kernel in the caller's order.
     dash::CoarseSort cs;
-    const bool coarse = dims == 4 && plan_coarse(cfg, N, &cs);
+    const bool coarse = plan_coarse(cfg, N, &cs, dims);
     const uint32_t l_first = coarse ? cs.levels : 0u;
     auto scatter_coarse = [&](bool hint) -> cudaError_t {
         const CoarseBuffers b = carve_coarse(workspace, cs, N);

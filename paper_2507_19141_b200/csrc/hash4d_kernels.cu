@@ -805,11 +805,10 @@ cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const in
                        const void* table, bool table_half, float* out, cudaStream_t s, const int32_t* order,
                        const float4* sorted_q) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
-    if (P.dims == 3 && order) return cudaErrorInvalidValue;
 #define DASH_FWD(FV, HV)                                                                                        \
     do {                                                                                                        \
         if (P.dims == 3)                                                                                        \
-            hash4d_fwd_kernel<FV, HV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, nullptr, nullptr); \
+            hash4d_fwd_kernel<FV, HV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, order, sorted_q); \
         else                                                                                                    \
             hash4d_fwd_kernel<FV, HV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, order, sorted_q); \
     } while (0)

@@ -140,28 +140,64 @@ def test_workspace_is_required_and_sized_by_the_library(set_debug):
     assert rc == 3
 
 
-def test_flag_is_ignored_by_g3d_and_by_the_deterministic_mode(set_debug):
+def test_flag_is_ignored_by_the_deterministic_mode(set_debug):
     set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 2)
     enc = EncoderParams(4, 2, 1 << 10, 8, 64, 4, 16)
     n = 2000
     rng = np.random.default_rng(2)
     xyz, t = make_queries_uniform(2, n)
     dout = rng.standard_normal((n, 8)).astype(np.float32)
-    # deterministic: bitwise equal with and without the flag
     got = []
     for flags in (DC | ZG | dh.FLAG_DETERMINISTIC_BWD, DC | ZG | dh.FLAG_DETERMINISTIC_BWD | SC):
         cfg = dh.config_from_params(enc, flags=flags)
         dt = torch.empty((4, 1 << 10, 2), device="cuda")
         dh.dash_hash4d_bwd(cfg, dev(xyz), dev(t), dev(dout), dt)
         got.append(dt.cpu().numpy())
-    assert np.array_equal(got[0], got[1])
-    # G_3D backward: the flag changes nothing (and needs no workspace)
-    o3 = oracle.make_config(4, 2, 1 << 10, 8, 64, 1, 1)
-    g3 = dh.make_config(4, 2, 1 << 10, 8, 64, 1, 1, flags=DC | ZG | SC)
-    ref, mag = oracle.oracle3d_bwd(o3, n, xyz, dout, want_abs=True)
-    dt = torch.empty((4, 1 << 10, 2), device="cuda")
-    dh.dash_hash3d_bwd(g3, dev(xyz), dev(dout), dt)
-    check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 4, what="g3d with the flag set")
+    assert np.array_equal(got[0], got[1])                      # bitwise equal with and without the flag
+
+
+def _g3d_parity(o3, g3, xyz, table, dout, index=None, what=""):
+    n = len(index) if index is not None else len(xyz)
+    L = g3.L
+    ref, mag = oracle.oracle3d_fwd(o3, n, xyz, table, index=index, want_abs=True)
+    out = dh.dash_hash3d_fwd(g3, dev(xyz), dev(table), index=dev(index))
+    tr = lambda a: np.asarray(a).reshape(n, L, g3.F).transpose(1, 0, 2)
+    check_close(tr(out.cpu().numpy()), tr(ref), tr(mag), RTOL_FP32, L, what=what + " g3d fwd")
+    plain = dh.dash_hash3d_fwd(dh.with_flags(g3, DC), dev(xyz), dev(table), index=dev(index))
+    assert torch.equal(out, plain)
+    refg, magg, hits = oracle.oracle3d_bwd(o3, n, xyz, dout, index=index, want_abs=True, want_hits=True)
+    dt = torch.full((L, g3.T, g3.F), 7.0, device="cuda")
+    dh.dash_hash3d_bwd(g3, dev(xyz), dev(dout), dt, index=dev(index))
+    check_close(dt.cpu().numpy(), refg, magg, RTOL_FP32, L, hits=hits, what=what + " g3d bwd")
+
+
+@pytest.mark.parametrize("levels", [1, 3, 6])
+def test_g3d_forced_levels(levels, set_debug):
+    """dash_hash3d_fwd / _bwd honour the flag: 3D cells, no t in the key, 4 corners per lane in the run kernel."""
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, levels)
+    rng = np.random.default_rng(levels)
+    for (L, F, T, n) in [(6, 2, 1 << 12, 3001), (5, 4, 30011, 1237), (3, 1, 1 << 10, 600)]:
+        o3 = oracle.make_config(L, F, T, 4, 200, 1, 1)
+        g3 = dh.make_config(L, F, T, 4, 200, 1, 1, flags=DC | ZG | SC)
+        assert dh.dash_hash3d_workspace_bytes(g3, n, dh.OP_BWD) >= 24 * n
+        xyz = np.clip(0.5 + 0.2 * rng.standard_normal((n, 3)), 0, 0.999).astype(np.float32)
+        table = rng.uniform(-1, 1, (L, T, F)).astype(np.float32)
+        dout = rng.standard_normal((n, L * F)).astype(np.float32)
+        _g3d_parity(o3, g3, xyz, table, dout, what=f"L{L} F{F} levels{levels}")
+        index = rng.integers(0, n, 2 * n).astype(np.int32)
+        _g3d_parity(o3, g3, xyz, table, rng.standard_normal((2 * n, L * F)).astype(np.float32), index=index,
+                    what=f"indexed L{L} F{F} levels{levels}")
+
+
+def test_g3d_full_size_workload():
+    """The bench's G_3D workload (1.5M Gaussians, L = 16, F = 2, T = 2^19) with the library's own choice of levels."""
+    from dash_inputs import make_g3d_workload
+    wl = make_g3d_workload()
+    enc = wl.spec.enc
+    o3 = oracle.make_config(enc.L, enc.F, enc.T, enc.res_s_min, enc.res_s_max, 1, 1)
+    g3 = dh.make_config(enc.L, enc.F, enc.T, enc.res_s_min, enc.res_s_max, 1, 1, flags=DC | ZG | SC)
+    assert dh.dash_hash3d_workspace_bytes(g3, wl.N, dh.OP_FWD) >= 24 * wl.N
+    _g3d_parity(o3, g3, wl.xyz, wl.table, wl.dout, what="G3D workload")
 
 
 def test_sorted_path_is_cuda_graph_capturable(set_debug):
