@@ -563,6 +563,9 @@ def run_cuda(args):
         cfg_x = dh.with_flags(cfg, flags & ~dh.FLAG_SORT_COARSE)   # the extras time the calls without the coarse sort
         extras = {"bwd_input_ms": timed(lambda: dh.dash_hash4d_bwd_input(cfg_x, xyz, t, table, dout, dq=dq,
                                                                            index=index))}
+        if sorted_path:   # the coordinate gradient walking the order the step's forward left in the workspace
+            extras["bwd_input_ms_sort_coarse_order_ready"] = timed(
+                lambda: dh.dash_hash4d_bwd_input(cfg_bwd, xyz, t, table, dout, dq=dq, index=index, workspace=bwd_ws))
         for delta in (1e-4, 1e-3, 1e-2):
             eps = (torch.rand((N, 4), device="cuda", generator=gen) * 2 - 1) * delta
             extras[f"smooth_loss+grad_ms(eps=U(-{delta:g},{delta:g}))"] = timed(

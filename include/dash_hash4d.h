@@ -61,7 +61,7 @@ enum dash_hash4d_flags {
     DASH_HASH4D_FLAG_ZERO_GRAD = 8u,        /* bwd OVERWRITES: the library zeroes each level group of dtable
                                                immediately before scattering into it (keeps it L2-resident)
                                                instead of accumulating into the caller's contents.          */
-    DASH_HASH4D_FLAG_SORT_COARSE = 16u,     /* dash_hash4d_fwd / _bwd, the high-collision case (BASELINE.json config 5):
+    DASH_HASH4D_FLAG_SORT_COARSE = 16u,     /* dash_hash4d_fwd / _bwd / _bwd_input, the high-collision case (BASELINE.json config 5):
                                                the queries are counting-sorted by their 4D cell on the coarse levels
                                                (cell count <= 2N; only for N >= 2^19, else the flag does nothing) and
                                                those levels are processed in that order — bwd: a segmented reduction,
@@ -69,10 +69,11 @@ enum dash_hash4d_flags {
                                                per run and corner; fwd: neighbouring lanes gather from the same cells.
                                                The other levels are unchanged.  Same values (fwd) / same sums in
                                                another order (bwd: same tolerance).  Needs workspace.  Honoured by
-                                               dash_hash4d_fwd / _bwd and dash_hash3d_fwd / _bwd (3D cells, no t in
-                                               the key); ignored under DETERMINISTIC_BWD and by the other calls.  */
+                                               dash_hash4d_fwd / _bwd / _bwd_input (the forward's gathers) and their
+                                               dash_hash3d_* forms (3D cells, no t in the key); ignored under
+                                               DETERMINISTIC_BWD and by the other calls.                          */
     DASH_HASH4D_FLAG_ORDER_READY = 32u      /* with SORT_COARSE: `workspace` still holds the order that an earlier
-                                               dash_hash4d_fwd / _bwd call with SORT_COARSE wrote for the SAME
+                                               dash_hash4d_fwd / _bwd / _bwd_input call with SORT_COARSE wrote for the SAME
                                                queries (N, xyz, t, index unchanged, e.g. the forward of this training
                                                step): the sort (five launches) is skipped.  A false claim gives
                                                wrong values but no out-of-bounds access.                        */

@@ -349,7 +349,8 @@ static size_t workspace_need(const dash_hash4d_config* cfg, int op, uint64_t N, 
     if (op == DASH_HASH4D_OP_BWD && (cfg->flags & DASH_HASH4D_FLAG_DETERMINISTIC_BWD))
         bytes = kHeaderBytes + table_elems(cfg) * sizeof(long long);
     dash::CoarseSort cs;
-    if ((op == DASH_HASH4D_OP_BWD || op == DASH_HASH4D_OP_FWD) && plan_coarse(cfg, N, &cs, dims))
+    if ((op == DASH_HASH4D_OP_BWD || op == DASH_HASH4D_OP_FWD || op == DASH_HASH4D_OP_BWD_INPUT) &&
+        plan_coarse(cfg, N, &cs, dims))
         bytes = kHeaderBytes + coarse_workspace(cs, N);
     return bytes;
 }
@@ -470,9 +471,24 @@ static int bwd_input_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, c
     uint32_t group = pick_group(cfg, level_bytes, DASH_DEBUG_FWD_GROUP);
     if (dims == 3 && group > 4 && 4 * cfg->F * sizeof(float) >= 32 && !debug_u32(DASH_DEBUG_FWD_GROUP)) group = 4;
     if (int rc = fill_plan(cfg, N, xyz_stride, t_stride, group, &P, dims)) return rc;
+    dash::CoarseSort cs;
+    const bool coarse = plan_coarse(cfg, N, &cs, dims);   // SORT_COARSE: the same gathers as the forward, same order
+    const size_t need = workspace_need(cfg, DASH_HASH4D_OP_BWD_INPUT, N, dims);
+    if (coarse && (!workspace || workspace_bytes < need))
+        return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "bwd_input needs %zu workspace bytes, got %zu", need,
+                    workspace_bytes);
+    if (coarse && !aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
     cudaError_t e = dash::launch_zero(dq, static_cast<size_t>(N) * dims * sizeof(float), s);
-    if (e == cudaSuccess) e = dash::launch_bwd_input(P, xyz, t, index, table, half, dout, dq, s);
+    if (e == cudaSuccess && coarse) {
+        const CoarseBuffers b = carve_coarse(workspace, cs, N);
+        if (!(cfg->flags & DASH_HASH4D_FLAG_ORDER_READY))
+            e = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s);
+        if (e == cudaSuccess)
+            e = dash::launch_bwd_input(P, xyz, t, index, table, half, dout, dq, s, b.order, b.sorted_q);
+    } else if (e == cudaSuccess) {
+        e = dash::launch_bwd_input(P, xyz, t, index, table, half, dout, dq, s);
+    }
     if (e != cudaSuccess) return cuda_fail(e, "bwd_input launch");
     return ok();
 }

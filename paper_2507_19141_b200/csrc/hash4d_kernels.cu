@@ -52,7 +52,7 @@ __device__ __forceinline__ Item this_item(const Plan& P) { return this_item(P, b
 // ------------------------------------------------------------------------------------------------
 // Forward: gather + quadrilinear interpolation (Eq. 9)
 // ------------------------------------------------------------------------------------------------
-template <int F, bool HALF, int D>
+template <int F, bool HALF, int D, bool ORDERED>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_fwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                   const float* __restrict__ t, const int32_t* __restrict__ index,
@@ -62,8 +62,8 @@ hash4d_fwd_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
     Item it = this_item(P);
     const LevelParams lp = P.lv[it.l];
     Query q;
-    if (order) {   // SORT_COARSE: position it.n of the cell-sorted order (bwd_runs_kernels.cu) — neighbouring lanes
-                   // then gather from the same cells; the row of `out` is the query's own
+    if constexpr (ORDERED) {   // SORT_COARSE: position it.n of the cell-sorted order (bwd_runs_kernels.cu): neighbouring
+                               // lanes then gather from the same cells; the row of `out` is the query's own
         const float4 c = __ldg(sorted_q + it.n);
         q = make_query<D>(lp, c.x, c.y, c.z, c.w);
         const uint64_t n = static_cast<uint64_t>(static_cast<uint32_t>(__ldg(order + it.n)));
@@ -209,19 +209,28 @@ hash4d_bwd_fixed_kernel(const __grid_constant__ Plan P, const float* __restrict_
 // interpolated value and the difference along the folded axis, so each axis derivative costs one
 // extra subtraction per fold instead of a second pass over the 16 corners.
 // ------------------------------------------------------------------------------------------------
-template <int F, bool HALF, int D>
+template <int F, bool HALF, int D, bool ORDERED>
 __global__ void __launch_bounds__(kBlockThreads)
 hash4d_bwd_input_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz,
                         const float* __restrict__ t, const int32_t* __restrict__ index,
                         const void* __restrict__ table, const float* __restrict__ dout,
-                        float* __restrict__ dq) {
+                        float* __restrict__ dq, const int32_t* __restrict__ order,
+                        const float4* __restrict__ sorted_q) {
     constexpr int NC = 1 << (D - 1);   // D = 3: G_3D, 4 (y,z) corners per lane, dq is [N][3]
-    const Item it = this_item(P);
+    Item it = this_item(P);
     const LevelParams lp = P.lv[it.l];
+    Query q;
     float g[F];
-    load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F,
-                 it.xc, g);
-    const Query q = load_query<D>(P, lp, it.n, xyz, t, index);
+    if constexpr (ORDERED) {   // SORT_COARSE: the it.n-th query of the cell-sorted order; rows of dout / dq are its own
+        const float4 c = __ldg(sorted_q + it.n);
+        q = make_query<D>(lp, c.x, c.y, c.z, c.w);
+        const uint64_t n = static_cast<uint64_t>(static_cast<uint32_t>(__ldg(order + it.n)));
+        it.n = n < P.N ? n : P.N - 1;
+        load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F, it.xc, g);
+    } else {                   // a separate instantiation: the plain kernel is the one that was tuned (32 registers)
+        load_dout<F>(dout + it.n * (static_cast<size_t>(P.L) * F) + static_cast<size_t>(it.l) * F, it.xc, g);
+        q = load_query<D>(P, lp, it.n, xyz, t, index);
+    }
     uint32_t slot[NC];
     float W[NC];
     half_cell<D>(P, lp, q, it.xc, slot, W);  // W unused here; slots shared with fwd
@@ -805,12 +814,19 @@ cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const in
                        const void* table, bool table_half, float* out, cudaStream_t s, const int32_t* order,
                        const float4* sorted_q) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
-#define DASH_FWD(FV, HV)                                                                                        \
-    do {                                                                                                        \
-        if (P.dims == 3)                                                                                        \
-            hash4d_fwd_kernel<FV, HV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, order, sorted_q); \
-        else                                                                                                    \
-            hash4d_fwd_kernel<FV, HV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, order, sorted_q); \
+#define DASH_FWD_D(FV, HV, DV)                                                                               \
+    do {                                                                                                     \
+        if (order)                                                                                           \
+            hash4d_fwd_kernel<FV, HV, DV, true><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, order,   \
+                                                                       sorted_q);                            \
+        else                                                                                                 \
+            hash4d_fwd_kernel<FV, HV, DV, false><<<grid, block, 0, s>>>(P, xyz, t, index, table, out, nullptr, \
+                                                                        nullptr);                            \
+    } while (0)
+#define DASH_FWD(FV, HV)                        \
+    do {                                        \
+        if (P.dims == 3) DASH_FWD_D(FV, HV, 3); \
+        else DASH_FWD_D(FV, HV, 4);             \
     } while (0)
     switch (P.F * 2 + (table_half ? 1 : 0)) {
         case 2: DASH_FWD(1, false); break;
@@ -824,19 +840,27 @@ cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const in
         default: return cudaErrorInvalidValue;
     }
 #undef DASH_FWD
+#undef DASH_FWD_D
     return after_launch();
 }
 
 cudaError_t launch_bwd_input(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                              const void* table, bool table_half, const float* dout, float* dq,
-                             cudaStream_t s) {
+                             cudaStream_t s, const int32_t* order, const float4* sorted_q) {
     const dim3 grid = item_grid(P), block(kBlockThreads);
-#define DASH_BWI(FV, HV)                                                                                \
-    do {                                                                                                \
-        if (P.dims == 3)                                                                                \
-            hash4d_bwd_input_kernel<FV, HV, 3><<<grid, block, 0, s>>>(P, xyz, t, index, table, dout, dq); \
-        else                                                                                            \
-            hash4d_bwd_input_kernel<FV, HV, 4><<<grid, block, 0, s>>>(P, xyz, t, index, table, dout, dq); \
+#define DASH_BWI_D(FV, HV, DV)                                                                                 \
+    do {                                                                                                       \
+        if (order)                                                                                             \
+            hash4d_bwd_input_kernel<FV, HV, DV, true><<<grid, block, 0, s>>>(P, xyz, t, index, table, dout, dq, \
+                                                                             order, sorted_q);                 \
+        else                                                                                                   \
+            hash4d_bwd_input_kernel<FV, HV, DV, false><<<grid, block, 0, s>>>(P, xyz, t, index, table, dout, dq, \
+                                                                              nullptr, nullptr);               \
+    } while (0)
+#define DASH_BWI(FV, HV)                        \
+    do {                                        \
+        if (P.dims == 3) DASH_BWI_D(FV, HV, 3); \
+        else DASH_BWI_D(FV, HV, 4);             \
     } while (0)
     switch (P.F * 2 + (table_half ? 1 : 0)) {
         case 2: DASH_BWI(1, false); break;
@@ -850,6 +874,7 @@ cudaError_t launch_bwd_input(const Plan& P, const float* xyz, const float* t, co
         default: return cudaErrorInvalidValue;
     }
 #undef DASH_BWI
+#undef DASH_BWI_D
     return after_launch();
 }
 

@@ -25,7 +25,7 @@ cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const in
                        const int32_t* order = nullptr, const float4* sorted_q = nullptr);
 cudaError_t launch_bwd_input(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                              const void* table, bool table_half, const float* dout, float* dq,
-                             cudaStream_t s);
+                             cudaStream_t s, const int32_t* order = nullptr, const float4* sorted_q = nullptr);
 cudaError_t launch_smooth(const Plan& P, const float* xyz, const float* t, const int32_t* index,
                           const float* eps, uint32_t eps_stride, const void* table, bool table_half,
                           float two_scale, float* loss, float* dtable, cudaStream_t s);

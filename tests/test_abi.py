@@ -103,7 +103,8 @@ def test_sort_coarse_workspace_and_flag_rules():
         assert need == 128 + 2 * 4 * n + 16 * n + 4 * bins + 4 * (bins // 1024)
         assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_FWD) == need
         assert dh.dash_hash4d_workspace_bytes(dh.with_flags(cfg, sc | dh.FLAG_ORDER_READY), n, dh.OP_BWD) == need
-        for op in (dh.OP_INDICES, dh.OP_BWD_INPUT, dh.OP_SMOOTH):
+        assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD_INPUT) == need
+        for op in (dh.OP_INDICES, dh.OP_SMOOTH):
             assert dh.dash_hash4d_workspace_bytes(cfg, n, op) == 0
         assert dh.dash_hash4d_workspace_bytes(cfg, (1 << 19) - 1, dh.OP_BWD) == 0     # below the threshold: plain path
         det = dh.with_flags(cfg, sc | dh.FLAG_DETERMINISTIC_BWD)

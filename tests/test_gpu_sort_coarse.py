@@ -15,7 +15,7 @@ import oracle
 import paper_2507_19141_b200 as dh
 from dash_inputs import EncoderParams, make_queries_uniform, make_workload
 from parity_utils import RTOL_FP32, check_close
-from test_gpu_parity import DC, both_configs, dev, run_bwd_parity, run_fwd_parity
+from test_gpu_parity import DC, both_configs, dev, run_bwd_input_parity, run_bwd_parity, run_fwd_parity
 
 pytestmark = pytest.mark.gpu
 
@@ -121,7 +121,8 @@ def test_workspace_is_required_and_sized_by_the_library(set_debug):
     need = dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD)
     assert need >= 24 * n
     assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_FWD) == need       # one buffer serves fwd and bwd of a step
-    assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD_INPUT) == 0    # the other calls ignore the flag
+    assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD_INPUT) == need
+    assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_SMOOTH) == 0       # the other calls ignore the flag
     assert dh.dash_hash4d_workspace_bytes(dh.with_flags(cfg, DC | SC | dh.FLAG_DETERMINISTIC_BWD), n, dh.OP_BWD) == \
         dh.dash_hash4d_workspace_bytes(dh.with_flags(cfg, DC | dh.FLAG_DETERMINISTIC_BWD), n, dh.OP_BWD)
     xyz, t = make_queries_uniform(1, n)
@@ -260,3 +261,33 @@ def test_packed_rows_custom_primes_non_power_of_two_table_and_validate_flag(set_
     bad = xyz.copy(); bad[5, 0] = np.nan
     with pytest.raises(dh.Hash4DError):
         dh.dash_hash4d_bwd(vcfg, dev(bad), dev(t), dev(dout), dt)
+
+
+def test_bwd_input_walks_the_sorted_order(set_debug):
+    """dash_hash4d_bwd_input / dash_hash3d_bwd_input under SORT_COARSE: the forward's gathers in the forward's order; the
+    coordinate gradient of every query is unchanged (compared with the oracle and, bitwise, with the plain call)."""
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 3)
+    rng = np.random.default_rng(8)
+    n = 3001
+    enc = EncoderParams(6, 2, 1 << 12, 8, 256, 4, 32)
+    xyz, t = make_queries_uniform(8, n)
+    table = rng.uniform(-1, 1, (6, 1 << 12, 2)).astype(np.float32)
+    dout = rng.standard_normal((n, 12)).astype(np.float32)
+    run_bwd_input_parity(enc, xyz, t, table, dout, flags=DC | SC, what="sort_coarse")
+    index = rng.integers(0, n, 2 * n).astype(np.int32)
+    t2 = rng.random(2 * n, dtype=np.float32)
+    d2 = rng.standard_normal((2 * n, 12)).astype(np.float32)
+    run_bwd_input_parity(enc, xyz, t2, table, d2, index=index, flags=DC | SC, what="sort_coarse, indexed")
+    gs, gp = dh.config_from_params(enc, flags=DC | SC), dh.config_from_params(enc, flags=DC)
+    a = dh.dash_hash4d_bwd_input(gs, dev(xyz), dev(t), dev(table), dev(dout))
+    b = dh.dash_hash4d_bwd_input(gp, dev(xyz), dev(t), dev(table), dev(dout))
+    assert torch.equal(a, b)
+    # the order of the step's forward serves it
+    ws = torch.empty(dh.dash_hash4d_workspace_bytes(gs, n, dh.OP_FWD), dtype=torch.uint8, device="cuda")
+    dh.dash_hash4d_fwd(gs, dev(xyz), dev(t), dev(table), workspace=ws)
+    c = dh.dash_hash4d_bwd_input(dh.with_flags(gs, DC | SC | READY), dev(xyz), dev(t), dev(table), dev(dout), workspace=ws)
+    assert torch.equal(c, b)
+    g3s = dh.make_config(6, 2, 1 << 12, 8, 256, 1, 1, flags=DC | SC)
+    g3p = dh.make_config(6, 2, 1 << 12, 8, 256, 1, 1, flags=DC)
+    assert torch.equal(dh.dash_hash3d_bwd_input(g3s, dev(xyz), dev(table), dev(dout)),
+                       dh.dash_hash3d_bwd_input(g3p, dev(xyz), dev(table), dev(dout)))
