@@ -73,8 +73,11 @@ DASH_API int dash_mlp_bwd(const dash_mlp_config* mlp, uint64_t N, const float* f
  *     dfeat, dparams += backward of the chain  dash_mlp_bwd
  *     dtable += J(x)^T dfeat                   dash_hash4d_bwd (enc->flags: DENSE_COARSE, ZERO_GRAD honoured)
  *     dq = d<dfeat, G_4D(x)>/d(x,y,z,t)        dash_hash4d_bwd_input, when dq ([N][4] fp32, overwritten) is not NULL
- * dL/d base is dout itself.  workspace: dash_deform_bwd_workspace_bytes = 2 * N * L*F * 4 bytes, 16-byte aligned.
- * enc->flags other than DENSE_COARSE | ZERO_GRAD: INVALID_ARG.  Errors of the composed calls are passed through. */
+ * dL/d base is dout itself.  workspace: dash_deform_bwd_workspace_bytes = 2 * N * L*F * 4 bytes (+ the encoder's sort
+ * workspace under SORT_COARSE), 16-byte aligned.  SORT_COARSE in enc->flags: ONE sort of the queries by coarse cell
+ * (inside the forward) serves all three encoder calls (dash_hash4d_bwd and _bwd_input run with ORDER_READY).
+ * enc->flags other than DENSE_COARSE | ZERO_GRAD | SORT_COARSE: INVALID_ARG.  Errors of the composed calls are passed
+ * through. */
 DASH_API size_t dash_deform_bwd_workspace_bytes(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N);
 DASH_API int dash_deform_bwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
                              const float* xyz, uint32_t xyz_stride, const float* t, uint32_t t_stride,

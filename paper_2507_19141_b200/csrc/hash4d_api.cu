@@ -986,7 +986,9 @@ DASH_API size_t dash_deform_bwd_workspace_bytes(const dash_hash4d_config* enc, c
                                                 uint64_t N) {
     if (check_config(enc) || check_mlp(mlp)) return 0;
     g_error[0] = '\0';
-    return 2 * round16(static_cast<size_t>(N) * enc->L * enc->F * sizeof(float));
+    // feature matrix + its gradient, then (SORT_COARSE) the encoder's sort workspace
+    return 2 * round16(static_cast<size_t>(N) * enc->L * enc->F * sizeof(float)) +
+           round16(workspace_need(enc, DASH_HASH4D_OP_FWD, N, 4));
 }
 
 DASH_API int dash_deform_bwd(const dash_hash4d_config* enc, const dash_mlp_config* mlp, uint64_t N,
@@ -996,27 +998,37 @@ DASH_API int dash_deform_bwd(const dash_hash4d_config* enc, const dash_mlp_confi
                              void* cuda_stream) {
     if (int rc = check_config(enc)) return rc;
     if (int rc = check_mlp(mlp)) return rc;
-    if (enc->flags & ~static_cast<uint32_t>(DASH_HASH4D_FLAG_DENSE_COARSE | DASH_HASH4D_FLAG_ZERO_GRAD))
-        return fail(DASH_HASH4D_INVALID_ARG, "deform_bwd: only DENSE_COARSE | ZERO_GRAD may be set in enc->flags");
+    constexpr uint32_t kAllowed = DASH_HASH4D_FLAG_DENSE_COARSE | DASH_HASH4D_FLAG_ZERO_GRAD | DASH_HASH4D_FLAG_SORT_COARSE;
+    if (enc->flags & ~kAllowed)
+        return fail(DASH_HASH4D_INVALID_ARG,
+                    "deform_bwd: only DENSE_COARSE | ZERO_GRAD | SORT_COARSE may be set in enc->flags");
     if (mlp->width[0] != enc->L * enc->F)
         return fail(DASH_HASH4D_INVALID_ARG, "mlp width[0] = %u != L*F = %u", mlp->width[0], enc->L * enc->F);
     const size_t half = round16(static_cast<size_t>(N) * enc->L * enc->F * sizeof(float));
-    if (N && (!workspace || workspace_bytes < 2 * half))
-        return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "deform_bwd needs %zu workspace bytes, got %zu", 2 * half,
-                    workspace_bytes);
+    const size_t sort_bytes = round16(workspace_need(enc, DASH_HASH4D_OP_FWD, N, 4));
+    if (N && (!workspace || workspace_bytes < 2 * half + sort_bytes))
+        return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "deform_bwd needs %zu workspace bytes, got %zu",
+                    2 * half + sort_bytes, workspace_bytes);
     if (N && !aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
     float* feat = static_cast<float*>(workspace);
     float* dfeat = reinterpret_cast<float*>(static_cast<char*>(workspace) + half);
-    dash_hash4d_config plain = *enc;
-    plain.flags = enc->flags & DASH_HASH4D_FLAG_DENSE_COARSE;
-    if (int rc = fwd_impl(4, &plain, N, xyz, xyz_stride, t, t_stride, index, table, feat, nullptr, 0, cuda_stream))
+    void* sort_ws = sort_bytes ? static_cast<char*>(workspace) + 2 * half : nullptr;
+    // SORT_COARSE: ONE sort (inside the forward) serves the forward, the table gradient and the coordinate gradient
+    const uint32_t sorted = enc->flags & DASH_HASH4D_FLAG_SORT_COARSE;
+    const uint32_t ready = sorted ? (sorted | DASH_HASH4D_FLAG_ORDER_READY) : 0u;
+    dash_hash4d_config fcfg = *enc, bcfg = *enc, icfg = *enc;
+    fcfg.flags = (enc->flags & DASH_HASH4D_FLAG_DENSE_COARSE) | sorted;
+    bcfg.flags = (enc->flags & (DASH_HASH4D_FLAG_DENSE_COARSE | DASH_HASH4D_FLAG_ZERO_GRAD)) | ready;
+    icfg.flags = (enc->flags & DASH_HASH4D_FLAG_DENSE_COARSE) | ready;
+    if (int rc = fwd_impl(4, &fcfg, N, xyz, xyz_stride, t, t_stride, index, table, feat, sort_ws, sort_bytes, cuda_stream))
         return rc;
     if (int rc = dash_mlp_bwd(mlp, N, feat, params, dout, dfeat, dparams, cuda_stream)) return rc;
-    if (int rc = bwd_impl(4, enc, N, xyz, xyz_stride, t, t_stride, index, dfeat, dtable, nullptr, 0, cuda_stream))
+    if (int rc = bwd_impl(4, &bcfg, N, xyz, xyz_stride, t, t_stride, index, dfeat, dtable, sort_ws, sort_bytes,
+                          cuda_stream))
         return rc;
     if (dq)
-        if (int rc = dash_hash4d_bwd_input(&plain, N, xyz, xyz_stride, t, t_stride, index, table, dfeat, dq, nullptr, 0,
-                                           cuda_stream))
+        if (int rc = dash_hash4d_bwd_input(&icfg, N, xyz, xyz_stride, t, t_stride, index, table, dfeat, dq, sort_ws,
+                                           sort_bytes, cuda_stream))
             return rc;
     return ok();
 }

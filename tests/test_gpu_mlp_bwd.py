@@ -7,6 +7,8 @@ delta (2^-8 of ONE term of the next sum): elementwise 4e-3 * A with A the oracle
 1e-3 (dfeat) / 4e-3 (dparams, which sums every row's flips).  The relu mask is a DECISION taken from a floating-point
 value: rows whose closest pre-activation is within 1e-3 of its rounding scale of a kink (oracle `margin`) have no unique
 gradient; for them only a validity bound is checked (|err| within twice the unmasked magnitude bound)."""
+import ctypes as C
+
 import numpy as np
 import pytest
 import torch
@@ -139,8 +141,9 @@ def test_mlp_bwd_errors():
         dh.dash_mlp_bwd(m, z(4, 32), z(330), z(4, 10), z(329))
 
 
-@pytest.mark.parametrize("dtype,with_index,zero_grad", [("fp32", False, True), ("fp16", True, False)])
-def test_deform_bwd_is_the_composition_and_matches_the_oracle(dtype, with_index, zero_grad):
+@pytest.mark.parametrize("dtype,with_index,zero_grad,sort", [("fp32", False, True, False), ("fp16", True, False, False),
+                                                             ("fp32", True, True, True), ("fp16", False, False, True)])
+def test_deform_bwd_is_the_composition_and_matches_the_oracle(dtype, with_index, zero_grad, sort, set_debug):
     """dash_deform_bwd = hash4d_fwd -> mlp_bwd -> hash4d_bwd (-> bwd_input).  Checked three ways: against the same
     four calls made one by one; dparams against the oracle chain (oracle_fwd -> oracle_mlp_bwd); dtable and dq against
     the oracle's scatter / coordinate gradient fed the GPU's own dfeat (both are linear in it: no mask ambiguity left)."""
@@ -158,8 +161,14 @@ def test_deform_bwd_is_the_composition_and_matches_the_oracle(dtype, with_index,
     params = make_mlp_params(4, widths)
     dout = rng.standard_normal((n, 10)).astype(np.float32)
     flags = dh.FLAG_DENSE_COARSE | (dh.FLAG_ZERO_GRAD if zero_grad else 0)
+    if sort:   # SORT_COARSE: one sort inside the forward serves the table gradient and the coordinate gradient too
+        set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 3)
+        flags |= dh.FLAG_SORT_COARSE
     gcfg, ocfg = dh.config_from_params(enc, flags=flags), oracle.config_from_params(enc)
     m = dh.make_mlp_config(widths)
+    if sort:
+        need = dh.binding._load().dash_deform_bwd_workspace_bytes(C.byref(gcfg), C.byref(m), n)
+        assert need >= 2 * n * L * F * 4 + 24 * n
     start = 7.0 if zero_grad else 0.0                                       # ZERO_GRAD must overwrite garbage
     dtable = torch.full((L, T, F), start, device="cuda")
     dparams = torch.zeros(params.size, device="cuda")
