@@ -765,7 +765,7 @@ def main():
     ap.add_argument("--sort-coarse", type=int, default=1,
                     help="1: DASH_HASH4D_FLAG_SORT_COARSE — fwd sorts the queries by coarse 4D cell and walks them in that "
                          "order, bwd reuses the order (ORDER_READY) and merges runs on the coarse levels; the library "
-                         "ignores the flag below 2^19 queries.  0: the plain path (A/B)")
+                         "ignores the flag when N*F < 2^21 (C2, C3).  0: the plain path (A/B)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", type=int, default=1,
                     help="1: also time bwd_input / smooth / one-timestamp fwd (information only)")

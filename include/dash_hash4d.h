@@ -63,7 +63,7 @@ enum dash_hash4d_flags {
                                                instead of accumulating into the caller's contents.          */
     DASH_HASH4D_FLAG_SORT_COARSE = 16u,     /* dash_hash4d_fwd / _bwd / _bwd_input, the high-collision case (BASELINE.json config 5):
                                                the queries are counting-sorted by their 4D cell on the coarse levels
-                                               (cell count <= 2N; only for N >= 2^19, else the flag does nothing) and
+                                               (cell count <= 2N; only for N*F >= 2^21, else the flag does nothing) and
                                                those levels are processed in that order — bwd: a segmented reduction,
                                                runs of queries in one cell summed in registers, one vector reduction
                                                per run and corner; fwd: neighbouring lanes gather from the same cells.

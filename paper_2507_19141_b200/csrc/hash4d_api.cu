@@ -290,7 +290,9 @@ static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSor
     const uint32_t forced = debug_u32(DASH_DEBUG_BWD_COARSE_LEVELS);
     if (forced) {
         nl = forced < c->L ? forced : c->L;
-    } else if (N >= (1ull << 19)) {   // below that the sort costs more than the merged reductions save (C3: +0.04 ms)
+    } else if (N * c->F >= (1ull << 21)) {
+        // below that the sort costs more than it saves: measured crossover ~350k queries at F = 4 (C4's encoder), ~750k at
+        // F = 2 (C3's encoder; C3 itself, 300k: +8 %) — profiles/experiments_r02.md §8
         while (nl < c->L && nl < 8) {
             const double cells = static_cast<double>(s.res_s[nl]) * s.res_s[nl] * s.res_s[nl] * s.res_t[nl];
             if (cells > 2.0 * static_cast<double>(N)) break;

@@ -93,7 +93,7 @@ def test_workspace_sizes():
 
 def test_sort_coarse_workspace_and_flag_rules():
     """DASH_HASH4D_FLAG_SORT_COARSE (include/dash_hash4d.h): needs a workspace only where the library takes the sorted
-    path (N >= 2^19, at least one level with Ns^3 Nt <= 2N), the same size for fwd and bwd, none for the other calls,
+    path (N*F >= 2^21, at least one level with Ns^3 Nt <= 2N), the same size for fwd and bwd, none for the other calls,
     none under DETERMINISTIC_BWD; ORDER_READY changes no size; bit 64 is still an unknown flag."""
     sc = dh.FLAG_DENSE_COARSE | dh.FLAG_SORT_COARSE
     for name, n in (("C4", 1_000_000), ("C5", 1_800_000)):
@@ -106,7 +106,9 @@ def test_sort_coarse_workspace_and_flag_rules():
         assert dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_BWD_INPUT) == need
         for op in (dh.OP_INDICES, dh.OP_SMOOTH):
             assert dh.dash_hash4d_workspace_bytes(cfg, n, op) == 0
-        assert dh.dash_hash4d_workspace_bytes(cfg, (1 << 19) - 1, dh.OP_BWD) == 0     # below the threshold: plain path
+        below = (1 << 21) // CONFIGS[name].enc.F - 1
+        assert dh.dash_hash4d_workspace_bytes(cfg, below, dh.OP_BWD) == 0              # below the threshold: plain path
+        assert dh.dash_hash4d_workspace_bytes(cfg, below + 1, dh.OP_BWD) > 24 * below
         det = dh.with_flags(cfg, sc | dh.FLAG_DETERMINISTIC_BWD)
         assert dh.dash_hash4d_workspace_bytes(det, n, dh.OP_FWD) == 0
     c3 = dh.config_from_params(CONFIGS["C3"].enc, flags=sc)

@@ -27,13 +27,13 @@ READY = dh.FLAG_ORDER_READY
 @pytest.mark.parametrize("name", ["C3", "C4", "C5"])
 def test_full_size_configs(name):
     """The bench's launch configuration (ZERO_GRAD + SORT_COARSE, the library's own choice of coarse levels; the forward
-    sorts, the backward of the same step reuses the order).  C3 (N < 2^19) takes the plain path and needs no workspace."""
+    sorts, the backward of the same step reuses the order).  C3 (N F < 2^21) takes the plain path and needs no workspace."""
     wl = make_workload(name)
     enc, N = wl.spec.enc, wl.N
     cfg = dh.config_from_params(enc, flags=DC | ZG | SC)
     need = dh.dash_hash4d_workspace_bytes(cfg, N, dh.OP_BWD)
     assert need == dh.dash_hash4d_workspace_bytes(cfg, N, dh.OP_FWD)
-    assert (need >= 24 * N) if N >= (1 << 19) else (need == 0)
+    assert (need >= 24 * N) if N * enc.F >= (1 << 21) else (need == 0)
     run_fwd_parity(enc, wl.xyz, wl.t, wl.table, index=wl.index, flags=DC | SC, what=name + " sort_coarse")
     run_bwd_parity(enc, wl.xyz, wl.t, wl.dout, index=wl.index, flags=DC | ZG | SC, what=name + " sort_coarse")
     if need:
