@@ -201,30 +201,39 @@ def test_g3d_full_size_workload():
     _g3d_parity(o3, g3, wl.xyz, wl.table, wl.dout, what="G3D workload")
 
 
-def test_sorted_path_is_cuda_graph_capturable(set_debug):
+def test_sorted_step_is_cuda_graph_capturable(set_debug):
+    """A whole step — forward with its sort, backward on the forward's order — captured once and replayed."""
     set_debug(dh.DEBUG_BWD_COARSE_LEVELS, 3)
     enc = EncoderParams(6, 2, 1 << 12, 8, 256, 4, 32)
     n = 5000
     rng = np.random.default_rng(4)
     xyz, t = make_queries_uniform(4, n)
+    table = rng.uniform(-1, 1, (6, 1 << 12, 2)).astype(np.float32)
     dout = rng.standard_normal((n, 12)).astype(np.float32)
     ocfg, gcfg = both_configs(enc, DC | ZG | SC)
+    bcfg = dh.with_flags(gcfg, DC | ZG | SC | READY)
+    ref_f, mag_f = oracle.oracle_fwd(ocfg, n, xyz, t, table, want_abs=True)
     ref, mag, hits = oracle.oracle_bwd(ocfg, n, xyz, t, dout, want_abs=True, want_hits=True)
-    xd, td, dd = dev(xyz), dev(t), dev(dout)
+    xd, td, tabd, dd = dev(xyz), dev(t), dev(table), dev(dout)
+    out = torch.empty((n, 12), device="cuda")
     dt = torch.full((6, 1 << 12, 2), 7.0, device="cuda")
     ws = torch.empty(dh.dash_hash4d_workspace_bytes(gcfg, n, dh.OP_BWD), dtype=torch.uint8, device="cuda")
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
-        dh.dash_hash4d_bwd(gcfg, xd, td, dd, dt, workspace=ws)                 # warm-up outside the capture
+        dh.dash_hash4d_fwd(gcfg, xd, td, tabd, out=out, workspace=ws)         # warm-up outside the capture
+        dh.dash_hash4d_bwd(bcfg, xd, td, dd, dt, workspace=ws)
         stream.synchronize()
         graph = torch.cuda.CUDAGraph()
         with torch.cuda.graph(graph, stream=stream):
-            dh.dash_hash4d_bwd(gcfg, xd, td, dd, dt, workspace=ws)
+            dh.dash_hash4d_fwd(gcfg, xd, td, tabd, out=out, workspace=ws)
+            dh.dash_hash4d_bwd(bcfg, xd, td, dd, dt, workspace=ws)
     for _ in range(2):
-        dt.fill_(3.0)
+        dt.fill_(3.0); out.fill_(5.0); ws.zero_()                              # the replay rebuilds the order itself
         graph.replay()
         torch.cuda.synchronize()
-        check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 6, hits=hits, what="graph replay")
+        check_close(dt.cpu().numpy(), ref, mag, RTOL_FP32, 6, hits=hits, what="graph replay bwd")
+        tr = lambda a: np.asarray(a).reshape(n, 6, 2).transpose(1, 0, 2)
+        check_close(tr(out.cpu().numpy()), tr(ref_f), tr(mag_f), RTOL_FP32, 6, what="graph replay fwd")
 
 
 def test_packed_rows_custom_primes_non_power_of_two_table_and_validate_flag(set_debug):
