@@ -520,6 +520,22 @@ def run_cuda(args):
             det_ms = None
     roofline["deterministic_bwd_ms"] = det_ms
 
+    # ---- what the coarse sort costs inside the forward call: the same forward on the order already in the workspace
+    if sorted_path:
+        def avg_ms(fn, iters=20):
+            fn(); fn()
+            torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record()
+            for _ in range(iters):
+                fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / iters
+        with_sort = avg_ms(lambda: dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index, workspace=bwd_ws))
+        ready = avg_ms(lambda: dh.dash_hash4d_fwd(cfg_bwd, xyz, t, table, out=out, index=index, workspace=bwd_ws))
+        roofline["step"]["ms"]["fwd_sort_part"] = with_sort - ready
+
     # ---- e2e: HOST (pinned) buffers through the binding's *_host calls, copies inside the timed region
     pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory()
     xyz_h, t_h, index_h, dout_h = pin(wl.xyz), pin(wl.t), pin(wl.index), pin(wl.dout)
