@@ -61,22 +61,27 @@ enum dash_hash4d_flags {
     DASH_HASH4D_FLAG_ZERO_GRAD = 8u,        /* bwd OVERWRITES: the library zeroes each level group of dtable
                                                immediately before scattering into it (keeps it L2-resident)
                                                instead of accumulating into the caller's contents.          */
-    DASH_HASH4D_FLAG_SORT_COARSE = 16u,     /* dash_hash4d_fwd / _bwd / _bwd_input, the high-collision case (BASELINE.json config 5):
-                                               the queries are counting-sorted by their 4D cell on the coarse levels
-                                               (cell count <= 2N; only for N*F >= 2^21, else the flag does nothing) and
-                                               those levels are processed in that order — bwd: a segmented reduction,
-                                               runs of queries in one cell summed in registers, one vector reduction
-                                               per run and corner; fwd: neighbouring lanes gather from the same cells.
-                                               The other levels are unchanged.  Same values (fwd) / same sums in
-                                               another order (bwd: same tolerance).  Needs workspace.  Honoured by
-                                               dash_hash4d_fwd / _bwd / _bwd_input (the forward's gathers) and their
-                                               dash_hash3d_* forms (3D cells, no t in the key); ignored under
+    DASH_HASH4D_FLAG_SORT_COARSE = 16u,     /* the high-collision case (BASELINE.json config 5; the gradient scatter is
+                                               the transpose of Eq. 9).  The queries are counting-
+                                               sorted by the Morton code of their 4D cell on the finest COARSE level
+                                               (the last level with Ns^3 Nt <= 2N) and walked in that order:
+                                                 fwd / bwd_input  every level: neighbouring lanes gather from the
+                                                                  same cells and lines; values unchanged (bitwise);
+                                                 bwd              the coarse levels: a segmented reduction — runs of
+                                                                  queries in one cell are summed in registers, one
+                                                                  vector reduction per run and corner (same sums in
+                                                                  another order: same tolerance); the finer levels
+                                                                  keep the caller's order.
+                                               Taken only when N*F >= 2^21 and a coarse level exists, else the flag
+                                               does nothing.  Needs workspace (dash_hash4d_workspace_bytes).  Honoured
+                                               by dash_hash4d_fwd / _bwd / _bwd_input, their dash_hash3d_* forms (3D
+                                               cells, no t in the key) and dash_deform_bwd; ignored under
                                                DETERMINISTIC_BWD and by the other calls.                          */
     DASH_HASH4D_FLAG_ORDER_READY = 32u      /* with SORT_COARSE: `workspace` still holds the order that an earlier
-                                               dash_hash4d_fwd / _bwd / _bwd_input call with SORT_COARSE wrote for the SAME
-                                               queries (N, xyz, t, index unchanged, e.g. the forward of this training
-                                               step): the sort (five launches) is skipped.  A false claim gives
-                                               wrong values but no out-of-bounds access.                        */
+                                               fwd / bwd / bwd_input call with SORT_COARSE wrote for the SAME queries
+                                               (N, xyz, t, index unchanged, e.g. the forward of this training step):
+                                               the sort (five launches) is skipped.  A false claim gives wrong
+                                               values but no out-of-bounds access.                              */
 };
 
 enum dash_hash4d_op { DASH_HASH4D_OP_FWD = 0, DASH_HASH4D_OP_BWD = 1, DASH_HASH4D_OP_INDICES = 2,
