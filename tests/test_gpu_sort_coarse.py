@@ -300,3 +300,52 @@ def test_bwd_input_walks_the_sorted_order(set_debug):
     g3p = dh.make_config(6, 2, 1 << 12, 8, 256, 1, 1, flags=DC)
     assert torch.equal(dh.dash_hash3d_bwd_input(g3s, dev(xyz), dev(table), dev(dout)),
                        dh.dash_hash3d_bwd_input(g3p, dev(xyz), dev(table), dev(dout)))
+
+
+def test_the_order_in_the_workspace_is_a_permutation_sorted_by_the_morton_key_of_the_cell(set_debug):
+    """What the speed of the path rests on (never its results): after a call with SORT_COARSE the workspace holds, behind
+    its 128-byte header, `order` [N] int32 — a permutation of the queries along which the Morton code of the 4D cell on the
+    key level (the last coarse level) never decreases — then the keys, then `sorted_q` [N] float4 = the coordinates of
+    query order[i].  The key is rebuilt here with numpy: one binary32 product and a floor per axis (the library's own cell
+    location), bit b of x, y, z (while b < bits_s) and of t (while b < bits_t) interleaved from bit 0 up."""
+    levels = 3
+    set_debug(dh.DEBUG_BWD_COARSE_LEVELS, levels)
+    enc = EncoderParams(6, 2, 1 << 12, 8, 256, 4, 32)
+    rng = np.random.default_rng(17)
+    rows = 3000
+    xyz = np.clip(0.5 + 0.25 * rng.standard_normal((rows, 3)), 0, 0.999).astype(np.float32)
+    index = rng.integers(0, rows, 5003).astype(np.int32)
+    n = len(index)
+    t = rng.random(n, dtype=np.float32)
+    cfg = dh.config_from_params(enc, flags=DC | SC)
+    ws = torch.zeros(dh.dash_hash4d_workspace_bytes(cfg, n, dh.OP_FWD), dtype=torch.uint8, device="cuda")
+    table = dev(rng.uniform(-1, 1, (6, 1 << 12, 2)).astype(np.float32))
+    dh.dash_hash4d_fwd(cfg, dev(xyz), dev(t), table, index=dev(index), workspace=ws)
+    torch.cuda.synchronize()
+    raw = ws.cpu().numpy()
+    r16 = lambda v: (v + 15) // 16 * 16
+    order = raw[128:128 + 4 * n].view(np.int32)
+    sq_at = 128 + 2 * r16(4 * n)
+    sorted_q = raw[sq_at:sq_at + 16 * n].view(np.float32).reshape(n, 4)
+    assert np.array_equal(np.sort(order), np.arange(n))
+    pts = np.concatenate([xyz[index], t[:, None]], axis=1)
+    assert np.array_equal(sorted_q, pts[order])
+    res_s, res_t, _ = dh.dash_hash4d_resolutions(cfg)
+    ns, nt = res_s[levels - 1], res_t[levels - 1]
+    bits_s, bits_t = int(np.ceil(np.log2(ns))), int(np.ceil(np.log2(nt)))
+    assert 3 * bits_s + bits_t <= 22 and max(bits_s, bits_t) <= 7      # no coarsening of the key at this size
+    cell = np.empty((n, 4), np.uint64)
+    for d in range(4):
+        cell[:, d] = np.floor(pts[:, d] * np.float32(nt if d == 3 else ns)).astype(np.uint64)
+    key = np.zeros(n, np.uint64)
+    pos = 0
+    for b in range(8):
+        if b < bits_s:
+            for d in range(3):
+                key |= ((cell[:, d] >> np.uint64(b)) & np.uint64(1)) << np.uint64(pos + d)
+            pos += 3
+        if b < bits_t:
+            key |= ((cell[:, 3] >> np.uint64(b)) & np.uint64(1)) << np.uint64(pos)
+            pos += 1
+    assert (np.diff(key[order].astype(np.int64)) >= 0).all()
+    assert len(np.unique(key)) > 50                                      # the check is not vacuous
