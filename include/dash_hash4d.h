@@ -276,6 +276,34 @@ DASH_API int dash_hash4d_sort_queries(uint64_t N, const float* xyz, uint32_t xyz
                                       uint32_t bits, int32_t* order, void* workspace, size_t workspace_bytes,
                                       void* cuda_stream);
 
+/* dash_hash4d_sort_queries for callers that are not able to allocate device memory.
+ *
+ * Who that is: code that runs inside somebody else's GPU budget.  A plug-in of a renderer or trainer is handed its input
+ * and output buffers by the host application, which owns every other byte of HBM through its own pool; a per-frame loop
+ * (the paper renders at 264 FPS) must not call cudaMalloc / cudaFree because they serialise the whole device
+ * and stall every other stream; and on a GPU whose memory is already committed to tables and Gaussians a late cudaMalloc
+ * can simply fail.  Such a caller has nowhere to get the `workspace` that dash_hash4d_sort_queries asks for.
+ *
+ * This call needs none: the sort's scratch (a key per query, the histogram bins, the scan totals) is a fixed array inside
+ * the library's own device data segment.  The call itself runs no cudaMalloc, cudaFree or any allocating library routine.
+ *   - The array is DASH_HASH4D_SORT_STATIC_MAX_N * 4 + 8^DASH_HASH4D_SORT_STATIC_MAX_BITS * 4 + 1024 bytes (5 243 904 B,
+ *     about 5 MB).  Every GPU on which this process uses the library carries it from the moment the library's device code
+ *     is loaded there until the process exits, whether or not this call is ever made.
+ *   - Limits: N <= DASH_HASH4D_SORT_STATIC_MAX_N and bits <= DASH_HASH4D_SORT_STATIC_MAX_BITS.  Anything larger returns
+ *     DASH_HASH4D_UNSUPPORTED with a message naming the limit (nothing is launched); use dash_hash4d_sort_queries then.
+ *   - The first call on each device looks up where the array lives on that device (cudaGetSymbolAddress, with that device
+ *     current) and remembers it; make that first call before starting any stream capture on that device.
+ *   - All calls on a device share the one array, and it keeps the previous call's contents; each call re-zeroes the part
+ *     it counts into, so back-to-back calls on one stream are fine.  Two calls that may execute on the GPU at the same
+ *     time (different streams, or different host threads on different streams) race on it and give a wrong `order`:
+ *     serialise them yourself.
+ * Arguments, key, result (`order` = query numbers by non-decreasing Morton key, ties in any order), launches (five, on
+ * `cuda_stream`, no synchronisation) and N == 0 behaviour are those of dash_hash4d_sort_queries. */
+#define DASH_HASH4D_SORT_STATIC_MAX_N 1048576ull /* 2^20 queries */
+#define DASH_HASH4D_SORT_STATIC_MAX_BITS 6       /* 2^18 bins    */
+DASH_API int dash_hash4d_sort_queries_static(uint64_t N, const float* xyz, uint32_t xyz_stride, const int32_t* index,
+                                             uint32_t bits, int32_t* order, void* cuda_stream);
+
 /* dtable <- 0 for the whole [L][T][F] fp32 gradient buffer (the accumulation's initial state), with the
  * library's own fill kernel on `cuda_stream`. */
 DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void* cuda_stream);

@@ -29,7 +29,8 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash3
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices", "dash_hash3d_bwd_input",
            "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_mlp_bwd", "dash_deform_bwd", "dash_deform_bwd_workspace_bytes", "dash_deform_workspace_bytes", "dash_deform_fwd",
            "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch",
-           "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_deform_slice_workspace_bytes",
+           "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_hash4d_sort_queries_static",
+           "dash_deform_slice_workspace_bytes",
            "dash_decompose_workspace_bytes", "dash_decompose"]
 
 
@@ -166,6 +167,8 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_hash4d_sort_workspace_bytes.restype = sz
     lib.dash_hash4d_sort_queries.argtypes = [u64, vp, u32, vp, u32, vp, vp, sz, vp]
     lib.dash_hash4d_sort_queries.restype = C.c_int
+    lib.dash_hash4d_sort_queries_static.argtypes = [u64, vp, u32, vp, u32, vp, vp]
+    lib.dash_hash4d_sort_queries_static.restype = C.c_int
     lib.dash_decompose_workspace_bytes.argtypes = [u64]
     lib.dash_decompose_workspace_bytes.restype = sz
     lib.dash_decompose.argtypes = [u64, vp, C.c_double, C.c_float, vp, vp, vp, vp, vp, sz, vp]
@@ -449,6 +452,36 @@ def dash_hash4d_sort_queries(xyz, index=None, bits=6, N=None, order=None, worksp
     _one_device(xyz, index, order, workspace)
     _check(_load().dash_hash4d_sort_queries(N, _ptr(xyz), xs, _ptr(index), int(bits), _ptr(order), _ptr(workspace),
                                             workspace.numel(), _stream()))
+    return order
+
+
+SORT_STATIC_MAX_N = 1 << 20   # DASH_HASH4D_SORT_STATIC_MAX_N
+SORT_STATIC_MAX_BITS = 6       # DASH_HASH4D_SORT_STATIC_MAX_BITS
+
+
+def dash_hash4d_sort_queries_static(xyz, order, index=None, bits=6, N=None):
+    """dash_hash4d_sort_queries without any device allocation, for callers that cannot make one: a plug-in whose host
+    application owns the GPU memory pool, a per-frame loop that must not stall the device in cudaMalloc / cudaFree, a
+    process whose HBM is already full.  The sort's scratch is a fixed ~5 MB array inside the library (held by every GPU
+    that loads it), so N <= SORT_STATIC_MAX_N and bits <= SORT_STATIC_MAX_BITS; beyond that the library refuses
+    (Hash4DError, UNSUPPORTED) and dash_hash4d_sort_queries with a workspace is the call to use.  `order` ([N] int32) is
+    the caller's buffer and is required: this wrapper, too, creates no tensor.  Calls share the scratch: do not let two of
+    them overlap on the GPU.  The first call on a device does a one-time address look-up; make it outside stream capture."""
+    _dev(xyz, torch.float32, "xyz"); _dev(index, torch.int32, "index"); _dev(order, torch.int32, "order")
+    if order is None:
+        raise ValueError("order is required: the no-allocation call writes into the caller's buffer")
+    if xyz.dim() != 2 or int(xyz.shape[1]) not in (3, 4):
+        raise ValueError("xyz must be [rows][3] or [rows][4]")
+    if N is None:
+        N = int(index.numel()) if index is not None else int(xyz.shape[0])
+    if index is not None:
+        _at_least(index, N, "index")
+    elif xyz.shape[0] < N:
+        raise ValueError(f"xyz has {xyz.shape[0]} rows, the call needs {N}")
+    _at_least(order, N, "order")
+    _one_device(xyz, index, order)
+    _check(_load().dash_hash4d_sort_queries_static(N, _ptr(xyz), int(xyz.shape[1]), _ptr(index), int(bits),
+                                                   _ptr(order), _stream()))
     return order
 
 

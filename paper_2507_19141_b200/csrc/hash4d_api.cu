@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 
 #include "../../include/dash_deform.h"
 #include "../../include/dash_hash4d.h"
@@ -792,6 +793,85 @@ DASH_API int dash_hash4d_zero(const dash_hash4d_config* cfg, float* dtable, void
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------
+// dash_hash4d_sort_queries_static: the query sort for callers that must not allocate device memory.
+//
+// The counting sort needs scratch besides its input and output: one key per query, the histogram bins and the
+// scan's per-CTA totals.  dash_hash4d_sort_queries takes that scratch from the caller; this variant takes it from
+// the array below, which lives in the library's own device data segment.  The CUDA runtime places the array on
+// every GPU whose context loads the library and keeps it there until the process exits, so no call ever
+// allocates, and the price is kSortStaticBytes (about 5 MB) of HBM per GPU whether or not the call is used.
+//
+// `g_sort_static` is only a device address inside device code.  In host code the same name is a host-side handle:
+// handing it to a kernel as if it were a pointer makes the kernel fault, or (on systems where the GPU can
+// dereference host addresses) scribble over host memory.  The host therefore asks the runtime where the array
+// lives on the CURRENT device (cudaGetSymbolAddress), once per device, and passes that address on.
+// ------------------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kSortStaticKeysBytes = static_cast<size_t>(DASH_HASH4D_SORT_STATIC_MAX_N) * 4;
+constexpr size_t kSortStaticBinsBytes = (static_cast<size_t>(1) << (3 * DASH_HASH4D_SORT_STATIC_MAX_BITS)) * 4;
+constexpr size_t kSortStaticTotalsBytes = 1024;  // >= one uint32 per 1024 bins at the maximum bin count
+constexpr size_t kSortStaticBytes = kSortStaticKeysBytes + kSortStaticBinsBytes + kSortStaticTotalsBytes;
+static_assert(kSortStaticTotalsBytes >= (kSortStaticBinsBytes / 4 + 1023) / 1024 * 4, "totals region too small");
+static_assert(kSortStaticKeysBytes % 256 == 0 && kSortStaticBinsBytes % 256 == 0, "regions keep the alignment");
+
+static __device__ __align__(256) unsigned char g_sort_static[kSortStaticBytes];
+
+constexpr int kSortStaticMaxDevices = 64;
+std::mutex g_sort_static_mutex;
+unsigned char* g_sort_static_addr[kSortStaticMaxDevices] = {};  // per device ordinal; NULL = not looked up yet
+
+// Device address of g_sort_static on the current device.  The first call on a device performs the look-up (which
+// also makes the runtime load the module there); later calls return the cached address.
+int sort_static_address(unsigned char** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (dev < 0 || dev >= kSortStaticMaxDevices)
+        return fail(DASH_HASH4D_UNSUPPORTED, "device ordinal %d outside 0..%d", dev, kSortStaticMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_sort_static_mutex);
+    if (!g_sort_static_addr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_sort_static);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(static sort scratch)");
+        if (!p) return fail(DASH_HASH4D_CUDA_ERROR, "cudaGetSymbolAddress returned NULL for the static sort scratch");
+        g_sort_static_addr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = g_sort_static_addr[dev];
+    return DASH_HASH4D_OK;
+}
+
+}  // namespace
+
+extern "C" DASH_API int dash_hash4d_sort_queries_static(uint64_t N, const float* xyz, uint32_t xyz_stride,
+                                                        const int32_t* index, uint32_t bits, int32_t* order,
+                                                        void* cuda_stream) {
+    if (bits < 1 || bits > DASH_HASH4D_SORT_STATIC_MAX_BITS)
+        return fail(DASH_HASH4D_UNSUPPORTED, "bits = %u outside 1..%d: the built-in scratch holds at most 2^%d bins; "
+                    "use dash_hash4d_sort_queries with a caller-supplied workspace", bits,
+                    DASH_HASH4D_SORT_STATIC_MAX_BITS, 3 * DASH_HASH4D_SORT_STATIC_MAX_BITS);
+    if (N > DASH_HASH4D_SORT_STATIC_MAX_N)
+        return fail(DASH_HASH4D_UNSUPPORTED, "N = %llu exceeds the %llu queries the built-in scratch holds; "
+                    "use dash_hash4d_sort_queries with a caller-supplied workspace",
+                    static_cast<unsigned long long>(N), static_cast<unsigned long long>(DASH_HASH4D_SORT_STATIC_MAX_N));
+    if (N == 0) return ok();
+    if (!xyz || !order) return fail(DASH_HASH4D_INVALID_ARG, "xyz or order is NULL");
+    if (!(xyz_stride == 3 || xyz_stride == 4))
+        return fail(DASH_HASH4D_INVALID_ARG, "xyz_stride = %u (want 3 or 4)", xyz_stride);
+    unsigned char* base = nullptr;
+    if (int rc = sort_static_address(&base)) return rc;
+    uint32_t* keys = reinterpret_cast<uint32_t*>(base);
+    uint32_t* bins = reinterpret_cast<uint32_t*>(base + kSortStaticKeysBytes);
+    uint32_t* totals = reinterpret_cast<uint32_t*>(base + kSortStaticKeysBytes + kSortStaticBinsBytes);
+    // Same five launches as dash_hash4d_sort_queries.  The array still holds whatever the previous call left: the
+    // first launch zeroes the bins this call counts into; keys[0..N) and the totals are fully rewritten before read.
+    cudaError_t e = dash::launch_sort_queries(N, xyz, xyz_stride, index, bits, order, keys, bins, totals,
+                                              static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(e, "static sort launch");
+    return ok();
+}
 
 // ------------------------------------------------------------------------------------------------------------
 // Render path: G_4D -> phi_d -> heads (include/dash_deform.h; Eq. 9-10; Q27)
