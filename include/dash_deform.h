@@ -62,7 +62,7 @@ DASH_API int dash_mlp_fwd(const dash_mlp_config* mlp, uint64_t N,
  *   dfeat    nullable, [N][width[0]] fp32, 16-byte aligned, written: dL/d feat — the `dout` of dash_hash4d_bwd /
  *            dash_hash4d_bwd_input when feat = G_4D(x).
  *   dparams  [dash_mlp_param_count] fp32, packed like params, ACCUMULATED into (+=): the caller zeroes it.
- * UNSUPPORTED when a width exceeds 240, or the tiles / accumulators of the chain exceed 227 KB of shared memory or
+ * UNSUPPORTED when width[0] exceeds 240 or any later width exceeds 128, or the tiles / accumulators of the chain exceed 227 KB of shared memory or
  * the 512 tensor-memory columns of an SM (accumulator + one kpad-wide weight-gradient block per layer). */
 DASH_API int dash_mlp_bwd(const dash_mlp_config* mlp, uint64_t N, const float* feat, const float* params,
                           const float* dout, float* dfeat, float* dparams, void* cuda_stream);

@@ -1006,6 +1006,11 @@ int fill_mlp_bwd_plan(const dash_mlp_config* m, uint64_t N, dash::MlpBwdPlan* B)
         if (M.kpad[l] > 256)
             return fail(DASH_HASH4D_UNSUPPORTED, "mlp_bwd: width[%u] = %u exceeds 240 (one wgrad MMA covers N <= 256)",
                         l, M.width[l]);
+        // One M = 128 wgrad issue and 16-chunk delta buffers per layer: a wider OUTPUT would lose rows >= 128 of dW / db
+        // and write its delta tile past the shared-memory allocation.
+        if (M.width[l + 1] > 128)
+            return fail(DASH_HASH4D_UNSUPPORTED, "mlp_bwd: width[%u] = %u exceeds 128 (a layer's output is one M = 128 "
+                        "weight-gradient tile)", l + 1, M.width[l + 1]);
         B->w_off[l] = off;
         off += (M.kpad[l] / 8) * (M.npad[l] * 16 + 16);
     }

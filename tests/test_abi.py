@@ -170,3 +170,15 @@ def test_set_debug_validates_and_reads_no_environment(monkeypatch):
     src = "".join(open(os.path.join(ROOT, "paper_2507_19141_b200", "csrc", f)).read()
                   for f in os.listdir(os.path.join(ROOT, "paper_2507_19141_b200", "csrc")))
     assert "getenv" not in src
+
+
+def test_mlp_bwd_refuses_layer_outputs_wider_than_one_tile():
+    """dash_mlp_bwd issues one M = 128 weight-gradient tile per layer: an output width above 128 is UNSUPPORTED (decided
+    on the host before any pointer is looked at), widths up to 128 pass the plan (NULL buffers then give INVALID_ARG)."""
+    lib = dh.binding._load()
+    call = lambda widths: lib.dash_mlp_bwd(C.byref(dh.make_mlp_config(widths)), 4, None, None, None, None, None, None)
+    for widths in ([32, 192, 10], [32, 64, 200], [32, 129]):
+        assert call(widths) == 2, widths
+        assert "128" in dh.dash_hash4d_last_error()
+    for widths in ([32, 128, 10], [32, 128, 128, 10], [240, 16]):
+        assert call(widths) == 1, widths

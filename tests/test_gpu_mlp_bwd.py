@@ -136,6 +136,11 @@ def test_mlp_bwd_errors():
     with pytest.raises(dh.Hash4DError) as e:
         dh.dash_mlp_bwd(wide, z(4, 250), z(dh.dash_mlp_param_count(wide)), z(4, 10), z(dh.dash_mlp_param_count(wide)))
     assert e.value.status == 2
+    for widths in ([32, 192, 10], [32, 64, 200]):                           # a layer output wider than one M = 128 tile
+        c = dh.make_mlp_config(widths)
+        with pytest.raises(dh.Hash4DError) as e:
+            dh.dash_mlp_bwd(c, z(4, 32), z(dh.dash_mlp_param_count(c)), z(4, widths[-1]), z(dh.dash_mlp_param_count(c)))
+        assert e.value.status == 2 and "128" in str(e.value)
     m = dh.make_mlp_config([32, 10])
     with pytest.raises(ValueError, match="dparams"):
         dh.dash_mlp_bwd(m, z(4, 32), z(330), z(4, 10), z(329))
