@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdash_hash4d.so")
 SOURCES = ["hash4d_kernels.cu", "bwd_runs_kernels.cu", "deform_kernels.cu", "mlp_bwd_kernels.cu", "hash4d_api.cu", "ceilings.cu", "decompose_kernels.cu"]
-DEPS = SOURCES + ["hash4d_kernels.h", "hash4d_plan.h", "hash4d_device.cuh", "deform_kernels.h", "deform_profile.cuh", "tcgen05_ptx.cuh", os.path.join("..", "..", "include", "dash_deform.h"), os.path.join("..", "..", "include", "dash_hash4d.h"),
+DEPS = SOURCES + ["api_errors.h", "hash4d_kernels.h", "hash4d_plan.h", "hash4d_device.cuh", "deform_kernels.h", "deform_profile.cuh", "tcgen05_ptx.cuh", os.path.join("..", "..", "include", "dash_deform.h"), os.path.join("..", "..", "include", "dash_hash4d.h"),
                os.path.join("..", "..", "include", "dash_ceilings.h"),
                os.path.join("..", "..", "include", "dash_decompose.h")]
 

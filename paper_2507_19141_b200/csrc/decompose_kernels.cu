@@ -7,6 +7,7 @@
 #include <cstdint>
 
 #include "../../include/dash_decompose.h"
+#include "api_errors.h"       // api_fail, api_cuda_fail, api_ok
 #include "deform_kernels.h"   // count_launch, device_sm_count
 
 namespace dash {
@@ -206,13 +207,20 @@ DASH_API int dash_decompose(uint64_t N, const float* dp, double k_percent, float
                             int32_t* dyn_index, dash_decompose_result* result, float* ddp, void* workspace,
                             size_t workspace_bytes, void* cuda_stream) {
     using namespace dash;
-    if (!(k_percent >= 0.0 && k_percent <= 100.0) || !result) return DASH_HASH4D_INVALID_ARG;
-    if (N > 0x7fffffffull) return DASH_HASH4D_UNSUPPORTED;
-    if (N && (!dp || !mag || !dyn_index)) return DASH_HASH4D_INVALID_ARG;
+    if (!(k_percent >= 0.0 && k_percent <= 100.0))
+        return api_fail(DASH_HASH4D_INVALID_ARG, "decompose: k_percent = %g outside [0, 100]", k_percent);
+    if (!result) return api_fail(DASH_HASH4D_INVALID_ARG, "decompose: result is NULL");
+    if (N > 0x7fffffffull) return api_fail(DASH_HASH4D_UNSUPPORTED, "decompose: N too large for an int32 index list");
+    if (N && (!dp || !mag || !dyn_index))
+        return api_fail(DASH_HASH4D_INVALID_ARG, "decompose: dp, mag or dyn_index is NULL");
     const size_t need = dash_decompose_workspace_bytes(N);
-    if (!workspace || workspace_bytes < need) return DASH_HASH4D_WORKSPACE_TOO_SMALL;
-    if ((reinterpret_cast<uintptr_t>(workspace) & 15u) || (reinterpret_cast<uintptr_t>(result) & 3u))
-        return DASH_HASH4D_INVALID_ARG;
+    if (!workspace || workspace_bytes < need)
+        return api_fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "decompose needs %zu workspace bytes, got %zu", need,
+                        workspace ? workspace_bytes : static_cast<size_t>(0));
+    if (reinterpret_cast<uintptr_t>(workspace) & 15u)
+        return api_fail(DASH_HASH4D_INVALID_ARG, "decompose: workspace not 16-byte aligned");
+    if (reinterpret_cast<uintptr_t>(result) & 3u)
+        return api_fail(DASH_HASH4D_INVALID_ARG, "decompose: result not 4-byte aligned");
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     const uint32_t blocks = static_cast<uint32_t>((N + kThreads - 1) / kThreads);
     char* w = static_cast<char*>(workspace);
@@ -221,36 +229,44 @@ DASH_API int dash_decompose(uint64_t N, const float* dp, double k_percent, float
     double* block_sum = reinterpret_cast<double*>(w + round16(sizeof(SelectState)) + round16(static_cast<size_t>(blocks) * 4));
     const double md = std::ceil(static_cast<double>(N) * k_percent / 100.0 - 1e-9);
     const uint64_t m = md <= 0.0 ? 0 : (md >= static_cast<double>(N) ? N : static_cast<uint64_t>(md));
+    // every launch is counted and checked on its own, so a failure names the kernel that caused it
+#define DASH_DECOMPOSE_LAUNCHED(what)                                                   \
+    do {                                                                                \
+        count_launch();                                                                 \
+        const cudaError_t le_ = cudaGetLastError();                                     \
+        if (le_ != cudaSuccess) return api_cuda_fail(le_, "decompose: " what " launch"); \
+    } while (0)
     zero_state_kernel<<<1, 256, 0, s>>>(st, static_cast<uint32_t>(m));
-    count_launch();
+    DASH_DECOMPOSE_LAUNCHED("zero_state");
     if (N) {
         magnitude_kernel<<<static_cast<unsigned>((N + 255) / 256), 256, 0, s>>>(N, dp, mag);
-        count_launch();
+        DASH_DECOMPOSE_LAUNCHED("magnitude");
     }
     if (m == 0 || m >= N) {
         set_tau_kernel<<<1, 1, 0, s>>>(st, m == 0 ? 0x7f800000u : 0xbf800000u);   // +inf / -1
-        count_launch();
+        DASH_DECOMPOSE_LAUNCHED("set_tau");
     } else {
         const size_t want = (N + 255) / 256, cap = static_cast<size_t>(device_sm_count()) * 8;
         const unsigned grid = static_cast<unsigned>(want > cap ? cap : want);
         for (int pass = 3; pass >= 0; --pass) {
             select_hist_kernel<<<grid, 256, 0, s>>>(N, mag, st, pass);
+            DASH_DECOMPOSE_LAUNCHED("select_hist");
             select_pick_kernel<<<1, 32, 0, s>>>(st, pass);
-            count_launch();
-            count_launch();
+            DASH_DECOMPOSE_LAUNCHED("select_pick");
         }
     }
     if (N) {
         classify_count_kernel<<<blocks, kThreads, 0, s>>>(N, mag, st, block_dyn, block_sum);
-        count_launch();
+        DASH_DECOMPOSE_LAUNCHED("classify_count");
     }
     scan_finalize_kernel<<<1, 1024, 0, s>>>(N, blocks, block_dyn, block_sum, st, result);
-    count_launch();
+    DASH_DECOMPOSE_LAUNCHED("scan_finalize");
     if (N) {
         compact_grad_kernel<<<blocks, kThreads, 0, s>>>(N, dp, mag, st, block_dyn, result, grad_scale, dyn_index, ddp);
-        count_launch();
+        DASH_DECOMPOSE_LAUNCHED("compact_grad");
     }
-    return cudaGetLastError() == cudaSuccess ? DASH_HASH4D_OK : DASH_HASH4D_CUDA_ERROR;
+#undef DASH_DECOMPOSE_LAUNCHED
+    return api_ok();
 }
 
 }  // extern "C"

@@ -15,6 +15,7 @@
 
 #include "../../include/dash_deform.h"
 #include "../../include/dash_hash4d.h"
+#include "api_errors.h"
 #include "deform_kernels.h"
 #include "hash4d_kernels.h"
 #include "hash4d_plan.h"
@@ -236,6 +237,20 @@ int run_validation(const dash_hash4d_config* c, const Plan& P, const float* xyz,
 }
 
 }  // namespace
+
+namespace dash {  // api_errors.h: the same channel for the other translation units
+
+int api_fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_error, sizeof(g_error), fmt, ap);
+    va_end(ap);
+    return code;
+}
+int api_cuda_fail(cudaError_t e, const char* what) { return cuda_fail(e, what); }
+int api_ok() { return ok(); }
+
+}  // namespace dash
 
 extern "C" {
 

@@ -182,3 +182,22 @@ def test_mlp_bwd_refuses_layer_outputs_wider_than_one_tile():
         assert "128" in dh.dash_hash4d_last_error()
     for widths in ([32, 128, 10], [32, 128, 128, 10], [240, 16]):
         assert call(widths) == 1, widths
+
+
+def test_decompose_failures_set_the_last_error_message():
+    """dash_decompose reports through the library's one error channel: each refusal (decided on the host, no GPU needed)
+    leaves its own message in dash_hash4d_last_error() rather than whatever an earlier call left there."""
+    lib = dh.binding._load()
+    call = lambda n, k, result, ws, ws_bytes: lib.dash_decompose(n, None, k, 1.0, None, None, result, None, ws, ws_bytes, None)
+    dh.dash_hash4d_set_debug(dh.DEBUG_FWD_GROUP, 0)                       # a successful call: message cleared
+    assert dh.dash_hash4d_last_error() == ""
+    assert call(4, 101.0, C.c_void_p(16), None, 0) == 1
+    assert "k_percent" in dh.dash_hash4d_last_error()
+    assert call(4, 10.0, None, None, 0) == 1
+    assert "result" in dh.dash_hash4d_last_error()
+    assert call(1 << 31, 10.0, C.c_void_p(16), None, 0) == 2
+    assert "int32" in dh.dash_hash4d_last_error()
+    assert call(0, 10.0, C.c_void_p(16), None, 0) == 3
+    assert "workspace bytes" in dh.dash_hash4d_last_error()
+    assert call(0, 10.0, C.c_void_p(16), C.c_void_p(8), 1 << 20) == 1
+    assert "aligned" in dh.dash_hash4d_last_error()
