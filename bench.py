@@ -94,6 +94,48 @@ def compulsory_bytes(dh, torch, cfg, enc, N, xyz, t, index):
     return {"fwd": fwd, "bwd": bwd, "step": fwd + bwd, "table_sectors_touched_bytes": table_touched}
 
 
+def time_step_of(dh, torch, wl, peak, l2_bytes, sort_coarse: bool, steps: int = 20):
+    """The timed step of run_cuda (ZERO_GRAD backward, SORT_COARSE forward, ORDER_READY backward, one shared workspace)
+    on another workload `wl`, in the same launch configuration, `steps` times after 3 warm-up steps.  CUDA events per
+    step; a 2 x L2 buffer is written between steps (outside the timed segments) when the working set is smaller than that."""
+    enc, N = wl.spec.enc, wl.N
+    flags = dh.FLAG_DENSE_COARSE | dh.FLAG_ZERO_GRAD | (dh.FLAG_SORT_COARSE if sort_coarse else 0)
+    cfg = dh.config_from_params(enc, flags=flags)
+    cfg_bwd = dh.with_flags(cfg, flags | dh.FLAG_ORDER_READY) if sort_coarse else cfg
+    need = dh.dash_hash4d_workspace_bytes(cfg, N, dh.OP_BWD)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda") if need else None
+    to_dev = lambda a: None if a is None else torch.from_numpy(a).cuda()
+    xyz, t, index, table, dout = to_dev(wl.xyz), to_dev(wl.t), to_dev(wl.index), to_dev(wl.table), to_dev(wl.dout)
+    out = torch.empty((N, enc.L * enc.F), dtype=torch.float32, device="cuda")
+    dtable = torch.empty((enc.L, enc.T, enc.F), dtype=torch.float32, device="cuda")
+    nbytes = lambda x: 0 if x is None else x.numel() * x.element_size()
+    working_set = sum(nbytes(x) for x in (xyz, t, table, dout, out, dtable))
+    flush = torch.empty(2 * l2_bytes, dtype=torch.uint8, device="cuda") if working_set < 2 * l2_bytes else None
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    seg = []
+    for i in range(steps + 3):
+        if flush is not None:
+            flush.zero_()
+        m = [ev(), ev(), ev()]
+        m[0].record()
+        dh.dash_hash4d_fwd(cfg, xyz, t, table, out=out, index=index, workspace=ws)
+        m[1].record()
+        dh.dash_hash4d_bwd(cfg_bwd, xyz, t, dout, dtable, index=index, workspace=ws)
+        m[2].record()
+        if i >= 3:
+            seg.append(m)
+    torch.cuda.synchronize()
+    ms_fwd = sum(m[0].elapsed_time(m[1]) for m in seg) / steps
+    ms_bwd = sum(m[1].elapsed_time(m[2]) for m in seg) / steps
+    ms = sum(m[0].elapsed_time(m[2]) for m in seg) / steps
+    b_fwd, b_bwd, b_zero = algorithmic_bytes(enc, index is not None)
+    step_bytes = (b_fwd + b_bwd) * N + b_zero
+    return {"N": N, "ms_per_step": ms, "Mqueries_per_s": N / (ms * 1e-3) / 1e6, "fwd_ms": ms_fwd, "bwd_ms": ms_bwd,
+            "step_frac_of_hbm_peak": step_bytes / (ms * 1e-3) / 1e9 / peak,
+            "sorted_path_taken": bool(sort_coarse and need), "steps": steps,
+            "l2_flush_between_steps": flush is not None}
+
+
 def measured_hbm_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -474,6 +516,20 @@ def run_cuda(args):
                  "ms": {"zero": ms_zero, "fwd": ms_fwd, "bwd": ms_bwd}},
     }
 
+    # `achieved` / `frac` divide the ALGORITHMIC bytes (one access per corner per query and level) by the
+    # time.  On the sorted path the kernels issue fewer accesses than that count (lines shared between neighbouring
+    # lanes, runs merged in registers), so the figure is a work-equivalent throughput, not HBM utilisation; the DRAM
+    # bytes ncu saw for the same call, over the same live time, are given beside it.
+    roofline["achieved_kind"] = ("algorithmic bytes / time" if not sorted_path else
+                                 "algorithmic bytes / time = work-equivalent throughput: SORT_COARSE issues fewer "
+                                 "accesses than the algorithmic count; see `dram` for the profiled DRAM bytes")
+    if roofline["traffic"]:
+        dram_gbs = roofline["traffic"] / (dom_ms * 1e-3) / 1e9
+        roofline["dram"] = {"bytes_per_call_ncu": roofline["traffic"], "GBps": dram_gbs, "frac": dram_gbs / peak,
+                            "note": "profiles/traffic.json bytes (ncu, cold-cache replay) over the live CUDA-event time of "
+                                    "the same call; the per-call write split under-counts late write-backs, so the step "
+                                    "figure (traffic_step) is the one to quote"}
+
     # ---- the stricter figures of SURVEY.md §8d, beside the algorithmic-bytes fraction
     bmin = compulsory_bytes(dh, torch, dh.config_from_params(enc, flags=dh.FLAG_DENSE_COARSE), enc, N, xyz, t, index)
     roofline["b_min"] = {"bytes": bmin, "step_GBps": bmin["step"] / (ms_step * 1e-3) / 1e9,
@@ -591,6 +647,23 @@ def run_cuda(args):
         one_t = t[:1].contiguous()
         extras["fwd_one_timestamp_ms"] = timed(lambda: dh.dash_hash4d_fwd(cfg_x, xyz, one_t, table, out=out,
                                                                            index=index, t_stride=0))
+        # every other BASELINE.json config's step in this bench's launch configuration (a bar per config)
+        if args.config == "C4":
+            extras["configs"] = {}
+            for name in ("C2", "C3", "C5"):
+                extras["configs"][name] = time_step_of(dh, torch, make_workload(name), peak, l2_bytes,
+                                                       bool(args.sort_coarse))
+            # The rule that turns the sorted path on (N*F >= 2^21, levels with Ns^3 Nt <= 2N) was fitted on clustered
+            # inputs (PAPER.md:241 is the basis for clustering).  A/B on C4's encoder with C1's distribution: 1M
+            # iid-uniform queries, where runs of queries in one cell are short.
+            import copy
+            wl_u = copy.copy(wl)
+            q_u = np.random.default_rng(20).random(size=(wl.N, 4), dtype=np.float32)
+            wl_u.xyz, wl_u.t, wl_u.index = np.ascontiguousarray(q_u[:, :3]), np.ascontiguousarray(q_u[:, 3]), None
+            extras["uniform_1M_on_C4_encoder"] = {
+                "sort_coarse_1": time_step_of(dh, torch, wl_u, peak, l2_bytes, True),
+                "sort_coarse_0": time_step_of(dh, torch, wl_u, peak, l2_bytes, False)}
+            del wl_u, q_u
         # G_3D of the decomposition stage on its own workload (dash_inputs.G3D_SPEC)
         from dash_inputs import make_g3d_workload
         g3 = make_g3d_workload()

@@ -832,8 +832,20 @@ class HostStep:
             d_ready = torch.cuda.Event(); d_ready.record(self.h2d)
         out_d = self._dev_like("out", out_h)
         dt_d = self._dev_like("dtable", dtable_h)
+        # ONE workspace, owned by this object, serves both calls of the step: under SORT_COARSE the forward leaves the
+        # cell-sorted order in it and the backward reuses it (ORDER_READY) instead of sorting again.
+        N = int(index_h.numel()) if index_h is not None else int(xyz_h.shape[0])   # as dash_hash4d_fwd counts them
+        need = max(dash_hash4d_workspace_bytes(cfg, N, OP_FWD), dash_hash4d_workspace_bytes(cfg, N, OP_BWD))
+        ws = self.buf.get("workspace")
+        if need and (ws is None or ws.numel() < need):
+            ws = self.buf["workspace"] = torch.empty(need, dtype=torch.uint8,
+                                                     device=torch.device("cuda", torch.cuda.current_device()))
+        ws = ws if need else None
+        cfg_bwd = cfg
+        if (cfg.flags & FLAG_SORT_COARSE) and not (cfg.flags & FLAG_DETERMINISTIC_BWD):
+            cfg_bwd = with_flags(cfg, cfg.flags | FLAG_ORDER_READY)
         main.wait_event(q_ready)
-        dash_hash4d_fwd(cfg, xyz_d, t_d, table_d, out=out_d, index=index_d, t_stride=t_stride)
+        dash_hash4d_fwd(cfg, xyz_d, t_d, table_d, out=out_d, index=index_d, t_stride=t_stride, workspace=ws)
         f_done = torch.cuda.Event(); f_done.record(main)
         with torch.cuda.stream(self.d2h):
             self.d2h.wait_event(f_done)
@@ -841,7 +853,7 @@ class HostStep:
         main.wait_event(d_ready)
         if not (cfg.flags & FLAG_ZERO_GRAD):
             dash_hash4d_zero(cfg, dt_d)
-        dash_hash4d_bwd(cfg, xyz_d, t_d, dout_d, dt_d, index=index_d, t_stride=t_stride)
+        dash_hash4d_bwd(cfg_bwd, xyz_d, t_d, dout_d, dt_d, index=index_d, t_stride=t_stride, workspace=ws)
         b_done = torch.cuda.Event(); b_done.record(main)
         with torch.cuda.stream(self.d2h):
             self.d2h.wait_event(b_done)

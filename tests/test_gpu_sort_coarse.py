@@ -349,3 +349,47 @@ def test_the_order_in_the_workspace_is_a_permutation_sorted_by_the_morton_key_of
             pos += 1
     assert (np.diff(key[order].astype(np.int64)) >= 0).all()
     assert len(np.unique(key)) > 50                                      # the check is not vacuous
+
+
+def test_host_step_runs_the_default_path_with_one_workspace():
+    """HostStep (the host-buffer call bench.py's e2e leg times) runs the same launches as the device-resident step: one
+    workspace owned by the object, the forward sorts into it, the backward reuses the order (ORDER_READY) and does not
+    sort a second time.  C4's encoder at N = 2^19 (N F = 2^21) takes the sorted path by the library's own rule.  The
+    results are those of the direct device calls: forward bitwise, gradient sums in another order."""
+    wl = make_workload("C4", n_override=1 << 19)
+    enc, N = wl.spec.enc, wl.N
+    cfg = dh.config_from_params(enc, flags=DC | ZG | SC)
+    need = dh.dash_hash4d_workspace_bytes(cfg, N, dh.OP_BWD)
+    assert need > 0, "the workload must take the sorted path"
+    xd, td, tab, dd = dev(wl.xyz), dev(wl.t), dev(wl.table), dev(wl.dout)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    out_d = torch.empty((N, enc.L * enc.F), device="cuda")
+    dt_d = torch.full((enc.L, enc.T, enc.F), 7.0, device="cuda")
+    dh.dash_hash4d_launch_count(reset=True)
+    dh.dash_hash4d_fwd(cfg, xd, td, tab, out=out_d, workspace=ws)
+    dh.dash_hash4d_bwd(dh.with_flags(cfg, DC | ZG | SC | READY), xd, td, dd, dt_d, workspace=ws)
+    device_step_launches = dh.dash_hash4d_launch_count(reset=True)
+    scratch = torch.empty_like(dt_d)
+    dh.dash_hash4d_bwd(cfg, xd, td, dd, scratch, workspace=ws)         # a backward that sorts again: more launches
+    bwd_resorting = dh.dash_hash4d_launch_count(reset=True)
+    dh.dash_hash4d_bwd(dh.with_flags(cfg, DC | ZG | SC | READY), xd, td, dd, scratch, workspace=ws)
+    assert bwd_resorting > dh.dash_hash4d_launch_count(reset=True), "ORDER_READY must save the sort's launches"
+    torch.cuda.synchronize()
+
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    out_h = torch.empty((N, enc.L * enc.F)).pin_memory()
+    dt_h = torch.empty((enc.L, enc.T, enc.F)).pin_memory()
+    step = dh.HostStep(cfg)
+    xyz_h, t_h, dout_h = pin(wl.xyz), pin(wl.t), pin(wl.dout)
+    for it in range(2):                                                 # the second step reuses buffers and workspace
+        out_h.fill_(-1); dt_h.fill_(-1)
+        dh.dash_hash4d_launch_count(reset=True)
+        step(xyz_h, t_h, tab, dout_h, out_h, dt_h)
+        assert dh.dash_hash4d_launch_count(reset=True) == device_step_launches
+        torch.cuda.synchronize()
+        assert torch.equal(out_h, out_d.cpu())
+        np.testing.assert_allclose(dt_h.numpy(), dt_d.cpu().numpy(), rtol=1e-4, atol=1e-5)
+        ws_ptr = step.buf["workspace"].data_ptr()
+        if it:
+            assert ws_ptr == first_ptr, "the workspace is allocated once"
+        first_ptr = ws_ptr
