@@ -117,7 +117,7 @@ uint32_t debug_u32(int key) { return static_cast<uint32_t>(g_debug[key].load(std
 
 // Level-group size G (power of two <= 8): as many levels as keep the group's randomly accessed
 // bytes (tables in fwd, fp32 gradient slices in bwd) within 0.3 x L2 — measured (profiles/
-// group_sweep_r01.md): B200's 126 MB L2 is two 63 MB halves and read-only lines are replicated in
+// group_sweep_r02.md): B200's 126 MB L2 is two 63 MB halves and read-only lines are replicated in
 // both, so ~40 MB is what stays resident next to the streamed inputs/outputs — but at least enough
 // that a query's slice of `out`/`dout` is one full 32-byte sector (G*F*4 >= 32), and without idling
 // more than a quarter of the lanes when L is not a multiple of G.  G = 16 (one query per warp) is

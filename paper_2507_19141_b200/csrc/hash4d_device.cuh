@@ -148,7 +148,7 @@ __device__ __forceinline__ void half_cell(const Plan& P, const LevelParams& lp, 
 // ------------------------------------------------------------------------------------------------
 
 // 8-byte table gather: ld.global.nc with default L1 allocation.  Measured alternatives on C4/C3/C5
-// (profiles/sorted_and_tma_experiments_r01.md §3): L1::no_allocate +41 %/+12 %/+28 % time, ld.global.cg
+// (profiles/experiments_r02.md §9b, a round-1 record): L1::no_allocate +41 %/+12 %/+28 % time, ld.global.cg
 // +3 %/+1 %/+5 %, L1::evict_last +-1 %.
 __device__ __forceinline__ uint2 gather8(const void* p) { return __ldg(static_cast<const uint2*>(p)); }
 

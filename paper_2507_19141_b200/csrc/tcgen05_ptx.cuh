@@ -145,7 +145,8 @@ __device__ __forceinline__ uint32_t operand_offset(uint32_t lbo, uint32_t row, u
 
 // Explicit shared-space stores on 32-bit shared addresses.  Stores through generic pointers into `extern
 // __shared__` made the compiler rebuild the shared window base (S2UR SR_CgaCtaId + ULEA) in the hot loop: 25 % of
-// the producers' stall samples were short-scoreboard waits on that chain (profiles/ncu_deform_adam_r01c.md).
+// the producers' stall samples were short-scoreboard waits on that chain (round-1 ncu source page; the
+// current kernel's stall mix is in profiles/ncu_render_r02.md).
 __device__ __forceinline__ void sts16(uint32_t a, uint16_t v) {
     asm volatile("st.shared.b16 [%0], %1;" ::"r"(a), "h"(v) : "memory");
 }
