@@ -412,7 +412,7 @@ def run_cuda(args):
 
     debug_keys = {"fwd_group": dh.DEBUG_FWD_GROUP, "bwd_group": dh.DEBUG_BWD_GROUP,
                   "smooth_group": dh.DEBUG_SMOOTH_GROUP, "deform_path": dh.DEBUG_DEFORM_PATH,
-                  "bwd_variant": dh.DEBUG_BWD_VARIANT, "fwd_variant": dh.DEBUG_FWD_VARIANT,
+                  "bwd_variant": dh.DEBUG_BWD_VARIANT,
                   "bwd_coarse_levels": dh.DEBUG_BWD_COARSE_LEVELS, "bwd_run_chunk": dh.DEBUG_BWD_RUN_CHUNK,
                   "fwd_ordered_levels": dh.DEBUG_FWD_ORDERED_LEVELS}
     for item in args.set_debug:
@@ -864,7 +864,7 @@ def main():
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), else null")
     ap.add_argument("--set-debug", action="append", default=[], metavar="KEY=VALUE",
                     help="dash_hash4d_set_debug override for A/B runs, e.g. bwd_group=1, bwd_variant=2 "
-                         "(keys: fwd_group bwd_group smooth_group deform_path bwd_variant fwd_variant)")
+                         "(keys: fwd_group bwd_group smooth_group deform_path bwd_variant bwd_coarse_levels bwd_run_chunk fwd_ordered_levels)")
     ap.add_argument("--ceilings", action="store_true",
                     help="run the microbenchmarks of include/dash_ceilings.h and print their JSON line instead")
     ap.add_argument("--md", default=None, help="with --ceilings: also write the table as markdown to this path")

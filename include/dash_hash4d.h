@@ -319,23 +319,6 @@ DASH_API uint64_t dash_hash4d_launch_count(int reset);
  * beside it and refuses (rebuilds, else raises) a library that is out of date. */
 DASH_API const char* dash_hash4d_build_id(void);
 
-/* Tuning overrides for sweeps and A/B measurements (bench.py --sweep, tests).  Process-wide; value 0 restores the
- * library's own choice; the library reads NO environment variable.  Not part of the method: every setting computes
- * the same result.  Returns INVALID_ARG for an unknown key or a negative value. */
-enum dash_debug_key {
-    DASH_DEBUG_FWD_GROUP = 0,    /* levels per level group G of fwd / bwd_input / slice_fwd (1..16, power of two) */
-    DASH_DEBUG_BWD_GROUP = 1,    /* ... of bwd */
-    DASH_DEBUG_SMOOTH_GROUP = 2, /* ... of smooth */
-    DASH_DEBUG_DEFORM_PATH = 3,  /* dash_deform_fwd: 1 = fused kernel, 2 = two-pass (encoder -> workspace -> MLP) */
-    DASH_DEBUG_BWD_VARIANT = 4,  /* bwd with ZERO_GRAD: 1 = no L2 eviction hints on the zero stores / reductions */
-    DASH_DEBUG_FWD_VARIANT = 5,  /* reserved (0) */
-    DASH_DEBUG_BWD_COARSE_LEVELS = 6, /* SORT_COARSE: number of leading levels the run-merged scatter takes */
-    DASH_DEBUG_BWD_RUN_CHUNK = 7,     /* SORT_COARSE: consecutive sorted queries per lane pair */
-    DASH_DEBUG_FWD_ORDERED_LEVELS = 8, /* SORT_COARSE: number of leading levels the forward walks in the sorted order */
-    DASH_DEBUG_KEY_COUNT = 9
-};
-DASH_API int dash_hash4d_set_debug(int key, int64_t value);
-
 #ifdef __cplusplus
 }
 #endif

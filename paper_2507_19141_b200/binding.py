@@ -28,10 +28,13 @@ EXPORTS = ["dash_hash4d_resolutions", "dash_hash4d_workspace_bytes", "dash_hash3
            "dash_hash4d_launch_count", "dash_hash4d_set_debug", "dash_hash4d_build_id",
            "dash_hash3d_resolutions", "dash_hash3d_fwd", "dash_hash3d_bwd", "dash_hash3d_indices", "dash_hash3d_bwd_input",
            "dash_hash4d_adam_step", "dash_mlp_param_count", "dash_mlp_fwd", "dash_mlp_bwd", "dash_deform_bwd", "dash_deform_bwd_workspace_bytes", "dash_deform_workspace_bytes", "dash_deform_fwd",
-           "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd", "dash_ceiling_launch",
+           "dash_hash4d_slice_t", "dash_hash4d_slice_fwd", "dash_deform_slice_fwd",
            "dash_hash4d_sort_workspace_bytes", "dash_hash4d_sort_queries", "dash_hash4d_sort_queries_static",
            "dash_deform_slice_workspace_bytes",
            "dash_decompose_workspace_bytes", "dash_decompose"]
+
+
+CEIL_EXPORTS = ["dash_ceiling_launch"]   # include/dash_ceilings.h, in libdash_ceilings.so (measurement tools, not the method)
 
 
 class Hash4DError(RuntimeError):
@@ -173,8 +176,6 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     lib.dash_decompose_workspace_bytes.restype = sz
     lib.dash_decompose.argtypes = [u64, vp, C.c_double, C.c_float, vp, vp, vp, vp, vp, sz, vp]
     lib.dash_decompose.restype = C.c_int
-    lib.dash_ceiling_launch.argtypes = [C.POINTER(CeilingParams), vp, vp, C.POINTER(C.c_uint64), vp]
-    lib.dash_ceiling_launch.restype = C.c_int
     lib.dash_hash4d_build_id.argtypes = []
     lib.dash_hash4d_build_id.restype = C.c_char_p
     lib.dash_hash4d_set_debug.argtypes = [C.c_int, C.c_int64]
@@ -183,8 +184,33 @@ def _bind(lib: C.CDLL) -> C.CDLL:
     return lib
 
 
+_ceil_lib: Optional[C.CDLL] = None
+
+
+def ceilings_library_path() -> str:
+    return _build.CEIL_LIB
+
+
+def _load_ceilings() -> C.CDLL:
+    """The microbenchmark library (include/dash_ceilings.h), separate from the product library."""
+    global _ceil_lib
+    if _ceil_lib is None:
+        if _build.ceilings_is_stale():
+            try:
+                _build.build_ceilings()
+            except Exception as exc:  # noqa: BLE001
+                raise ImportError(f"libdash_ceilings.so is missing or older than its sources and the nvcc build "
+                                  f"failed: {exc}") from exc
+        lib = C.CDLL(_build.CEIL_LIB)
+        lib.dash_ceiling_launch.argtypes = [C.POINTER(CeilingParams), C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64),
+                                            C.c_void_p]
+        lib.dash_ceiling_launch.restype = C.c_int
+        _ceil_lib = lib
+    return _ceil_lib
+
+
 def exported_symbols() -> list[str]:
-    """Names include/dash_hash4d.h declares that resolve in the loaded library."""
+    """Names the product headers declare that resolve in the product library."""
     lib = _load()
     return [n for n in EXPORTS if hasattr(lib, n)]
 
@@ -293,12 +319,12 @@ def dash_hash4d_launch_count(reset: bool = False) -> int:
     return int(_load().dash_hash4d_launch_count(1 if reset else 0))
 
 
-(DEBUG_FWD_GROUP, DEBUG_BWD_GROUP, DEBUG_SMOOTH_GROUP, DEBUG_DEFORM_PATH, DEBUG_BWD_VARIANT, DEBUG_FWD_VARIANT,
- DEBUG_BWD_COARSE_LEVELS, DEBUG_BWD_RUN_CHUNK, DEBUG_FWD_ORDERED_LEVELS) = range(9)
+(DEBUG_FWD_GROUP, DEBUG_BWD_GROUP, DEBUG_SMOOTH_GROUP, DEBUG_DEFORM_PATH, DEBUG_BWD_VARIANT,
+ DEBUG_BWD_COARSE_LEVELS, DEBUG_BWD_RUN_CHUNK, DEBUG_FWD_ORDERED_LEVELS) = range(8)   # include/dash_debug.h
 
 
 def dash_hash4d_set_debug(key: int, value: int) -> None:
-    """Tuning override for sweeps (include/dash_hash4d.h `dash_debug_key`); 0 restores the library's choice."""
+    """Tuning override for sweeps (include/dash_debug.h `dash_debug_key`); 0 restores the library's choice."""
     _check(_load().dash_hash4d_set_debug(int(key), int(value)))
 
 
@@ -877,7 +903,7 @@ def dash_ceiling_launch(kind, buf, sink, width=8, pattern=CEIL_INDEPENDENT, foot
         raise ValueError("buf / sink smaller than the footprint")
     p.grid, p.block, p.dyn_smem, p.iters, p.seed = int(grid), int(block), int(dyn_smem), int(iters), int(seed)
     ops = C.c_uint64(0)
-    rc = _load().dash_ceiling_launch(C.byref(p), _ptr(buf), _ptr(sink), C.byref(ops), _stream())
+    rc = _load_ceilings().dash_ceiling_launch(C.byref(p), _ptr(buf), _ptr(sink), C.byref(ops), _stream())
     if rc != 0:
         raise Hash4DError(rc, "dash_ceiling_launch: bad parameters or launch failure")
     return int(ops.value)

@@ -6,8 +6,6 @@
 #include <cstdint>
 
 #include "../../include/dash_ceilings.h"
-#include "deform_kernels.h"  // device_sm_count
-#include "hash4d_kernels.h"
 
 namespace dash {
 namespace {
@@ -163,13 +161,28 @@ __global__ void tma_gather_kernel(const CeilArgs a) {
 }  // namespace
 }  // namespace dash
 
+namespace {
+// Built as its own library (libdash_ceilings.so): nothing here is shared with the product library.
+uint32_t sm_count_of_current_device() {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+        return 148u;
+    return static_cast<uint32_t>(sms);
+}
+#ifndef DASH_CEIL_BUILD_ID_STRING
+#define DASH_CEIL_BUILD_ID_STRING "unknown"
+#endif
+__attribute__((used)) const char kCeilBuildId[] = "DASH_CEIL_BUILD_ID=" DASH_CEIL_BUILD_ID_STRING;
+}  // namespace
+
 extern "C" DASH_API int dash_ceiling_launch(const dash_ceiling_params* p, void* buf, void* sink,
                                             uint64_t* lane_ops, void* cuda_stream) {
     using namespace dash;
     if (!p || p->struct_size != sizeof(dash_ceiling_params) || !buf || !sink) return DASH_HASH4D_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(buf) | reinterpret_cast<uintptr_t>(sink)) & 15u) return DASH_HASH4D_INVALID_ARG;
     const uint32_t block = p->block ? p->block : 256u;
-    const uint32_t grid = p->grid ? p->grid : 8u * static_cast<uint32_t>(device_sm_count());
+    const uint32_t grid = p->grid ? p->grid : 8u * sm_count_of_current_device();
     if (block % 32u || block > 1024u || p->iters == 0 || p->pattern > DASH_CEIL_PAIR_XCORNER)
         return DASH_HASH4D_INVALID_ARG;
     const uint32_t w = p->width;
@@ -222,7 +235,6 @@ extern "C" DASH_API int dash_ceiling_launch(const dash_ceiling_params* p, void* 
 #undef DASH_CEIL_LAUNCH
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return DASH_HASH4D_CUDA_ERROR;
-    count_launch();
     if (lane_ops) *lane_ops = static_cast<uint64_t>(grid) * block * p->iters * kUnroll;
     return DASH_HASH4D_OK;
 }

@@ -13,6 +13,7 @@
 #include <cstring>
 #include <mutex>
 
+#include "../../include/dash_debug.h"
 #include "../../include/dash_deform.h"
 #include "../../include/dash_hash4d.h"
 #include "api_errors.h"
