@@ -81,7 +81,11 @@ enum dash_hash4d_flags {
                                                fwd / bwd / bwd_input call with SORT_COARSE wrote for the SAME queries
                                                (N, xyz, t, index unchanged, e.g. the forward of this training step):
                                                the sort (five launches) is skipped.  A false claim gives wrong
-                                               values but no out-of-bounds access.                              */
+                                               values but no out-of-bounds access.  The sort leaves a stamp (N, strides,
+                                               sort key, the xyz / t / index pointers) in the workspace; together with
+                                               VALIDATE_INPUTS, which synchronises anyway, the claim is checked against it
+                                               and a mismatch is INVALID_ARG.  Changed CONTENTS behind unchanged pointers
+                                               are not detected.                                                */
 };
 
 enum dash_hash4d_op { DASH_HASH4D_OP_FWD = 0, DASH_HASH4D_OP_BWD = 1, DASH_HASH4D_OP_INDICES = 2,

@@ -81,7 +81,9 @@ __global__ void __launch_bounds__(kBlockThreads)
 sort4d_scatter_kernel(const __grid_constant__ Plan P, const float* __restrict__ xyz, const float* __restrict__ t,
                       const int32_t* __restrict__ index, const uint32_t* __restrict__ keys,
                       uint32_t* __restrict__ cursor, const uint32_t* __restrict__ tile_offset,
-                      int32_t* __restrict__ order, float4* __restrict__ sorted_q) {
+                      int32_t* __restrict__ order, float4* __restrict__ sorted_q, WorkspaceHeader* __restrict__ hdr,
+                      const OrderStamp stamp) {
+    if (blockIdx.x == 0 && threadIdx.x < 12) hdr->order_stamp.w[threadIdx.x] = stamp.w[threadIdx.x];
     const size_t stride = static_cast<size_t>(gridDim.x) * kBlockThreads;
     for (uint64_t n = static_cast<uint64_t>(blockIdx.x) * kBlockThreads + threadIdx.x; n < P.N; n += stride) {
         float c[4];
@@ -202,7 +204,7 @@ inline cudaError_t launched() {
 
 cudaError_t launch_coarse_sort(const Plan& P, const CoarseSort& cs, const float* xyz, const float* t,
                                const int32_t* index, int32_t* order, float4* sorted_q, uint32_t* keys, uint32_t* bins,
-                               uint32_t* totals, cudaStream_t s) {
+                               uint32_t* totals, cudaStream_t s, WorkspaceHeader* hdr, const OrderStamp& stamp) {
     const size_t want = (P.N + kBlockThreads - 1) / kBlockThreads;
     const size_t cap = static_cast<size_t>(device_sm_count()) * 16;
     const unsigned blocks = static_cast<unsigned>(want < 1 ? 1 : (want > cap ? cap : want));
@@ -213,9 +215,11 @@ cudaError_t launch_coarse_sort(const Plan& P, const CoarseSort& cs, const float*
     if ((e = launched()) != cudaSuccess) return e;
     if ((e = launch_exclusive_scan_u32(bins, cs.n_bins, totals, s, false)) != cudaSuccess) return e;
     if (P.dims == 3)
-        sort4d_scatter_kernel<3><<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, totals, order, sorted_q);
+        sort4d_scatter_kernel<3><<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, totals, order, sorted_q, hdr,
+                                                                  stamp);
     else
-        sort4d_scatter_kernel<4><<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, totals, order, sorted_q);
+        sort4d_scatter_kernel<4><<<blocks, kBlockThreads, 0, s>>>(P, xyz, t, index, keys, bins, totals, order, sorted_q, hdr,
+                                                                  stamp);
     return launched();
 }
 

@@ -225,7 +225,7 @@ int run_validation(const dash_hash4d_config* c, const Plan& P, const float* xyz,
         return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "VALIDATE_INPUTS needs %zu workspace bytes",
                     kHeaderBytes);
     WorkspaceHeader* hdr = static_cast<WorkspaceHeader*>(workspace);
-    cudaError_t e = dash::launch_zero(hdr, kHeaderBytes, s);
+    cudaError_t e = dash::launch_zero(hdr, dash::kHeaderScratchBytes, s);   // not the order stamp behind it
     if (e == cudaSuccess) e = dash::launch_validate(P, xyz, t, index, hdr, s);
     if (e != cudaSuccess) return cuda_fail(e, "validate launch");
     uint32_t bad = 0;
@@ -361,6 +361,46 @@ static CoarseBuffers carve_coarse(void* workspace, const dash::CoarseSort& cs, u
     return b;
 }
 
+// What identifies the queries and the key an order was computed for.  The sort writes it behind the order; a later
+// ORDER_READY call can compare it (verify_order).
+static dash::OrderStamp order_stamp(const Plan& P, const dash::CoarseSort& cs, const float* xyz, const float* t,
+                                    const int32_t* index) {
+    dash::OrderStamp st;
+    const uint64_t px = reinterpret_cast<uintptr_t>(xyz), pt = reinterpret_cast<uintptr_t>(t),
+                   pi = reinterpret_cast<uintptr_t>(index);
+    st.w[0] = 0x44415348u;   // "DASH": a workspace that no sort has written never matches
+    st.w[1] = static_cast<uint32_t>(P.N);
+    st.w[2] = static_cast<uint32_t>(P.N >> 32);
+    st.w[3] = P.dims | (P.xyz_stride << 8) | (P.t_stride << 16);
+    st.w[4] = cs.key_level | (cs.bits_s << 8) | (cs.bits_t << 16);
+    st.w[5] = cs.shift_s | (cs.shift_t << 8);
+    st.w[6] = static_cast<uint32_t>(px); st.w[7] = static_cast<uint32_t>(px >> 32);
+    st.w[8] = static_cast<uint32_t>(pt); st.w[9] = static_cast<uint32_t>(pt >> 32);
+    st.w[10] = static_cast<uint32_t>(pi); st.w[11] = static_cast<uint32_t>(pi >> 32);
+    return st;
+}
+
+// ORDER_READY is a promise the library cannot check without reading the workspace back.  Under VALIDATE_INPUTS, which
+// synchronises the stream anyway, it does: the stamp the sort left must be the one this call would write.
+static int verify_order(const dash_hash4d_config* cfg, const Plan& P, const dash::CoarseSort& cs, const float* xyz,
+                        const float* t, const int32_t* index, void* workspace, cudaStream_t s) {
+    constexpr uint32_t kBoth = DASH_HASH4D_FLAG_ORDER_READY | DASH_HASH4D_FLAG_VALIDATE_INPUTS;
+    if ((cfg->flags & kBoth) != kBoth) return DASH_HASH4D_OK;
+    dash::OrderStamp got;
+    cudaError_t e = cudaMemcpyAsync(&got, &static_cast<WorkspaceHeader*>(workspace)->order_stamp, sizeof(got),
+                                    cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(e, "ORDER_READY stamp readback");
+    const dash::OrderStamp want = order_stamp(P, cs, xyz, t, index);
+    if (std::memcmp(&got, &want, sizeof(want)) != 0)
+        return fail(DASH_HASH4D_INVALID_ARG, "ORDER_READY: the workspace does not hold an order for these queries (%s)",
+                    got.w[0] != want.w[0] ? "no SORT_COARSE call has sorted into it" :
+                    (got.w[1] != want.w[1] || got.w[2] != want.w[2]) ? "it was computed for a different N" :
+                    std::memcmp(&got.w[6], &want.w[6], 24) != 0 ? "xyz, t or index pointer differs" :
+                    "strides or sort key differ");
+    return DASH_HASH4D_OK;
+}
+
 static size_t workspace_need(const dash_hash4d_config* cfg, int op, uint64_t N, int dims = 4) {
     size_t bytes = 0;
     if ((cfg->flags & DASH_HASH4D_FLAG_VALIDATE_INPUTS) && op != DASH_HASH4D_OP_INDICES)
@@ -413,13 +453,16 @@ static int fwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
         return fail(DASH_HASH4D_WORKSPACE_TOO_SMALL, "fwd needs %zu workspace bytes, got %zu", need, workspace_bytes);
     if (coarse && !aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
+    if (coarse)
+        if (int rc = verify_order(cfg, P, cs, xyz, t, index, workspace, s)) return rc;
     cudaError_t e = cudaSuccess;
     if (coarse) {
         // SORT_COARSE: the coarse levels in cell-sorted order (a warp's lanes then share cells and lines: C4 levels 0-3
         // 120 -> 72 us, profiles/experiments_r02.md §8), the others in the caller's order
         const CoarseBuffers b = carve_coarse(workspace, cs, N);
         if (!(cfg->flags & DASH_HASH4D_FLAG_ORDER_READY))
-            e = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s);
+            e = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s,
+                                         static_cast<WorkspaceHeader*>(workspace), order_stamp(P, cs, xyz, t, index));
         if (e != cudaSuccess) return cuda_fail(e, "coarse sort launch");
         Plan Pc = P;
         const uint32_t lf = cs.levels_fwd;
@@ -501,11 +544,14 @@ static int bwd_input_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, c
                     workspace_bytes);
     if (coarse && !aligned16(workspace)) return fail(DASH_HASH4D_INVALID_ARG, "workspace not 16-byte aligned");
     if (int rc = run_validation(cfg, P, xyz, t, index, workspace, workspace_bytes, s)) return rc;
+    if (coarse)
+        if (int rc = verify_order(cfg, P, cs, xyz, t, index, workspace, s)) return rc;
     cudaError_t e = dash::launch_zero(dq, static_cast<size_t>(N) * dims * sizeof(float), s);
     if (e == cudaSuccess && coarse) {
         const CoarseBuffers b = carve_coarse(workspace, cs, N);
         if (!(cfg->flags & DASH_HASH4D_FLAG_ORDER_READY))
-            e = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s);
+            e = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s,
+                                         static_cast<WorkspaceHeader*>(workspace), order_stamp(P, cs, xyz, t, index));
         if (e == cudaSuccess)
             e = dash::launch_bwd_input(P, xyz, t, index, table, half, dout, dq, s, b.order, b.sorted_q);
     } else if (e == cudaSuccess) {
@@ -622,12 +668,15 @@ static int bwd_impl(int dims, const dash_hash4d_config* cfg, uint64_t N, const f
     // the others through the one-reduction-per-corner kernel in the caller's order.
     dash::CoarseSort cs;
     const bool coarse = plan_coarse(cfg, N, &cs, dims);
+    if (coarse)
+        if (int rc = verify_order(cfg, P, cs, xyz, t, index, workspace, s)) return rc;
     const uint32_t l_first = coarse ? cs.levels : 0u;
     auto scatter_coarse = [&](bool hint) -> cudaError_t {
         const CoarseBuffers b = carve_coarse(workspace, cs, N);
         cudaError_t ce = cudaSuccess;
         if (!(cfg->flags & DASH_HASH4D_FLAG_ORDER_READY))
-            ce = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s);
+            ce = dash::launch_coarse_sort(P, cs, xyz, t, index, b.order, b.sorted_q, b.keys, b.bins, b.totals, s,
+                                         static_cast<WorkspaceHeader*>(workspace), order_stamp(P, cs, xyz, t, index));
         if (ce == cudaSuccess) ce = dash::launch_bwd_runs(P, cs, dout, dtable, b.order, b.sorted_q, s, hint);
         return ce;
     };

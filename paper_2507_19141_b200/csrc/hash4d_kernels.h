@@ -10,14 +10,23 @@
 namespace dash {
 
 // Header of the caller's workspace when a flag needs one (DETERMINISTIC_BWD / VALIDATE_INPUTS).
+// What a SORT_COARSE sort was computed for: written behind the order by the sort's last kernel, compared by a later
+// ORDER_READY call when VALIDATE_INPUTS lets it synchronise (hash4d_api.cu).  Plain words so that memcmp decides.
+struct OrderStamp {
+    uint32_t w[12];
+};
+
 struct WorkspaceHeader {
     uint32_t absmax_bits;   // max |dout| as binary32 bits (deterministic bwd)
     float scale;            // fixed-point scale 2^s
     double inv_scale;       // 2^-s
     uint32_t bad_inputs;    // VALIDATE_INPUTS: coordinates that are NaN or outside [0,1)
-    uint32_t pad[27];
+    uint32_t pad0[11];      // the first 64 bytes are per-call scratch (zeroed by VALIDATE_INPUTS)
+    OrderStamp order_stamp; // bytes 64..111: survives from the call that sorted to the calls that reuse the order
+    uint32_t pad1[4];
 };
 static_assert(sizeof(WorkspaceHeader) == 128, "workspace header is 128 bytes");
+constexpr size_t kHeaderScratchBytes = 64;
 
 // order / sorted_q (both or neither; G_4D only): walk the queries in the cell-sorted order of launch_coarse_sort
 cudaError_t launch_fwd(const Plan& P, const float* xyz, const float* t, const int32_t* index,
@@ -60,7 +69,7 @@ struct CoarseSort {
 // order[i] = number of the i-th query in key order, sorted_q[i] = its (x, y, z, t); keys / bins / totals: scratch
 cudaError_t launch_coarse_sort(const Plan& P, const CoarseSort& cs, const float* xyz, const float* t,
                                const int32_t* index, int32_t* order, float4* sorted_q, uint32_t* keys, uint32_t* bins,
-                               uint32_t* totals, cudaStream_t s);
+                               uint32_t* totals, cudaStream_t s, WorkspaceHeader* hdr, const OrderStamp& stamp);
 cudaError_t launch_bwd_runs(const Plan& P, const CoarseSort& cs, const float* dout, float* dtable, const int32_t* order,
                             const float4* sorted_q, cudaStream_t s, bool l2_hint);
 cudaError_t launch_slice_t(const Plan& P, const float* t, const void* table, bool table_half, float* slice,

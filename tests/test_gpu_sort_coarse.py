@@ -393,3 +393,39 @@ def test_host_step_runs_the_default_path_with_one_workspace():
         if it:
             assert ws_ptr == first_ptr, "the workspace is allocated once"
         first_ptr = ws_ptr
+
+
+def test_order_ready_claim_is_checked_under_validate_inputs():
+    """ORDER_READY is a promise about the workspace.  The sort stamps what it sorted (N, strides, key, the query pointers);
+    with VALIDATE_INPUTS (which synchronises anyway) a call that claims ORDER_READY for other queries, or on a workspace no
+    sort has written, is refused with INVALID_ARG instead of silently computing with a foreign order."""
+    wl = make_workload("C4", n_override=(1 << 19) + 64)   # N - 1 still takes the sorted path (N F >= 2^21)
+    enc, N = wl.spec.enc, wl.N
+    V = dh.FLAG_VALIDATE_INPUTS
+    cfg = dh.config_from_params(enc, flags=DC | ZG | SC)
+    ready = dh.with_flags(cfg, DC | ZG | SC | READY | V)
+    need = dh.dash_hash4d_workspace_bytes(ready, N, dh.OP_BWD)
+    assert need > 0
+    xd, td, tab, dd = dev(wl.xyz), dev(wl.t), dev(wl.table), dev(wl.dout)
+    dt = torch.empty((enc.L, enc.T, enc.F), device="cuda")
+    fresh = torch.zeros(need, dtype=torch.uint8, device="cuda")
+    with pytest.raises(dh.Hash4DError) as e:                            # nothing has sorted into this workspace
+        dh.dash_hash4d_bwd(ready, xd, td, dd, dt, workspace=fresh)
+    assert e.value.status == 1 and "ORDER_READY" in str(e.value)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    out = dh.dash_hash4d_fwd(cfg, xd, td, tab, workspace=ws)            # sorts and stamps
+    dh.dash_hash4d_bwd(ready, xd, td, dd, dt, workspace=ws)             # the honest claim passes, validation included
+    want = dh.dash_hash4d_bwd(dh.with_flags(cfg, DC | ZG | SC | READY), xd, td, dd, torch.empty_like(dt), workspace=ws)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(dt.cpu().numpy(), want.cpu().numpy(), rtol=1e-4, atol=1e-5)
+    assert torch.equal(dh.dash_hash4d_fwd(ready, xd, td, tab, workspace=ws), out)
+    with pytest.raises(dh.Hash4DError) as e:                            # fewer queries than the order was built for
+        dh.dash_hash4d_bwd(ready, xd, td, dd, dt, N=N - 1, workspace=ws)
+    assert e.value.status == 1 and "different N" in str(e.value)
+    with pytest.raises(dh.Hash4DError) as e:                            # other coordinates (a copy at another address)
+        dh.dash_hash4d_bwd(ready, xd.clone(), td, dd, dt, workspace=ws)
+    assert e.value.status == 1 and "pointer" in str(e.value)
+    with pytest.raises(dh.Hash4DError):                                 # an index list appears
+        dh.dash_hash4d_bwd_input(ready, xd, td, tab, dd, index=torch.arange(N, dtype=torch.int32, device="cuda"),
+                                 workspace=ws)
+    dh.dash_hash4d_bwd(ready, xd, td, dd, dt, workspace=ws)             # the refused calls left the stamp intact
