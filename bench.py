@@ -414,7 +414,7 @@ def run_cuda(args):
                   "smooth_group": dh.DEBUG_SMOOTH_GROUP, "deform_path": dh.DEBUG_DEFORM_PATH,
                   "bwd_variant": dh.DEBUG_BWD_VARIANT,
                   "bwd_coarse_levels": dh.DEBUG_BWD_COARSE_LEVELS, "bwd_run_chunk": dh.DEBUG_BWD_RUN_CHUNK,
-                  "fwd_ordered_levels": dh.DEBUG_FWD_ORDERED_LEVELS}
+                  "fwd_ordered_levels": dh.DEBUG_FWD_ORDERED_LEVELS, "sort_key_bits": dh.DEBUG_SORT_KEY_BITS}
     for item in args.set_debug:
         key, _, val = item.partition("=")
         dh.dash_hash4d_set_debug(debug_keys[key], int(val))
@@ -864,7 +864,7 @@ def main():
                     help="ncu dram bytes per launch of the dominant kernel (from profiles/), else null")
     ap.add_argument("--set-debug", action="append", default=[], metavar="KEY=VALUE",
                     help="dash_hash4d_set_debug override for A/B runs, e.g. bwd_group=1, bwd_variant=2 "
-                         "(keys: fwd_group bwd_group smooth_group deform_path bwd_variant bwd_coarse_levels bwd_run_chunk fwd_ordered_levels)")
+                         "(keys: fwd_group bwd_group smooth_group deform_path bwd_variant bwd_coarse_levels bwd_run_chunk fwd_ordered_levels sort_key_bits)")
     ap.add_argument("--ceilings", action="store_true",
                     help="run the microbenchmarks of include/dash_ceilings.h and print their JSON line instead")
     ap.add_argument("--md", default=None, help="with --ceilings: also write the table as markdown to this path")

@@ -26,7 +26,8 @@ enum dash_debug_key {
     DASH_DEBUG_BWD_COARSE_LEVELS = 5, /* SORT_COARSE: number of leading levels the run-merged scatter takes */
     DASH_DEBUG_BWD_RUN_CHUNK = 6,     /* SORT_COARSE: consecutive sorted queries per lane pair */
     DASH_DEBUG_FWD_ORDERED_LEVELS = 7, /* SORT_COARSE: number of leading levels the forward walks in the sorted order */
-    DASH_DEBUG_KEY_COUNT = 8
+    DASH_DEBUG_SORT_KEY_BITS = 8,      /* SORT_COARSE: cap on the bits of the sort key, 8..22 (bins = 2^bits) */
+    DASH_DEBUG_KEY_COUNT = 9
 };
 DASH_API int dash_hash4d_set_debug(int key, int64_t value);
 

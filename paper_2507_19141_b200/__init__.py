@@ -15,7 +15,7 @@ from .binding import (  # noqa: F401
     MlpConfig, make_mlp_config, dash_mlp_param_count, dash_mlp_fwd, dash_mlp_bwd, dash_deform_bwd, dash_deform_workspace_bytes, dash_deform_fwd,
     dash_hash4d_fwd_host, dash_hash4d_bwd_host, exported_symbols, with_flags, HostStep,
     dash_hash4d_sort_queries, dash_hash4d_sort_queries_static, dash_decompose, dash_decompose_read, DecomposeResult, dash_hash4d_set_debug, DEBUG_FWD_GROUP, DEBUG_BWD_GROUP, DEBUG_SMOOTH_GROUP, DEBUG_DEFORM_PATH,
-    DEBUG_BWD_VARIANT, DEBUG_BWD_COARSE_LEVELS, DEBUG_BWD_RUN_CHUNK, DEBUG_FWD_ORDERED_LEVELS,
+    DEBUG_BWD_VARIANT, DEBUG_BWD_COARSE_LEVELS, DEBUG_BWD_RUN_CHUNK, DEBUG_FWD_ORDERED_LEVELS, DEBUG_SORT_KEY_BITS,
     dash_ceiling_launch, CEIL_COPY, CEIL_GATHER, CEIL_RED, CEIL_SMEM_ATOMIC, CEIL_TMA_GATHER, CEIL_SMEM_ATOMIC_U64,
     CEIL_INDEPENDENT, CEIL_PAIR_ALIGNED, CEIL_PAIR_XCORNER,
 )

@@ -320,7 +320,7 @@ def dash_hash4d_launch_count(reset: bool = False) -> int:
 
 
 (DEBUG_FWD_GROUP, DEBUG_BWD_GROUP, DEBUG_SMOOTH_GROUP, DEBUG_DEFORM_PATH, DEBUG_BWD_VARIANT,
- DEBUG_BWD_COARSE_LEVELS, DEBUG_BWD_RUN_CHUNK, DEBUG_FWD_ORDERED_LEVELS) = range(8)   # include/dash_debug.h
+ DEBUG_BWD_COARSE_LEVELS, DEBUG_BWD_RUN_CHUNK, DEBUG_FWD_ORDERED_LEVELS, DEBUG_SORT_KEY_BITS) = range(9)   # include/dash_debug.h
 
 
 def dash_hash4d_set_debug(key: int, value: int) -> None:

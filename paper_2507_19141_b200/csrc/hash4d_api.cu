@@ -321,7 +321,9 @@ static bool plan_coarse(const dash_hash4d_config* c, uint64_t N, dash::CoarseSor
     cs->key_level = nl - 1;
     auto ceil_log2 = [](uint32_t v) { uint32_t b = 0; while ((1ull << b) < v) ++b; return b; };
     uint32_t bs = ceil_log2(s.res_s[nl - 1]), bt = ceil_log2(s.res_t[nl - 1]);
-    while (3 * (bs - cs->shift_s) + (bt - cs->shift_t) > 22 || bs - cs->shift_s > 7 || bt - cs->shift_t > 7) {
+    uint32_t max_bits = debug_u32(DASH_DEBUG_SORT_KEY_BITS);
+    max_bits = max_bits ? (max_bits < 8 ? 8u : (max_bits > 22 ? 22u : max_bits)) : 22u;
+    while (3 * (bs - cs->shift_s) + (bt - cs->shift_t) > max_bits || bs - cs->shift_s > 7 || bt - cs->shift_t > 7) {
         if (bt - cs->shift_t > bs - cs->shift_s) ++cs->shift_t; else ++cs->shift_s;
     }
     cs->bits_s = bs - cs->shift_s;
