@@ -34,7 +34,9 @@ def unmasked_bound(widths, params, dout):
     return D
 
 
-def check_bwd(widths, feat, params, dout, dfeat, dparams, what):
+def check_bwd(widths, feat, params, dout, dfeat, dparams, what, p_slack=0.0):
+    """p_slack: elementwise absolute allowance on dparams for error that is not the kernel's (the rounding of an fp32
+    '+=' into a non-zero start); both dparams checks run on the values as they came back, nothing is clipped."""
     fq, pq, fa, pa, mg = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout,
                                                want_abs=True)
     dfeat, dparams = np.asarray(dfeat, np.float64), np.asarray(dparams, np.float64)
@@ -48,8 +50,9 @@ def check_bwd(widths, feat, params, dout, dfeat, dparams, what):
     loose = 2.0 * unmasked_bound(widths, params, dout)
     assert (err[~ok] <= loose[~ok] + 1e-30).all(), f"{what}: dfeat of a near-kink row outside the validity bound"
     errp = np.abs(dparams - pq)
-    assert (errp <= 4e-3 * pa + 1e-30).all(), f"{what}: dparams worst err/A {(errp / (pa + 1e-300)).max():.3e}"
-    nrmp = np.linalg.norm(dparams - pq) / max(np.linalg.norm(pq), 1e-300)
+    assert (errp <= 4e-3 * pa + p_slack + 1e-30).all(), f"{what}: dparams worst err/A {(errp / (pa + 1e-300)).max():.3e}"
+    slack_norm = float(np.linalg.norm(np.broadcast_to(p_slack, pq.shape)))
+    nrmp = (np.linalg.norm(dparams - pq) - slack_norm) / max(np.linalg.norm(pq), 1e-300)
     assert nrmp <= 4e-3, f"{what}: dparams normwise {nrmp:.3e}"
     return float(ok.mean())
 
@@ -85,12 +88,12 @@ def test_mlp_bwd_parity(widths, N):
 
 
 def check_bwd_with_start(widths, feat, params, dout, dfeat, got_p, start, what):
-    fq, pq, fa, pa, mg = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout,
-                                               want_abs=True)
+    """dparams was accumulated into a random `start`: the fp32 '+=' rounds at the magnitude of start + gradient, which is
+    not the kernel's error.  That rounding is passed on as an absolute slack; the UNCLIPPED difference is what is checked,
+    element by element and normwise."""
+    _, pq = oracle.oracle_mlp_bwd(oracle.make_mlp_config(widths, quant_bf16=True), feat, params, dout)
     slack = 2.0 ** -22 * (np.abs(start) + np.abs(pq))
-    errp = np.abs(got_p - pq)
-    assert (errp <= 4e-3 * pa + slack + 1e-30).all(), f"{what}: dparams worst err/A {(errp / (pa + 1e-300)).max():.3e}"
-    return check_bwd(widths, feat, params, dout, dfeat, pq + np.clip(got_p - pq, -4e-3 * pa, 4e-3 * pa), what)
+    return check_bwd(widths, feat, params, dout, dfeat, got_p, what, p_slack=slack)
 
 
 def test_mlp_bwd_without_dfeat_and_twice_accumulates():
